@@ -1,0 +1,146 @@
+/*
+ * pz.h -- C ABI of the B200-native Poisson + wall-normal Helmholtz hot path of
+ * arxiv/paper_2502_06296 (Diez, Peeters, Costa: pencil-distributed finite-difference
+ * solver for turbulent wall flows).  Citations are PAPER.md:<line>.
+ *
+ * Everything behind this boundary is hand-written CUDA for sm_100a in FP64.  There is no
+ * CPU fallback: without a CUDA device every compute entry point returns PZ_ECUDA.
+ *
+ * Conventions
+ *   - Fields are compact C-order arrays p[k][j][i] of nx*ny*nz doubles, x (i) fastest,
+ *     z (k) slowest, no ghost cells.  Element offsets are 64-bit.
+ *   - "device" pointers are CUDA device addresses, "host" pointers are ordinary host
+ *     addresses (pinned memory is faster for the *_host calls but not required).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - All solves are IN PLACE ("only the array d' is modified in-place"),
+ *     asynchronous on `stream`, allocate nothing, never synchronise the host, use no
+ *     atomics (bitwise run-to-run deterministic) and can be captured into a CUDA graph.
+ *   - The caller owns every array it passes; zc/zf are copied at plan creation.  The plan
+ *     owns its device tables and workspace until poisson_plan_destroy.
+ *   - Every function returns a pz_status; on failure pz_last_error() holds a message
+ *     (thread-local) and no output array has a defined value.
+ *
+ * Grid: uniform spacing lx/nx, ly/ny in the periodic directions; wall-normal cell faces
+ * zf[0..nz] (strictly increasing) and cell centres zc[0..nz-1] with zf[k] < zc[k] < zf[k+1]
+ * (staggered grid, uniform x,y, non-uniform z, second-order differences).
+ *   dzf_k = zf[k+1]-zf[k], dzc_k = zc[k+1]-zc[k],
+ *   A_k = 1/(dzf_k dzc_{k-1}) (A_0 = 0),  C_k = 1/(dzf_k dzc_k) (C_{nz-1} = 0).
+ */
+#ifndef PZ_H
+#define PZ_H
+
+#if defined(__GNUC__)
+#define PZ_API __attribute__((visibility("default")))
+#else
+#define PZ_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pz_plan pz_plan; /* opaque */
+
+enum pz_status {
+    PZ_OK = 0,
+    PZ_EINVAL = 1,       /* null pointer, non-positive size, non-monotone grid, a < 0, ... */
+    PZ_EUNSUPPORTED = 2, /* nx or ny not a power of two in [8, 4096], nz < 4, unknown bc/option */
+    PZ_ENOMEM = 3,       /* host or device allocation failed */
+    PZ_ECUDA = 4,        /* CUDA runtime error (message in pz_last_error) */
+    PZ_ENOTSETUP = 5     /* helmholtz_z_solve before helmholtz_z_setup */
+};
+
+/* The only boundary-condition set on the hot path: x, y periodic; Poisson: zero wall-normal
+ * gradient at both walls (Neumann); Helmholtz: u = 0 at both wall faces (Dirichlet). */
+enum pz_bc { PZ_BC_PERIODIC_XY_NEUMANN_P_DIRICHLET_U = 0 };
+
+/*
+ * Plan / pre-processing (PAPER.md:199 "only once as an initialization step", :338
+ * "inexpensive operation ... during the initialization").  Builds on the host and uploads:
+ * the z-metric tables A_k, C_k, dzf_k; the modified wavenumbers lambda_x, lambda_y
+ * re-ordered for the packed half-complex layout; the FFT
+ * twiddle tables.  No field-sized device memory is allocated by the default solver variants.
+ *   out    receives the plan (host pointer to host pointer)
+ *   zc,zf  host arrays of nz and nz+1 doubles
+ * Errors: PZ_EINVAL, PZ_EUNSUPPORTED, PZ_ENOMEM, PZ_ECUDA.
+ */
+PZ_API int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double ly,
+                        const double *zc, const double *zf, int bc);
+
+/*
+ * Pressure Poisson solve, Eq. (4)/(12), steps 2-8 of PAPER.md:124-131:
+ * real FFT along x, FFT along y, one tridiagonal solve along z per (kx,ky) with the
+ * eigenvalue lambda_x(i)+lambda_y(j) added to the diagonal -(A_k+C_k) (Neumann walls),
+ * inverse FFTs, 1/(nx ny) scaling.  On entry p = right-hand side f, on return p = phi with
+ *   (L_h phi) = f   and   sum_ijk dzf_k phi_ijk = 0   (the singular (0,0) mode is solved with
+ * its last wall-normal equation replaced by the gauge and carries zero volume mean).
+ * f must be compatible (sum_ijk dzf_k f_ijk = 0); this is not checked.
+ *   p  device, nx*ny*nz doubles, 16-byte aligned, in place.
+ */
+PZ_API int poisson_solve(pz_plan *plan, double *p, void *stream);
+
+/*
+ * Wall-normal implicit diffusion, Eq. (11), with the paper's split of the
+ * cyclic-reduction solver into pre-processing and runtime (Algorithm 2).
+ *
+ * helmholtz_z_setup: pre-processing for (I - a L_z), a = gamma_k nu dt / 2 >= 0.  Computes the
+ * k-only coefficient sub-arrays of Algorithm 2 Step 1 for every sub-domain, and the per-level
+ * multipliers of the cyclic reduction of the boundary system, on the host (O(nz) work), and
+ * uploads them into the table set not used by solves still in flight.  May be called once
+ * per Runge-Kutta sub-step ("time-dependent").
+ *
+ * helmholtz_z_solve: runtime.  For every (i,j) column solves
+ *   u_k - a [A_k (u_{k-1}-u_k) + C_k (u_{k+1}-u_k) - W_k u_k] = r_k,
+ * W_k = 0 except W_0 = 1/(dzf_0 (zc_0-zf_0)), W_{nz-1} = 1/(dzf_{nz-1} (zf_nz-zc_{nz-1}))
+ * (u = 0 on the wall faces), touching only the right-hand side (Algorithm 2 Steps 2-4).
+ *   u  device, nx*ny*nz doubles, in place: on entry r, on return u.
+ * helmholtz_z_solve_n applies the same operator to n fields (the three velocity components).
+ * Errors: PZ_ENOTSETUP before the first setup; PZ_EINVAL for a < 0 or null pointers.
+ */
+PZ_API int helmholtz_z_setup(pz_plan *plan, double a);
+PZ_API int helmholtz_z_solve(pz_plan *plan, double *u, void *stream);
+PZ_API int helmholtz_z_solve_n(pz_plan *plan, double *const *u, int n, void *stream);
+
+/*
+ * End-to-end variants with HOST buffers: copy host -> device workspace (owned by the plan,
+ * allocated on first use: nx*ny*nz doubles), solve, copy back, all asynchronously on
+ * `stream`.  The host buffer must stay valid until the stream has been synchronised.
+ */
+PZ_API int poisson_solve_host(pz_plan *plan, double *p_host, void *stream);
+PZ_API int helmholtz_z_solve_host(pz_plan *plan, double *u_host, void *stream);
+
+/* Frees every device and host resource of the plan.  NULL is accepted. */
+PZ_API int poisson_plan_destroy(pz_plan *plan);
+
+/* Message of the last failure on the calling thread ("" if none). */
+PZ_API const char *pz_last_error(void);
+
+/* ------------------------------------------------------------------ diagnostics
+ * Used by the tests, the benchmark and the profiles; not needed by a solver user. */
+
+/* Stages of poisson_solve, runnable one at a time on a device field (in place). */
+enum pz_stage {
+    PZ_STAGE_FFT_X_FWD = 0, /* a1: R2C along x into the packed layout                     */
+    PZ_STAGE_FFT_Y_FWD = 1, /* a2: FFT along y of the packed complex pairs                */
+    PZ_STAGE_Z_SOLVE = 2,   /* a3: tridiagonal solves in spectral space                   */
+    PZ_STAGE_FFT_Y_INV = 3, /* a4                                                         */
+    PZ_STAGE_FFT_X_INV = 4  /* a5: C2R along x and 1/(nx ny) scaling                      */
+};
+PZ_API int pz_poisson_stage(pz_plan *plan, double *p, int stage, void *stream);
+
+/* Integer tuning options (kernel variants, tile widths, slab sizes).  Unknown keys or
+ * unsupported values return PZ_EUNSUPPORTED and change nothing.  Keys are listed in
+ * DESIGN.md ("Options"). */
+PZ_API int pz_set_option(pz_plan *plan, const char *key, int value);
+PZ_API int pz_get_option(const pz_plan *plan, const char *key, int *value);
+
+/* Number of kernels this library has launched since it was loaded (host-side counter). */
+PZ_API long long pz_launch_count(void);
+
+/* Library version: major*10000 + minor*100 + patch. */
+PZ_API int pz_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PZ_H */

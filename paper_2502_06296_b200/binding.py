@@ -1,0 +1,189 @@
+"""Thin ctypes binding of include/pz.h -- argument marshalling only.
+
+Same names as the C ABI.  PyTorch is used for device memory and streams: a field is a
+contiguous float64 CUDA tensor of shape (nz, ny, nx) (or any shape with nx*ny*nz elements),
+passed by ``data_ptr()``; ``stream`` defaults to ``torch.cuda.current_stream()``.
+
+There is no CPU fallback: if ``libpz_b200.so`` is missing, or no CUDA device is present, the
+calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpz_b200.so")
+
+PZ_OK, PZ_EINVAL, PZ_EUNSUPPORTED, PZ_ENOMEM, PZ_ECUDA, PZ_ENOTSETUP = range(6)
+PZ_BC_PERIODIC_XY_NEUMANN_P_DIRICHLET_U = 0
+PZ_STAGE_FFT_X_FWD, PZ_STAGE_FFT_Y_FWD, PZ_STAGE_Z_SOLVE, PZ_STAGE_FFT_Y_INV, PZ_STAGE_FFT_X_INV = range(5)
+
+# every symbol include/pz.h declares: (name, restype, argtypes)
+_vp, _i, _d = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+_dp = ctypes.POINTER(ctypes.c_double)
+SIGNATURES = {
+    "poisson_plan_create": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _d, _d, _dp, _dp, _i]),
+    "poisson_solve": (_i, [_vp, _vp, _vp]),
+    "helmholtz_z_setup": (_i, [_vp, _d]),
+    "helmholtz_z_solve": (_i, [_vp, _vp, _vp]),
+    "helmholtz_z_solve_n": (_i, [_vp, ctypes.POINTER(_vp), _i, _vp]),
+    "poisson_solve_host": (_i, [_vp, _vp, _vp]),
+    "helmholtz_z_solve_host": (_i, [_vp, _vp, _vp]),
+    "poisson_plan_destroy": (_i, [_vp]),
+    "pz_last_error": (ctypes.c_char_p, []),
+    "pz_poisson_stage": (_i, [_vp, _vp, _i, _vp]),
+    "pz_set_option": (_i, [_vp, ctypes.c_char_p, _i]),
+    "pz_get_option": (_i, [_vp, ctypes.c_char_p, ctypes.POINTER(_i)]),
+    "pz_launch_count": (ctypes.c_longlong, []),
+    "pz_version": (_i, []),
+}
+
+_lib = None
+
+
+class PzError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"pz status {status}: {message}")
+        self.status = status
+
+
+def lib() -> ctypes.CDLL:
+    """Load libpz_b200.so (built by ``python -m paper_2502_06296_b200.build``).  Fails loudly."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} not found: build the CUDA extension with "
+                "`python -m paper_2502_06296_b200.build` (there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def _check(status: int):
+    if status != PZ_OK:
+        raise PzError(status, lib().pz_last_error().decode())
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        import torch
+
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def _dev_ptr(t, n: int) -> int:
+    import torch
+
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError("field must be a contiguous float64 CUDA tensor")
+    if t.numel() != n:
+        raise ValueError(f"field has {t.numel()} elements, plan expects {n}")
+    return t.data_ptr()
+
+
+def _host_ptr(t, n: int) -> int:
+    import torch
+
+    if isinstance(t, np.ndarray):
+        if t.dtype != np.float64 or not t.flags["C_CONTIGUOUS"] or t.size != n:
+            raise TypeError("host field must be a C-contiguous float64 array of nx*ny*nz elements")
+        return t.ctypes.data
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError("host field must be a contiguous float64 CPU tensor or numpy array")
+    if t.numel() != n:
+        raise ValueError(f"field has {t.numel()} elements, plan expects {n}")
+    return t.data_ptr()
+
+
+class Plan:
+    """Owner of a ``pz_plan*``; destroyed with :func:`poisson_plan_destroy` or on garbage collection."""
+
+    def __init__(self, handle: int, nx: int, ny: int, nz: int):
+        self.handle, self.nx, self.ny, self.nz = handle, nx, ny, nz
+        self.n = nx * ny * nz
+
+    def __del__(self):
+        try:
+            poisson_plan_destroy(self)
+        except Exception:
+            pass
+
+
+def poisson_plan_create(nx: int, ny: int, nz: int, lx: float, ly: float, zc, zf,
+                        bc: int = PZ_BC_PERIODIC_XY_NEUMANN_P_DIRICHLET_U) -> Plan:
+    zc = np.ascontiguousarray(zc, dtype=np.float64)
+    zf = np.ascontiguousarray(zf, dtype=np.float64)
+    if zc.size != nz or zf.size != nz + 1:
+        raise ValueError("zc must have nz entries and zf nz+1")
+    out = _vp()
+    _check(lib().poisson_plan_create(ctypes.byref(out), nx, ny, nz, float(lx), float(ly),
+                                     zc.ctypes.data_as(_dp), zf.ctypes.data_as(_dp), bc))
+    return Plan(out.value, nx, ny, nz)
+
+
+def poisson_plan_destroy(plan: Plan) -> None:
+    if plan is not None and plan.handle:
+        h, plan.handle = plan.handle, 0
+        _check(lib().poisson_plan_destroy(h))
+
+
+def poisson_solve(plan: Plan, p, stream=None) -> None:
+    _check(lib().poisson_solve(plan.handle, _dev_ptr(p, plan.n), _stream_ptr(stream)))
+
+
+def helmholtz_z_setup(plan: Plan, a: float) -> None:
+    _check(lib().helmholtz_z_setup(plan.handle, float(a)))
+
+
+def helmholtz_z_solve(plan: Plan, u, stream=None) -> None:
+    _check(lib().helmholtz_z_solve(plan.handle, _dev_ptr(u, plan.n), _stream_ptr(stream)))
+
+
+def helmholtz_z_solve_n(plan: Plan, fields, stream=None) -> None:
+    ptrs = (_vp * len(fields))(*[_dev_ptr(u, plan.n) for u in fields])
+    _check(lib().helmholtz_z_solve_n(plan.handle, ptrs, len(fields), _stream_ptr(stream)))
+
+
+def poisson_solve_host(plan: Plan, p_host, stream=None) -> None:
+    _check(lib().poisson_solve_host(plan.handle, _host_ptr(p_host, plan.n), _stream_ptr(stream)))
+
+
+def helmholtz_z_solve_host(plan: Plan, u_host, stream=None) -> None:
+    _check(lib().helmholtz_z_solve_host(plan.handle, _host_ptr(u_host, plan.n), _stream_ptr(stream)))
+
+
+def pz_poisson_stage(plan: Plan, p, stage: int, stream=None) -> None:
+    _check(lib().pz_poisson_stage(plan.handle, _dev_ptr(p, plan.n), int(stage), _stream_ptr(stream)))
+
+
+def pz_set_option(plan: Plan, key: str, value: int) -> None:
+    _check(lib().pz_set_option(plan.handle, key.encode(), int(value)))
+
+
+def pz_get_option(plan: Plan, key: str) -> int:
+    v = _i()
+    _check(lib().pz_get_option(plan.handle, key.encode(), ctypes.byref(v)))
+    return v.value
+
+
+def pz_launch_count() -> int:
+    return int(lib().pz_launch_count())
+
+
+def pz_version() -> int:
+    return int(lib().pz_version())
+
+
+def pz_last_error() -> str:
+    return lib().pz_last_error().decode()

@@ -1,0 +1,383 @@
+// pz_api.cu -- the C ABI of include/pz.h: plan / pre-processing (step a0), solve orchestration,
+// options, error reporting.  Host code only; kernels live in the other translation units.
+#include "pz_internal.h"
+
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+namespace pz {
+
+static thread_local char g_err[512] = "";
+static std::atomic<long long> g_launches{0};
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    set_error("CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
+    return PZ_ECUDA;
+}
+
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+namespace {
+
+bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+typedef long double ld;
+const ld kPi = 3.141592653589793238462643383279502884L;
+
+// lambda_q = -4 sin^2(pi q / n) / delta^2, folded to q <= n/2 (R1, R6)
+double lambda(int q, int n, double length)
+{
+    if (q > n - q) q = n - q;
+    const ld delta = (ld)length / (ld)n;
+    const ld s = sinl(kPi * (ld)q / (ld)n);
+    return (double)(-(ld)4 * s * s / (delta * delta));
+}
+
+// exp(-2 pi i k / n) with the argument folded into the first octant
+void twiddle(int k, int n, double *re, double *im)
+{
+    // angle = 2 pi k / n, k in [0, n); use symmetries about multiples of pi/4 (n is a power of two >= 8)
+    const int e = n / 8;
+    int oct = (e > 0) ? k / e : 0;
+    int rem = (e > 0) ? k % e : 0;
+    ld c, s;
+    if (e == 0) {
+        c = cosl(2 * kPi * (ld)k / (ld)n);
+        s = sinl(2 * kPi * (ld)k / (ld)n);
+    } else {
+        // theta = (oct*e + rem) * 2 pi / n = oct*pi/4 + rem*2pi/n
+        ld base_c, base_s;
+        const bool odd = oct & 1;
+        const ld th = odd ? (ld)(e - rem) * 2 * kPi / (ld)n : (ld)rem * 2 * kPi / (ld)n; // in [0, pi/4]
+        const ld ct = cosl(th), st = sinl(th);
+        // angle within the quadrant: odd octant -> pi/2 - th
+        if (odd) { base_c = st; base_s = ct; } else { base_c = ct; base_s = st; }
+        switch (oct / 2) { // quadrant rotation
+        case 0: c = base_c; s = base_s; break;
+        case 1: c = -base_s; s = base_c; break;
+        case 2: c = -base_c; s = -base_s; break;
+        default: c = base_s; s = -base_c; break;
+        }
+    }
+    *re = (double)c;
+    *im = (double)(-s);
+}
+
+int ensure_zwork(pz_plan *pl)
+{
+    if (pl->d_zwork) return PZ_OK;
+    cudaError_t e = cudaMalloc(&pl->d_zwork, pl->n * sizeof(double));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        set_error("z-solve variant 0 workspace (%zu bytes): %s", pl->n * sizeof(double), cudaGetErrorString(e));
+        return PZ_ENOMEM;
+    }
+    return PZ_OK;
+}
+
+int slab_planes(const pz_plan *pl)
+{
+    if (pl->opt.slab_planes > 0) return pl->opt.slab_planes < pl->nz ? pl->opt.slab_planes : pl->nz;
+    // auto: keep a slab of planes (x- then y-transformed back to back) inside the 126 MB L2
+    const size_t plane_bytes = (size_t)pl->nx * pl->ny * sizeof(double);
+    size_t sp = (32u << 20) / plane_bytes;
+    if (sp < 1) sp = 1;
+    if (sp > (size_t)pl->nz) sp = pl->nz;
+    return (int)sp;
+}
+
+int forward_xy(pz_plan *pl, double *p, cudaStream_t st)
+{
+    const int sp = slab_planes(pl);
+    for (int k0 = 0; k0 < pl->nz; k0 += sp) {
+        const int nk = (k0 + sp <= pl->nz) ? sp : pl->nz - k0;
+        int rc = launch_fft_x(pl, p, k0, nk, false, st);
+        if (rc) return rc;
+        rc = launch_fft_y(pl, p, k0, nk, false, st);
+        if (rc) return rc;
+        rc = launch_pair0(pl, p, k0, nk, false, st);
+        if (rc) return rc;
+    }
+    return PZ_OK;
+}
+
+int inverse_xy(pz_plan *pl, double *p, cudaStream_t st)
+{
+    const int sp = slab_planes(pl);
+    for (int k0 = 0; k0 < pl->nz; k0 += sp) {
+        const int nk = (k0 + sp <= pl->nz) ? sp : pl->nz - k0;
+        int rc = launch_pair0(pl, p, k0, nk, true, st);
+        if (rc) return rc;
+        rc = launch_fft_y(pl, p, k0, nk, true, st);
+        if (rc) return rc;
+        rc = launch_fft_x(pl, p, k0, nk, true, st);
+        if (rc) return rc;
+    }
+    return PZ_OK;
+}
+
+} // namespace
+} // namespace pz
+
+using namespace pz;
+
+extern "C" {
+
+const char *pz_last_error(void) { return g_err; }
+long long pz_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+int pz_version(void) { return 100; }
+
+int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double ly, const double *zc,
+                        const double *zf, int bc)
+{
+    g_err[0] = 0;
+    if (!out) { set_error("poisson_plan_create: out is NULL"); return PZ_EINVAL; }
+    *out = nullptr;
+    if (!zc || !zf) { set_error("poisson_plan_create: zc/zf is NULL"); return PZ_EINVAL; }
+    if (nx <= 0 || ny <= 0 || nz <= 0) { set_error("poisson_plan_create: non-positive size %d x %d x %d", nx, ny, nz); return PZ_EINVAL; }
+    if (!(lx > 0.0) || !(ly > 0.0) || !std::isfinite(lx) || !std::isfinite(ly)) { set_error("poisson_plan_create: lx, ly must be positive and finite"); return PZ_EINVAL; }
+    if (bc != PZ_BC_PERIODIC_XY_NEUMANN_P_DIRICHLET_U) { set_error("poisson_plan_create: unsupported bc %d", bc); return PZ_EUNSUPPORTED; }
+    if (!is_pow2(nx) || !is_pow2(ny) || nx < 8 || ny < 8 || nx > 4096 || ny > 4096) {
+        set_error("poisson_plan_create: nx, ny must be powers of two in [8, 4096] (got %d, %d)", nx, ny);
+        return PZ_EUNSUPPORTED;
+    }
+    if (nz < 4) { set_error("poisson_plan_create: nz must be >= 4 (got %d)", nz); return PZ_EUNSUPPORTED; }
+    for (int k = 0; k < nz; ++k) {
+        if (!(zf[k + 1] > zf[k]) || !std::isfinite(zf[k]) || !std::isfinite(zf[k + 1])) { set_error("poisson_plan_create: zf not strictly increasing at k = %d", k); return PZ_EINVAL; }
+        if (!(zc[k] > zf[k] && zc[k] < zf[k + 1])) { set_error("poisson_plan_create: zc[%d] outside its cell", k); return PZ_EINVAL; }
+    }
+
+    int dev_count = 0;
+    cudaError_t ce = cudaGetDeviceCount(&dev_count);
+    if (ce != cudaSuccess || dev_count == 0) {
+        cudaGetLastError();
+        set_error("poisson_plan_create: no CUDA device (%s); there is no CPU fallback", cudaGetErrorString(ce));
+        return PZ_ECUDA;
+    }
+
+    pz_plan *pl = new (std::nothrow) pz_plan();
+    if (!pl) { set_error("poisson_plan_create: out of host memory"); return PZ_ENOMEM; }
+    pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->lx = lx; pl->ly = ly;
+    pl->n = (size_t)nx * ny * nz;
+    int rc = PZ_OK;
+    auto fail = [&](int code) { poisson_plan_destroy(pl); return code; };
+    if (cudaGetDevice(&pl->device) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaGetDevice"));
+    cudaDeviceGetAttribute(&pl->num_sms, cudaDevAttrMultiProcessorCount, pl->device);
+
+    // z-metric tables in double, exactly as the definition states them (one division each)
+    pl->zc.assign(zc, zc + nz);
+    pl->zf.assign(zf, zf + nz + 1);
+    pl->dzf.resize(nz); pl->dzc.resize(nz > 1 ? nz - 1 : 0); pl->A.resize(nz); pl->C.resize(nz);
+    double lz = 0.0;
+    for (int k = 0; k < nz; ++k) { pl->dzf[k] = zf[k + 1] - zf[k]; lz += pl->dzf[k]; }
+    for (int k = 0; k + 1 < nz; ++k) pl->dzc[k] = zc[k + 1] - zc[k];
+    for (int k = 0; k < nz; ++k) {
+        pl->A[k] = (k >= 1) ? 1.0 / (pl->dzf[k] * pl->dzc[k - 1]) : 0.0;
+        pl->C[k] = (k + 1 < nz) ? 1.0 / (pl->dzf[k] * pl->dzc[k]) : 0.0;
+    }
+    pl->inv_lz = 1.0 / lz;
+
+    // one device allocation for all tables
+    const size_t ndbl = 3 * (size_t)nz + (size_t)nx + 2 * (size_t)ny + 2 * (size_t)nx + 2 * (size_t)ny + 8;
+    std::vector<double> host(ndbl, 0.0);
+    size_t off = 0;
+    auto take = [&](size_t cnt) { size_t o = off; off += (cnt + 1) & ~(size_t)1; return o; }; // keep 16-B alignment
+    const size_t oA = take(nz), oC = take(nz), oD = take(nz), oLx = take(nx), oLyn = take(ny), oLyp = take(ny);
+    const size_t oTx = take(2 * (size_t)nx), oTy = take(2 * (size_t)ny);
+    for (int k = 0; k < nz; ++k) { host[oA + k] = pl->A[k]; host[oC + k] = pl->C[k]; host[oD + k] = pl->dzf[k]; }
+    // modified wavenumbers re-ordered for the packed layout
+    for (int i = 0; i < nx; ++i) host[oLx + i] = lambda(i == 0 ? 0 : (i == 1 ? nx / 2 : i / 2), nx, lx);
+    for (int j = 0; j < ny; ++j) {
+        host[oLyn + j] = lambda(j, ny, ly);
+        host[oLyp + j] = lambda(j == 0 ? 0 : (j == 1 ? ny / 2 : j / 2), ny, ly);
+    }
+    for (int k = 0; k < nx; ++k) twiddle(k, nx, &host[oTx + 2 * k], &host[oTx + 2 * k + 1]);
+    for (int k = 0; k < ny; ++k) twiddle(k, ny, &host[oTy + 2 * k], &host[oTy + 2 * k + 1]);
+
+    ce = cudaMalloc(&pl->tables, off * sizeof(double));
+    if (ce != cudaSuccess) { cudaGetLastError(); set_error("plan tables: %s", cudaGetErrorString(ce)); return fail(PZ_ENOMEM); }
+    ce = cudaMemcpy(pl->tables, host.data(), off * sizeof(double), cudaMemcpyHostToDevice);
+    if (ce != cudaSuccess) return fail(cuda_fail(ce, "cudaMemcpy(tables)"));
+    pl->d_A = pl->tables + oA; pl->d_C = pl->tables + oC; pl->d_dzf = pl->tables + oD;
+    pl->d_lamx = pl->tables + oLx; pl->d_lamy_nat = pl->tables + oLyn; pl->d_lamy_pk = pl->tables + oLyp;
+    pl->d_twx = reinterpret_cast<double2 *>(pl->tables + oTx);
+    pl->d_twy = reinterpret_cast<double2 *>(pl->tables + oTy);
+
+    ce = cudaStreamCreateWithFlags(&pl->upload_stream, cudaStreamNonBlocking);
+    if (ce != cudaSuccess) return fail(cuda_fail(ce, "cudaStreamCreate"));
+    for (int b = 0; b < 2; ++b) {
+        if ((ce = cudaEventCreateWithFlags(&pl->helm[b].uploaded, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
+        if ((ce = cudaEventCreateWithFlags(&pl->helm[b].last_use, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
+    }
+    pl->opt.zsolve_variant = (nz <= 1024) ? 1 : 0;
+    if (pl->opt.zsolve_variant == 0 && (rc = ensure_zwork(pl)) != PZ_OK) return fail(rc);
+    *out = pl;
+    return PZ_OK;
+}
+
+int poisson_plan_destroy(pz_plan *pl)
+{
+    if (!pl) return PZ_OK;
+    cudaDeviceSynchronize();
+    if (pl->tables) cudaFree(pl->tables);
+    if (pl->d_zwork) cudaFree(pl->d_zwork);
+    if (pl->d_host_stage) cudaFree(pl->d_host_stage);
+    for (int b = 0; b < 2; ++b) {
+        if (pl->helm[b].dev) cudaFree(pl->helm[b].dev);
+        if (pl->helm[b].uploaded) cudaEventDestroy(pl->helm[b].uploaded);
+        if (pl->helm[b].last_use) cudaEventDestroy(pl->helm[b].last_use);
+    }
+    if (pl->helm_host) cudaFreeHost(pl->helm_host);
+    if (pl->upload_stream) cudaStreamDestroy(pl->upload_stream);
+    cudaGetLastError();
+    delete pl;
+    return PZ_OK;
+}
+
+int pz_poisson_stage(pz_plan *pl, double *p, int stage, void *stream)
+{
+    if (!pl || !p) { set_error("pz_poisson_stage: NULL argument"); return PZ_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    switch (stage) {
+    case PZ_STAGE_FFT_X_FWD: return launch_fft_x(pl, p, 0, pl->nz, false, st);
+    case PZ_STAGE_FFT_Y_FWD:
+        if ((rc = launch_fft_y(pl, p, 0, pl->nz, false, st)) != PZ_OK) return rc;
+        return launch_pair0(pl, p, 0, pl->nz, false, st);
+    case PZ_STAGE_Z_SOLVE: return launch_zsolve(pl, p, st);
+    case PZ_STAGE_FFT_Y_INV:
+        if ((rc = launch_pair0(pl, p, 0, pl->nz, true, st)) != PZ_OK) return rc;
+        return launch_fft_y(pl, p, 0, pl->nz, true, st);
+    case PZ_STAGE_FFT_X_INV: return launch_fft_x(pl, p, 0, pl->nz, true, st);
+    default: set_error("pz_poisson_stage: unknown stage %d", stage); return PZ_EINVAL;
+    }
+}
+
+int poisson_solve(pz_plan *pl, double *p, void *stream)
+{
+    if (!pl || !p) { set_error("poisson_solve: NULL argument"); return PZ_EINVAL; }
+    if (((uintptr_t)p & 15) != 0) { set_error("poisson_solve: p must be 16-byte aligned"); return PZ_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if ((rc = forward_xy(pl, p, st)) != PZ_OK) return rc;
+    if ((rc = launch_zsolve(pl, p, st)) != PZ_OK) return rc;
+    return inverse_xy(pl, p, st);
+}
+
+int helmholtz_z_setup(pz_plan *pl, double a)
+{
+    if (!pl) { set_error("helmholtz_z_setup: plan is NULL"); return PZ_EINVAL; }
+    if (!(a >= 0.0) || !std::isfinite(a)) { set_error("helmholtz_z_setup: a must be finite and >= 0"); return PZ_EINVAL; }
+    return helmholtz_build_tables(pl, a);
+}
+
+int helmholtz_z_solve(pz_plan *pl, double *u, void *stream)
+{
+    if (!pl || !u) { set_error("helmholtz_z_solve: NULL argument"); return PZ_EINVAL; }
+    if (pl->helm_cur < 0) { set_error("helmholtz_z_solve: call helmholtz_z_setup first"); return PZ_ENOTSETUP; }
+    return launch_helmholtz(pl, u, (cudaStream_t)stream);
+}
+
+int helmholtz_z_solve_n(pz_plan *pl, double *const *u, int n, void *stream)
+{
+    if (!pl || !u || n < 0) { set_error("helmholtz_z_solve_n: bad argument"); return PZ_EINVAL; }
+    for (int c = 0; c < n; ++c) {
+        const int rc = helmholtz_z_solve(pl, u[c], stream);
+        if (rc != PZ_OK) return rc;
+    }
+    return PZ_OK;
+}
+
+static int ensure_host_stage(pz_plan *pl)
+{
+    if (pl->d_host_stage) return PZ_OK;
+    cudaError_t e = cudaMalloc(&pl->d_host_stage, pl->n * sizeof(double));
+    if (e != cudaSuccess) { cudaGetLastError(); set_error("host staging field: %s", cudaGetErrorString(e)); return PZ_ENOMEM; }
+    return PZ_OK;
+}
+
+int poisson_solve_host(pz_plan *pl, double *p_host, void *stream)
+{
+    if (!pl || !p_host) { set_error("poisson_solve_host: NULL argument"); return PZ_EINVAL; }
+    int rc = ensure_host_stage(pl);
+    if (rc != PZ_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    PZ_CUDA(cudaMemcpyAsync(pl->d_host_stage, p_host, pl->n * sizeof(double), cudaMemcpyHostToDevice, st));
+    if ((rc = poisson_solve(pl, pl->d_host_stage, stream)) != PZ_OK) return rc;
+    PZ_CUDA(cudaMemcpyAsync(p_host, pl->d_host_stage, pl->n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    return PZ_OK;
+}
+
+int helmholtz_z_solve_host(pz_plan *pl, double *u_host, void *stream)
+{
+    if (!pl || !u_host) { set_error("helmholtz_z_solve_host: NULL argument"); return PZ_EINVAL; }
+    if (pl->helm_cur < 0) { set_error("helmholtz_z_solve_host: call helmholtz_z_setup first"); return PZ_ENOTSETUP; }
+    int rc = ensure_host_stage(pl);
+    if (rc != PZ_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    PZ_CUDA(cudaMemcpyAsync(pl->d_host_stage, u_host, pl->n * sizeof(double), cudaMemcpyHostToDevice, st));
+    if ((rc = helmholtz_z_solve(pl, pl->d_host_stage, stream)) != PZ_OK) return rc;
+    PZ_CUDA(cudaMemcpyAsync(u_host, pl->d_host_stage, pl->n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    return PZ_OK;
+}
+
+static int *option_slot(pz_plan *pl, const char *key)
+{
+    if (!std::strcmp(key, "zsolve_variant")) return &pl->opt.zsolve_variant;
+    if (!std::strcmp(key, "slab_planes")) return &pl->opt.slab_planes;
+    if (!std::strcmp(key, "helm_tx")) return &pl->opt.helm_tx;
+    if (!std::strcmp(key, "helm_m")) return &pl->opt.helm_m;
+    if (!std::strcmp(key, "fft_y_tc")) return &pl->opt.fft_y_tc;
+    if (!std::strcmp(key, "fft_x_lpb")) return &pl->opt.fft_x_lpb;
+    return nullptr;
+}
+
+int pz_set_option(pz_plan *pl, const char *key, int value)
+{
+    if (!pl || !key) { set_error("pz_set_option: NULL argument"); return PZ_EINVAL; }
+    int *slot = option_slot(pl, key);
+    if (!slot) { set_error("pz_set_option: unknown key '%s'", key); return PZ_EUNSUPPORTED; }
+    if (slot == &pl->opt.zsolve_variant) {
+        if (value != 0 && value != 1) { set_error("zsolve_variant must be 0 or 1"); return PZ_EUNSUPPORTED; }
+        if (value == 1 && pl->nz > 1024) { set_error("zsolve_variant 1 supports nz <= 1024"); return PZ_EUNSUPPORTED; }
+        if (value == 0) { const int rc = ensure_zwork(pl); if (rc != PZ_OK) return rc; }
+    } else if (value < 0) {
+        set_error("pz_set_option: '%s' must be >= 0", key);
+        return PZ_EUNSUPPORTED;
+    }
+    *slot = value;
+    if ((slot == &pl->opt.helm_tx || slot == &pl->opt.helm_m) && pl->helm_cur >= 0)
+        return helmholtz_build_tables(pl, pl->helm_a); // geometry changed: rebuild the tables
+    return PZ_OK;
+}
+
+int pz_get_option(const pz_plan *pl, const char *key, int *value)
+{
+    if (!pl || !key || !value) { set_error("pz_get_option: NULL argument"); return PZ_EINVAL; }
+    int *slot = option_slot(const_cast<pz_plan *>(pl), key);
+    if (!slot) {
+        if (!std::strcmp(key, "helm_m_actual")) { *value = pl->helm_m; return PZ_OK; }
+        if (!std::strcmp(key, "helm_tx_actual")) { *value = pl->helm_tx; return PZ_OK; }
+        if (!std::strcmp(key, "helm_p_actual")) { *value = pl->helm_P; return PZ_OK; }
+        if (!std::strcmp(key, "slab_planes_actual")) { *value = slab_planes(pl); return PZ_OK; }
+        set_error("pz_get_option: unknown key '%s'", key);
+        return PZ_EUNSUPPORTED;
+    }
+    *value = *slot;
+    return PZ_OK;
+}
+
+} // extern "C"

@@ -1,0 +1,191 @@
+// pz_fft_y.cu -- steps a2 / a4 of the hot path: FFT along y (PAPER.md:126 step 3, :130 step 7).
+//
+// In the paper the y transform sits behind an x->y pencil transpose, which takes 81.7-90.5 % of
+// the Poisson time at scale.  On one GPU the transpose is removed: a CTA
+// transforms TC neighbouring columns at once, reading and writing rows of TC*16 contiguous
+// bytes with stride nx, so every access is coalesced and the field is never re-laid-out.
+//
+// After the packed x transform, the two reals at (2q, 2q+1) of a line are Re/Im of x-mode q, so
+// along y the data is already a COMPLEX sequence per q: one complex-to-complex FFT of length ny
+// per pair gives the 2-D spectrum F(q, r), r = 0..ny-1, in the same storage.  Pair q = 0 holds
+// two real sequences (x-modes 0 and nx/2) instead; a tiny kernel separates their spectra into
+// the packed layout along y (and re-merges them before the inverse), DESIGN.md "Spectral layout".
+#include "pz_fft.cuh"
+#include "pz_internal.h"
+
+namespace pz {
+
+namespace {
+
+template <int TC>
+struct XchgY {
+    double2 *buf; // [pos][TC]
+    int c;
+    __device__ __forceinline__ void put(int pos, double2 v) const { buf[pos * TC + c] = v; }
+    __device__ __forceinline__ double2 get(int pos) const { return buf[pos * TC + c]; }
+    __device__ __forceinline__ void sync() const { __syncthreads(); }
+};
+
+template <int L, int TC, bool INV>
+__global__ void __launch_bounds__(FftPlan<L>::T *TC)
+    fft_y_kernel(double *__restrict__ p, const double2 *__restrict__ tw, int nx)
+{
+    using P = FftPlan<L>;
+    constexpr int E = P::E, T = P::T;
+    extern __shared__ double2 smem_y[];
+
+    const int c = threadIdx.x % TC, tid = threadIdx.x / TC;
+    const size_t pair = (size_t)blockIdx.x * TC + c;
+    double *base = p + (size_t)blockIdx.y * L * nx + 2 * pair;
+    XchgY<TC> xc{smem_y, c};
+
+    double2 v[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const double2 t = *reinterpret_cast<const double2 *>(base + (size_t)(tid + e * T) * nx);
+        v[e] = INV ? cconj(t) : t;
+    }
+    fft_line<L, 1>(v, tid, tw, xc);
+#pragma unroll
+    for (int e = 0; e < E; ++e)
+        *reinterpret_cast<double2 *>(base + (size_t)(tid + e * T) * nx) = INV ? cconj(v[e]) : v[e];
+}
+
+// Pair q = 0: W_r = A_r + i B_r with A, B the spectra of the real sequences in columns 0 and 1.
+// Forward: rows (2r, 2r+1) <- (Re A_r, Re B_r), (Im A_r, Im B_r); rows 0, 1 <- r = 0, ny/2.
+// Inverse: the reverse.  One CTA per plane; the whole column pair is staged in shared memory.
+template <bool INV>
+__global__ void pair0_kernel(double *__restrict__ p, int nx, int ny)
+{
+    extern __shared__ double2 smem_p0[];
+    double *base = p + (size_t)blockIdx.x * ny * nx;
+    for (int r = threadIdx.x; r < ny; r += blockDim.x)
+        smem_p0[r] = *reinterpret_cast<const double2 *>(base + (size_t)r * nx);
+    __syncthreads();
+    const int h = ny / 2;
+    for (int r = threadIdx.x; r <= h; r += blockDim.x) {
+        if constexpr (!INV) {
+            double2 lo, hi;
+            if (r == 0 || r == h) {
+                const double2 w = smem_p0[r];
+                *reinterpret_cast<double2 *>(base + (size_t)(r == 0 ? 0 : 1) * nx) = w;
+                continue;
+            }
+            const double2 w = smem_p0[r], wm = cconj(smem_p0[ny - r]);
+            const double2 a = make_double2(0.5 * (w.x + wm.x), 0.5 * (w.y + wm.y));
+            const double2 d = csub(w, wm);
+            const double2 b = make_double2(0.5 * d.y, -0.5 * d.x);
+            lo = make_double2(a.x, b.x);
+            hi = make_double2(a.y, b.y);
+            *reinterpret_cast<double2 *>(base + (size_t)(2 * r) * nx) = lo;
+            *reinterpret_cast<double2 *>(base + (size_t)(2 * r + 1) * nx) = hi;
+        } else {
+            if (r == 0 || r == h) {
+                const double2 w = smem_p0[r == 0 ? 0 : 1];
+                *reinterpret_cast<double2 *>(base + (size_t)r * nx) = w;
+                continue;
+            }
+            const double2 lo = smem_p0[2 * r], hi = smem_p0[2 * r + 1];
+            const double2 a = make_double2(lo.x, hi.x), b = make_double2(lo.y, hi.y);
+            // W_r = A + iB,  W_{ny-r} = conj(A) + i conj(B)
+            *reinterpret_cast<double2 *>(base + (size_t)r * nx) = make_double2(a.x - b.y, a.y + b.x);
+            *reinterpret_cast<double2 *>(base + (size_t)(ny - r) * nx) = make_double2(a.x + b.y, b.x - a.y);
+        }
+    }
+}
+
+template <int L, int TC, bool INV>
+int launch_ltc(const pz_plan *pl, double *p, int nk, cudaStream_t st)
+{
+    using P = FftPlan<L>;
+    constexpr int threads = P::T * TC;
+    constexpr size_t smem = (P::R2 > 1) ? (size_t)L * TC * sizeof(double2) : 0;
+    static bool attr_done = false;
+    if (smem > 48 * 1024 && !attr_done) {
+        PZ_CUDA(cudaFuncSetAttribute(fft_y_kernel<L, TC, INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    dim3 grid((unsigned)(pl->nx / 2 / TC), (unsigned)nk);
+    fft_y_kernel<L, TC, INV><<<grid, threads, smem, st>>>(p, pl->d_twy, pl->nx);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+// TC (complex pairs per CTA): 128-byte rows (TC = 8) while the exchange tile stays <= 64 KB,
+// narrower for long lines; never more pairs than the field has.  A (L, TC) combination is
+// instantiated only if its CTA has at most 512 threads and its tile at most 128 KB.
+template <int L, int TC>
+constexpr bool tc_valid() { return FftPlan<L>::T * TC <= 512 && (size_t)L * TC * sizeof(double2) <= 128 * 1024; }
+
+template <int L, int TC, bool INV>
+int try_ltc(const pz_plan *pl, double *p, int nk, cudaStream_t st)
+{
+    if constexpr (tc_valid<L, TC>()) {
+        return launch_ltc<L, TC, INV>(pl, p, nk, st);
+    } else {
+        set_error("fft_y: no kernel for ny = %d with %d pairs per CTA", L, TC);
+        return PZ_EUNSUPPORTED;
+    }
+}
+
+template <int L, bool INV>
+int launch_l(const pz_plan *pl, double *p, int nk, cudaStream_t st)
+{
+    const int npairs = pl->nx / 2;
+    int tc = pl->opt.fft_y_tc;
+    if (tc == 0) tc = (L <= 512) ? 8 : 4;
+    if (tc > npairs) tc = npairs;
+    if (tc >= 16 && tc_valid<L, 16>()) return try_ltc<L, 16, INV>(pl, p, nk, st);
+    if (tc >= 8 && tc_valid<L, 8>()) return try_ltc<L, 8, INV>(pl, p, nk, st);
+    if (tc >= 4 && tc_valid<L, 4>()) return try_ltc<L, 4, INV>(pl, p, nk, st);
+    return try_ltc<L, 2, INV>(pl, p, nk, st);
+}
+
+template <bool INV>
+int dispatch(const pz_plan *pl, double *p, int nk, cudaStream_t st)
+{
+    switch (pl->ny) {
+    case 8: return launch_l<8, INV>(pl, p, nk, st);
+    case 16: return launch_l<16, INV>(pl, p, nk, st);
+    case 32: return launch_l<32, INV>(pl, p, nk, st);
+    case 64: return launch_l<64, INV>(pl, p, nk, st);
+    case 128: return launch_l<128, INV>(pl, p, nk, st);
+    case 256: return launch_l<256, INV>(pl, p, nk, st);
+    case 512: return launch_l<512, INV>(pl, p, nk, st);
+    case 1024: return launch_l<1024, INV>(pl, p, nk, st);
+    case 2048: return launch_l<2048, INV>(pl, p, nk, st);
+    case 4096: return launch_l<4096, INV>(pl, p, nk, st);
+    default: set_error("fft_y: unsupported ny = %d", pl->ny); return PZ_EUNSUPPORTED;
+    }
+}
+
+} // namespace
+
+int launch_fft_y(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st)
+{
+    double *base = p + (size_t)k0 * pl->nx * pl->ny;
+    return inverse ? dispatch<true>(pl, base, nk, st) : dispatch<false>(pl, base, nk, st);
+}
+
+int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st)
+{
+    double *base = p + (size_t)k0 * pl->nx * pl->ny;
+    const size_t smem = (size_t)pl->ny * sizeof(double2);
+    const int threads = pl->ny / 2 >= 256 ? 256 : (pl->ny / 2 < 32 ? 32 : pl->ny / 2);
+    static bool attr_done = false;
+    if (smem > 48 * 1024 && !attr_done) {
+        PZ_CUDA(cudaFuncSetAttribute(pair0_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
+        PZ_CUDA(cudaFuncSetAttribute(pair0_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
+        attr_done = true;
+    }
+    if (inverse)
+        pair0_kernel<true><<<(unsigned)nk, threads, smem, st>>>(base, pl->nx, pl->ny);
+    else
+        pair0_kernel<false><<<(unsigned)nk, threads, smem, st>>>(base, pl->nx, pl->ny);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+} // namespace pz

@@ -1,0 +1,268 @@
+// pz_helmholtz.cu -- step a6 of the hot path: wall-normal implicit diffusion (Eq. 11,
+// PAPER.md:74-78) with the paper's split of cyclic reduction into pre-processing and runtime
+// (Algorithm 2).
+//
+// Pre-processing (helmholtz_build_tables, host, long double -> double): the matrix I - a L_z is
+// the same for every (i,j) column ("identical for all (i,j) indexes"), so the
+// coefficient sub-arrays (a, b, c) of Algorithm 2 Step 1 are 1-D arrays in k.  The z direction is
+// cut into P sub-domains of m rows (padded with identity rows to P*m); for the boundary system of
+// size 2P the multipliers of every parallel-cyclic-reduction level are precomputed too, so the
+// runtime applies numbers and never divides ("store 1/b").
+//
+// Runtime (helmholtz_kernel): a CTA owns TX neighbouring columns (TX*8 contiguous bytes per row);
+// thread (column, sub-domain) loads its m rows straight into registers (one coalesced HBM read),
+// runs Step 2 (forward / backward sweeps touching only d), exchanges the two boundary rows through
+// shared memory, applies the precomputed PCR levels (Step 3), reconstructs (Step 4) and stores
+// (one HBM write): 16 bytes and about 5 FMAs per point.
+#include "pz_internal.h"
+
+#include <cmath>
+#include <cstring>
+
+namespace pz {
+
+namespace {
+
+// Table layout (doubles), nzp = P*m, n2 = 2P, LV = levels:
+//   [0, nzp)        fA_k  = A_i / b_{i-1}          (Step 2 forward, i = 2..m-1, else 0)
+//   [nzp, 2nzp)     bC_k  = C_i / b_{i+1}          (Step 2 backward, i = 0..m-3, else 0)
+//   [2nzp, 3nzp)    rb_k  = 1 / b_i                (Step 4)
+//   [3nzp, 4nzp)    ra_k  = a_i / b_i
+//   [4nzp, 5nzp)    rc_k  = c_i / b_i
+//   [5nzp, +LV*2*n2)   per level l and reduced row r: k1, k2 (d_r += k1 d_{r-h} + k2 d_{r+h})
+//   then n2         rbr_r = 1 / b_r after the last level
+template <int M>
+__global__ void __launch_bounds__(M >= 16 ? 512 : 1024)
+    helmholtz_kernel(double *__restrict__ u, const double *__restrict__ tab, size_t plane, int nz, int P,
+                     int levels, int tx)
+{
+    extern __shared__ double smem_h[]; // 2 buffers x (2P rows) x tx
+    const int c = threadIdx.x % tx, s = threadIdx.x / tx;
+    const size_t col = (size_t)blockIdx.x * tx + c;
+    const int nzp = P * M, n2 = 2 * P;
+    const int k0 = s * M;
+    const double *fA = tab + k0, *bC = tab + nzp + k0, *rb = tab + 2 * nzp + k0;
+    const double *ra = tab + 3 * nzp + k0, *rc = tab + 4 * nzp + k0;
+    const double *pcr = tab + 5 * (size_t)nzp;
+    double *up = u + col;
+
+    double d[M];
+#pragma unroll
+    for (int i = 0; i < M; ++i) d[i] = (k0 + i < nz) ? up[(size_t)(k0 + i) * plane] : 0.0;
+
+    // Step 2: runtime reduction, d only
+#pragma unroll
+    for (int i = 2; i < M; ++i) d[i] = fma(-__ldg(&fA[i]), d[i - 1], d[i]);
+#pragma unroll
+    for (int i = M - 3; i >= 0; --i) d[i] = fma(-__ldg(&bC[i]), d[i + 1], d[i]);
+
+    // Step 3: boundary system, rows (2s, 2s+1) = (first, last) row of sub-domain s
+    double *buf0 = smem_h, *buf1 = smem_h + (size_t)n2 * tx;
+    double x0 = d[0], x1 = d[M - 1];
+    buf0[(2 * s) * tx + c] = x0;
+    buf0[(2 * s + 1) * tx + c] = x1;
+    __syncthreads();
+    double *cur = buf0, *nxt = buf1;
+    int h = 1;
+    for (int l = 0; l < levels; ++l, h *= 2) {
+        const double *kk = pcr + (size_t)l * 2 * n2;
+        const int r0 = 2 * s, r1 = 2 * s + 1;
+        double y0 = x0, y1 = x1;
+        if (r0 - h >= 0) y0 = fma(__ldg(&kk[2 * r0]), cur[(r0 - h) * tx + c], y0);
+        if (r0 + h < n2) y0 = fma(__ldg(&kk[2 * r0 + 1]), cur[(r0 + h) * tx + c], y0);
+        if (r1 - h >= 0) y1 = fma(__ldg(&kk[2 * r1]), cur[(r1 - h) * tx + c], y1);
+        if (r1 + h < n2) y1 = fma(__ldg(&kk[2 * r1 + 1]), cur[(r1 + h) * tx + c], y1);
+        x0 = y0;
+        x1 = y1;
+        if (l + 1 < levels) {
+            nxt[r0 * tx + c] = x0;
+            nxt[r1 * tx + c] = x1;
+            __syncthreads();
+            double *t = cur; cur = nxt; nxt = t;
+        }
+    }
+    {
+        const double *rbr = pcr + (size_t)levels * 2 * n2;
+        x0 *= __ldg(&rbr[2 * s]);
+        x1 *= __ldg(&rbr[2 * s + 1]);
+    }
+
+    // Step 4: reconstruct in place and store
+    if (k0 < nz) up[(size_t)k0 * plane] = x0;
+#pragma unroll
+    for (int i = 1; i < M - 1; ++i) {
+        const double v = fma(-__ldg(&rc[i]), x1, fma(-__ldg(&ra[i]), x0, __ldg(&rb[i]) * d[i]));
+        if (k0 + i < nz) up[(size_t)(k0 + i) * plane] = v;
+    }
+    if (k0 + M - 1 < nz) up[(size_t)(k0 + M - 1) * plane] = x1;
+}
+
+int ilog2_ceil(int n)
+{
+    int l = 0;
+    while ((1 << l) < n) ++l;
+    return l;
+}
+
+} // namespace
+
+// Choose the sub-domain size m and count P for this nz (and the CTA width) -- launch geometry.
+static void helm_geometry(pz_plan *pl)
+{
+    int m = pl->opt.helm_m;
+    if (m != 4 && m != 8 && m != 16 && m != 32) m = (pl->nz <= 128) ? 4 : (pl->nz <= 256) ? 8 : (pl->nz <= 512 ? 16 : 32);
+    int P = (pl->nz + m - 1) / m;
+    int tx = pl->opt.helm_tx;
+    if (tx != 4 && tx != 8 && tx != 16 && tx != 32) tx = 16;
+    while (m < 32 && 4 * P > 1024) { m *= 2; P = (pl->nz + m - 1) / m; }
+    const int limit = (m >= 16) ? 512 : 1024; // __launch_bounds__ of helmholtz_kernel<m>
+    while (tx > 4 && tx * P > limit) tx /= 2;
+    pl->helm_m = m;
+    pl->helm_P = P;
+    pl->helm_tx = tx;
+    pl->helm_levels = ilog2_ceil(2 * P);
+}
+
+// Algorithm 2 Step 1 on the host, plus the precomputed PCR of the boundary system.
+int helmholtz_build_tables(pz_plan *pl, double a)
+{
+    typedef long double ld;
+    helm_geometry(pl);
+    const int nz = pl->nz, m = pl->helm_m, P = pl->helm_P, nzp = P * m, n2 = 2 * P, LV = pl->helm_levels;
+    if (pl->helm_tx * P > ((m >= 16) ? 512 : 1024)) {
+        set_error("helmholtz: nz = %d needs more than 1024 threads per CTA", nz);
+        return PZ_EUNSUPPORTED;
+    }
+    const size_t ndbl = 5 * (size_t)nzp + (size_t)LV * 2 * n2 + n2;
+    const size_t bytes = ndbl * sizeof(double);
+
+    // matrix of I - a L_z with Dirichlet walls, padded with identity rows
+    std::vector<ld> A(nzp, 0), B(nzp, 1), C(nzp, 0);
+    for (int k = 0; k < nz; ++k) {
+        ld W = 0;
+        if (k == 0) W += (ld)2 / ((ld)pl->dzf[0] * ((ld)2 * ((ld)pl->zc[0] - (ld)pl->zf[0])));
+        if (k == nz - 1) W += (ld)2 / ((ld)pl->dzf[nz - 1] * ((ld)2 * ((ld)pl->zf[nz] - (ld)pl->zc[nz - 1])));
+        A[k] = -(ld)a * (ld)pl->A[k];
+        C[k] = -(ld)a * (ld)pl->C[k];
+        B[k] = (ld)1 + (ld)a * ((ld)pl->A[k] + (ld)pl->C[k] + W);
+    }
+    std::vector<double> host(ndbl, 0.0);
+    double *fA = host.data(), *bC = fA + nzp, *rb = bC + nzp, *ra = rb + nzp, *rc = ra + nzp;
+    double *pcr = rc + nzp;
+    std::vector<ld> ra2(n2), rbd(n2), rc2(n2); // boundary system
+    std::vector<ld> ca(m), cb(m), cc(m);
+    for (int s = 0; s < P; ++s) {
+        const ld *As = &A[s * m], *Bs = &B[s * m], *Cs = &C[s * m];
+        // Algorithm 2, Step 1
+        for (int i = 0; i < m; ++i) ca[i] = cb[i] = cc[i] = 0;
+        ca[1] = As[1];
+        cb[1] = Bs[1];
+        for (int i = 2; i < m; ++i) {
+            cb[i] = Bs[i] - As[i] * Cs[i - 1] / cb[i - 1];
+            ca[i] = -As[i] * ca[i - 1] / cb[i - 1];
+        }
+        cc[m - 1] = Cs[m - 1];
+        cc[m - 2] = Cs[m - 2];
+        for (int i = m - 3; i >= 1; --i) {
+            ca[i] = ca[i] - Cs[i] * ca[i + 1] / cb[i + 1];
+            cc[i] = -Cs[i] * cc[i + 1] / cb[i + 1];
+        }
+        ca[0] = As[0];
+        cb[0] = Bs[0] - Cs[0] * ca[1] / Bs[1];
+        cc[0] = -Cs[0] * cc[1] / Bs[1];
+        for (int i = 0; i < m; ++i) {
+            const int k = s * m + i;
+            fA[k] = (i >= 2) ? (double)(As[i] / cb[i - 1]) : 0.0;
+            bC[k] = (i <= m - 3) ? (double)(Cs[i] / cb[i + 1]) : 0.0;
+            if (i >= 1 && i <= m - 2) {
+                rb[k] = (double)((ld)1 / cb[i]);
+                ra[k] = (double)(ca[i] / cb[i]);
+                rc[k] = (double)(cc[i] / cb[i]);
+            }
+        }
+        ra2[2 * s] = ca[0];         rbd[2 * s] = cb[0];         rc2[2 * s] = cc[0];
+        ra2[2 * s + 1] = ca[m - 1]; rbd[2 * s + 1] = cb[m - 1]; rc2[2 * s + 1] = cc[m - 1];
+    }
+    ra2[0] = 0;
+    rc2[n2 - 1] = 0;
+    // PCR of the boundary system with the multipliers recorded per level
+    {
+        std::vector<ld> na(n2), nb(n2), nc(n2);
+        int h = 1;
+        for (int l = 0; l < LV; ++l, h *= 2) {
+            double *kk = pcr + (size_t)l * 2 * n2;
+            for (int r = 0; r < n2; ++r) {
+                ld k1 = 0, k2 = 0;
+                ld b = rbd[r], an = 0, cn = 0;
+                if (r - h >= 0) { k1 = ra2[r] / rbd[r - h]; b -= k1 * rc2[r - h]; an = -k1 * ra2[r - h]; }
+                if (r + h < n2) { k2 = rc2[r] / rbd[r + h]; b -= k2 * ra2[r + h]; cn = -k2 * rc2[r + h]; }
+                kk[2 * r] = (double)(-k1);
+                kk[2 * r + 1] = (double)(-k2);
+                na[r] = an; nb[r] = b; nc[r] = cn;
+            }
+            ra2 = na; rbd = nb; rc2 = nc;
+        }
+        double *rbr = pcr + (size_t)LV * 2 * n2;
+        for (int r = 0; r < n2; ++r) rbr[r] = (double)((ld)1 / rbd[r]);
+    }
+
+    // upload into the table set that no in-flight solve reads (double buffering)
+    const int nb = (pl->helm_cur < 0) ? 0 : 1 - pl->helm_cur;
+    HelmTables &t = pl->helm[nb];
+    if (t.bytes < bytes) {
+        if (t.dev) PZ_CUDA(cudaFree(t.dev));
+        t.dev = nullptr;
+        cudaError_t e = cudaMalloc(&t.dev, bytes);
+        if (e != cudaSuccess) { set_error("helmholtz tables: %s", cudaGetErrorString(e)); return PZ_ENOMEM; }
+        t.bytes = bytes;
+    }
+    if (pl->helm_host_bytes < 2 * bytes) {
+        PZ_CUDA(cudaStreamSynchronize(pl->upload_stream));
+        if (pl->helm_host) PZ_CUDA(cudaFreeHost(pl->helm_host));
+        pl->helm_host = nullptr;
+        cudaError_t e = cudaMallocHost(&pl->helm_host, 2 * bytes);
+        if (e != cudaSuccess) { set_error("helmholtz staging: %s", cudaGetErrorString(e)); return PZ_ENOMEM; }
+        pl->helm_host_bytes = 2 * bytes;
+    }
+    if (t.used) PZ_CUDA(cudaStreamWaitEvent(pl->upload_stream, t.last_use, 0)); // old readers done
+    // the staging half was last read by the upload two setups ago: that copy has completed
+    // because its event has been waited on by every later solve's stream; be safe and sync it
+    if (t.used) PZ_CUDA(cudaEventSynchronize(t.uploaded));
+    double *stage = pl->helm_host + (size_t)nb * (pl->helm_host_bytes / 2 / sizeof(double));
+    std::memcpy(stage, host.data(), bytes);
+    PZ_CUDA(cudaMemcpyAsync(t.dev, stage, bytes, cudaMemcpyHostToDevice, pl->upload_stream));
+    PZ_CUDA(cudaEventRecord(t.uploaded, pl->upload_stream));
+    t.used = true;
+    pl->helm_cur = nb;
+    pl->helm_a = a;
+    return PZ_OK;
+}
+
+int launch_helmholtz(pz_plan *pl, double *u, cudaStream_t st)
+{
+    HelmTables &t = pl->helm[pl->helm_cur];
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    PZ_CUDA(cudaStreamIsCapturing(st, &cap));
+    const bool capturing = (cap != cudaStreamCaptureStatusNone);
+    // order after the table upload unless it is known to have completed (always the case when
+    // capturing a graph after a warm-up solve)
+    if (!capturing && cudaEventQuery(t.uploaded) != cudaSuccess) PZ_CUDA(cudaStreamWaitEvent(st, t.uploaded, 0));
+    const size_t plane = (size_t)pl->nx * pl->ny;
+    const int tx = pl->helm_tx, P = pl->helm_P;
+    const unsigned blocks = (unsigned)(plane / tx);
+    const size_t smem = 2 * (size_t)(2 * P) * tx * sizeof(double);
+    const int threads = tx * P;
+    switch (pl->helm_m) {
+    case 4: helmholtz_kernel<4><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); break;
+    case 8: helmholtz_kernel<8><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); break;
+    case 16: helmholtz_kernel<16><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); break;
+    case 32: helmholtz_kernel<32><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); break;
+    default: set_error("helmholtz: bad sub-domain size %d", pl->helm_m); return PZ_EINVAL;
+    }
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    if (!capturing) PZ_CUDA(cudaEventRecord(t.last_use, st));
+    return PZ_OK;
+}
+
+} // namespace pz

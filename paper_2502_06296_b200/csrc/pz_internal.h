@@ -1,0 +1,92 @@
+// pz_internal.h -- plan object and launch declarations shared by the translation units of
+// libpz_b200.so.  Not installed; the public boundary is include/pz.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstddef>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/pz.h"
+
+namespace pz {
+
+// Helmholtz pre-processing tables of Algorithm 2, one set per buffer.
+// Rows are padded to nzp = P*m with identity rows so that every sub-domain has m rows.
+struct HelmTables {
+    double *dev = nullptr;      // one allocation: [fA | bC | rb | ra | rc] (5*nzp) + reduced PCR tables
+    size_t bytes = 0;
+    cudaEvent_t uploaded = nullptr;   // recorded on the upload stream after the H2D copy
+    cudaEvent_t last_use = nullptr;   // recorded on the caller's stream after each solve
+    bool used = false;
+};
+
+struct Options {
+    int zsolve_variant = 0;   // 0 = thread-per-column Thomas through global memory (2 sweeps)
+                              // 1 = chunked cyclic reduction in shared memory
+    int slab_planes = 0;      // 0 = auto: z-planes per L2-resident slab for the fused x/y FFT passes
+    int helm_tx = 0;          // 0 = auto: columns per CTA in the Helmholtz kernel
+    int helm_m = 0;           // 0 = auto: rows per sub-domain in the Helmholtz kernel
+    int fft_y_tc = 0;         // 0 = auto: complex column pairs per CTA in the y FFT
+    int fft_x_lpb = 0;        // 0 = auto: lines per CTA in the x FFT
+};
+
+} // namespace pz
+
+struct pz_plan {
+    int nx = 0, ny = 0, nz = 0;
+    double lx = 0, ly = 0;
+    int device = 0;
+    int num_sms = 0;
+    size_t n = 0;
+
+    // host copies
+    std::vector<double> zc, zf, dzf, dzc, A, C;
+
+    // device tables (one allocation, freed as `tables`)
+    double *tables = nullptr;
+    double *d_A = nullptr, *d_C = nullptr, *d_dzf = nullptr;   // nz each
+    double *d_lamx = nullptr;        // nx: lambda_x per real column i in packed order
+    double *d_lamy_nat = nullptr;    // ny: lambda_y, natural order (complex pairs i >= 2)
+    double *d_lamy_pk = nullptr;     // ny: lambda_y, packed order (columns i = 0, 1)
+    double2 *d_twx = nullptr;        // nx: exp(-2 pi i k / nx)
+    double2 *d_twy = nullptr;        // ny: exp(-2 pi i k / ny)
+    double inv_lz = 0;               // 1 / sum dzf
+
+    // optional workspaces (allocated on first use)
+    double *d_zwork = nullptr;       // variant-0 z solve: N doubles
+    double *d_host_stage = nullptr;  // *_host calls: N doubles
+
+    // Helmholtz
+    double helm_a = -1.0;
+    int helm_m = 0, helm_P = 0, helm_tx = 0, helm_levels = 0;
+    pz::HelmTables helm[2];
+    int helm_cur = -1;
+    cudaStream_t upload_stream = nullptr;
+    double *helm_host = nullptr;     // pinned staging for uploads, 2 halves
+    size_t helm_host_bytes = 0;
+
+    pz::Options opt;
+};
+
+namespace pz {
+
+void set_error(const char *fmt, ...);
+int cuda_fail(cudaError_t e, const char *what);
+void count_launch(int n = 1);
+
+#define PZ_CUDA(call)                                                                              \
+    do {                                                                                           \
+        cudaError_t e__ = (call);                                                                  \
+        if (e__ != cudaSuccess) return ::pz::cuda_fail(e__, #call);                                \
+    } while (0)
+
+// kernels (each returns a pz_status)
+int launch_fft_x(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
+int launch_fft_y(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
+int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
+int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st);
+int launch_helmholtz(pz_plan *pl, double *u, cudaStream_t st);
+int helmholtz_build_tables(pz_plan *pl, double a);
+
+} // namespace pz

@@ -1,0 +1,96 @@
+// pz_zsolve.cu -- step a3 of the hot path: one real tridiagonal solve along z per spectral
+// column (Eq. 12; steps 4-6 of PAPER.md:127-129):
+//     A_k phi_{k-1} + (-(A_k+C_k) + lambda) phi_k + C_k phi_{k+1} = d_k,   lambda = lambda_x + lambda_y.
+// Real and imaginary parts are separate real systems with the same matrix.
+//
+// Numerics (reading R5).  Every row is kept in M-matrix form
+//     -alpha x_{k-1} + (alpha + gamma + eps) x_k - gamma x_{k+1} = r,   alpha, gamma, eps >= 0,
+// with the excess eps (= sigma = -lambda at the start) carried explicitly.  Elimination then
+// only ever ADDS non-negative numbers (eps' = eps + m eps_prev), so the near-singular low modes
+// on strongly stretched grids are solved to ~1e-14 instead of ~1e-11 (forming -(A+C)+lambda in
+// double and subtracting loses 4-5 digits).
+//
+// Variant 0 (this file, reference variant): one thread per column, serial Thomas sweeps through
+// global memory ("each i,j index is assigned to a thread, which serially performs
+// operations along the third domain direction"), forward result and C_k/p_k staged in HBM.
+// Variant 1 (pz_zsolve_cr.cu): chunked cyclic reduction in shared memory (Algorithm 1).
+#include "pz_internal.h"
+
+namespace pz {
+
+int launch_zsolve_cr(pz_plan *pl, double *p, cudaStream_t st);
+
+namespace {
+
+__global__ void __launch_bounds__(128)
+    zsolve_thomas_kernel(double *__restrict__ p, double *__restrict__ work, const double *__restrict__ A,
+                         const double *__restrict__ C, const double *__restrict__ dzf,
+                         const double *__restrict__ lamx, const double *__restrict__ lamy_nat,
+                         const double *__restrict__ lamy_pk, int nx, int ny, int nz, double inv_lz)
+{
+    const size_t plane = (size_t)nx * ny;
+    const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= plane) return;
+    const int i = (int)(col % nx), j = (int)(col / nx);
+    const double sigma = -(lamx[i] + (i < 2 ? lamy_pk[j] : lamy_nat[j]));
+    const bool singular = (i == 0 && j == 0);
+
+    // forward: p_k = C_k + e_k, e_k = sigma + A_k e_{k-1}/p_{k-1}; g_k = (-d_k + A_k g_{k-1})/p_k
+    double e = sigma;
+    double pk = C[0] + e;
+    double rp = 1.0 / pk;
+    double g = -p[col] * rp;
+    p[col] = g;
+    work[col] = C[0] * rp;
+    for (int k = 1; k < nz; ++k) {
+        const double a = A[k], c = C[k];
+        const double d = p[(size_t)k * plane + col];
+        e = fma(a * e, rp, sigma);
+        pk = c + e;
+        if (singular && k == nz - 1) {
+            // gauge: the last equation of the singular (0,0) system is replaced by phi = 0
+            g = 0.0;
+            rp = 0.0;
+        } else {
+            rp = 1.0 / pk;
+            g = fma(a, g, -d) * rp;
+        }
+        p[(size_t)k * plane + col] = g;
+        work[(size_t)k * plane + col] = c * rp;
+    }
+    // backward: phi_k = g_k + (C_k/p_k) phi_{k+1}
+    double x = g;
+    for (int k = nz - 2; k >= 0; --k) {
+        x = fma(work[(size_t)k * plane + col], x, p[(size_t)k * plane + col]);
+        p[(size_t)k * plane + col] = x;
+    }
+    if (singular) {
+        double s = 0.0;
+        for (int k = 0; k < nz; ++k) s = fma(dzf[k], p[(size_t)k * plane + col], s);
+        s *= inv_lz;
+        for (int k = 0; k < nz; ++k) p[(size_t)k * plane + col] -= s;
+    }
+}
+
+} // namespace
+
+int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st)
+{
+    if (pl->opt.zsolve_variant == 1) return launch_zsolve_cr(pl, p, st);
+    if (!pl->d_zwork) {
+        cudaError_t e = cudaMalloc(&pl->d_zwork, pl->n * sizeof(double));
+        if (e != cudaSuccess) {
+            set_error("z-solve variant 0 workspace (%zu bytes): %s", pl->n * sizeof(double), cudaGetErrorString(e));
+            return PZ_ENOMEM;
+        }
+    }
+    const size_t plane = (size_t)pl->nx * pl->ny;
+    const unsigned blocks = (unsigned)((plane + 127) / 128);
+    zsolve_thomas_kernel<<<blocks, 128, 0, st>>>(p, pl->d_zwork, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
+                                                  pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, pl->nz, pl->inv_lz);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+} // namespace pz

@@ -1,0 +1,280 @@
+// pz_zsolve_cr.cu -- step a3, variant 1: the paper's parallel tridiagonal algorithm
+// (Algorithm 1 at :157-197) applied INSIDE one GPU.
+//
+// In the paper the z direction is cut into p_z sub-domains owned by different GPUs: each reduces
+// its rows to the two boundary unknowns, a small system of size 2 p_z is solved, and the interior
+// is reconstructed.  Here a CTA stages a tile of 16 neighbouring spectral columns x all nz rows in
+// shared memory (one coalesced HBM read, one write: 16 B/point), a warp owns one complex column
+// (the packed pair (2q, 2q+1): Re and Im share the matrix, so pivots are computed once for both),
+// and its 32 lanes are the 32 "sub-domains" of m = nz/32 rows.  The boundary system is solved
+// with warp-shuffle parallel cyclic reduction.  Coefficients depend on (i,j,k) for the Poisson
+// problem, so Algorithm 1's private a', c' arrays live in registers and are
+// recomputed every solve; storing them would cost 8-16 more HBM bytes per point.
+//
+// All rows are kept in M-matrix form with an explicit diagonal excess (see pz_zsolve.cu): the
+// sub-domain sweeps, the reduced system and the PCR levels only add non-negative numbers.
+#include "pz_internal.h"
+
+namespace pz {
+
+namespace {
+
+constexpr int kTX = 16;    // real columns per tile (128-byte rows)
+constexpr int kPairs = 8;  // complex pairs per tile = warps per CTA
+constexpr int kLanes = 32; // sub-domains per column
+
+// 1/x to ~1 ulp: hardware seed + two Newton steps (x is a positive, normal pivot).
+__device__ __forceinline__ double fast_rcp(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    return r;
+}
+
+__device__ __forceinline__ double shfl_up(double v, int d) { return __shfl_up_sync(0xffffffffu, v, d); }
+__device__ __forceinline__ double shfl_down(double v, int d) { return __shfl_down_sync(0xffffffffu, v, d); }
+
+// One column pair, one sub-domain per lane.  d points at this lane's first row inside the tile
+// (row stride kTX/2 double2).  al/ga: this lane's alpha_i, gamma_i (sub-/super-diagonal
+// magnitudes, zero on padding rows and at the walls) in shared memory.  MASK bit 0 / 1: which
+// component (x / y of the double2) is solved and written back.
+template <int M, int MASK, bool pin>
+__device__ __forceinline__ void solve_pair(double2 *d, const double *al, const double *ga, double sigma,
+                                           int k0, int nz, const double *__restrict__ dzf, double inv_lz)
+{
+    constexpr int RS = kTX / 2;
+    // row coefficients: real rows have excess sigma, padding rows (k >= nz) are x = 0,
+    // the pinned row (gauge of the singular column) likewise.
+    auto eps_of = [&](int i) { return (k0 + i < nz && !(pin && k0 + i == nz - 1)) ? sigma : 1.0; };
+    auto alpha_of = [&](int i) { return (pin && k0 + i == nz - 1) ? 0.0 : al[i]; };
+    auto rhs_of = [&](int i) {
+        const double2 v = d[i * RS];
+        const bool live = (k0 + i < nz) && !(pin && k0 + i == nz - 1);
+        return live ? make_double2(-v.x, -v.y) : make_double2(0.0, 0.0);
+    };
+
+    // ---- UL sweep (read only), rows M-2 .. 1: Schur complement of the interior onto row 0
+    double chat = ga[M - 2], eps2 = eps_of(M - 2);
+    double2 rp2 = rhs_of(M - 2);
+    double rb2 = fast_rcp(alpha_of(M - 2) + chat + eps2);
+#pragma unroll
+    for (int i = M - 3; i >= 1; --i) {
+        const double nn = ga[i] * rb2;
+        const double2 r = rhs_of(i);
+        chat = nn * chat;
+        eps2 = fma(nn, eps2, eps_of(i));
+        rp2.x = fma(nn, rp2.x, r.x);
+        rp2.y = fma(nn, rp2.y, r.y);
+        rb2 = fast_rcp(alpha_of(i) + chat + eps2);
+    }
+    double a0, c0, e0;
+    double2 r0;
+    {
+        const double nn = ga[0] * rb2;
+        const double2 r = rhs_of(0);
+        a0 = alpha_of(0);
+        c0 = nn * chat;
+        e0 = fma(nn, eps2, eps_of(0));
+        r0.x = fma(nn, rp2.x, r.x);
+        r0.y = fma(nn, rp2.y, r.y);
+        const double rb = fast_rcp(a0 + c0 + e0);
+        a0 *= rb; c0 *= rb; e0 *= rb; r0.x *= rb; r0.y *= rb;
+    }
+
+    // ---- LU sweep, rows 1 .. M-1: x_i = Rn_i + Ah_i x_0 + W_i x_{i+1}; Rn overwrites the tile
+    double Ah[M], W[M];
+    double ahat = alpha_of(1), eps = eps_of(1);
+    double2 rp = rhs_of(1);
+    double rb = fast_rcp(ahat + ga[1] + eps);
+    Ah[1] = ahat * rb;
+    W[1] = ga[1] * rb;
+    {
+        double2 t = d[1 * RS];
+        if (MASK & 1) t.x = rp.x * rb;
+        if (MASK & 2) t.y = rp.y * rb;
+        d[1 * RS] = t;
+    }
+#pragma unroll
+    for (int i = 2; i < M; ++i) {
+        const double mm = alpha_of(i) * rb;
+        const double2 r = rhs_of(i);
+        ahat = mm * ahat;
+        eps = fma(mm, eps, eps_of(i));
+        rp.x = fma(mm, rp.x, r.x);
+        rp.y = fma(mm, rp.y, r.y);
+        rb = fast_rcp(ahat + ga[i] + eps);
+        Ah[i] = ahat * rb;
+        W[i] = ga[i] * rb;
+        double2 t = d[i * RS];
+        if (MASK & 1) t.x = rp.x * rb;
+        if (MASK & 2) t.y = rp.y * rb;
+        d[i * RS] = t;
+    }
+    // last row of the sub-domain, normalised: -a x_0 + x_{M-1} - c x_{next 0} = r, excess e
+    double a = Ah[M - 1], c = W[M - 1], e = eps * rb;
+    double2 r = make_double2(rp.x * rb, rp.y * rb);
+
+    // ---- reduced system: first eliminate the x_0 unknowns (local row 0 and the next lane's)
+    {
+        const double c0n = shfl_down(c0, 1), e0n = shfl_down(e0, 1);
+        const double r0nx = shfl_down(r0.x, 1), r0ny = shfl_down(r0.y, 1);
+        const double k1 = a, k2 = c; // c = 0 on the last lane (wall or padding)
+        a = k1 * a0;
+        c = k2 * c0n;
+        e = fma(k1, e0, fma(k2, e0n, e));
+        r.x = fma(k1, r0.x, fma(k2, r0nx, r.x));
+        r.y = fma(k1, r0.y, fma(k2, r0ny, r.y));
+        const double rbn = fast_rcp(a + c + e);
+        a *= rbn; c *= rbn; e *= rbn; r.x *= rbn; r.y *= rbn;
+    }
+    // ---- parallel cyclic reduction across the 32 lanes (unknown X_s = last row of lane s)
+#pragma unroll
+    for (int h = 1; h < kLanes; h *= 2) {
+        const double am = shfl_up(a, h), em = shfl_up(e, h), rmx = shfl_up(r.x, h), rmy = shfl_up(r.y, h);
+        const double cp = shfl_down(c, h), ep = shfl_down(e, h), rpx = shfl_down(r.x, h), rpy = shfl_down(r.y, h);
+        // a == 0 whenever lane-h < 0 and c == 0 whenever lane+h > 31, so out-of-range partners
+        // (whose shuffled values are the lane's own, finite) contribute nothing.
+        const double k1 = a, k2 = c;
+        a = k1 * am;
+        c = k2 * cp;
+        e = fma(k1, em, fma(k2, ep, e));
+        r.x = fma(k1, rmx, fma(k2, rpx, r.x));
+        r.y = fma(k1, rmy, fma(k2, rpy, r.y));
+        const double rbn = fast_rcp(a + c + e);
+        a *= rbn; c *= rbn; e *= rbn; r.x *= rbn; r.y *= rbn;
+    }
+    // r = X_s.  x_0 of this lane from its normalised row 0:  x_0 = r0 + a0 X_{s-1} + c0 X_s
+    const double xpx = shfl_up(r.x, 1), xpy = shfl_up(r.y, 1); // lane 0: a0 = 0
+    double2 x0 = make_double2(fma(a0, xpx, fma(c0, r.x, r0.x)), fma(a0, xpy, fma(c0, r.y, r0.y)));
+
+    // ---- reconstruct the interior (back substitution with the stored LU rows)
+    double2 x = r;
+    double2 wsum = make_double2(0.0, 0.0);
+    auto put = [&](int i, double2 val) {
+        double2 t = d[i * RS];
+        if (MASK & 1) t.x = val.x;
+        if (MASK & 2) t.y = val.y;
+        d[i * RS] = t;
+        if (pin && k0 + i < nz) wsum.x = fma(dzf[k0 + i], val.x, wsum.x);
+    };
+    put(M - 1, x);
+#pragma unroll
+    for (int i = M - 2; i >= 1; --i) {
+        const double2 rn = d[i * RS];
+        x.x = fma(W[i], x.x, fma(Ah[i], x0.x, rn.x));
+        x.y = fma(W[i], x.y, fma(Ah[i], x0.y, rn.y));
+        put(i, x);
+    }
+    put(0, x0);
+
+    if constexpr (pin) {
+        // zero volume mean of the (0,0) mode: subtract sum_k dzf_k phi_k / sum_k dzf_k
+        double s = wsum.x;
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        s *= inv_lz;
+#pragma unroll
+        for (int i = 0; i < M; ++i)
+            if (k0 + i < nz) d[i * RS].x -= s;
+    }
+}
+
+template <int M>
+__global__ void __launch_bounds__(kPairs *kLanes)
+    zsolve_cr_kernel(double *__restrict__ p, const double *__restrict__ A, const double *__restrict__ C,
+                     const double *__restrict__ dzf, const double *__restrict__ lamx,
+                     const double *__restrict__ lamy_nat, const double *__restrict__ lamy_pk, int nx, int ny,
+                     int nz, double inv_lz)
+{
+    constexpr int CH = M * kTX + 2;  // doubles per sub-domain in the tile (+2: bank spread, 16-B aligned)
+    constexpr int CS = M + 1;        // coefficient stride per lane (bank spread)
+    extern __shared__ double smem_z[];
+    double *tile = smem_z;                     // kLanes * CH
+    double *s_al = tile + kLanes * CH;         // kLanes * CS
+    double *s_ga = s_al + kLanes * CS;
+
+    const size_t plane = (size_t)nx * ny;
+    const size_t col0 = (size_t)blockIdx.x * kTX;
+
+    // stage the tile: 8 threads x 16 B per row, 32 rows per sweep
+    {
+        const int c2 = (threadIdx.x & 7) * 2;
+        for (int k = threadIdx.x >> 3; k < nz; k += 32) {
+            const double2 v = *reinterpret_cast<const double2 *>(p + (size_t)k * plane + col0 + c2);
+            *reinterpret_cast<double2 *>(tile + (k / M) * CH + (k % M) * kTX + c2) = v;
+        }
+        for (int k = threadIdx.x; k < kLanes * M; k += blockDim.x) {
+            s_al[(k / M) * CS + (k % M)] = (k < nz) ? A[k] : 0.0;
+            s_ga[(k / M) * CS + (k % M)] = (k < nz) ? C[k] : 0.0;
+        }
+    }
+    __syncthreads();
+
+    {
+        const int lane = threadIdx.x & 31, q = threadIdx.x >> 5;
+        const size_t col = col0 + 2 * q;
+        const int i = (int)(col % nx), j = (int)(col / nx);
+        const double ly = (i < 2) ? lamy_pk[j] : lamy_nat[j];
+        const double sig0 = -(lamx[i] + ly), sig1 = -(lamx[i + 1] + ly);
+        double2 *d = reinterpret_cast<double2 *>(tile + lane * CH + 2 * q);
+        const double *al = s_al + lane * CS, *ga = s_ga + lane * CS;
+        const int k0 = lane * M;
+        if (sig0 == sig1) {
+            solve_pair<M, 3, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
+        } else {
+            // pair 0 of a row: x-modes 0 and nx/2 have different eigenvalues; (0,0) is singular
+            if (i == 0 && j == 0)
+                solve_pair<M, 1, true>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
+            else
+                solve_pair<M, 1, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
+            solve_pair<M, 2, false>(d, al, ga, sig1, k0, nz, dzf, inv_lz);
+        }
+    }
+    __syncthreads();
+
+    {
+        const int c2 = (threadIdx.x & 7) * 2;
+        for (int k = threadIdx.x >> 3; k < nz; k += 32) {
+            const double2 v = *reinterpret_cast<const double2 *>(tile + (k / M) * CH + (k % M) * kTX + c2);
+            *reinterpret_cast<double2 *>(p + (size_t)k * plane + col0 + c2) = v;
+        }
+    }
+}
+
+template <int M>
+int launch_m(pz_plan *pl, double *p, cudaStream_t st)
+{
+    constexpr size_t smem = ((size_t)kLanes * (M * kTX + 2) + 2 * (size_t)kLanes * (M + 1)) * sizeof(double);
+    static bool attr_done = false;
+    if (smem > 48 * 1024 && !attr_done) {
+        PZ_CUDA(cudaFuncSetAttribute(zsolve_cr_kernel<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    const size_t plane = (size_t)pl->nx * pl->ny;
+    const unsigned blocks = (unsigned)(plane / kTX);
+    zsolve_cr_kernel<M><<<blocks, kPairs * kLanes, smem, st>>>(p, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
+                                                                pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny,
+                                                                pl->nz, pl->inv_lz);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+} // namespace
+
+int launch_zsolve_cr(pz_plan *pl, double *p, cudaStream_t st)
+{
+    const int nz = pl->nz;
+    if (nz <= 32 * 4) return launch_m<4>(pl, p, st);
+    if (nz <= 32 * 8) return launch_m<8>(pl, p, st);
+    if (nz <= 32 * 16) return launch_m<16>(pl, p, st);
+    if (nz <= 32 * 32) return launch_m<32>(pl, p, st);
+    set_error("z-solve variant 1 supports nz <= 1024 (got %d); use zsolve_variant = 0", nz);
+    return PZ_EUNSUPPORTED;
+}
+
+} // namespace pz

@@ -1,0 +1,309 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Bar (BASELINE.json north_star): max|gpu - oracle| / max|oracle| <= 1e-11.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+
+    assert t.cuda.is_available()
+    return t
+
+
+@pytest.fixture(scope="module")
+def pz():
+    from paper_2502_06296_b200 import binding
+
+    binding.lib()  # fails loudly if the extension is missing
+    return binding
+
+
+@pytest.fixture(scope="module")
+def wl():
+    from paper_2502_06296_b200 import workloads
+
+    return workloads
+
+
+@pytest.fixture(scope="module")
+def oracle():
+    import oracle as o
+
+    return o
+
+
+def rel_err(got, ref):
+    return float(np.abs(got - ref).max() / np.abs(ref).max())
+
+
+def gpu_poisson(torch, pz, w, zc, zf, f, options=()):
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    for k, v in options:
+        pz.pz_set_option(plan, k, v)
+    p = torch.from_numpy(f).cuda()
+    pz.poisson_solve(plan, p)
+    torch.cuda.synchronize()
+    out = p.cpu().numpy()
+    pz.poisson_plan_destroy(plan)
+    return out
+
+
+# ------------------------------------------------------------------------ Poisson
+
+POISSON_SHAPES = [
+    # (base config, nx, ny, nz)   small enough for the oracle in seconds, several tiles + ragged tails
+    ("c0", 64, 64, 64),       # BASELINE config 0 itself
+    ("c0", 8, 8, 4),          # minimum sizes
+    ("c0", 16, 8, 5),
+    ("c1", 32, 64, 48),       # stretched, nz not a multiple of 32
+    ("c1", 128, 32, 100),
+    ("c1", 64, 128, 129),     # one row past a sub-domain multiple
+    ("c3", 256, 64, 96),      # beta = 2.0, long x
+    ("c3", 32, 256, 33),
+    ("c2", 64, 64, 128),      # few-mode right-hand side
+]
+
+
+@pytest.mark.parametrize("base,nx,ny,nz", POISSON_SHAPES)
+@pytest.mark.parametrize("variant", [0, 1])
+def test_poisson_matches_oracle(torch, pz, wl, oracle, base, nx, ny, nz, variant):
+    w = wl.scaled(wl.CONFIGS[base], nx, ny, nz)
+    zc, zf = wl.grid(w)
+    f = wl.poisson_rhs(w)
+    ref = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 0 if nx * ny <= 64 * 64 else 1)
+    got = gpu_poisson(torch, pz, w, zc, zf, f, [("zsolve_variant", variant)])
+    assert rel_err(got, ref) <= TOL
+    dzf = np.diff(zf)
+    wm = np.einsum("k,kji->", dzf, got) / (dzf.sum() * nx * ny)
+    assert abs(wm) <= 1e-13 * np.abs(got).max()
+
+
+@pytest.mark.parametrize("slab", [1, 3, 1000])
+def test_poisson_slab_size_does_not_change_the_result(torch, pz, wl, slab):
+    w = wl.scaled(wl.CONFIGS["c1"], 64, 32, 40)
+    zc, zf = wl.grid(w)
+    f = wl.poisson_rhs(w)
+    a = gpu_poisson(torch, pz, w, zc, zf, f, [("slab_planes", slab)])
+    b = gpu_poisson(torch, pz, w, zc, zf, f, [])
+    assert np.array_equal(a, b)  # bitwise: no atomics, same arithmetic per point
+
+
+def test_poisson_is_bitwise_deterministic_and_plan_is_reusable(torch, pz, wl):
+    w = wl.scaled(wl.CONFIGS["c1"], 64, 64, 64)
+    zc, zf = wl.grid(w)
+    f = wl.poisson_rhs(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    outs = []
+    for _ in range(3):
+        p = torch.from_numpy(f).cuda()
+        pz.poisson_solve(plan, p)
+        outs.append(p.cpu().numpy())
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+
+
+def test_poisson_on_a_side_stream_and_graph_capture(torch, pz, wl):
+    w = wl.scaled(wl.CONFIGS["c1"], 32, 32, 64)
+    zc, zf = wl.grid(w)
+    f = wl.poisson_rhs(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    p0 = torch.from_numpy(f).cuda()
+    pz.poisson_solve(plan, p0)
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    p1 = torch.from_numpy(f).cuda()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        pz.poisson_solve(plan, p1)
+    s.synchronize()
+    assert torch.equal(p0, p1)
+    # CUDA graph: no allocation, no host sync inside the solve
+    static = torch.from_numpy(f).cuda()
+    g = torch.cuda.CUDAGraph()
+    torch.cuda.synchronize()
+    with torch.cuda.graph(g):
+        pz.poisson_solve(plan, static)
+    static.copy_(torch.from_numpy(f))
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(static, p0)
+
+
+def test_poisson_stages_against_oracle_dft(torch, pz, wl, oracle):
+    """Stage a1+a2 produce the 2-D DFT of every plane (in the packed spectral layout)."""
+    from oracle import algorithms as alg
+
+    w = wl.scaled(wl.CONFIGS["c1"], 32, 16, 6)
+    zc, zf = wl.grid(w)
+    f = wl.poisson_rhs(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    p = torch.from_numpy(f).cuda()
+    pz.pz_poisson_stage(plan, p, pz.PZ_STAGE_FFT_X_FWD)
+    gx = p.cpu().numpy()
+    X = np.fft.rfft(f, axis=2)
+    for k in range(w.nz):
+        for j in range(w.ny):
+            assert np.abs(alg.unpack_halfcomplex(gx[k, j])[1:-1] - X[k, j, 1:-1]).max() <= 1e-12 * np.abs(X).max()
+            assert abs(gx[k, j, 0] - X[k, j, 0].real) <= 1e-12 * np.abs(X).max()
+            assert abs(gx[k, j, 1] - X[k, j, -1].real) <= 1e-12 * np.abs(X).max()
+    pz.pz_poisson_stage(plan, p, pz.PZ_STAGE_FFT_Y_FWD)
+    gy = p.cpu().numpy()
+    F = oracle.dft_xy(f, -1, 0)                      # full complex 2-D DFT, [k][qy][qx]
+    scale = np.abs(F).max()
+    nxh = w.nx // 2
+    for q in range(1, nxh):                          # complex pairs: natural order in y
+        got = gy[:, :, 2 * q] + 1j * gy[:, :, 2 * q + 1]
+        assert np.abs(got - F[:, :, q]).max() <= 1e-12 * scale
+    for col, q in ((0, 0), (1, nxh)):                # x-modes 0 and nx/2: packed order in y
+        for k in range(w.nz):
+            got = alg.unpack_halfcomplex(gy[k, :, col])
+            assert np.abs(got - F[k, : w.ny // 2 + 1, q]).max() <= 1e-12 * scale
+    # inverse stages undo the forward ones (up to the 1/(nx ny) applied in a5)
+    pz.pz_poisson_stage(plan, p, pz.PZ_STAGE_FFT_Y_INV)
+    pz.pz_poisson_stage(plan, p, pz.PZ_STAGE_FFT_X_INV)
+    back = p.cpu().numpy()
+    assert np.abs(back - f).max() <= 1e-13 * np.abs(f).max()
+
+
+@pytest.mark.parametrize("nx,ny", [(8, 8), (16, 8), (8, 32), (64, 16), (128, 64), (256, 128), (512, 256),
+                                   (1024, 8), (8, 1024), (2048, 16), (16, 2048), (4096, 8), (8, 4096)])
+def test_fft_roundtrip_and_spectrum_every_size(torch, pz, wl, nx, ny):
+    """Every supported transform length: forward stages against numpy.fft (library routine as
+    an independent check of the layout), then the inverse stages return the input."""
+    nz = 4
+    w = wl.scaled(wl.CONFIGS["c0"], nx, ny, nz)
+    zc, zf = wl.grid(w)
+    rng = np.random.default_rng(nx + ny)
+    f = rng.standard_normal((nz, ny, nx))
+    plan = pz.poisson_plan_create(nx, ny, nz, w.lx, w.ly, zc, zf)
+    p = torch.from_numpy(f).cuda()
+    pz.pz_poisson_stage(plan, p, pz.PZ_STAGE_FFT_X_FWD)
+    pz.pz_poisson_stage(plan, p, pz.PZ_STAGE_FFT_Y_FWD)
+    g = p.cpu().numpy()
+    F = np.fft.fft(np.fft.rfft(f, axis=2), axis=1)   # [k][qy][qx], qx = 0..nx/2
+    scale = np.abs(F).max()
+    for q in range(1, nx // 2):
+        got = g[:, :, 2 * q] + 1j * g[:, :, 2 * q + 1]
+        assert np.abs(got - F[:, :, q]).max() <= 1e-12 * scale, q
+    assert np.abs(g[:, 0, 0] - F[:, 0, 0].real).max() <= 1e-12 * scale
+    assert np.abs(g[:, 1, 1] - F[:, ny // 2, nx // 2].real).max() <= 1e-12 * scale
+    pz.pz_poisson_stage(plan, p, pz.PZ_STAGE_FFT_Y_INV)
+    pz.pz_poisson_stage(plan, p, pz.PZ_STAGE_FFT_X_INV)
+    assert np.abs(p.cpu().numpy() - f).max() <= 1e-13 * np.abs(f).max()
+
+
+# ---------------------------------------------------------------------- Helmholtz
+
+HELM_CASES = [
+    # (nx, ny, nz, beta, a, options)
+    (8, 8, 4, 0.0, 0.1, []),
+    (16, 8, 7, 1.8, 5e-5, []),
+    (32, 16, 64, 1.8, 5e-5, []),
+    (32, 16, 100, 1.8, 5e-5, []),
+    (64, 8, 129, 2.0, 2.5e-5, []),
+    (16, 16, 256, 1.8, 5e-5, []),
+    (16, 16, 256, 1.8, 1e-2, [("helm_m", 4)]),
+    (16, 16, 256, 1.8, 5e-5, [("helm_m", 32), ("helm_tx", 8)]),
+    (8, 16, 512, 1.8, 5e-5, []),
+    (8, 16, 512, 1.8, 5e-5, [("helm_tx", 32)]),
+    (8, 8, 1024, 1.8, 2.5e-5, []),
+    (8, 8, 1024, 1.8, 2.5e-5, [("helm_m", 16), ("helm_tx", 8)]),
+    (8, 8, 1594, 1.8, 2.5e-5, []),       # the paper's nz
+    (8, 8, 64, 0.0, 0.0, []),            # a = 0: identity
+    (8, 8, 64, 1.8, 10.0, []),           # strongly implicit
+]
+
+
+@pytest.mark.parametrize("nx,ny,nz,beta,a,options", HELM_CASES)
+def test_helmholtz_matches_oracle(torch, pz, wl, oracle, nx, ny, nz, beta, a, options):
+    zf = wl.z_faces(nz, 2.0, beta)
+    zc = wl.z_centres(zf)
+    rng = np.random.default_rng(nz * 7 + nx)
+    r = rng.standard_normal((nz, ny, nx))
+    ref = oracle.helmholtz_z_solve(zc, zf, a, r)
+    plan = pz.poisson_plan_create(nx, ny, nz, 1.0, 1.0, zc, zf)
+    for k, v in options:
+        pz.pz_set_option(plan, k, v)
+    pz.helmholtz_z_setup(plan, a)
+    u = torch.from_numpy(r).cuda()
+    pz.helmholtz_z_solve(plan, u)
+    torch.cuda.synchronize()
+    assert rel_err(u.cpu().numpy(), ref) <= TOL
+    if a == 0.0:
+        assert np.array_equal(u.cpu().numpy(), r)
+
+
+def test_helmholtz_not_setup_and_resetup(torch, pz, wl, oracle):
+    nx, ny, nz = 16, 16, 96
+    zf = wl.z_faces(nz, 2.0, 1.8)
+    zc = wl.z_centres(zf)
+    plan = pz.poisson_plan_create(nx, ny, nz, 1.0, 1.0, zc, zf)
+    r = np.random.default_rng(1).standard_normal((nz, ny, nx))
+    u = torch.from_numpy(r).cuda()
+    with pytest.raises(pz.PzError) as ei:
+        pz.helmholtz_z_solve(plan, u)
+    assert ei.value.status == pz.PZ_ENOTSETUP
+    with pytest.raises(pz.PzError) as ei:
+        pz.helmholtz_z_setup(plan, -1.0)
+    assert ei.value.status == pz.PZ_EINVAL
+    # a changes every Runge-Kutta sub-step: re-setup between solves, no sync
+    fields, refs = [], []
+    for a in (8 / 15 * 5e-5, 2 / 15 * 5e-5, 1 / 3 * 5e-5, 1e-3):
+        pz.helmholtz_z_setup(plan, a)
+        v = torch.from_numpy(r).cuda()
+        pz.helmholtz_z_solve(plan, v)
+        fields.append(v)
+        refs.append(oracle.helmholtz_z_solve(zc, zf, a, r))
+    torch.cuda.synchronize()
+    for v, ref in zip(fields, refs):
+        assert rel_err(v.cpu().numpy(), ref) <= TOL
+    # three components in one call
+    pz.helmholtz_z_setup(plan, 5e-5)
+    comps = [torch.from_numpy(r * (c + 1)).cuda() for c in range(3)]
+    pz.helmholtz_z_solve_n(plan, comps)
+    torch.cuda.synchronize()
+    ref = oracle.helmholtz_z_solve(zc, zf, 5e-5, r)
+    for c, v in enumerate(comps):
+        assert rel_err(v.cpu().numpy(), ref * (c + 1)) <= TOL
+
+
+def test_host_buffer_entry_points(torch, pz, wl, oracle):
+    w = wl.scaled(wl.CONFIGS["c1"], 32, 32, 48)
+    zc, zf = wl.grid(w)
+    f = wl.poisson_rhs(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    host = torch.from_numpy(f.copy()).pin_memory()
+    pz.poisson_solve_host(plan, host)
+    torch.cuda.synchronize()
+    ref = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)
+    assert rel_err(host.numpy(), ref) <= TOL
+    r = wl.helmholtz_rhs(w)
+    pz.helmholtz_z_setup(plan, w.a)
+    hb = torch.from_numpy(r.copy()).pin_memory()
+    pz.helmholtz_z_solve_host(plan, hb)
+    torch.cuda.synchronize()
+    assert rel_err(hb.numpy(), oracle.helmholtz_z_solve(zc, zf, w.a, r)) <= TOL
+
+
+# ------------------------------------------------------- BASELINE configs 1 and 2 in full
+
+def test_config1_poisson_and_helmholtz_full(torch, pz, wl, oracle):
+    w = wl.CONFIGS["c1"]
+    zc, zf = wl.grid(w)
+    f = wl.poisson_rhs(w)
+    ref = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)
+    for variant in (0, 1):
+        got = gpu_poisson(torch, pz, w, zc, zf, f, [("zsolve_variant", variant)])
+        assert rel_err(got, ref) <= TOL
+    r = wl.helmholtz_rhs(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    pz.helmholtz_z_setup(plan, w.a)
+    u = torch.from_numpy(r).cuda()
+    pz.helmholtz_z_solve(plan, u)
+    assert rel_err(u.cpu().numpy(), oracle.helmholtz_z_solve(zc, zf, w.a, r)) <= TOL
