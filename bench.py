@@ -1,0 +1,396 @@
+#!/usr/bin/env python
+"""bench.py -- FP64 Poisson + wall-normal Helmholtz grid points/s on B200, fraction of the HBM roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input: one pressure
+Poisson solve (steps a1..a5) plus the wall-normal Helmholtz solve of every velocity component
+(step a6) on the workload's grid.  Fields stay resident in HBM and are solved in place, step
+after step (the solution of one step is the right-hand side of the next; the kernels' cost does
+not depend on the values).  Every field is larger than the 126 MB L2, so no L2 flush is needed
+between iterations.
+
+Prints ONE JSON line.  With N > 1 (torchrun, one rank per GPU)
+every rank solves its own independent problem -- the path shards by replicating independent
+fields, no data-path collective -- and the value is the sum over ranks divided by the slowest
+rank's time ("weak" scaling).
+
+--impl reference times the CPU oracle (as it stands, never tuned) on the host cores on a bounded
+sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "FP64 Poisson+Helmholtz grid points/s on 1 B200; % of HBM roofline"
+UNIT = "grid points/s"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.lines = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+                pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample_shape(w, budget_pts):
+    """Largest power-of-two sub-grid of the workload (same recipe) with at most budget_pts points."""
+    nx, ny, nz = w.nx, w.ny, w.nz
+    while nx * ny * nz > budget_pts:
+        if nz >= nx and nz >= ny and nz > 16:
+            nz //= 2
+        elif nx >= ny and nx > 16:
+            nx //= 2
+        elif ny > 16:
+            ny //= 2
+        else:
+            break
+    return nx, ny, nz
+
+
+def run_oracle_step(w_s, zc, zf, f, rs):
+    import oracle
+
+    t0 = time.perf_counter()
+    if w_s.poisson:
+        oracle.poisson_solve(w_s.lx, w_s.ly, zc, zf, f, 1)
+    for r in rs:
+        oracle.helmholtz_z_solve(zc, zf, w_s.a, r)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(w, target_seconds=15.0):
+    """The oracle as it stands, timed on the host cores on a bounded sample of the workload."""
+    import oracle
+    from paper_2502_06296_b200 import workloads as wl
+
+    cores = oracle.num_threads()
+    fields = (1 if w.poisson else 0) + w.n_helmholtz
+    # calibrate on a small sub-grid, then pick the sample size for ~target_seconds
+    cal = wl.scaled(w, *oracle_sample_shape(w, 2 ** 21))
+    zc, zf = wl.grid(cal)
+    f = wl.poisson_rhs(cal) if cal.poisson else None
+    rs = [wl.helmholtz_rhs(cal, c) for c in range(cal.n_helmholtz)]
+    t_cal = run_oracle_step(cal, zc, zf, f, rs)
+    rate = fields * cal.n / t_cal
+    budget = min(w.n, max(cal.n, int(rate * target_seconds / fields)))
+    smp = wl.scaled(w, *oracle_sample_shape(w, budget))
+    zc, zf = wl.grid(smp)
+    f = wl.poisson_rhs(smp) if smp.poisson else None
+    rs = [wl.helmholtz_rhs(smp, c) for c in range(smp.n_helmholtz)]
+    t = run_oracle_step(smp, zc, zf, f, rs)
+    return {"value": fields * smp.n / t, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"1 step (1 Poisson + {w.n_helmholtz} Helmholtz solves, radix-2 FFT oracle variant) of the "
+                      f"{w.name} recipe on a {smp.nx}x{smp.ny}x{smp.nz} sub-grid, {t:.2f} s",
+            "seconds": t}
+
+
+def bench_reference(args, w):
+    """--impl reference: the oracle on the host cores, K steps, each a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    from paper_2502_06296_b200 import workloads as wl
+
+    fields = (1 if w.poisson else 0) + w.n_helmholtz
+    steps, warm = max(args.steps, 1), max(args.warmup, 0)
+    # size each step for about 60 s total
+    cal = wl.scaled(w, *oracle_sample_shape(w, 2 ** 21))
+    zc, zf = wl.grid(cal)
+    f = wl.poisson_rhs(cal) if cal.poisson else None
+    rs = [wl.helmholtz_rhs(cal, c) for c in range(cal.n_helmholtz)]
+    t_cal = run_oracle_step(cal, zc, zf, f, rs)
+    rate = fields * cal.n / t_cal
+    per_step = 60.0 / (steps + warm)
+    smp = wl.scaled(w, *oracle_sample_shape(w, min(w.n, max(2 ** 18, int(rate * per_step / fields)))))
+    zc, zf = wl.grid(smp)
+    f = wl.poisson_rhs(smp) if smp.poisson else None
+    rs = [wl.helmholtz_rhs(smp, c) for c in range(smp.n_helmholtz)]
+    for _ in range(warm):
+        run_oracle_step(smp, zc, zf, f, rs)
+    t = sum(run_oracle_step(smp, zc, zf, f, rs) for _ in range(steps))
+    value = fields * smp.n * steps / t
+    sample = (f"each step = 1 Poisson + {w.n_helmholtz} Helmholtz solves of the {w.name} recipe on a "
+              f"{smp.nx}x{smp.ny}x{smp.nz} sub-grid")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": warm, "ms_per_step": 1e3 * t / steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "sample_grid": [smp.nx, smp.ny, smp.nz]},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="c2", help="c1, c2 (default), c3 or c4 of BASELINE.json")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--option", action="append", default=[], help="key=value passed to pz_set_option")
+    args = ap.parse_args()
+
+    from paper_2502_06296_b200 import workloads as wl
+
+    w = wl.CONFIGS[args.workload]
+    if args.impl == "reference":
+        return bench_reference(args, w)
+
+    import numpy as np
+    import torch
+
+    from paper_2502_06296_b200 import binding as pz
+
+    pz.lib()  # fail loudly if the CUDA extension is missing
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; there is no CPU fallback")
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    steps, warm = max(args.steps, 1), max(args.warmup, 3)
+
+    # ---- synthetic inputs, resident in HBM (device-side seeded generators; rank-dependent seeds)
+    zc, zf = wl.grid(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    for kv in args.option:
+        k, v = kv.split("=")
+        pz.pz_set_option(plan, k, int(v))
+    fields = (1 if w.poisson else 0) + w.n_helmholtz
+    p = None
+    if w.poisson:
+        p = wl.device_remove_weighted_mean(wl.device_field(w, w.poisson_seed + 1000 * rank), zf)
+    us = [wl.device_field(w, s + 1000 * rank) for s in w.helmholtz_seeds]
+    if w.n_helmholtz:
+        pz.helmholtz_z_setup(plan, w.a)
+
+    def step():
+        if p is not None:
+            pz.poisson_solve(plan, p)
+        if us:
+            pz.helmholtz_z_solve_n(plan, us)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(warm):
+        step()
+    barrier()
+
+    # ---- timed region: exactly K steps, CUDA events on the launching stream, per-kernel events on
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    pz.pz_profile_enable(plan, True)
+    n0 = pz.pz_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(steps):
+        step()
+    ev1.record()
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    launches = pz.pz_launch_count() - n0
+    pz.pz_profile_enable(plan, False)
+    clocks = sampler.stop()
+    kernel_ms = {}
+    for ci, nm in enumerate(pz.KERNEL_CLASSES):
+        ms, cnt = pz.pz_profile_read(plan, ci)
+        if cnt:
+            kernel_ms[nm] = {"ms_total": ms, "launches": cnt, "ms_per_launch": ms / cnt}
+
+    t_max = ms_total
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_max = float(t.item())
+    value = fields * w.n * world * steps / (t_max * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        host = torch.empty(w.n, dtype=torch.float64).pin_memory()
+        host.copy_((p if p is not None else us[0]).flatten())
+        torch.cuda.synchronize()
+
+        def e2e_step():
+            if w.poisson:
+                pz.poisson_solve_host(plan, host)
+            for _ in range(w.n_helmholtz):
+                pz.helmholtz_z_solve_host(plan, host)
+
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.e2e_steps):
+            e2e_step()
+        e1.record()
+        barrier()
+        e_ms = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([e_ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e_ms = float(t.item())
+        e2e = {"value": fields * w.n * world * args.e2e_steps / (e_ms * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": fields * w.n * 8, "d2h_bytes_per_step": fields * w.n * 8,
+               "steps": args.e2e_steps, "ms_per_step": e_ms / args.e2e_steps,
+               "api": "poisson_solve_host + helmholtz_z_solve_host (pinned host buffers)"}
+        del host
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (largest share of the step), live event timings
+    peak, peak_src = measured_peak()
+    dom = max(kernel_ms, key=lambda k: kernel_ms[k]["ms_total"])
+    bytes_per_launch = {  # algorithmic: every kernel reads and writes each of its points once
+        nm: 16.0 * w.n * (steps * (w.n_helmholtz if nm == "helmholtz" else 1)) / kernel_ms[nm]["launches"]
+        for nm in kernel_ms if not nm.startswith("pair0")}
+    achieved = bytes_per_launch[dom] / (kernel_ms[dom]["ms_per_launch"] * 1e-3) / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(args.workload, {}).get(dom)
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": bytes_per_launch[dom],
+                "share_of_step": kernel_ms[dom]["ms_total"] / ms_total}
+    # whole-step figures: 48 B/pt structural minimum for Poisson (3 sweeps), 16 B/pt per Helmholtz field
+    step_bytes = ((48.0 if w.poisson else 0.0) + 16.0 * w.n_helmholtz) * w.n
+    step_frac = step_bytes * steps / (ms_total * 1e-3) / 1e9 / peak
+    per_kernel = {nm: {"ms_per_launch": round(v["ms_per_launch"], 5), "launches_per_step": v["launches"] / steps,
+                       "share": round(v["ms_total"] / ms_total, 4),
+                       "GBps_algorithmic": (round(bytes_per_launch[nm] / (v["ms_per_launch"] * 1e-3) / 1e9, 1)
+                                            if nm in bytes_per_launch else None)}
+                  for nm, v in kernel_ms.items()}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
+        "ms_per_step": t_max / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "fields_per_step": fields,
+                   "step": f"{1 if w.poisson else 0} Poisson solve + {w.n_helmholtz} Helmholtz solves, in place",
+                   "l2": "every field (%.2f GB) is larger than the 126 MB L2; no flush" % (w.n * 8 / 1e9),
+                   "parallelism": "replicas" if world > 1 else "single GPU",
+                   "options": args.option},
+        "clocks": clocks, "gpu_launches": launches,
+        "roofline": roofline,
+        "hbm_roofline_step": {"bytes_per_step": step_bytes, "frac": step_frac,
+                              "model": "48 B/pt Poisson (3 read+write sweeps) + 16 B/pt per Helmholtz field",
+                              "strict_16B_poisson_frac": ((16.0 * fields) * w.n * steps / (ms_total * 1e-3) / 1e9 / peak)},
+        "kernels": per_kernel,
+    }
+    if e2e is not None:
+        line["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        # free the device first: nothing depends on it, and the oracle only uses host memory
+        line["cpu_baseline"] = cpu_baseline(w)
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

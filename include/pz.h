@@ -134,6 +134,20 @@ PZ_API int pz_poisson_stage(pz_plan *plan, double *p, int stage, void *stream);
 PZ_API int pz_set_option(pz_plan *plan, const char *key, int value);
 PZ_API int pz_get_option(const pz_plan *plan, const char *key, int *value);
 
+/* Per-kernel device timing for the benchmark's roofline figures.  While enabled, every kernel
+ * launch of this plan is bracketed by a pair of CUDA events recorded on the launching stream
+ * (no host synchronisation, a few microseconds of stream time per launch).
+ * pz_profile_enable(plan, 1) clears the records and starts; (plan, 0) stops.
+ * pz_profile_read synchronises on the recorded events and returns, for one kernel class, the
+ * summed device time in milliseconds and the number of launches.  Not capturable in a graph. */
+enum pz_kernel_class {
+    PZ_K_FFT_X_FWD = 0, PZ_K_FFT_Y_FWD = 1, PZ_K_PAIR0_FWD = 2, PZ_K_Z_SOLVE = 3,
+    PZ_K_PAIR0_INV = 4, PZ_K_FFT_Y_INV = 5, PZ_K_FFT_X_INV = 6, PZ_K_HELMHOLTZ = 7,
+    PZ_K_COUNT = 8
+};
+PZ_API int pz_profile_enable(pz_plan *plan, int on);
+PZ_API int pz_profile_read(pz_plan *plan, int kernel_class, double *total_ms, long long *launches);
+
 /* Number of kernels this library has launched since it was loaded (host-side counter). */
 PZ_API long long pz_launch_count(void);
 

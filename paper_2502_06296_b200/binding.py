@@ -37,6 +37,8 @@ SIGNATURES = {
     "pz_poisson_stage": (_i, [_vp, _vp, _i, _vp]),
     "pz_set_option": (_i, [_vp, ctypes.c_char_p, _i]),
     "pz_get_option": (_i, [_vp, ctypes.c_char_p, ctypes.POINTER(_i)]),
+    "pz_profile_enable": (_i, [_vp, _i]),
+    "pz_profile_read": (_i, [_vp, _i, ctypes.POINTER(_d), ctypes.POINTER(ctypes.c_longlong)]),
     "pz_launch_count": (ctypes.c_longlong, []),
     "pz_version": (_i, []),
 }
@@ -175,6 +177,20 @@ def pz_get_option(plan: Plan, key: str) -> int:
     v = _i()
     _check(lib().pz_get_option(plan.handle, key.encode(), ctypes.byref(v)))
     return v.value
+
+
+KERNEL_CLASSES = ("fft_x_fwd", "fft_y_fwd", "pair0_fwd", "z_solve", "pair0_inv", "fft_y_inv", "fft_x_inv", "helmholtz")
+
+
+def pz_profile_enable(plan: Plan, on: bool) -> None:
+    _check(lib().pz_profile_enable(plan.handle, 1 if on else 0))
+
+
+def pz_profile_read(plan: Plan, kernel_class: int):
+    """-> (summed device milliseconds, launches) of one kernel class since pz_profile_enable(plan, True)."""
+    ms, cnt = _d(), ctypes.c_longlong()
+    _check(lib().pz_profile_read(plan.handle, int(kernel_class), ctypes.byref(ms), ctypes.byref(cnt)))
+    return ms.value, cnt.value
 
 
 def pz_launch_count() -> int:

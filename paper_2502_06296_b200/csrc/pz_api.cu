@@ -30,6 +30,28 @@ int cuda_fail(cudaError_t e, const char *what)
 
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+static cudaEvent_t prof_event(pz_plan *pl)
+{
+    cudaEvent_t e = nullptr;
+    if (!pl->prof_pool.empty()) { e = pl->prof_pool.back(); pl->prof_pool.pop_back(); return e; }
+    if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return e;
+}
+
+ProfScope::ProfScope(const pz_plan *plan, int cls, cudaStream_t stream) : pl(const_cast<pz_plan *>(plan)), st(stream)
+{
+    if (!pl->prof_on) return;
+    cudaEvent_t a = prof_event(pl), b = prof_event(pl);
+    if (!a || !b) return;
+    cudaEventRecord(a, st);
+    pl->prof_recs.push_back({cls, a, b});
+    stop = b;
+}
+ProfScope::~ProfScope()
+{
+    if (stop) cudaEventRecord(stop, st);
+}
+
 namespace {
 
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
@@ -242,6 +264,8 @@ int poisson_plan_destroy(pz_plan *pl)
     }
     if (pl->helm_host) cudaFreeHost(pl->helm_host);
     if (pl->upload_stream) cudaStreamDestroy(pl->upload_stream);
+    for (auto &r : pl->prof_recs) { cudaEventDestroy(r.start); cudaEventDestroy(r.stop); }
+    for (auto e : pl->prof_pool) cudaEventDestroy(e);
     cudaGetLastError();
     delete pl;
     return PZ_OK;
@@ -331,6 +355,35 @@ int helmholtz_z_solve_host(pz_plan *pl, double *u_host, void *stream)
     PZ_CUDA(cudaMemcpyAsync(pl->d_host_stage, u_host, pl->n * sizeof(double), cudaMemcpyHostToDevice, st));
     if ((rc = helmholtz_z_solve(pl, pl->d_host_stage, stream)) != PZ_OK) return rc;
     PZ_CUDA(cudaMemcpyAsync(u_host, pl->d_host_stage, pl->n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    return PZ_OK;
+}
+
+int pz_profile_enable(pz_plan *pl, int on)
+{
+    if (!pl) { set_error("pz_profile_enable: plan is NULL"); return PZ_EINVAL; }
+    if (on) {
+        for (auto &r : pl->prof_recs) { pl->prof_pool.push_back(r.start); pl->prof_pool.push_back(r.stop); }
+        pl->prof_recs.clear();
+    }
+    pl->prof_on = (on != 0);
+    return PZ_OK;
+}
+
+int pz_profile_read(pz_plan *pl, int cls, double *total_ms, long long *launches)
+{
+    if (!pl || !total_ms || !launches || cls < 0 || cls >= PZ_K_COUNT) { set_error("pz_profile_read: bad argument"); return PZ_EINVAL; }
+    double sum = 0.0;
+    long long cnt = 0;
+    for (auto &r : pl->prof_recs) {
+        if (r.cls != cls) continue;
+        PZ_CUDA(cudaEventSynchronize(r.stop));
+        float ms = 0.f;
+        PZ_CUDA(cudaEventElapsedTime(&ms, r.start, r.stop));
+        sum += ms;
+        ++cnt;
+    }
+    *total_ms = sum;
+    *launches = cnt;
     return PZ_OK;
 }
 

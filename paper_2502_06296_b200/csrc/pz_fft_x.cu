@@ -116,6 +116,7 @@ int launch_m(const pz_plan *pl, double *p, long long nlines, cudaStream_t st)
     static_assert(smem <= 48 * 1024, "x-FFT exchange buffer must fit the default shared-memory limit");
     const long long blocks = (nlines + LPB - 1) / LPB;
     const double scale = 1.0 / ((double)pl->nx * (double)pl->ny);
+    ProfScope prof(pl, INV ? PZ_K_FFT_X_INV : PZ_K_FFT_X_FWD, st);
     fft_x_kernel<M, LPB, INV><<<(unsigned)blocks, threads, smem, st>>>(p, pl->d_twx, nlines, scale);
     count_launch();
     PZ_CUDA(cudaGetLastError());

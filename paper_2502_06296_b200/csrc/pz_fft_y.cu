@@ -106,6 +106,7 @@ int launch_ltc(const pz_plan *pl, double *p, int nk, cudaStream_t st)
         attr_done = true;
     }
     dim3 grid((unsigned)(pl->nx / 2 / TC), (unsigned)nk);
+    ProfScope prof(pl, INV ? PZ_K_FFT_Y_INV : PZ_K_FFT_Y_FWD, st);
     fft_y_kernel<L, TC, INV><<<grid, threads, smem, st>>>(p, pl->d_twy, pl->nx);
     count_launch();
     PZ_CUDA(cudaGetLastError());
@@ -179,6 +180,7 @@ int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cud
         PZ_CUDA(cudaFuncSetAttribute(pair0_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
         attr_done = true;
     }
+    ProfScope prof(pl, inverse ? PZ_K_PAIR0_INV : PZ_K_PAIR0_FWD, st);
     if (inverse)
         pair0_kernel<true><<<(unsigned)nk, threads, smem, st>>>(base, pl->nx, pl->ny);
     else

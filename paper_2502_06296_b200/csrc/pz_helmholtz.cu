@@ -252,6 +252,7 @@ int launch_helmholtz(pz_plan *pl, double *u, cudaStream_t st)
     const unsigned blocks = (unsigned)(plane / tx);
     const size_t smem = 2 * (size_t)(2 * P) * tx * sizeof(double);
     const int threads = tx * P;
+    ProfScope prof(pl, PZ_K_HELMHOLTZ, st);
     switch (pl->helm_m) {
     case 4: helmholtz_kernel<4><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); break;
     case 8: helmholtz_kernel<8><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); break;

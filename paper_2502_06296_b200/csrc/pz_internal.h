@@ -67,6 +67,12 @@ struct pz_plan {
     size_t helm_host_bytes = 0;
 
     pz::Options opt;
+
+    // optional per-launch event timing (pz_profile_enable)
+    bool prof_on = false;
+    struct ProfRec { int cls; cudaEvent_t start, stop; };
+    std::vector<ProfRec> prof_recs;
+    std::vector<cudaEvent_t> prof_pool;
 };
 
 namespace pz {
@@ -80,6 +86,13 @@ void count_launch(int n = 1);
         cudaError_t e__ = (call);                                                                  \
         if (e__ != cudaSuccess) return ::pz::cuda_fail(e__, #call);                                \
     } while (0)
+
+// Brackets one kernel launch with events when profiling is on.
+struct ProfScope {
+    pz_plan *pl; cudaStream_t st; cudaEvent_t stop = nullptr;
+    ProfScope(const pz_plan *plan, int cls, cudaStream_t stream);
+    ~ProfScope();
+};
 
 // kernels (each returns a pz_status)
 int launch_fft_x(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);

@@ -86,6 +86,7 @@ int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st)
     }
     const size_t plane = (size_t)pl->nx * pl->ny;
     const unsigned blocks = (unsigned)((plane + 127) / 128);
+    ProfScope prof(pl, PZ_K_Z_SOLVE, st);
     zsolve_thomas_kernel<<<blocks, 128, 0, st>>>(p, pl->d_zwork, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
                                                   pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, pl->nz, pl->inv_lz);
     count_launch();

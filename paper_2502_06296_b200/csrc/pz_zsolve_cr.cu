@@ -256,6 +256,7 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st)
     }
     const size_t plane = (size_t)pl->nx * pl->ny;
     const unsigned blocks = (unsigned)(plane / kTX);
+    ProfScope prof(pl, PZ_K_Z_SOLVE, st);
     zsolve_cr_kernel<M><<<blocks, kPairs * kLanes, smem, st>>>(p, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
                                                                 pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny,
                                                                 pl->nz, pl->inv_lz);
