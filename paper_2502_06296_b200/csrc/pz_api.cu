@@ -113,11 +113,10 @@ int ensure_zwork(pz_plan *pl)
 int slab_planes(const pz_plan *pl)
 {
     if (pl->opt.slab_planes > 0) return pl->opt.slab_planes < pl->nz ? pl->opt.slab_planes : pl->nz;
-    // auto: keep a slab of planes (x- then y-transformed back to back) inside the 126 MB L2
-    const size_t plane_bytes = (size_t)pl->nx * pl->ny * sizeof(double);
-    size_t sp = (32u << 20) / plane_bytes;
-    if (sp < 1) sp = 1;
-    if (sp > (size_t)pl->nz) sp = pl->nz;
+    // auto: one launch per transform direction over the whole field.  (Slabs of planes that stay
+    // inside the 126 MB L2 between the x and y transforms save HBM traffic but, as separate small
+    // launches, lose more to launch tails than they save: profiles/r01a.)
+    size_t sp = (size_t)pl->nz;
     return (int)sp;
 }
 

@@ -103,7 +103,11 @@ __host__ __device__ constexpr int bitrev(int p, int bits)
 
 // Twiddle + butterflies of one pass, in registers.  tw[k] = exp(-2 pi i k / LT), k < LT, where
 // LT is a multiple of L (table stride LT/L lets the x kernels share the length-n table).
-template <int L, int E, int R, int NS, int TWSTRIDE>
+// TWMODE 0: every twiddle w^{r jm} is looked up (cheap when all lanes of a warp share jm: the y
+// kernels).  TWMODE 1: only w^{jm}, w^{2jm}, w^{4jm}, w^{8jm} are looked up and the other powers are
+// products of two of them (one rounding more; the x kernels, whose lanes hit 16-32 different
+// table lines per lookup and would otherwise be bound by L1 wavefronts).
+template <int L, int E, int R, int NS, int TWSTRIDE, int TWMODE>
 __device__ __forceinline__ void pass_butterflies(double2 (&v)[E], int tid, const double2 *__restrict__ tw)
 {
     constexpr int T = L / E, S = E / R;
@@ -112,10 +116,27 @@ __device__ __forceinline__ void pass_butterflies(double2 (&v)[E], int tid, const
     for (int b = 0; b < S; ++b) {
         if constexpr (NS > 1) {
             const int jm = (tid + b * T) & (NS - 1);
+            constexpr int STEP = (L / (NS * R)) * TWSTRIDE;
+            if constexpr (TWMODE == 0 || R <= 2) {
 #pragma unroll
-            for (int r = 1; r < R; ++r) {
-                const double2 w = __ldg(&tw[r * jm * (L / (NS * R)) * TWSTRIDE]);
-                v[b + r * S] = cmul(v[b + r * S], w);
+                for (int r = 1; r < R; ++r) {
+                    const double2 w = __ldg(&tw[r * jm * STEP]);
+                    v[b + r * S] = cmul(v[b + r * S], w);
+                }
+            } else {
+                double2 w[R];
+#pragma unroll
+                for (int r = 1; r < R; r *= 2) w[r] = __ldg(&tw[r * jm * STEP]);
+#pragma unroll
+                for (int r = 3; r < R; ++r) {
+                    if ((r & (r - 1)) != 0) { // not a power of two: highest set bit times the rest
+                        int hb = 1;
+                        while (hb * 2 <= r) hb *= 2;
+                        w[r] = cmul(w[hb], w[r - hb]);
+                    }
+                }
+#pragma unroll
+                for (int r = 1; r < R; ++r) v[b + r * S] = cmul(v[b + r * S], w[r]);
             }
         }
         dif<R, S>(&v[b]);
@@ -172,14 +193,14 @@ PZ_FFT_PLAN(4096, 16, 16, 16, 16)
 //   xchg.get(pos)         load it back
 //   xchg.sync()           barrier covering every thread that shares the buffer
 // On return v[e] = X[tid + e T] (natural order).
-template <int L, int TWSTRIDE, class Xchg>
+template <int L, int TWSTRIDE, int TWMODE, class Xchg>
 __device__ __forceinline__ void fft_line(double2 (&v)[FftPlan<L>::E], int tid, const double2 *__restrict__ tw,
                                          Xchg &xchg)
 {
     using P = FftPlan<L>;
     constexpr int E = P::E, T = P::T, R1 = P::R1, R2 = P::R2, R3 = P::R3;
 
-    pass_butterflies<L, E, R1, 1, TWSTRIDE>(v, tid, tw);
+    pass_butterflies<L, E, R1, 1, TWSTRIDE, TWMODE>(v, tid, tw);
     if constexpr (R2 == 1) {
         unscramble<E, R1>(v);
         return;
@@ -195,7 +216,7 @@ __device__ __forceinline__ void fft_line(double2 (&v)[FftPlan<L>::E], int tid, c
         xchg.sync();
 #pragma unroll
         for (int e = 0; e < E; ++e) v[e] = xchg.get(tid + e * T);
-        pass_butterflies<L, E, R2, R1, TWSTRIDE>(v, tid, tw);
+        pass_butterflies<L, E, R2, R1, TWSTRIDE, TWMODE>(v, tid, tw);
         if constexpr (R3 == 1) {
             unscramble<E, R2>(v);
             return;
@@ -212,7 +233,7 @@ __device__ __forceinline__ void fft_line(double2 (&v)[FftPlan<L>::E], int tid, c
             xchg.sync();
 #pragma unroll
             for (int e = 0; e < E; ++e) v[e] = xchg.get(tid + e * T);
-            pass_butterflies<L, E, R3, R1 * R2, TWSTRIDE>(v, tid, tw);
+            pass_butterflies<L, E, R3, R1 * R2, TWSTRIDE, TWMODE>(v, tid, tw);
             unscramble<E, R3>(v);
         }
     }

@@ -27,7 +27,7 @@ struct XchgY {
 };
 
 template <int L, int TC, bool INV>
-__global__ void __launch_bounds__(FftPlan<L>::T *TC)
+__global__ void __launch_bounds__(FftPlan<L>::T *TC, (FftPlan<L>::T * TC <= 256) ? 2 : 1)
     fft_y_kernel(double *__restrict__ p, const double2 *__restrict__ tw, int nx)
 {
     using P = FftPlan<L>;
@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(FftPlan<L>::T *TC)
         const double2 t = *reinterpret_cast<const double2 *>(base + (size_t)(tid + e * T) * nx);
         v[e] = INV ? cconj(t) : t;
     }
-    fft_line<L, 1>(v, tid, tw, xc);
+    fft_line<L, 1, 0>(v, tid, tw, xc);
 #pragma unroll
     for (int e = 0; e < E; ++e)
         *reinterpret_cast<double2 *>(base + (size_t)(tid + e * T) * nx) = INV ? cconj(v[e]) : v[e];

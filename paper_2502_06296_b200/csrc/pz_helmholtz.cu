@@ -31,24 +31,30 @@ namespace {
 //   [4nzp, 5nzp)    rc_k  = c_i / b_i
 //   [5nzp, +LV*2*n2)   per level l and reduced row r: k1, k2 (d_r += k1 d_{r-h} + k2 d_{r+h})
 //   then n2         rbr_r = 1 / b_r after the last level
-template <int M>
-__global__ void __launch_bounds__(M >= 16 ? 512 : 1024)
+// Threads per CTA = tx * P.  Register budget per sub-domain size (whole tile lives in registers):
+// m <= 16: 64 registers (up to 1024 threads per SM), m = 32: 128 registers.
+template <int M> struct HelmLimits {
+    static constexpr int kMaxThreads = (M >= 32) ? 256 : 512;
+    static constexpr int kMinBlocks = 2;
+};
+
+template <int M, bool FULL>
+__global__ void __launch_bounds__(HelmLimits<M>::kMaxThreads, HelmLimits<M>::kMinBlocks)
     helmholtz_kernel(double *__restrict__ u, const double *__restrict__ tab, size_t plane, int nz, int P,
                      int levels, int tx)
 {
     extern __shared__ double smem_h[]; // 2 buffers x (2P rows) x tx
     const int c = threadIdx.x % tx, s = threadIdx.x / tx;
-    const size_t col = (size_t)blockIdx.x * tx + c;
     const int nzp = P * M, n2 = 2 * P;
     const int k0 = s * M;
     const double *fA = tab + k0, *bC = tab + nzp + k0, *rb = tab + 2 * nzp + k0;
     const double *ra = tab + 3 * nzp + k0, *rc = tab + 4 * nzp + k0;
     const double *pcr = tab + 5 * (size_t)nzp;
-    double *up = u + col;
+    double *up = u + ((size_t)blockIdx.x * tx + c) + (size_t)k0 * plane;
 
     double d[M];
 #pragma unroll
-    for (int i = 0; i < M; ++i) d[i] = (k0 + i < nz) ? up[(size_t)(k0 + i) * plane] : 0.0;
+    for (int i = 0; i < M; ++i) d[i] = (FULL || k0 + i < nz) ? up[(size_t)i * plane] : 0.0;
 
     // Step 2: runtime reduction, d only
 #pragma unroll
@@ -57,23 +63,21 @@ __global__ void __launch_bounds__(M >= 16 ? 512 : 1024)
     for (int i = M - 3; i >= 0; --i) d[i] = fma(-__ldg(&bC[i]), d[i + 1], d[i]);
 
     // Step 3: boundary system, rows (2s, 2s+1) = (first, last) row of sub-domain s
-    double *buf0 = smem_h, *buf1 = smem_h + (size_t)n2 * tx;
+    double *cur = smem_h, *nxt = smem_h + (size_t)n2 * tx;
     double x0 = d[0], x1 = d[M - 1];
-    buf0[(2 * s) * tx + c] = x0;
-    buf0[(2 * s + 1) * tx + c] = x1;
+    const int r0 = 2 * s, r1 = 2 * s + 1;
+    cur[r0 * tx + c] = x0;
+    cur[r1 * tx + c] = x1;
     __syncthreads();
-    double *cur = buf0, *nxt = buf1;
     int h = 1;
     for (int l = 0; l < levels; ++l, h *= 2) {
         const double *kk = pcr + (size_t)l * 2 * n2;
-        const int r0 = 2 * s, r1 = 2 * s + 1;
-        double y0 = x0, y1 = x1;
-        if (r0 - h >= 0) y0 = fma(__ldg(&kk[2 * r0]), cur[(r0 - h) * tx + c], y0);
-        if (r0 + h < n2) y0 = fma(__ldg(&kk[2 * r0 + 1]), cur[(r0 + h) * tx + c], y0);
-        if (r1 - h >= 0) y1 = fma(__ldg(&kk[2 * r1]), cur[(r1 - h) * tx + c], y1);
-        if (r1 + h < n2) y1 = fma(__ldg(&kk[2 * r1 + 1]), cur[(r1 + h) * tx + c], y1);
-        x0 = y0;
-        x1 = y1;
+        // multipliers are zero where the partner row does not exist; clamp the index instead of branching
+        const int a0 = max(r0 - h, 0), b0 = min(r0 + h, n2 - 1), a1 = max(r1 - h, 0), b1 = min(r1 + h, n2 - 1);
+        const double2 k0v = __ldg(reinterpret_cast<const double2 *>(kk) + r0);
+        const double2 k1v = __ldg(reinterpret_cast<const double2 *>(kk) + r1);
+        x0 = fma(k0v.x, cur[a0 * tx + c], fma(k0v.y, cur[b0 * tx + c], x0));
+        x1 = fma(k1v.x, cur[a1 * tx + c], fma(k1v.y, cur[b1 * tx + c], x1));
         if (l + 1 < levels) {
             nxt[r0 * tx + c] = x0;
             nxt[r1 * tx + c] = x1;
@@ -82,19 +86,19 @@ __global__ void __launch_bounds__(M >= 16 ? 512 : 1024)
         }
     }
     {
-        const double *rbr = pcr + (size_t)levels * 2 * n2;
-        x0 *= __ldg(&rbr[2 * s]);
-        x1 *= __ldg(&rbr[2 * s + 1]);
+        const double2 rbr = __ldg(reinterpret_cast<const double2 *>(pcr + (size_t)levels * 2 * n2) + s);
+        x0 *= rbr.x;
+        x1 *= rbr.y;
     }
 
     // Step 4: reconstruct in place and store
-    if (k0 < nz) up[(size_t)k0 * plane] = x0;
+    if (FULL || k0 < nz) up[0] = x0;
 #pragma unroll
     for (int i = 1; i < M - 1; ++i) {
         const double v = fma(-__ldg(&rc[i]), x1, fma(-__ldg(&ra[i]), x0, __ldg(&rb[i]) * d[i]));
-        if (k0 + i < nz) up[(size_t)(k0 + i) * plane] = v;
+        if (FULL || k0 + i < nz) up[(size_t)i * plane] = v;
     }
-    if (k0 + M - 1 < nz) up[(size_t)(k0 + M - 1) * plane] = x1;
+    if (FULL || k0 + M - 1 < nz) up[(size_t)(M - 1) * plane] = x1;
 }
 
 int ilog2_ceil(int n)
@@ -113,9 +117,9 @@ static void helm_geometry(pz_plan *pl)
     if (m != 4 && m != 8 && m != 16 && m != 32) m = (pl->nz <= 128) ? 4 : (pl->nz <= 256) ? 8 : (pl->nz <= 512 ? 16 : 32);
     int P = (pl->nz + m - 1) / m;
     int tx = pl->opt.helm_tx;
-    if (tx != 4 && tx != 8 && tx != 16 && tx != 32) tx = 16;
-    while (m < 32 && 4 * P > 1024) { m *= 2; P = (pl->nz + m - 1) / m; }
-    const int limit = (m >= 16) ? 512 : 1024; // __launch_bounds__ of helmholtz_kernel<m>
+    if (tx != 4 && tx != 8 && tx != 16 && tx != 32) tx = 8;
+    while (m < 32 && 4 * P > 512) { m *= 2; P = (pl->nz + m - 1) / m; }
+    const int limit = (m >= 32) ? 256 : 512; // __launch_bounds__ of helmholtz_kernel<m>
     while (tx > 4 && tx * P > limit) tx /= 2;
     pl->helm_m = m;
     pl->helm_P = P;
@@ -129,8 +133,8 @@ int helmholtz_build_tables(pz_plan *pl, double a)
     typedef long double ld;
     helm_geometry(pl);
     const int nz = pl->nz, m = pl->helm_m, P = pl->helm_P, nzp = P * m, n2 = 2 * P, LV = pl->helm_levels;
-    if (pl->helm_tx * P > ((m >= 16) ? 512 : 1024)) {
-        set_error("helmholtz: nz = %d needs more than 1024 threads per CTA", nz);
+    if (pl->helm_tx * P > ((m >= 32) ? 256 : 512)) {
+        set_error("helmholtz: nz = %d is too large for the register-tile kernel (P = %d sub-domains)", nz, P);
         return PZ_EUNSUPPORTED;
     }
     const size_t ndbl = 5 * (size_t)nzp + (size_t)LV * 2 * n2 + n2;
@@ -253,13 +257,20 @@ int launch_helmholtz(pz_plan *pl, double *u, cudaStream_t st)
     const size_t smem = 2 * (size_t)(2 * P) * tx * sizeof(double);
     const int threads = tx * P;
     ProfScope prof(pl, PZ_K_HELMHOLTZ, st);
+    const bool full = (P * pl->helm_m == pl->nz);
+#define PZ_HELM_LAUNCH(MM)                                                                                       \
+    do {                                                                                                         \
+        if (full) helmholtz_kernel<MM, true><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); \
+        else helmholtz_kernel<MM, false><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx);    \
+    } while (0)
     switch (pl->helm_m) {
-    case 4: helmholtz_kernel<4><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); break;
-    case 8: helmholtz_kernel<8><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); break;
-    case 16: helmholtz_kernel<16><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); break;
-    case 32: helmholtz_kernel<32><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); break;
+    case 4: PZ_HELM_LAUNCH(4); break;
+    case 8: PZ_HELM_LAUNCH(8); break;
+    case 16: PZ_HELM_LAUNCH(16); break;
+    case 32: PZ_HELM_LAUNCH(32); break;
     default: set_error("helmholtz: bad sub-domain size %d", pl->helm_m); return PZ_EINVAL;
     }
+#undef PZ_HELM_LAUNCH
     count_launch();
     PZ_CUDA(cudaGetLastError());
     if (!capturing) PZ_CUDA(cudaEventRecord(t.last_use, st));

@@ -42,6 +42,15 @@ __device__ __forceinline__ double shfl_down(double v, int d) { return __shfl_dow
 // (row stride kTX/2 double2).  al/ga: this lane's alpha_i, gamma_i (sub-/super-diagonal
 // magnitudes, zero on padding rows and at the walls) in shared memory.  MASK bit 0 / 1: which
 // component (x / y of the double2) is solved and written back.
+//
+// Sweeps (Algorithm 1 re-ordered so that only the pivot reciprocals are thread-private):
+//   A  rows M-2..1, read only: UL elimination -> this sub-domain's row 0 in terms of
+//      (x_{M-1} of the previous lane, x_0, x_{M-1})
+//   B  rows 1..M-1, read only: LU elimination -> row M-1 in terms of (x_0, x_{M-1}, next x_0);
+//      keeps rb_i = 1/pivot_i in registers.  A and B run interleaved (two independent chains).
+//   reduced system across lanes (warp shuffles, parallel cyclic reduction)
+//   C  rows 1..M-2 forward: g_i = (r_i + alpha_i g_{i-1}) rb_i with g_0 := x_0  (overwrites the tile)
+//   D  rows M-2..1 backward: x_i = g_i + gamma_i rb_i x_{i+1}
 template <int M, int MASK, bool pin>
 __device__ __forceinline__ void solve_pair(double2 *d, const double *al, const double *ga, double sigma,
                                            int k0, int nz, const double *__restrict__ dzf, double inv_lz)
@@ -57,20 +66,40 @@ __device__ __forceinline__ void solve_pair(double2 *d, const double *al, const d
         return live ? make_double2(-v.x, -v.y) : make_double2(0.0, 0.0);
     };
 
-    // ---- UL sweep (read only), rows M-2 .. 1: Schur complement of the interior onto row 0
+    // ---- sweeps A (UL, descending) and B (LU, ascending), interleaved
+    double rb[M];
     double chat = ga[M - 2], eps2 = eps_of(M - 2);
     double2 rp2 = rhs_of(M - 2);
     double rb2 = fast_rcp(alpha_of(M - 2) + chat + eps2);
+    double ahat = alpha_of(1), eps = eps_of(1);
+    double2 rp = rhs_of(1);
+    rb[1] = fast_rcp(ahat + ga[1] + eps);
 #pragma unroll
-    for (int i = M - 3; i >= 1; --i) {
-        const double nn = ga[i] * rb2;
-        const double2 r = rhs_of(i);
-        chat = nn * chat;
-        eps2 = fma(nn, eps2, eps_of(i));
-        rp2.x = fma(nn, rp2.x, r.x);
-        rp2.y = fma(nn, rp2.y, r.y);
-        rb2 = fast_rcp(alpha_of(i) + chat + eps2);
+    for (int t = 0; t < M - 2; ++t) {
+        {   // A: row i = M-3-t (for t < M-3)
+            const int i = M - 3 - t;
+            if (i >= 1) {
+                const double nn = ga[i] * rb2;
+                const double2 r = rhs_of(i);
+                chat = nn * chat;
+                eps2 = fma(nn, eps2, eps_of(i));
+                rp2.x = fma(nn, rp2.x, r.x);
+                rp2.y = fma(nn, rp2.y, r.y);
+                rb2 = fast_rcp(alpha_of(i) + chat + eps2);
+            }
+        }
+        {   // B: row i = 2+t
+            const int i = 2 + t;
+            const double mm = alpha_of(i) * rb[i - 1];
+            const double2 r = rhs_of(i);
+            ahat = mm * ahat;
+            eps = fma(mm, eps, eps_of(i));
+            rp.x = fma(mm, rp.x, r.x);
+            rp.y = fma(mm, rp.y, r.y);
+            rb[i] = fast_rcp(ahat + ga[i] + eps);
+        }
     }
+    // normalised row 0:  -a0 X_{s-1} + x_0 - c0 X_s = r0, excess e0
     double a0, c0, e0;
     double2 r0;
     {
@@ -81,42 +110,12 @@ __device__ __forceinline__ void solve_pair(double2 *d, const double *al, const d
         e0 = fma(nn, eps2, eps_of(0));
         r0.x = fma(nn, rp2.x, r.x);
         r0.y = fma(nn, rp2.y, r.y);
-        const double rb = fast_rcp(a0 + c0 + e0);
-        a0 *= rb; c0 *= rb; e0 *= rb; r0.x *= rb; r0.y *= rb;
+        const double rbn = fast_rcp(a0 + c0 + e0);
+        a0 *= rbn; c0 *= rbn; e0 *= rbn; r0.x *= rbn; r0.y *= rbn;
     }
-
-    // ---- LU sweep, rows 1 .. M-1: x_i = Rn_i + Ah_i x_0 + W_i x_{i+1}; Rn overwrites the tile
-    double Ah[M], W[M];
-    double ahat = alpha_of(1), eps = eps_of(1);
-    double2 rp = rhs_of(1);
-    double rb = fast_rcp(ahat + ga[1] + eps);
-    Ah[1] = ahat * rb;
-    W[1] = ga[1] * rb;
-    {
-        double2 t = d[1 * RS];
-        if (MASK & 1) t.x = rp.x * rb;
-        if (MASK & 2) t.y = rp.y * rb;
-        d[1 * RS] = t;
-    }
-#pragma unroll
-    for (int i = 2; i < M; ++i) {
-        const double mm = alpha_of(i) * rb;
-        const double2 r = rhs_of(i);
-        ahat = mm * ahat;
-        eps = fma(mm, eps, eps_of(i));
-        rp.x = fma(mm, rp.x, r.x);
-        rp.y = fma(mm, rp.y, r.y);
-        rb = fast_rcp(ahat + ga[i] + eps);
-        Ah[i] = ahat * rb;
-        W[i] = ga[i] * rb;
-        double2 t = d[i * RS];
-        if (MASK & 1) t.x = rp.x * rb;
-        if (MASK & 2) t.y = rp.y * rb;
-        d[i * RS] = t;
-    }
-    // last row of the sub-domain, normalised: -a x_0 + x_{M-1} - c x_{next 0} = r, excess e
-    double a = Ah[M - 1], c = W[M - 1], e = eps * rb;
-    double2 r = make_double2(rp.x * rb, rp.y * rb);
+    // normalised last row:  -a x_0 + X_s - c (next lane's x_0) = r, excess e
+    double a = ahat * rb[M - 1], c = ga[M - 1] * rb[M - 1], e = eps * rb[M - 1];
+    double2 r = make_double2(rp.x * rb[M - 1], rp.y * rb[M - 1]);
 
     // ---- reduced system: first eliminate the x_0 unknowns (local row 0 and the next lane's)
     {
@@ -149,27 +148,48 @@ __device__ __forceinline__ void solve_pair(double2 *d, const double *al, const d
     }
     // r = X_s.  x_0 of this lane from its normalised row 0:  x_0 = r0 + a0 X_{s-1} + c0 X_s
     const double xpx = shfl_up(r.x, 1), xpy = shfl_up(r.y, 1); // lane 0: a0 = 0
-    double2 x0 = make_double2(fma(a0, xpx, fma(c0, r.x, r0.x)), fma(a0, xpy, fma(c0, r.y, r0.y)));
+    const double2 x0 = make_double2(fma(a0, xpx, fma(c0, r.x, r0.x)), fma(a0, xpy, fma(c0, r.y, r0.y)));
 
-    // ---- reconstruct the interior (back substitution with the stored LU rows)
-    double2 x = r;
     double2 wsum = make_double2(0.0, 0.0);
     auto put = [&](int i, double2 val) {
-        double2 t = d[i * RS];
-        if (MASK & 1) t.x = val.x;
-        if (MASK & 2) t.y = val.y;
+        double2 t = val;
+        if (MASK != 3) {
+            t = d[i * RS];
+            if (MASK & 1) t.x = val.x;
+            if (MASK & 2) t.y = val.y;
+        }
         d[i * RS] = t;
+    };
+    auto acc = [&](int i, double2 val) {
         if (pin && k0 + i < nz) wsum.x = fma(dzf[k0 + i], val.x, wsum.x);
     };
+
+    // ---- sweep C: forward substitution of the right-hand side with x_0 known
+    // (rows 1..M-2; unmasked components of the tile stay untouched)
+    double2 gprev = x0;
+#pragma unroll
+    for (int i = 1; i <= M - 2; ++i) {
+        const double2 rr = rhs_of(i);
+        const double av = alpha_of(i);
+        gprev.x = fma(av, gprev.x, rr.x) * rb[i];
+        gprev.y = fma(av, gprev.y, rr.y) * rb[i];
+        put(i, gprev);
+    }
+    // ---- sweep D: back substitution
+    double2 x = r;
     put(M - 1, x);
+    acc(M - 1, x);
 #pragma unroll
     for (int i = M - 2; i >= 1; --i) {
-        const double2 rn = d[i * RS];
-        x.x = fma(W[i], x.x, fma(Ah[i], x0.x, rn.x));
-        x.y = fma(W[i], x.y, fma(Ah[i], x0.y, rn.y));
+        const double2 gi = d[i * RS];
+        const double w = ga[i] * rb[i];
+        x.x = fma(w, x.x, gi.x);
+        x.y = fma(w, x.y, gi.y);
         put(i, x);
+        acc(i, x);
     }
     put(0, x0);
+    acc(0, x0);
 
     if constexpr (pin) {
         // zero volume mean of the (0,0) mode: subtract sum_k dzf_k phi_k / sum_k dzf_k
@@ -184,7 +204,7 @@ __device__ __forceinline__ void solve_pair(double2 *d, const double *al, const d
 }
 
 template <int M>
-__global__ void __launch_bounds__(kPairs *kLanes)
+__global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 1))
     zsolve_cr_kernel(double *__restrict__ p, const double *__restrict__ A, const double *__restrict__ C,
                      const double *__restrict__ dzf, const double *__restrict__ lamx,
                      const double *__restrict__ lamy_nat, const double *__restrict__ lamy_pk, int nx, int ny,
