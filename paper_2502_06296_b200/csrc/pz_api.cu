@@ -311,17 +311,17 @@ int helmholtz_z_solve(pz_plan *pl, double *u, void *stream)
 {
     if (!pl || !u) { set_error("helmholtz_z_solve: NULL argument"); return PZ_EINVAL; }
     if (pl->helm_cur < 0) { set_error("helmholtz_z_solve: call helmholtz_z_setup first"); return PZ_ENOTSETUP; }
-    return launch_helmholtz(pl, u, (cudaStream_t)stream);
+    double *one[1] = {u};
+    return launch_helmholtz_n(pl, one, 1, (cudaStream_t)stream);
 }
 
 int helmholtz_z_solve_n(pz_plan *pl, double *const *u, int n, void *stream)
 {
     if (!pl || !u || n < 0) { set_error("helmholtz_z_solve_n: bad argument"); return PZ_EINVAL; }
-    for (int c = 0; c < n; ++c) {
-        const int rc = helmholtz_z_solve(pl, u[c], stream);
-        if (rc != PZ_OK) return rc;
-    }
-    return PZ_OK;
+    if (pl->helm_cur < 0) { set_error("helmholtz_z_solve_n: call helmholtz_z_setup first"); return PZ_ENOTSETUP; }
+    for (int c = 0; c < n; ++c)
+        if (!u[c]) { set_error("helmholtz_z_solve_n: field %d is NULL", c); return PZ_EINVAL; }
+    return launch_helmholtz_n(pl, u, n, (cudaStream_t)stream);
 }
 
 static int ensure_host_stage(pz_plan *pl)
@@ -390,6 +390,7 @@ static int *option_slot(pz_plan *pl, const char *key)
 {
     if (!std::strcmp(key, "zsolve_variant")) return &pl->opt.zsolve_variant;
     if (!std::strcmp(key, "slab_planes")) return &pl->opt.slab_planes;
+    if (!std::strcmp(key, "helm_variant")) return &pl->opt.helm_variant;
     if (!std::strcmp(key, "helm_tx")) return &pl->opt.helm_tx;
     if (!std::strcmp(key, "helm_m")) return &pl->opt.helm_m;
     if (!std::strcmp(key, "fft_y_tc")) return &pl->opt.fft_y_tc;
@@ -411,7 +412,7 @@ int pz_set_option(pz_plan *pl, const char *key, int value)
         return PZ_EUNSUPPORTED;
     }
     *slot = value;
-    if ((slot == &pl->opt.helm_tx || slot == &pl->opt.helm_m) && pl->helm_cur >= 0)
+    if ((slot == &pl->opt.helm_tx || slot == &pl->opt.helm_m || slot == &pl->opt.helm_variant) && pl->helm_cur >= 0)
         return helmholtz_build_tables(pl, pl->helm_a); // geometry changed: rebuild the tables
     return PZ_OK;
 }
@@ -422,6 +423,7 @@ int pz_get_option(const pz_plan *pl, const char *key, int *value)
     int *slot = option_slot(const_cast<pz_plan *>(pl), key);
     if (!slot) {
         if (!std::strcmp(key, "helm_m_actual")) { *value = pl->helm_m; return PZ_OK; }
+        if (!std::strcmp(key, "helm_variant_actual")) { *value = pl->helm_variant; return PZ_OK; }
         if (!std::strcmp(key, "helm_tx_actual")) { *value = pl->helm_tx; return PZ_OK; }
         if (!std::strcmp(key, "helm_p_actual")) { *value = pl->helm_P; return PZ_OK; }
         if (!std::strcmp(key, "slab_planes_actual")) { *value = slab_planes(pl); return PZ_OK; }

@@ -113,7 +113,21 @@ int ilog2_ceil(int n)
 // Choose the sub-domain size m and count P for this nz (and the CTA width) -- launch geometry.
 static void helm_geometry(pz_plan *pl)
 {
+    int variant = pl->opt.helm_variant;
+    if (variant != 0 && variant != 1) variant = (pl->nz <= 1024) ? 1 : 0;
+    if (variant == 1 && pl->nz > 1024) variant = 0;
+    pl->helm_variant = variant;
     int m = pl->opt.helm_m;
+    if (variant == 1) {
+        // 16 columns x P sub-domains per CTA, P <= 32
+        if (m != 4 && m != 8 && m != 16 && m != 32) m = 4;
+        while (m < 32 && (pl->nz + m - 1) / m > 32) m *= 2;
+        pl->helm_m = m;
+        pl->helm_P = (pl->nz + m - 1) / m;
+        pl->helm_tx = 16;
+        pl->helm_levels = ilog2_ceil(2 * pl->helm_P);
+        return;
+    }
     if (m != 4 && m != 8 && m != 16 && m != 32) m = (pl->nz <= 128) ? 4 : (pl->nz <= 256) ? 8 : (pl->nz <= 512 ? 16 : 32);
     int P = (pl->nz + m - 1) / m;
     int tx = pl->opt.helm_tx;
@@ -133,7 +147,10 @@ int helmholtz_build_tables(pz_plan *pl, double a)
     typedef long double ld;
     helm_geometry(pl);
     const int nz = pl->nz, m = pl->helm_m, P = pl->helm_P, nzp = P * m, n2 = 2 * P, LV = pl->helm_levels;
-    if (pl->helm_tx * P > ((m >= 32) ? 256 : 512)) {
+    if (pl->helm_variant == 1) {
+        const int rc = helmholtz_tma_prepare(pl);
+        if (rc != PZ_OK) return rc;
+    } else if (pl->helm_tx * P > ((m >= 32) ? 256 : 512)) {
         set_error("helmholtz: nz = %d is too large for the register-tile kernel (P = %d sub-domains)", nz, P);
         return PZ_EUNSUPPORTED;
     }
@@ -242,8 +259,9 @@ int helmholtz_build_tables(pz_plan *pl, double a)
     return PZ_OK;
 }
 
-int launch_helmholtz(pz_plan *pl, double *u, cudaStream_t st)
+int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st)
 {
+    if (n == 0) return PZ_OK;
     HelmTables &t = pl->helm[pl->helm_cur];
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     PZ_CUDA(cudaStreamIsCapturing(st, &cap));
@@ -253,26 +271,37 @@ int launch_helmholtz(pz_plan *pl, double *u, cudaStream_t st)
     if (!capturing && cudaEventQuery(t.uploaded) != cudaSuccess) PZ_CUDA(cudaStreamWaitEvent(st, t.uploaded, 0));
     const size_t plane = (size_t)pl->nx * pl->ny;
     const int tx = pl->helm_tx, P = pl->helm_P;
-    const unsigned blocks = (unsigned)(plane / tx);
-    const size_t smem = 2 * (size_t)(2 * P) * tx * sizeof(double);
-    const int threads = tx * P;
-    ProfScope prof(pl, PZ_K_HELMHOLTZ, st);
-    const bool full = (P * pl->helm_m == pl->nz);
+    if (pl->helm_variant == 1) {
+        for (int f0 = 0; f0 < n; f0 += 4) {
+            const int nf = (n - f0 < 4) ? n - f0 : 4;
+            ProfScope prof(pl, PZ_K_HELMHOLTZ, st);
+            const int rc = launch_helmholtz_tma(pl, u + f0, nf, t.dev, st);
+            if (rc != PZ_OK) return rc;
+        }
+    } else {
+        const unsigned blocks = (unsigned)(plane / tx);
+        const size_t smem = 2 * (size_t)(2 * P) * tx * sizeof(double);
+        const int threads = tx * P;
+        const bool full = (P * pl->helm_m == pl->nz);
 #define PZ_HELM_LAUNCH(MM)                                                                                       \
     do {                                                                                                         \
-        if (full) helmholtz_kernel<MM, true><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx); \
-        else helmholtz_kernel<MM, false><<<blocks, threads, smem, st>>>(u, t.dev, plane, pl->nz, P, pl->helm_levels, tx);    \
+        if (full) helmholtz_kernel<MM, true><<<blocks, threads, smem, st>>>(u[f], t.dev, plane, pl->nz, P, pl->helm_levels, tx); \
+        else helmholtz_kernel<MM, false><<<blocks, threads, smem, st>>>(u[f], t.dev, plane, pl->nz, P, pl->helm_levels, tx);    \
     } while (0)
-    switch (pl->helm_m) {
-    case 4: PZ_HELM_LAUNCH(4); break;
-    case 8: PZ_HELM_LAUNCH(8); break;
-    case 16: PZ_HELM_LAUNCH(16); break;
-    case 32: PZ_HELM_LAUNCH(32); break;
-    default: set_error("helmholtz: bad sub-domain size %d", pl->helm_m); return PZ_EINVAL;
-    }
+        for (int f = 0; f < n; ++f) {
+            ProfScope prof(pl, PZ_K_HELMHOLTZ, st);
+            switch (pl->helm_m) {
+            case 4: PZ_HELM_LAUNCH(4); break;
+            case 8: PZ_HELM_LAUNCH(8); break;
+            case 16: PZ_HELM_LAUNCH(16); break;
+            case 32: PZ_HELM_LAUNCH(32); break;
+            default: set_error("helmholtz: bad sub-domain size %d", pl->helm_m); return PZ_EINVAL;
+            }
+            count_launch();
+            PZ_CUDA(cudaGetLastError());
+        }
 #undef PZ_HELM_LAUNCH
-    count_launch();
-    PZ_CUDA(cudaGetLastError());
+    }
     if (!capturing) PZ_CUDA(cudaEventRecord(t.last_use, st));
     return PZ_OK;
 }

@@ -25,7 +25,8 @@ struct Options {
     int zsolve_variant = 0;   // 0 = thread-per-column Thomas through global memory (2 sweeps)
                               // 1 = chunked cyclic reduction in shared memory
     int slab_planes = 0;      // 0 = auto: z-planes per L2-resident slab for the fused x/y FFT passes
-    int helm_tx = 0;          // 0 = auto: columns per CTA in the Helmholtz kernel
+    int helm_variant = -1;    // -1 = auto; 1 = persistent TMA-fed pipeline (nz <= 1024); 0 = register tile, direct loads
+    int helm_tx = 0;          // 0 = auto: columns per CTA in the Helmholtz kernel (variant 0)
     int helm_m = 0;           // 0 = auto: rows per sub-domain in the Helmholtz kernel
     int fft_y_tc = 0;         // 0 = auto: complex column pairs per CTA in the y FFT
     int fft_x_lpb = 0;        // 0 = auto: lines per CTA in the x FFT
@@ -60,6 +61,8 @@ struct pz_plan {
     // Helmholtz
     double helm_a = -1.0;
     int helm_m = 0, helm_P = 0, helm_tx = 0, helm_levels = 0;
+    int helm_variant = 0;            // variant the current tables were built for
+    int helm_bps = 0;                // variant 1: resident CTAs per SM
     pz::HelmTables helm[2];
     int helm_cur = -1;
     cudaStream_t upload_stream = nullptr;
@@ -99,7 +102,9 @@ int launch_fft_x(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cud
 int launch_fft_y(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
 int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
 int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st);
-int launch_helmholtz(pz_plan *pl, double *u, cudaStream_t st);
+int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st);
+int launch_helmholtz_tma(pz_plan *pl, double *const *u, int n, const double *tab, cudaStream_t st);
+int helmholtz_tma_prepare(pz_plan *pl);
 int helmholtz_build_tables(pz_plan *pl, double a);
 
 } // namespace pz

@@ -1,0 +1,53 @@
+// pz_tma.cu -- host side of pz_tma.cuh: tensor-map encoding through the driver entry point.
+#include "pz_tma.cuh"
+#include "pz_internal.h"
+
+#include <mutex>
+
+namespace pz {
+
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn g_encode = nullptr;
+std::once_flag g_once;
+
+void resolve()
+{
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult q = cudaDriverEntryPointSymbolNotFound;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+        g_encode = reinterpret_cast<EncodeTiledFn>(fn);
+    else
+        cudaGetLastError();
+}
+
+} // namespace
+
+int encode_column_tile_map(CUtensorMap *map, const double *field, size_t ncols, int nz, int tx, int box_rows)
+{
+    std::call_once(g_once, resolve);
+    if (!g_encode) {
+        set_error("cuTensorMapEncodeTiled is not available from this driver");
+        return PZ_ECUDA;
+    }
+    const cuuint64_t gdim[2] = {(cuuint64_t)ncols, (cuuint64_t)nz};
+    const cuuint64_t gstride[1] = {(cuuint64_t)ncols * sizeof(double)};
+    const cuuint32_t box[2] = {(cuuint32_t)tx, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = g_encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double *>(field), gdim, gstride, box,
+                                estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("cuTensorMapEncodeTiled failed (%d) for %zu columns x %d rows, box %d x %d", (int)r, ncols, nz, tx,
+                  box_rows);
+        return PZ_ECUDA;
+    }
+    return PZ_OK;
+}
+
+} // namespace pz

@@ -217,20 +217,25 @@ HELM_CASES = [
     (8, 8, 1594, 1.8, 2.5e-5, []),       # the paper's nz
     (8, 8, 64, 0.0, 0.0, []),            # a = 0: identity
     (8, 8, 64, 1.8, 10.0, []),           # strongly implicit
+    (256, 128, 300, 1.8, 5e-5, []),      # 2048 tiles of 16 columns: several per resident CTA; 2 TMA boxes
+    (128, 64, 48, 1.8, 5e-5, []),
 ]
 
 
 @pytest.mark.parametrize("nx,ny,nz,beta,a,options", HELM_CASES)
-def test_helmholtz_matches_oracle(torch, pz, wl, oracle, nx, ny, nz, beta, a, options):
+@pytest.mark.parametrize("variant", [0, 1])   # 0: register tile, direct loads; 1: persistent TMA pipeline
+def test_helmholtz_matches_oracle(torch, pz, wl, oracle, nx, ny, nz, beta, a, options, variant):
     zf = wl.z_faces(nz, 2.0, beta)
     zc = wl.z_centres(zf)
     rng = np.random.default_rng(nz * 7 + nx)
     r = rng.standard_normal((nz, ny, nx))
     ref = oracle.helmholtz_z_solve(zc, zf, a, r)
     plan = pz.poisson_plan_create(nx, ny, nz, 1.0, 1.0, zc, zf)
+    pz.pz_set_option(plan, "helm_variant", variant)
     for k, v in options:
         pz.pz_set_option(plan, k, v)
     pz.helmholtz_z_setup(plan, a)
+    assert pz.pz_get_option(plan, "helm_variant_actual") == (variant if nz <= 1024 else 0)
     u = torch.from_numpy(r).cuda()
     pz.helmholtz_z_solve(plan, u)
     torch.cuda.synchronize()
