@@ -391,6 +391,10 @@ static int *option_slot(pz_plan *pl, const char *key)
     if (!std::strcmp(key, "zsolve_variant")) return &pl->opt.zsolve_variant;
     if (!std::strcmp(key, "slab_planes")) return &pl->opt.slab_planes;
     if (!std::strcmp(key, "helm_variant")) return &pl->opt.helm_variant;
+    if (!std::strcmp(key, "helm_probe")) return &pl->opt.helm_probe;
+    if (!std::strcmp(key, "helm_cluster")) return &pl->opt.helm_cluster;
+    if (!std::strcmp(key, "helm_box_rows")) return &pl->opt.helm_box_rows;
+    if (!std::strcmp(key, "helm_l2promo")) return &pl->opt.helm_l2promo;
     if (!std::strcmp(key, "helm_tx")) return &pl->opt.helm_tx;
     if (!std::strcmp(key, "helm_m")) return &pl->opt.helm_m;
     if (!std::strcmp(key, "fft_y_tc")) return &pl->opt.fft_y_tc;

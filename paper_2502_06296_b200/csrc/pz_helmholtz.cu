@@ -119,9 +119,9 @@ static void helm_geometry(pz_plan *pl)
     pl->helm_variant = variant;
     int m = pl->opt.helm_m;
     if (variant == 1) {
-        // 16 columns x P sub-domains per CTA, P <= 32
-        if (m != 4 && m != 8 && m != 16 && m != 32) m = 4;
-        while (m < 32 && (pl->nz + m - 1) / m > 32) m *= 2;
+        // 8 column pairs x P sub-domains per CTA, P <= 64, m in {4, 8, 16}
+        if (m != 4 && m != 8 && m != 16) m = (pl->nz <= 128) ? 4 : (pl->nz <= 256 ? 8 : 16);
+        while (m < 16 && (pl->nz + m - 1) / m > 64) m *= 2;
         pl->helm_m = m;
         pl->helm_P = (pl->nz + m - 1) / m;
         pl->helm_tx = 16;

@@ -8,14 +8,19 @@
 // fields:
 //   * the tile {16 columns x all nz rows} (128-byte rows, zero-filled past nz) is fetched by the
 //     TMA unit into shared memory and signalled on an mbarrier;
-//   * thread (c, s) copies the m rows of sub-domain s of column c into registers, the CTA
-//     synchronises once and thread 0 immediately issues the fetch of the NEXT tile into the same
-//     buffer, so loads stay in flight through Steps 2-4 and the stores of this tile;
+//   * thread (cp, s) copies the m rows of sub-domain s of the column PAIR cp into registers with
+//     16-byte shared-memory loads (one k-only table value then serves two points and every load /
+//     store instruction moves 16 bytes: with one column per thread the kernel is bound by LSU
+//     instruction issue, ncu r01c), the CTA synchronises once and thread 0 immediately issues
+//     the fetch of the NEXT tile into the same buffer, so loads stay in flight through Steps 2-4
+//     and the stores of this tile;
 //   * Step 2 (forward / backward sweeps on d only), Step 3 (boundary system: precomputed
 //     parallel-cyclic-reduction multipliers applied through a small shared-memory exchange),
-//     Step 4 (reconstruction) run in registers; results go back with coalesced 128-byte stores;
-//   * the k-only tables are staged once per CTA in shared memory with a padded stride, so the
-//     two sub-domains that share a warp read them without bank conflicts.
+//     Step 4 (reconstruction) run in registers; results go back with 16-byte stores, 128
+//     contiguous bytes per 8 lanes;
+//   * the k-only tables and the PCR multipliers are staged once per CTA in shared memory; the
+//     table stride per sub-domain is padded so that the four sub-domains of a warp hit different
+//     bank groups.
 // 16 bytes and five FMAs per point; the paper's "store 1/b" makes it division-free.
 #include "pz_internal.h"
 #include "pz_tma.cuh"
@@ -33,27 +38,47 @@ struct HelmArgs {
 };
 
 template <int M> struct Limits {
-    static constexpr int kMaxThreads = 512;                // P <= 32 sub-domains
-    static constexpr int kMinBlocks = (M >= 32) ? 1 : 2;   // m = 32 keeps 64 doubles of d + addresses
+    static constexpr int kMaxThreads = 512;                // 8 column pairs x P <= 64 sub-domains
+    static constexpr int kMinBlocks = (M >= 16) ? 1 : 2;   // m = 16: 2 x 16 doubles of d per thread
 };
 
+__device__ __forceinline__ double2 ld2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
+__device__ __forceinline__ void st2(double *p, double2 v) { *reinterpret_cast<double2 *>(p) = v; }
+
+// Shared-memory carve-up in doubles; host and device agree through these helpers.
+template <int M> struct Smem {
+    static constexpr int TS = M + 2; // table stride per sub-domain: even (16-byte pairs)
+    __host__ __device__ static int box_rows(int P) { return P * M <= 256 ? P * M : 256; }
+    __host__ __device__ static int nbox(int P) { return (P * M + box_rows(P) - 1) / box_rows(P); }
+    __host__ __device__ static size_t tile(int P) { return (size_t)box_rows(P) * nbox(P) * kTX; }
+    __host__ __device__ static size_t xch(int P) { return (size_t)2 * 2 * P * kTX; }
+    __host__ __device__ static size_t tab(int P) { return (size_t)5 * P * TS; }
+    __host__ __device__ static size_t pcr(int P, int levels) { return (size_t)levels * 4 * P + 2 * P; }
+    __host__ __device__ static size_t bytes(int P, int levels)
+    {
+        return (tile(P) + xch(P) + tab(P) + pcr(P, levels)) * sizeof(double) + 16;
+    }
+};
+
+// Thread (cp, s): columns (2cp, 2cp+1) of the tile, sub-domain s (rows s*M .. s*M+M-1).
 template <int M, bool FULL>
 __global__ void __launch_bounds__(Limits<M>::kMaxThreads, Limits<M>::kMinBlocks)
     helmholtz_tma_kernel(const __grid_constant__ HelmArgs args, const double *__restrict__ tab, size_t plane, int nz,
-                         int P, int levels, int box_rows, int nbox, int tiles_per_field, int total_tiles)
+                         int P, int levels, int tiles_per_field, int total_tiles, int probe, int box_rows, int nbox, int csz)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    constexpr int TS = M + 1; // padded table stride per sub-domain
+    using L = Smem<M>;
+    constexpr int TS = L::TS;
     const int nzp = P * M, n2 = 2 * P;
-    const int rows_alloc = box_rows * nbox;
-    double *tile = reinterpret_cast<double *>(smem_raw);                  // rows_alloc x 16
-    double *xch = tile + (size_t)rows_alloc * kTX;                        // 2 buffers x 2 x P x 16
-    double *stab = xch + (size_t)2 * n2 * kTX;                            // 5 x P x TS
-    uint64_t *bar = reinterpret_cast<uint64_t *>(stab + (size_t)5 * P * TS);
+    double *tile = reinterpret_cast<double *>(smem_raw);   // rows x 16
+    double *xch = tile + L::tile(P);                       // [buffer][first/last][s][16]
+    double *stab = xch + L::xch(P);                        // [table][s][TS]
+    double *spcr = stab + L::tab(P);                       // [level][s][4], then [s][2]
+    uint64_t *bar = reinterpret_cast<uint64_t *>(spcr + L::pcr(P, levels));
 
-    const int tid = threadIdx.x, c = tid & (kTX - 1), s = tid >> 4;
+    const int tid = threadIdx.x, c2 = 2 * (tid & 7), s = tid >> 3;
     const int k0 = s * M;
-    const unsigned tile_bytes = (unsigned)rows_alloc * kTX * sizeof(double);
+    const unsigned tile_bytes = (unsigned)(L::tile(P) * sizeof(double));
 
     if (tid == 0) {
         mbar_init(bar, 1);
@@ -63,11 +88,17 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, Limits<M>::kMinBlocks)
         const int t = q / nzp, k = q - t * nzp;
         stab[(size_t)t * P * TS + (k / M) * TS + (k % M)] = tab[q];
     }
+    for (int q = tid; q < (int)L::pcr(P, levels); q += blockDim.x) spcr[q] = tab[5 * (size_t)nzp + q];
     __syncthreads();
 
     auto fetch = [&](int t) {
-        const int f = t / tiles_per_field, col0 = (t - f * tiles_per_field) * kTX;
+        const int f = t / tiles_per_field, tt = t - f * tiles_per_field, col0 = tt * kTX;
         mbar_arrive_expect_tx(bar, tile_bytes);
+        if (probe == 3) { // diagnostic: same bytes fetched as 32-column boxes (256-byte rows)
+            for (int b = 0; b < nbox; ++b)
+                tma_load_2d(tile + (size_t)b * box_rows * 32, &args.map[f], (tt >> 1) * 32, (tt & 1) * (nzp / 2) + b * box_rows, bar);
+            return;
+        }
         for (int b = 0; b < nbox; ++b) tma_load_2d(tile + (size_t)b * box_rows * kTX, &args.map[f], col0, b * box_rows, bar);
     };
 
@@ -75,87 +106,126 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, Limits<M>::kMinBlocks)
     if (tid == 0 && t < total_tiles) fetch(t);
 
     const double *fA = stab + s * TS, *bC = fA + P * TS, *rb = bC + P * TS, *ra = rb + P * TS, *rc = ra + P * TS;
-    const double *pcr = tab + 5 * (size_t)nzp;
     const int sm1 = max(s - 1, 0), sp1 = min(s + 1, P - 1);
     unsigned phase = 0;
 
     for (; t < total_tiles; t += gridDim.x) {
-        double d[M];
+        double da[M], db[M]; // the two columns
         mbar_wait(bar, phase);
         phase ^= 1;
 #pragma unroll
-        for (int i = 0; i < M; ++i) d[i] = tile[(k0 + i) * kTX + c];
-        __syncthreads(); // every thread holds its rows: the buffer is free again
+        for (int i = 0; i < M; ++i) {
+            const double2 v = ld2(tile + (k0 + i) * kTX + c2);
+            da[i] = v.x;
+            db[i] = v.y;
+        }
+        // every thread holds its rows: the buffer is free again.  With a cluster (csz > 1) the
+        // CTAs of the cluster, which own neighbouring tiles, also meet here, so that their next
+        // fetches (and their stores) reach DRAM together as 128*csz contiguous bytes per row.
+        if (csz > 1) {
+            asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+        } else {
+            __syncthreads();
+        }
         if (tid == 0 && t + (int)gridDim.x < total_tiles) fetch(t + gridDim.x);
 
-        // Step 2: runtime reduction, d only
+        if (probe == 2) { // diagnostic: pipeline skeleton only (load, store)
+            const int f = t / tiles_per_field;
+            double *up = args.u[f] + (size_t)(t - f * tiles_per_field) * kTX + c2 + (size_t)k0 * plane;
 #pragma unroll
-        for (int i = 2; i < M; ++i) d[i] = fma(-fA[i], d[i - 1], d[i]);
+            for (int i = 0; i < M; ++i)
+                if (FULL || k0 + i < nz) st2(up + (size_t)i * plane, make_double2(da[i], db[i]));
+            continue;
+        }
+        // Step 2: runtime reduction, d only (forward i = 2..M-1, backward i = M-3..0)
 #pragma unroll
-        for (int i = M - 3; i >= 0; --i) d[i] = fma(-bC[i], d[i + 1], d[i]);
+        for (int i = 2; i < M; i += 2) {
+            const double2 f = ld2(fA + i);
+            da[i] = fma(-f.x, da[i - 1], da[i]);
+            db[i] = fma(-f.x, db[i - 1], db[i]);
+            da[i + 1] = fma(-f.y, da[i], da[i + 1]);
+            db[i + 1] = fma(-f.y, db[i], db[i + 1]);
+        }
+#pragma unroll
+        for (int i = M - 4; i >= 0; i -= 2) {
+            const double2 g = ld2(bC + i);
+            da[i + 1] = fma(-g.y, da[i + 2], da[i + 1]);
+            db[i + 1] = fma(-g.y, db[i + 2], db[i + 1]);
+            da[i] = fma(-g.x, da[i + 1], da[i]);
+            db[i] = fma(-g.x, db[i + 1], db[i]);
+        }
 
-        // Step 3: boundary system.  Row 2s = first row of sub-domain s (x0), row 2s+1 = last (x1);
-        // shared layout [buffer][first/last][s][c].
-        double x0 = d[0], x1 = d[M - 1];
+        // Step 3: boundary system.  Row 2s = first row of sub-domain s (x0), row 2s+1 = last (x1).
+        double2 x0 = make_double2(da[0], db[0]), x1 = make_double2(da[M - 1], db[M - 1]);
         double *cur = xch, *nxt = xch + (size_t)n2 * kTX;
-        cur[(s)*kTX + c] = x0;
-        cur[(P + s) * kTX + c] = x1;
+        st2(cur + s * kTX + c2, x0);
+        st2(cur + (P + s) * kTX + c2, x1);
         __syncthreads();
         {
             // level 0 (h = 1): partners of x0 are (x1 of s-1, own x1), of x1 (own x0, x0 of s+1)
-            const double2 ka = __ldg(reinterpret_cast<const double2 *>(pcr) + 2 * s);
-            const double2 kb = __ldg(reinterpret_cast<const double2 *>(pcr) + 2 * s + 1);
-            const double n0 = fma(ka.x, cur[(P + sm1) * kTX + c], fma(ka.y, x1, x0));
-            const double n1 = fma(kb.x, x0, fma(kb.y, cur[sp1 * kTX + c], x1));
+            const double2 ka = ld2(spcr + 4 * s), kb = ld2(spcr + 4 * s + 2);
+            const double2 pm = ld2(cur + (P + sm1) * kTX + c2), pp = ld2(cur + sp1 * kTX + c2);
+            const double2 n0 = make_double2(fma(ka.x, pm.x, fma(ka.y, x1.x, x0.x)), fma(ka.x, pm.y, fma(ka.y, x1.y, x0.y)));
+            const double2 n1 = make_double2(fma(kb.x, x0.x, fma(kb.y, pp.x, x1.x)), fma(kb.x, x0.y, fma(kb.y, pp.y, x1.y)));
             x0 = n0;
             x1 = n1;
         }
         for (int l = 1, hs = 1; l < levels; ++l, hs *= 2) {
-            nxt[s * kTX + c] = x0;
-            nxt[(P + s) * kTX + c] = x1;
+            st2(nxt + s * kTX + c2, x0);
+            st2(nxt + (P + s) * kTX + c2, x1);
             __syncthreads();
             double *tmp = cur; cur = nxt; nxt = tmp;
-            const double2 ka = __ldg(reinterpret_cast<const double2 *>(pcr + (size_t)l * 2 * n2) + 2 * s);
-            const double2 kb = __ldg(reinterpret_cast<const double2 *>(pcr + (size_t)l * 2 * n2) + 2 * s + 1);
+            const double *kk = spcr + (size_t)l * 4 * P + 4 * s;
+            const double2 ka = ld2(kk), kb = ld2(kk + 2);
             const int sa = max(s - hs, 0), sb = min(s + hs, P - 1);
-            x0 = fma(ka.x, cur[sa * kTX + c], fma(ka.y, cur[sb * kTX + c], x0));
-            x1 = fma(kb.x, cur[(P + sa) * kTX + c], fma(kb.y, cur[(P + sb) * kTX + c], x1));
+            const double2 am = ld2(cur + sa * kTX + c2), ap = ld2(cur + sb * kTX + c2);
+            const double2 bm = ld2(cur + (P + sa) * kTX + c2), bp = ld2(cur + (P + sb) * kTX + c2);
+            x0.x = fma(ka.x, am.x, fma(ka.y, ap.x, x0.x));
+            x0.y = fma(ka.x, am.y, fma(ka.y, ap.y, x0.y));
+            x1.x = fma(kb.x, bm.x, fma(kb.y, bp.x, x1.x));
+            x1.y = fma(kb.x, bm.y, fma(kb.y, bp.y, x1.y));
         }
         {
-            const double2 rbr = __ldg(reinterpret_cast<const double2 *>(pcr + (size_t)levels * 2 * n2) + s);
-            x0 *= rbr.x;
-            x1 *= rbr.y;
+            const double2 rbr = ld2(spcr + (size_t)levels * 4 * P + 2 * s);
+            x0.x *= rbr.x; x0.y *= rbr.x;
+            x1.x *= rbr.y; x1.y *= rbr.y;
         }
 
         // Step 4: reconstruct and store
+        if ((probe == 1 || probe == 3) && x0.x != 1.2345e300) continue; // diagnostic: no stores
         const int f = t / tiles_per_field;
-        double *up = args.u[f] + (size_t)(t - f * tiles_per_field) * kTX + c + (size_t)k0 * plane;
-        if (FULL || k0 < nz) up[0] = x0;
+        double *up = args.u[f] + (size_t)(t - f * tiles_per_field) * kTX + c2 + (size_t)k0 * plane;
 #pragma unroll
-        for (int i = 1; i < M - 1; ++i) {
-            const double v = fma(-rc[i], x1, fma(-ra[i], x0, rb[i] * d[i]));
-            if (FULL || k0 + i < nz) up[(size_t)i * plane] = v;
+        for (int i = 0; i < M; i += 2) {
+            const double2 qb = ld2(rb + i), qa = ld2(ra + i), qc = ld2(rc + i);
+            double2 v, w;
+            if (i == 0) {
+                v = x0;
+            } else {
+                v.x = fma(-qc.x, x1.x, fma(-qa.x, x0.x, qb.x * da[i]));
+                v.y = fma(-qc.x, x1.y, fma(-qa.x, x0.y, qb.x * db[i]));
+            }
+            if (i + 1 == M - 1) {
+                w = x1;
+            } else {
+                w.x = fma(-qc.y, x1.x, fma(-qa.y, x0.x, qb.y * da[i + 1]));
+                w.y = fma(-qc.y, x1.y, fma(-qa.y, x0.y, qb.y * db[i + 1]));
+            }
+            if (FULL || k0 + i < nz) st2(up + (size_t)i * plane, v);
+            if (FULL || k0 + i + 1 < nz) st2(up + (size_t)(i + 1) * plane, w);
         }
-        if (FULL || k0 + M - 1 < nz) up[(size_t)(M - 1) * plane] = x1;
     }
-}
-
-template <int M>
-size_t smem_bytes(int P)
-{
-    const int nzp = P * M, box_rows = nzp <= 256 ? nzp : 256, nbox = (nzp + box_rows - 1) / box_rows;
-    return ((size_t)box_rows * nbox * kTX + (size_t)2 * 2 * P * kTX + (size_t)5 * P * (M + 1)) * sizeof(double) + 16;
 }
 
 template <int M, bool FULL>
 int prepare_mf(pz_plan *pl)
 {
-    const size_t smem = smem_bytes<M>(pl->helm_P);
+    const size_t smem = Smem<M>::bytes(pl->helm_P, pl->helm_levels);
     auto kern = helmholtz_tma_kernel<M, FULL>;
     if (smem > 227 * 1024) { set_error("helmholtz (TMA variant): tile of %zu bytes does not fit shared memory", smem); return PZ_EUNSUPPORTED; }
     PZ_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     int bps = 0;
-    PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, kTX * pl->helm_P, smem));
+    PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, (kTX / 2) * pl->helm_P, smem));
     if (bps < 1) { set_error("helmholtz (TMA variant): kernel does not fit an SM"); return PZ_ECUDA; }
     pl->helm_bps = bps;
     return PZ_OK;
@@ -164,14 +234,19 @@ int prepare_mf(pz_plan *pl)
 template <int M, bool FULL>
 int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStream_t st)
 {
-    const int P = pl->helm_P, nzp = P * M;
-    const int box_rows = nzp <= 256 ? nzp : 256;
-    const int nbox = (nzp + box_rows - 1) / box_rows;
+    const int P = pl->helm_P;
     const size_t plane = (size_t)pl->nx * pl->ny;
-    const size_t smem = smem_bytes<M>(P);
+    const size_t smem = Smem<M>::bytes(P, pl->helm_levels);
+    const bool wide = (pl->opt.helm_probe == 3) && (P * M) % 512 == 0;
+    int box_rows = Smem<M>::box_rows(P), nbox = Smem<M>::nbox(P);
+    if (pl->opt.helm_box_rows > 0 && (P * M) % pl->opt.helm_box_rows == 0 && pl->opt.helm_box_rows <= 256) {
+        box_rows = pl->opt.helm_box_rows;
+        nbox = P * M / box_rows;
+    }
+    if (wide) { box_rows = 256; nbox = P * M / 512; }
     HelmArgs args;
     for (int f = 0; f < n; ++f) {
-        const int rc = encode_column_tile_map(&args.map[f], u[f], plane, pl->nz, kTX, box_rows);
+        const int rc = encode_column_tile_map(&args.map[f], u[f], plane, pl->nz, wide ? 32 : kTX, box_rows, pl->opt.helm_l2promo);
         if (rc != PZ_OK) return rc;
         args.u[f] = u[f];
     }
@@ -180,8 +255,36 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
     const long long total = (long long)tiles_per_field * n;
     long long blocks = (long long)pl->num_sms * pl->helm_bps;
     if (blocks > total) blocks = total;
-    helmholtz_tma_kernel<M, FULL><<<(unsigned)blocks, kTX * P, smem, st>>>(args, tab, plane, pl->nz, P, pl->helm_levels,
-                                                                            box_rows, nbox, tiles_per_field, (int)total);
+    // CTAs of a cluster own neighbouring tiles and meet once per tile, so their fetches and stores
+    // reach DRAM together (256 contiguous bytes per row for a pair).  Measured (profiles/r01c):
+    // +15-20 % with m = 16, a loss with the smaller sub-domains (two or more CTAs per SM).
+    int csz = pl->opt.helm_cluster;
+    if (csz == 0) csz = (M == 16) ? 2 : 1;
+    if (csz != 2 && csz != 4 && csz != 8) csz = 1;
+    while (csz > 1 && (tiles_per_field % csz != 0 || blocks < csz)) csz /= 2;
+    const int probe = wide ? 3 : (pl->opt.helm_probe == 3 ? 1 : pl->opt.helm_probe);
+    cudaLaunchConfig_t cfg = {};
+    cfg.blockDim = dim3((kTX / 2) * P);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = csz;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (csz > 1) {
+        cfg.gridDim = dim3((unsigned)(blocks / csz * csz));
+        int nclusters = 0;
+        PZ_CUDA(cudaOccupancyMaxActiveClusters(&nclusters, helmholtz_tma_kernel<M, FULL>, &cfg));
+        if (nclusters < 1) { set_error("helmholtz (TMA variant): no cluster of %d CTAs fits", csz); return PZ_ECUDA; }
+        if ((long long)nclusters * csz < blocks) blocks = (long long)nclusters * csz;
+    }
+    blocks = blocks / csz * csz;
+    cfg.gridDim = dim3((unsigned)blocks);
+    PZ_CUDA(cudaLaunchKernelEx(&cfg, helmholtz_tma_kernel<M, FULL>, args, tab, plane, pl->nz, P, pl->helm_levels,
+                               tiles_per_field, (int)total, probe, box_rows, nbox, csz));
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
@@ -198,7 +301,6 @@ int helmholtz_tma_prepare(pz_plan *pl)
     case 4: return PZ_HP(4);
     case 8: return PZ_HP(8);
     case 16: return PZ_HP(16);
-    case 32: return PZ_HP(32);
     default: set_error("helmholtz: bad sub-domain size %d", pl->helm_m); return PZ_EINVAL;
     }
 #undef PZ_HP
@@ -209,13 +311,14 @@ int helmholtz_tma_prepare(pz_plan *pl)
 int launch_helmholtz_tma(pz_plan *pl, double *const *u, int n, const double *tab, cudaStream_t st)
 {
     if (n < 1 || n > kMaxFields) { set_error("helmholtz (TMA variant): 1..4 fields per launch"); return PZ_EINVAL; }
+    for (int f = 0; f < n; ++f)
+        if (((uintptr_t)u[f] & 15) != 0) { set_error("helmholtz_z_solve: u must be 16-byte aligned"); return PZ_EINVAL; }
     const bool full = (pl->helm_P * pl->helm_m == pl->nz);
 #define PZ_HT(MM) (full ? launch_mf<MM, true>(pl, u, n, tab, st) : launch_mf<MM, false>(pl, u, n, tab, st))
     switch (pl->helm_m) {
     case 4: return PZ_HT(4);
     case 8: return PZ_HT(8);
     case 16: return PZ_HT(16);
-    case 32: return PZ_HT(32);
     default: set_error("helmholtz: bad sub-domain size %d", pl->helm_m); return PZ_EINVAL;
     }
 #undef PZ_HT

@@ -26,6 +26,10 @@ struct Options {
                               // 1 = chunked cyclic reduction in shared memory
     int slab_planes = 0;      // 0 = auto: z-planes per L2-resident slab for the fused x/y FFT passes
     int helm_variant = -1;    // -1 = auto; 1 = persistent TMA-fed pipeline (nz <= 1024); 0 = register tile, direct loads
+    int helm_box_rows = 0;    // diagnostic (variant 1): rows per TMA box (0 = 256)
+    int helm_l2promo = 1;     // diagnostic (variant 1): tensor-map L2 promotion 0 none, 1 128 B, 2 256 B, 3 64 B
+    int helm_cluster = 0;     // variant 1: CTAs per cluster walking neighbouring tiles in step (0 = auto)
+    int helm_probe = 0;       // diagnostic (variant 1): 1 = no stores, 2 = no arithmetic (results are wrong)
     int helm_tx = 0;          // 0 = auto: columns per CTA in the Helmholtz kernel (variant 0)
     int helm_m = 0;           // 0 = auto: rows per sub-domain in the Helmholtz kernel
     int fft_y_tc = 0;         // 0 = auto: complex column pairs per CTA in the y FFT

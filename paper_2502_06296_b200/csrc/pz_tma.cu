@@ -28,7 +28,7 @@ void resolve()
 
 } // namespace
 
-int encode_column_tile_map(CUtensorMap *map, const double *field, size_t ncols, int nz, int tx, int box_rows)
+int encode_column_tile_map(CUtensorMap *map, const double *field, size_t ncols, int nz, int tx, int box_rows, int l2promo)
 {
     std::call_once(g_once, resolve);
     if (!g_encode) {
@@ -41,7 +41,10 @@ int encode_column_tile_map(CUtensorMap *map, const double *field, size_t ncols, 
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = g_encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double *>(field), gdim, gstride, box,
                                 estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                l2promo == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE : l2promo == 2 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+                                                                               : l2promo == 3 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B
+                                                                                              : CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         set_error("cuTensorMapEncodeTiled failed (%d) for %zu columns x %d rows, box %d x %d", (int)r, ncols, nz, tx,
                   box_rows);

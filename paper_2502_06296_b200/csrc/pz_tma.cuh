@@ -48,6 +48,11 @@ __device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *map, i
         "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
         ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
 }
+// hint: bring the box at (c0, c1) into L2 (no shared-memory destination, no completion signal)
+__device__ __forceinline__ void tma_prefetch_l2_2d(const CUtensorMap *map, int c0, int c1)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(map), "r"(c0), "r"(c1) : "memory");
+}
 // orders generic-proxy shared-memory writes before later async-proxy (TMA store) reads
 __device__ __forceinline__ void fence_proxy_async_smem()
 {
@@ -71,6 +76,7 @@ template <int N> __device__ __forceinline__ void tma_store_wait_all()
 
 // ---------------------------------------------------------------- host side
 // Encodes the {ncols, nz} view of a field with boxes of {tx, box_rows}.  Returns a pz_status.
-int encode_column_tile_map(CUtensorMap *map, const double *field, size_t ncols, int nz, int tx, int box_rows);
+int encode_column_tile_map(CUtensorMap *map, const double *field, size_t ncols, int nz, int tx, int box_rows,
+                           int l2promo = 1);
 
 } // namespace pz

@@ -209,7 +209,7 @@ HELM_CASES = [
     (64, 8, 129, 2.0, 2.5e-5, []),
     (16, 16, 256, 1.8, 5e-5, []),
     (16, 16, 256, 1.8, 1e-2, [("helm_m", 4)]),
-    (16, 16, 256, 1.8, 5e-5, [("helm_m", 32), ("helm_tx", 8)]),
+    (16, 16, 256, 1.8, 5e-5, [("helm_m", 16), ("helm_tx", 8)]),
     (8, 16, 512, 1.8, 5e-5, []),
     (8, 16, 512, 1.8, 5e-5, [("helm_tx", 32)]),
     (8, 8, 1024, 1.8, 2.5e-5, []),
