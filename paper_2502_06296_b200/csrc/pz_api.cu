@@ -243,7 +243,7 @@ int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double
         if ((ce = cudaEventCreateWithFlags(&pl->helm[b].uploaded, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
         if ((ce = cudaEventCreateWithFlags(&pl->helm[b].last_use, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
     }
-    pl->opt.zsolve_variant = (nz <= 1024) ? 1 : 0;
+    pl->opt.zsolve_variant = (nz <= 512) ? 2 : (nz <= 1024) ? 1 : 0;
     if (pl->opt.zsolve_variant == 0 && (rc = ensure_zwork(pl)) != PZ_OK) return fail(rc);
     *out = pl;
     return PZ_OK;
@@ -389,6 +389,7 @@ int pz_profile_read(pz_plan *pl, int cls, double *total_ms, long long *launches)
 static int *option_slot(pz_plan *pl, const char *key)
 {
     if (!std::strcmp(key, "zsolve_variant")) return &pl->opt.zsolve_variant;
+    if (!std::strcmp(key, "zsolve_stages")) return &pl->opt.zsolve_stages;
     if (!std::strcmp(key, "slab_planes")) return &pl->opt.slab_planes;
     if (!std::strcmp(key, "helm_variant")) return &pl->opt.helm_variant;
     if (!std::strcmp(key, "helm_probe")) return &pl->opt.helm_probe;
@@ -408,8 +409,8 @@ int pz_set_option(pz_plan *pl, const char *key, int value)
     int *slot = option_slot(pl, key);
     if (!slot) { set_error("pz_set_option: unknown key '%s'", key); return PZ_EUNSUPPORTED; }
     if (slot == &pl->opt.zsolve_variant) {
-        if (value != 0 && value != 1) { set_error("zsolve_variant must be 0 or 1"); return PZ_EUNSUPPORTED; }
-        if (value == 1 && pl->nz > 1024) { set_error("zsolve_variant 1 supports nz <= 1024"); return PZ_EUNSUPPORTED; }
+        if (value < 0 || value > 2) { set_error("zsolve_variant must be 0, 1 or 2"); return PZ_EUNSUPPORTED; }
+        if (value >= 1 && pl->nz > 1024) { set_error("zsolve_variant %d supports nz <= 1024", value); return PZ_EUNSUPPORTED; }
         if (value == 0) { const int rc = ensure_zwork(pl); if (rc != PZ_OK) return rc; }
     } else if (value < 0) {
         set_error("pz_set_option: '%s' must be >= 0", key);

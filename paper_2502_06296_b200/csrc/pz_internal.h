@@ -24,6 +24,8 @@ struct HelmTables {
 struct Options {
     int zsolve_variant = 0;   // 0 = thread-per-column Thomas through global memory (2 sweeps)
                               // 1 = chunked cyclic reduction in shared memory
+                              // 2 = the same solve inside a TMA load / solve / TMA store pipeline
+    int zsolve_stages = 0;    // variant 2: shared-memory stages (0 = as many as fit, at most 3)
     int slab_planes = 0;      // 0 = auto: z-planes per L2-resident slab for the fused x/y FFT passes
     int helm_variant = -1;    // -1 = auto; 1 = persistent TMA-fed pipeline (nz <= 1024); 0 = register tile, direct loads
     int helm_box_rows = 0;    // diagnostic (variant 1): rows per TMA box (0 = 256)

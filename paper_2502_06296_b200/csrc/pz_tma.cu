@@ -28,7 +28,8 @@ void resolve()
 
 } // namespace
 
-int encode_column_tile_map(CUtensorMap *map, const double *field, size_t ncols, int nz, int tx, int box_rows, int l2promo)
+int encode_column_tile_map(CUtensorMap *map, const double *field, size_t ncols, int nz, int tx, int box_rows, int l2promo,
+                           bool swizzle128)
 {
     std::call_once(g_once, resolve);
     if (!g_encode) {
@@ -40,7 +41,8 @@ int encode_column_tile_map(CUtensorMap *map, const double *field, size_t ncols, 
     const cuuint32_t box[2] = {(cuuint32_t)tx, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = g_encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double *>(field), gdim, gstride, box,
-                                estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
                                 l2promo == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE : l2promo == 2 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
                                                                                : l2promo == 3 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B
                                                                                               : CU_TENSOR_MAP_L2_PROMOTION_L2_128B,

@@ -76,7 +76,8 @@ template <int N> __device__ __forceinline__ void tma_store_wait_all()
 
 // ---------------------------------------------------------------- host side
 // Encodes the {ncols, nz} view of a field with boxes of {tx, box_rows}.  Returns a pz_status.
+// swizzle128: shared-memory side uses the 128-byte swizzle (tx * 8 must be 128).
 int encode_column_tile_map(CUtensorMap *map, const double *field, size_t ncols, int nz, int tx, int box_rows,
-                           int l2promo = 1);
+                           int l2promo = 1, bool swizzle128 = false);
 
 } // namespace pz

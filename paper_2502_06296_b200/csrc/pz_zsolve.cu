@@ -19,6 +19,7 @@
 namespace pz {
 
 int launch_zsolve_cr(pz_plan *pl, double *p, cudaStream_t st);
+int launch_zsolve_tma(pz_plan *pl, double *p, cudaStream_t st);
 
 namespace {
 
@@ -77,6 +78,7 @@ __global__ void __launch_bounds__(128)
 int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st)
 {
     if (pl->opt.zsolve_variant == 1) return launch_zsolve_cr(pl, p, st);
+    if (pl->opt.zsolve_variant == 2) return launch_zsolve_tma(pl, p, st);
     if (!pl->d_zwork) {
         cudaError_t e = cudaMalloc(&pl->d_zwork, pl->n * sizeof(double));
         if (e != cudaSuccess) {

@@ -14,6 +14,7 @@
 // All rows are kept in M-matrix form with an explicit diagonal excess (see pz_zsolve.cu): the
 // sub-domain sweeps, the reduced system and the PCR levels only add non-negative numbers.
 #include "pz_internal.h"
+#include "pz_zsolve_pair.cuh"
 
 namespace pz {
 
@@ -21,187 +22,12 @@ namespace {
 
 constexpr int kTX = 16;    // real columns per tile (128-byte rows)
 constexpr int kPairs = 8;  // complex pairs per tile = warps per CTA
-constexpr int kLanes = 32; // sub-domains per column
 
-// 1/x to ~1 ulp: hardware seed + two Newton steps (x is a positive, normal pivot).
-__device__ __forceinline__ double fast_rcp(double x)
-{
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    double e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    return r;
-}
-
-__device__ __forceinline__ double shfl_up(double v, int d) { return __shfl_up_sync(0xffffffffu, v, d); }
-__device__ __forceinline__ double shfl_down(double v, int d) { return __shfl_down_sync(0xffffffffu, v, d); }
-
-// One column pair, one sub-domain per lane.  d points at this lane's first row inside the tile
-// (row stride kTX/2 double2).  al/ga: this lane's alpha_i, gamma_i (sub-/super-diagonal
-// magnitudes, zero on padding rows and at the walls) in shared memory.  MASK bit 0 / 1: which
-// component (x / y of the double2) is solved and written back.
-//
-// Sweeps (Algorithm 1 re-ordered so that only the pivot reciprocals are thread-private):
-//   A  rows M-2..1, read only: UL elimination -> this sub-domain's row 0 in terms of
-//      (x_{M-1} of the previous lane, x_0, x_{M-1})
-//   B  rows 1..M-1, read only: LU elimination -> row M-1 in terms of (x_0, x_{M-1}, next x_0);
-//      keeps rb_i = 1/pivot_i in registers.  A and B run interleaved (two independent chains).
-//   reduced system across lanes (warp shuffles, parallel cyclic reduction)
-//   C  rows 1..M-2 forward: g_i = (r_i + alpha_i g_{i-1}) rb_i with g_0 := x_0  (overwrites the tile)
-//   D  rows M-2..1 backward: x_i = g_i + gamma_i rb_i x_{i+1}
-template <int M, int MASK, bool pin>
-__device__ __forceinline__ void solve_pair(double2 *d, const double *al, const double *ga, double sigma,
-                                           int k0, int nz, const double *__restrict__ dzf, double inv_lz)
-{
-    constexpr int RS = kTX / 2;
-    // row coefficients: real rows have excess sigma, padding rows (k >= nz) are x = 0,
-    // the pinned row (gauge of the singular column) likewise.
-    auto eps_of = [&](int i) { return (k0 + i < nz && !(pin && k0 + i == nz - 1)) ? sigma : 1.0; };
-    auto alpha_of = [&](int i) { return (pin && k0 + i == nz - 1) ? 0.0 : al[i]; };
-    auto rhs_of = [&](int i) {
-        const double2 v = d[i * RS];
-        const bool live = (k0 + i < nz) && !(pin && k0 + i == nz - 1);
-        return live ? make_double2(-v.x, -v.y) : make_double2(0.0, 0.0);
-    };
-
-    // ---- sweeps A (UL, descending) and B (LU, ascending), interleaved
-    double rb[M];
-    double chat = ga[M - 2], eps2 = eps_of(M - 2);
-    double2 rp2 = rhs_of(M - 2);
-    double rb2 = fast_rcp(alpha_of(M - 2) + chat + eps2);
-    double ahat = alpha_of(1), eps = eps_of(1);
-    double2 rp = rhs_of(1);
-    rb[1] = fast_rcp(ahat + ga[1] + eps);
-#pragma unroll
-    for (int t = 0; t < M - 2; ++t) {
-        {   // A: row i = M-3-t (for t < M-3)
-            const int i = M - 3 - t;
-            if (i >= 1) {
-                const double nn = ga[i] * rb2;
-                const double2 r = rhs_of(i);
-                chat = nn * chat;
-                eps2 = fma(nn, eps2, eps_of(i));
-                rp2.x = fma(nn, rp2.x, r.x);
-                rp2.y = fma(nn, rp2.y, r.y);
-                rb2 = fast_rcp(alpha_of(i) + chat + eps2);
-            }
-        }
-        {   // B: row i = 2+t
-            const int i = 2 + t;
-            const double mm = alpha_of(i) * rb[i - 1];
-            const double2 r = rhs_of(i);
-            ahat = mm * ahat;
-            eps = fma(mm, eps, eps_of(i));
-            rp.x = fma(mm, rp.x, r.x);
-            rp.y = fma(mm, rp.y, r.y);
-            rb[i] = fast_rcp(ahat + ga[i] + eps);
-        }
-    }
-    // normalised row 0:  -a0 X_{s-1} + x_0 - c0 X_s = r0, excess e0
-    double a0, c0, e0;
-    double2 r0;
-    {
-        const double nn = ga[0] * rb2;
-        const double2 r = rhs_of(0);
-        a0 = alpha_of(0);
-        c0 = nn * chat;
-        e0 = fma(nn, eps2, eps_of(0));
-        r0.x = fma(nn, rp2.x, r.x);
-        r0.y = fma(nn, rp2.y, r.y);
-        const double rbn = fast_rcp(a0 + c0 + e0);
-        a0 *= rbn; c0 *= rbn; e0 *= rbn; r0.x *= rbn; r0.y *= rbn;
-    }
-    // normalised last row:  -a x_0 + X_s - c (next lane's x_0) = r, excess e
-    double a = ahat * rb[M - 1], c = ga[M - 1] * rb[M - 1], e = eps * rb[M - 1];
-    double2 r = make_double2(rp.x * rb[M - 1], rp.y * rb[M - 1]);
-
-    // ---- reduced system: first eliminate the x_0 unknowns (local row 0 and the next lane's)
-    {
-        const double c0n = shfl_down(c0, 1), e0n = shfl_down(e0, 1);
-        const double r0nx = shfl_down(r0.x, 1), r0ny = shfl_down(r0.y, 1);
-        const double k1 = a, k2 = c; // c = 0 on the last lane (wall or padding)
-        a = k1 * a0;
-        c = k2 * c0n;
-        e = fma(k1, e0, fma(k2, e0n, e));
-        r.x = fma(k1, r0.x, fma(k2, r0nx, r.x));
-        r.y = fma(k1, r0.y, fma(k2, r0ny, r.y));
-        const double rbn = fast_rcp(a + c + e);
-        a *= rbn; c *= rbn; e *= rbn; r.x *= rbn; r.y *= rbn;
-    }
-    // ---- parallel cyclic reduction across the 32 lanes (unknown X_s = last row of lane s)
-#pragma unroll
-    for (int h = 1; h < kLanes; h *= 2) {
-        const double am = shfl_up(a, h), em = shfl_up(e, h), rmx = shfl_up(r.x, h), rmy = shfl_up(r.y, h);
-        const double cp = shfl_down(c, h), ep = shfl_down(e, h), rpx = shfl_down(r.x, h), rpy = shfl_down(r.y, h);
-        // a == 0 whenever lane-h < 0 and c == 0 whenever lane+h > 31, so out-of-range partners
-        // (whose shuffled values are the lane's own, finite) contribute nothing.
-        const double k1 = a, k2 = c;
-        a = k1 * am;
-        c = k2 * cp;
-        e = fma(k1, em, fma(k2, ep, e));
-        r.x = fma(k1, rmx, fma(k2, rpx, r.x));
-        r.y = fma(k1, rmy, fma(k2, rpy, r.y));
-        const double rbn = fast_rcp(a + c + e);
-        a *= rbn; c *= rbn; e *= rbn; r.x *= rbn; r.y *= rbn;
-    }
-    // r = X_s.  x_0 of this lane from its normalised row 0:  x_0 = r0 + a0 X_{s-1} + c0 X_s
-    const double xpx = shfl_up(r.x, 1), xpy = shfl_up(r.y, 1); // lane 0: a0 = 0
-    const double2 x0 = make_double2(fma(a0, xpx, fma(c0, r.x, r0.x)), fma(a0, xpy, fma(c0, r.y, r0.y)));
-
-    double2 wsum = make_double2(0.0, 0.0);
-    auto put = [&](int i, double2 val) {
-        double2 t = val;
-        if (MASK != 3) {
-            t = d[i * RS];
-            if (MASK & 1) t.x = val.x;
-            if (MASK & 2) t.y = val.y;
-        }
-        d[i * RS] = t;
-    };
-    auto acc = [&](int i, double2 val) {
-        if (pin && k0 + i < nz) wsum.x = fma(dzf[k0 + i], val.x, wsum.x);
-    };
-
-    // ---- sweep C: forward substitution of the right-hand side with x_0 known
-    // (rows 1..M-2; unmasked components of the tile stay untouched)
-    double2 gprev = x0;
-#pragma unroll
-    for (int i = 1; i <= M - 2; ++i) {
-        const double2 rr = rhs_of(i);
-        const double av = alpha_of(i);
-        gprev.x = fma(av, gprev.x, rr.x) * rb[i];
-        gprev.y = fma(av, gprev.y, rr.y) * rb[i];
-        put(i, gprev);
-    }
-    // ---- sweep D: back substitution
-    double2 x = r;
-    put(M - 1, x);
-    acc(M - 1, x);
-#pragma unroll
-    for (int i = M - 2; i >= 1; --i) {
-        const double2 gi = d[i * RS];
-        const double w = ga[i] * rb[i];
-        x.x = fma(w, x.x, gi.x);
-        x.y = fma(w, x.y, gi.y);
-        put(i, x);
-        acc(i, x);
-    }
-    put(0, x0);
-    acc(0, x0);
-
-    if constexpr (pin) {
-        // zero volume mean of the (0,0) mode: subtract sum_k dzf_k phi_k / sum_k dzf_k
-        double s = wsum.x;
-#pragma unroll
-        for (int o = 16; o >= 1; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        s *= inv_lz;
-#pragma unroll
-        for (int i = 0; i < M; ++i)
-            if (k0 + i < nz) d[i * RS].x -= s;
-    }
-}
+// rows of one sub-domain inside the manually staged tile: stride kTX doubles
+struct RowAcc {
+    double2 *d;
+    __device__ __forceinline__ double2 &operator()(int i) const { return d[i * (kTX / 2)]; }
+};
 
 template <int M>
 __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 1))
@@ -240,7 +66,7 @@ __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 
         const int i = (int)(col % nx), j = (int)(col / nx);
         const double ly = (i < 2) ? lamy_pk[j] : lamy_nat[j];
         const double sig0 = -(lamx[i] + ly), sig1 = -(lamx[i + 1] + ly);
-        double2 *d = reinterpret_cast<double2 *>(tile + lane * CH + 2 * q);
+        const RowAcc d{reinterpret_cast<double2 *>(tile + lane * CH + 2 * q)};
         const double *al = s_al + lane * CS, *ga = s_ga + lane * CS;
         const int k0 = lane * M;
         if (sig0 == sig1) {

@@ -1,0 +1,192 @@
+// pz_zsolve_tma.cu -- step a3, variant 2 (default for nz <= 512): the chunked cyclic reduction of
+// pz_zsolve_cr.cu (Algorithm 1 inside one GPU) fed by an asynchronous pipeline.
+//
+// Variant 1 stages its tile with ordinary loads, solves, and writes back: the three phases of a
+// CTA do not overlap and only two CTAs fit an SM (ncu r01b: 35 % of DRAM peak, 24 % of the warp
+// slots active, every pipe below 55 %).  Here one CTA per SM stays resident:
+//   * a producer warp drives the TMA unit: the tile {16 columns x nz rows} of spectral column
+//     block t is fetched into one of S shared-memory stages as 32 boxes {16 columns x m rows}, one
+//     per sub-domain; a stage that has been solved is written back by TMA stores straight from
+//     shared memory, and is refilled as soon as the store has read it;
+//   * eight solver warps, one per complex column pair, wait for "stage full", solve their pair in
+//     place (lanes = the 32 sub-domains; warp-shuffle PCR for the boundary system) and signal
+//     "stage done".  Solver warps never wait for one another: each walks the tile sequence at its
+//     own pace, so loads, solves and stores of neighbouring tiles overlap.
+//   * Shared-memory layout: a warp reads the same 16-byte slot (its pair) of 32 different rows,
+//     which in a dense [row][128 B] tile is a 32-way bank conflict.  The boxes use the TMA
+//     128-byte swizzle (the 16-byte slot index is XORed with the row index mod 8) and each
+//     sub-domain slot is m+1 rows long, so the 8 lanes of a shared-memory wavefront sit in 8
+//     different rows mod 8: conflict-free.
+#include "pz_internal.h"
+#include "pz_tma.cuh"
+#include "pz_zsolve_pair.cuh"
+
+namespace pz {
+
+namespace {
+
+constexpr int kTX = 16;      // real columns per tile (128-byte rows)
+constexpr int kSolvers = 8;  // solver warps = complex pairs per tile
+constexpr int kThreads = (kSolvers + 1) * 32;
+
+// Row i of a sub-domain whose slot starts at absolute row R0 of a 1024-byte aligned stage:
+// byte offset (R0+i)*128 + ((pair ^ ((R0+i) & 7)) << 4).
+struct SwzAcc {
+    unsigned char *slot; // stage base + R0*128
+    int off[8];          // ((pair ^ ((R0 + j) & 7)) << 4), j = 0..7
+    __device__ __forceinline__ double2 &operator()(int i) const
+    {
+        return *reinterpret_cast<double2 *>(slot + i * 128 + off[i & 7]);
+    }
+};
+
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+template <int M> struct Geo {
+    static constexpr int SLOT = M + 1;                       // rows per sub-domain slot
+    static constexpr size_t STAGE = (size_t)kLanes * SLOT * 128;
+    static constexpr int CS = M + 1;                         // coefficient stride per lane
+    static constexpr size_t COEF = (size_t)2 * kLanes * CS * sizeof(double);
+    __host__ __device__ static size_t bytes(int stages) { return 1024 + stages * STAGE + COEF + 64; }
+};
+
+template <int M>
+__global__ void __launch_bounds__(kThreads, 1)
+    zsolve_tma_kernel(const __grid_constant__ CUtensorMap map, const double *__restrict__ A,
+                      const double *__restrict__ C, const double *__restrict__ dzf, const double *__restrict__ lamx,
+                      const double *__restrict__ lamy_nat, const double *__restrict__ lamy_pk, int nx, int ny, int nz,
+                      double inv_lz, int ntiles, int stages)
+{
+    using G = Geo<M>;
+    extern __shared__ unsigned char smem_zt[];
+    // 1024-byte aligned stage area (the swizzle pattern is a function of the address)
+    unsigned char *base = smem_zt + ((1024u - (smem_u32(smem_zt) & 1023u)) & 1023u);
+    double *s_al = reinterpret_cast<double *>(base + stages * G::STAGE);
+    double *s_ga = s_al + kLanes * G::CS;
+    uint64_t *full = reinterpret_cast<uint64_t *>(s_ga + kLanes * G::CS);
+    uint64_t *done = full + 4;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < stages; ++b) {
+            mbar_init(&full[b], 1);
+            mbar_init(&done[b], kSolvers);
+        }
+        mbar_fence_init();
+    }
+    for (int k = threadIdx.x; k < kLanes * M; k += blockDim.x) {
+        s_al[(k / M) * G::CS + (k % M)] = (k < nz) ? A[k] : 0.0;
+        s_ga[(k / M) * G::CS + (k % M)] = (k < nz) ? C[k] : 0.0;
+    }
+    __syncthreads();
+
+    const int my_tiles = (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    constexpr unsigned kStageTx = (unsigned)(kLanes * M * 128);
+
+    if (warp == kSolvers) {
+        // ---------------------------------------------------------------- producer
+        if (lane == 0) {
+            auto load = [&](int it) {
+                const int b = it % stages, col0 = ((int)blockIdx.x + it * (int)gridDim.x) * kTX;
+                mbar_arrive_expect_tx(&full[b], kStageTx);
+                for (int l = 0; l < kLanes; ++l)
+                    tma_load_2d(base + b * G::STAGE + (size_t)l * G::SLOT * 128, &map, col0, l * M, &full[b]);
+            };
+            for (int it = 0; it < stages && it < my_tiles; ++it) load(it);
+            for (int it = 0; it < my_tiles; ++it) {
+                const int b = it % stages, col0 = ((int)blockIdx.x + it * (int)gridDim.x) * kTX;
+                mbar_wait(&done[b], (it / stages) & 1);
+                for (int l = 0; l < kLanes; ++l)
+                    if (l * M < nz) tma_store_2d(&map, base + b * G::STAGE + (size_t)l * G::SLOT * 128, col0, l * M);
+                tma_store_commit();
+                if (it + stages < my_tiles) {
+                    tma_store_wait_read<0>();
+                    load(it + stages);
+                }
+            }
+            tma_store_wait_all<0>();
+        }
+        return;
+    }
+
+    // -------------------------------------------------------------------- solvers
+    const int q = warp;
+    const double *al = s_al + lane * G::CS, *ga = s_ga + lane * G::CS;
+    const int k0 = lane * M, R0 = lane * G::SLOT;
+    SwzAcc d;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) d.off[j] = (q ^ ((R0 + j) & 7)) << 4;
+
+    for (int it = 0; it < my_tiles; ++it) {
+        const int b = it % stages;
+        const size_t col = ((size_t)blockIdx.x + (size_t)it * gridDim.x) * kTX + 2 * q;
+        const int i = (int)(col % nx), j = (int)(col / nx);
+        const double ly = (i < 2) ? lamy_pk[j] : lamy_nat[j];
+        const double sig0 = -(lamx[i] + ly), sig1 = -(lamx[i + 1] + ly);
+        d.slot = base + b * G::STAGE + (size_t)R0 * 128;
+        mbar_wait(&full[b], (it / stages) & 1);
+        if (sig0 == sig1) {
+            solve_pair<M, 3, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
+        } else {
+            // pair 0 of a row: x-modes 0 and nx/2 have different eigenvalues; (0,0) is singular
+            if (i == 0 && j == 0)
+                solve_pair<M, 1, true>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
+            else
+                solve_pair<M, 1, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
+            solve_pair<M, 2, false>(d, al, ga, sig1, k0, nz, dzf, inv_lz);
+        }
+        fence_proxy_async_smem(); // this lane's shared-memory writes -> visible to the TMA store
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&done[b]);
+    }
+}
+
+template <int M>
+int launch_m(pz_plan *pl, double *p, cudaStream_t st)
+{
+    using G = Geo<M>;
+    int stages = (int)((227 * 1024 - 1024 - G::COEF - 64) / G::STAGE);
+    if (stages > 3) stages = 3;
+    if (pl->opt.zsolve_stages > 0 && pl->opt.zsolve_stages < stages) stages = pl->opt.zsolve_stages;
+    if (stages < 1) { set_error("z-solve variant 2: nz = %d does not fit shared memory", pl->nz); return PZ_EUNSUPPORTED; }
+    const size_t smem = G::bytes(stages);
+    static bool attr_done = false;
+    if (!attr_done) {
+        PZ_CUDA(cudaFuncSetAttribute(zsolve_tma_kernel<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        attr_done = true;
+    }
+    const size_t plane = (size_t)pl->nx * pl->ny;
+    CUtensorMap map;
+    const int rc = encode_column_tile_map(&map, p, plane, pl->nz, kTX, M, 1, /*swizzle128=*/true);
+    if (rc != PZ_OK) return rc;
+    const int ntiles = (int)(plane / kTX);
+    int occ = 1;
+    if (smem * 2 <= 227 * 1024) PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, zsolve_tma_kernel<M>, kThreads, smem));
+    if (occ < 1) occ = 1;
+    int blocks = pl->num_sms * occ;
+    if (blocks > ntiles) blocks = ntiles;
+    ProfScope prof(pl, PZ_K_Z_SOLVE, st);
+    zsolve_tma_kernel<M><<<blocks, kThreads, smem, st>>>(map, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx, pl->d_lamy_nat,
+                                                          pl->d_lamy_pk, pl->nx, pl->ny, pl->nz, pl->inv_lz, ntiles, stages);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+} // namespace
+
+int launch_zsolve_tma(pz_plan *pl, double *p, cudaStream_t st)
+{
+    const int nz = pl->nz;
+    if (nz <= 32 * 4) return launch_m<4>(pl, p, st);
+    if (nz <= 32 * 8) return launch_m<8>(pl, p, st);
+    if (nz <= 32 * 16) return launch_m<16>(pl, p, st);
+    if (nz <= 32 * 32) return launch_m<32>(pl, p, st);
+    set_error("z-solve variant 2 supports nz <= 1024 (got %d); use zsolve_variant = 0", nz);
+    return PZ_EUNSUPPORTED;
+}
+
+} // namespace pz

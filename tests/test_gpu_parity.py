@@ -72,7 +72,7 @@ POISSON_SHAPES = [
 
 
 @pytest.mark.parametrize("base,nx,ny,nz", POISSON_SHAPES)
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_poisson_matches_oracle(torch, pz, wl, oracle, base, nx, ny, nz, variant):
     w = wl.scaled(wl.CONFIGS[base], nx, ny, nz)
     zc, zf = wl.grid(w)
@@ -303,7 +303,7 @@ def test_config1_poisson_and_helmholtz_full(torch, pz, wl, oracle):
     zc, zf = wl.grid(w)
     f = wl.poisson_rhs(w)
     ref = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)
-    for variant in (0, 1):
+    for variant in (0, 1, 2):
         got = gpu_poisson(torch, pz, w, zc, zf, f, [("zsolve_variant", variant)])
         assert rel_err(got, ref) <= TOL
     r = wl.helmholtz_rhs(w)
