@@ -37,18 +37,27 @@ __device__ __forceinline__ double shfl_down(double v, int d) { return __shfl_dow
 //   reduced system across lanes (warp shuffles, parallel cyclic reduction)
 //   C  rows 1..M-2 forward: g_i = (r_i + alpha_i g_{i-1}) rb_i with g_0 := x_0  (overwrites the tile)
 //   D  rows M-2..1 backward: x_i = g_i + gamma_i rb_i x_{i+1}
-template <int M, int MASK, bool pin, class Acc>
+// FULL: nz == 32 M and the column is not the pinned one: no padding rows, no row tests.
+template <int M, int MASK, bool pin, bool FULL = false, class Acc>
 __device__ __forceinline__ void solve_pair(const Acc d, const double *al, const double *ga, double sigma,
                                            int k0, int nz, const double *__restrict__ dzf, double inv_lz)
 {
     // row coefficients: real rows have excess sigma, padding rows (k >= nz) are x = 0,
     // the pinned row (gauge of the singular column) likewise.
-    auto eps_of = [&](int i) { return (k0 + i < nz && !(pin && k0 + i == nz - 1)) ? sigma : 1.0; };
+    static_assert(!(FULL && pin), "the pinned column takes the general path");
+    auto eps_of = [&](int i) {
+        if constexpr (FULL) return sigma;
+        else return (k0 + i < nz && !(pin && k0 + i == nz - 1)) ? sigma : 1.0;
+    };
     auto alpha_of = [&](int i) { return (pin && k0 + i == nz - 1) ? 0.0 : al[i]; };
     auto rhs_of = [&](int i) {
         const double2 v = d(i);
-        const bool live = (k0 + i < nz) && !(pin && k0 + i == nz - 1);
-        return live ? make_double2(-v.x, -v.y) : make_double2(0.0, 0.0);
+        if constexpr (FULL) {
+            return make_double2(-v.x, -v.y);
+        } else {
+            const bool live = (k0 + i < nz) && !(pin && k0 + i == nz - 1);
+            return live ? make_double2(-v.x, -v.y) : make_double2(0.0, 0.0);
+        }
     };
 
     // ---- sweeps A (UL, descending) and B (LU, ascending), interleaved

@@ -114,6 +114,7 @@ __global__ void __launch_bounds__(kThreads, 1)
 
     // -------------------------------------------------------------------- solvers
     const int q = warp;
+    const bool no_pad = (nz == kLanes * M);
     const double *al = s_al + lane * G::CS, *ga = s_ga + lane * G::CS;
     const int k0 = lane * M, R0 = lane * G::SLOT;
     SwzAcc d;
@@ -129,7 +130,8 @@ __global__ void __launch_bounds__(kThreads, 1)
         d.slot = base + b * G::STAGE + (size_t)R0 * 128;
         mbar_wait(&full[b], (it / stages) & 1);
         if (sig0 == sig1) {
-            solve_pair<M, 3, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
+            if (no_pad) solve_pair<M, 3, false, true>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
+            else solve_pair<M, 3, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
         } else {
             // pair 0 of a row: x-modes 0 and nx/2 have different eigenvalues; (0,0) is singular
             if (i == 0 && j == 0)
