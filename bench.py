@@ -223,14 +223,13 @@ def main():
     import torch
 
     from paper_2502_06296_b200 import binding as pz
+    from paper_2502_06296_b200 import ranks
 
     pz.lib()  # fail loudly if the CUDA extension is missing
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; there is no CPU fallback")
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = ranks.env_rank()
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
@@ -249,8 +248,8 @@ def main():
     fields = (1 if w.poisson else 0) + w.n_helmholtz
     p = None
     if w.poisson:
-        p = wl.device_remove_weighted_mean(wl.device_field(w, w.poisson_seed + 1000 * rank), zf)
-    us = [wl.device_field(w, s + 1000 * rank) for s in w.helmholtz_seeds]
+        p = wl.device_remove_weighted_mean(wl.device_field(w, ranks.rank_seed(w.poisson_seed, rank)), zf)
+    us = [wl.device_field(w, ranks.rank_seed(s, rank)) for s in w.helmholtz_seeds]
     if w.n_helmholtz:
         pz.helmholtz_z_setup(plan, w.a)
 
@@ -293,12 +292,8 @@ def main():
         if cnt:
             kernel_ms[nm] = {"ms_total": ms, "launches": cnt, "ms_per_launch": ms / cnt}
 
-    t_max = ms_total
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_max = float(t.item())
-    value = fields * w.n * world * steps / (t_max * 1e-3)
+    t_max = ranks.max_over_ranks(ms_total, dist, "cuda")
+    value = ranks.whole_job_rate(fields * w.n * steps, world, t_max)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -323,10 +318,7 @@ def main():
         e1.record()
         barrier()
         e_ms = e0.elapsed_time(e1)
-        if dist is not None:
-            t = torch.tensor([e_ms], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e_ms = float(t.item())
+        e_ms = ranks.max_over_ranks(e_ms, dist, "cuda")
         e2e = {"value": fields * w.n * world * args.e2e_steps / (e_ms * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": fields * w.n * 8, "d2h_bytes_per_step": fields * w.n * 8,
                "steps": args.e2e_steps, "ms_per_step": e_ms / args.e2e_steps,
