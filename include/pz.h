@@ -124,7 +124,9 @@ enum pz_stage {
     PZ_STAGE_FFT_Y_FWD = 1, /* a2: FFT along y of the packed complex pairs                */
     PZ_STAGE_Z_SOLVE = 2,   /* a3: tridiagonal solves in spectral space                   */
     PZ_STAGE_FFT_Y_INV = 3, /* a4                                                         */
-    PZ_STAGE_FFT_X_INV = 4  /* a5: C2R along x and 1/(nx ny) scaling                      */
+    PZ_STAGE_FFT_X_INV = 4, /* a5: C2R along x and 1/(nx ny) scaling                      */
+    PZ_STAGE_FFT_XY_FWD = 5, /* a1+a2 by the fused kernel (nx, ny in {256,512,1024,2048})  */
+    PZ_STAGE_FFT_XY_INV = 6  /* a4+a5 by the fused kernel                                  */
 };
 PZ_API int pz_poisson_stage(pz_plan *plan, double *p, int stage, void *stream);
 
@@ -143,7 +145,9 @@ PZ_API int pz_get_option(const pz_plan *plan, const char *key, int *value);
 enum pz_kernel_class {
     PZ_K_FFT_X_FWD = 0, PZ_K_FFT_Y_FWD = 1, PZ_K_PAIR0_FWD = 2, PZ_K_Z_SOLVE = 3,
     PZ_K_PAIR0_INV = 4, PZ_K_FFT_Y_INV = 5, PZ_K_FFT_X_INV = 6, PZ_K_HELMHOLTZ = 7,
-    PZ_K_COUNT = 8
+    PZ_K_FFT_XY_FWD = 8, /* a1+a2 in one kernel (second trip of the plane through L2 only) */
+    PZ_K_FFT_XY_INV = 9, /* a4+a5 in one kernel */
+    PZ_K_COUNT = 10
 };
 PZ_API int pz_profile_enable(pz_plan *plan, int on);
 PZ_API int pz_profile_read(pz_plan *plan, int kernel_class, double *total_ms, long long *launches);

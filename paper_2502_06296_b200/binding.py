@@ -20,6 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libpz_b200.so")
 PZ_OK, PZ_EINVAL, PZ_EUNSUPPORTED, PZ_ENOMEM, PZ_ECUDA, PZ_ENOTSETUP = range(6)
 PZ_BC_PERIODIC_XY_NEUMANN_P_DIRICHLET_U = 0
 PZ_STAGE_FFT_X_FWD, PZ_STAGE_FFT_Y_FWD, PZ_STAGE_Z_SOLVE, PZ_STAGE_FFT_Y_INV, PZ_STAGE_FFT_X_INV = range(5)
+PZ_STAGE_FFT_XY_FWD, PZ_STAGE_FFT_XY_INV = 5, 6
 
 # every symbol include/pz.h declares: (name, restype, argtypes)
 _vp, _i, _d = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
@@ -179,7 +180,8 @@ def pz_get_option(plan: Plan, key: str) -> int:
     return v.value
 
 
-KERNEL_CLASSES = ("fft_x_fwd", "fft_y_fwd", "pair0_fwd", "z_solve", "pair0_inv", "fft_y_inv", "fft_x_inv", "helmholtz")
+KERNEL_CLASSES = ("fft_x_fwd", "fft_y_fwd", "pair0_fwd", "z_solve", "pair0_inv", "fft_y_inv", "fft_x_inv", "helmholtz",
+                  "fft_xy_fwd", "fft_xy_inv")
 
 
 def pz_profile_enable(plan: Plan, on: bool) -> None:

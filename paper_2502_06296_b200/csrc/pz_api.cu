@@ -120,8 +120,24 @@ int slab_planes(const pz_plan *pl)
     return (int)sp;
 }
 
+bool fused_sizes(const pz_plan *pl)
+{
+    auto ok = [](int n) { return n == 256 || n == 512 || n == 1024 || n == 2048; };
+    return ok(pl->nx) && ok(pl->ny);
+}
+
+bool use_fused(const pz_plan *pl)
+{
+    if (pl->opt.slab_planes > 0) return false;
+    // auto = separate kernels: the fused kernel halves the DRAM traffic of the transforms (ncu r01d:
+    // 16 instead of 32 B/point) but is bound by the on-SM work of the two transforms, which the
+    // separate kernels overlap with their own HBM time just as well (0.85 vs 0.72 ms at 512^3)
+    return pl->opt.fft_fused == 1 && fused_sizes(pl);
+}
+
 int forward_xy(pz_plan *pl, double *p, cudaStream_t st)
 {
+    if (use_fused(pl)) return launch_fft_xy_fwd(pl, p, st);
     const int sp = slab_planes(pl);
     for (int k0 = 0; k0 < pl->nz; k0 += sp) {
         const int nk = (k0 + sp <= pl->nz) ? sp : pl->nz - k0;
@@ -137,6 +153,7 @@ int forward_xy(pz_plan *pl, double *p, cudaStream_t st)
 
 int inverse_xy(pz_plan *pl, double *p, cudaStream_t st)
 {
+    if (use_fused(pl)) return launch_fft_xy_inv(pl, p, st);
     const int sp = slab_planes(pl);
     for (int k0 = 0; k0 < pl->nz; k0 += sp) {
         const int nk = (k0 + sp <= pl->nz) ? sp : pl->nz - k0;
@@ -243,6 +260,8 @@ int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double
         if ((ce = cudaEventCreateWithFlags(&pl->helm[b].uploaded, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
         if ((ce = cudaEventCreateWithFlags(&pl->helm[b].last_use, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
     }
+    ce = cudaMalloc(&pl->d_xyctr, 2 * (size_t)(nz + 1) * sizeof(int));
+    if (ce != cudaSuccess) { cudaGetLastError(); set_error("plan counters: %s", cudaGetErrorString(ce)); return fail(PZ_ENOMEM); }
     pl->opt.zsolve_variant = (nz <= 512) ? 2 : (nz <= 1024) ? 1 : 0;
     if (pl->opt.zsolve_variant == 0 && (rc = ensure_zwork(pl)) != PZ_OK) return fail(rc);
     *out = pl;
@@ -256,6 +275,7 @@ int poisson_plan_destroy(pz_plan *pl)
     if (pl->tables) cudaFree(pl->tables);
     if (pl->d_zwork) cudaFree(pl->d_zwork);
     if (pl->d_host_stage) cudaFree(pl->d_host_stage);
+    if (pl->d_xyctr) cudaFree(pl->d_xyctr);
     for (int b = 0; b < 2; ++b) {
         if (pl->helm[b].dev) cudaFree(pl->helm[b].dev);
         if (pl->helm[b].uploaded) cudaEventDestroy(pl->helm[b].uploaded);
@@ -285,6 +305,11 @@ int pz_poisson_stage(pz_plan *pl, double *p, int stage, void *stream)
         if ((rc = launch_pair0(pl, p, 0, pl->nz, true, st)) != PZ_OK) return rc;
         return launch_fft_y(pl, p, 0, pl->nz, true, st);
     case PZ_STAGE_FFT_X_INV: return launch_fft_x(pl, p, 0, pl->nz, true, st);
+    case PZ_STAGE_FFT_XY_FWD:
+    case PZ_STAGE_FFT_XY_INV:
+        if (!fused_sizes(pl)) { set_error("pz_poisson_stage: the fused x/y kernel needs nx, ny in {256, 512, 1024, 2048}"); return PZ_EUNSUPPORTED; }
+        PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 1) * sizeof(int), st));
+        return stage == PZ_STAGE_FFT_XY_FWD ? launch_fft_xy_fwd(pl, p, st) : launch_fft_xy_inv(pl, p, st);
     default: set_error("pz_poisson_stage: unknown stage %d", stage); return PZ_EINVAL;
     }
 }
@@ -295,6 +320,7 @@ int poisson_solve(pz_plan *pl, double *p, void *stream)
     if (((uintptr_t)p & 15) != 0) { set_error("poisson_solve: p must be 16-byte aligned"); return PZ_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
+    if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 1) * sizeof(int), st));
     if ((rc = forward_xy(pl, p, st)) != PZ_OK) return rc;
     if ((rc = launch_zsolve(pl, p, st)) != PZ_OK) return rc;
     return inverse_xy(pl, p, st);
@@ -391,6 +417,8 @@ static int *option_slot(pz_plan *pl, const char *key)
     if (!std::strcmp(key, "zsolve_variant")) return &pl->opt.zsolve_variant;
     if (!std::strcmp(key, "zsolve_stages")) return &pl->opt.zsolve_stages;
     if (!std::strcmp(key, "slab_planes")) return &pl->opt.slab_planes;
+    if (!std::strcmp(key, "fft_fused")) return &pl->opt.fft_fused;
+    if (!std::strcmp(key, "xy_lag")) return &pl->opt.xy_lag;
     if (!std::strcmp(key, "helm_variant")) return &pl->opt.helm_variant;
     if (!std::strcmp(key, "helm_probe")) return &pl->opt.helm_probe;
     if (!std::strcmp(key, "helm_cluster")) return &pl->opt.helm_cluster;

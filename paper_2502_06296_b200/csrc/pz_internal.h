@@ -26,6 +26,9 @@ struct Options {
                               // 1 = chunked cyclic reduction in shared memory
                               // 2 = the same solve inside a TMA load / solve / TMA store pipeline
     int zsolve_stages = 0;    // variant 2: shared-memory stages (0 = as many as fit, at most 3)
+    int fft_fused = -1;       // -1 = auto (currently the separate kernels); 0 = separate kernels; 1 = fused x/y kernel
+                              // (nx, ny in {256, 512, 1024, 2048})
+    int xy_lag = 0;           // fused kernel: planes by which the first phase runs ahead (0 = auto)
     int slab_planes = 0;      // 0 = auto: z-planes per L2-resident slab for the fused x/y FFT passes
     int helm_variant = -1;    // -1 = auto; 1 = persistent TMA-fed pipeline (nz <= 1024); 0 = register tile, direct loads
     int helm_box_rows = 0;    // diagnostic (variant 1): rows per TMA box (0 = 256)
@@ -63,6 +66,7 @@ struct pz_plan {
     // optional workspaces (allocated on first use)
     double *d_zwork = nullptr;       // variant-0 z solve: N doubles
     double *d_host_stage = nullptr;  // *_host calls: N doubles
+    int *d_xyctr = nullptr;          // fused x/y kernels: 2 x (1 + nz) ticket / per-plane counters
 
     // Helmholtz
     double helm_a = -1.0;
@@ -108,6 +112,8 @@ int launch_fft_x(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cud
 int launch_fft_y(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
 int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
 int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st);
+int launch_fft_xy_fwd(pz_plan *pl, double *p, cudaStream_t st);
+int launch_fft_xy_inv(pz_plan *pl, double *p, cudaStream_t st);
 int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st);
 int launch_helmholtz_tma(pz_plan *pl, double *const *u, int n, const double *tab, cudaStream_t st);
 int helmholtz_tma_prepare(pz_plan *pl);
