@@ -337,13 +337,19 @@ def main():
         nm: 16.0 * w.n * (steps * (w.n_helmholtz if nm == "helmholtz" else 1)) / kernel_ms[nm]["launches"]
         for nm in kernel_ms if not nm.startswith("pair0")}
     achieved = bytes_per_launch[dom] / (kernel_ms[dom]["ms_per_launch"] * 1e-3) / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath)).get(args.workload, {}).get(dom)
-        except Exception:
-            traffic = None
+    traffic = None  # dram bytes per launch of the dominant kernel from the committed ncu --set full capture
+    try:
+        import csv
+        import glob
+
+        tfiles = sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv")))
+        if tfiles:
+            with open(tfiles[-1]) as f:
+                for row in csv.DictReader(f):
+                    if row["workload"] == args.workload and row["kernel"] == dom:
+                        traffic = float(row["dram_bytes_per_launch"])
+    except Exception:
+        traffic = None
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": bytes_per_launch[dom],
