@@ -44,6 +44,7 @@ template <int M> struct Limits {
 
 __device__ __forceinline__ double2 ld2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
 __device__ __forceinline__ void st2(double *p, double2 v) { *reinterpret_cast<double2 *>(p) = v; }
+__device__ __forceinline__ void st2g(double *p, double2 v) { __stcs(reinterpret_cast<double2 *>(p), v); }
 
 // Shared-memory carve-up in doubles; host and device agree through these helpers.
 template <int M> struct Smem {
@@ -91,6 +92,7 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, Limits<M>::kMinBlocks)
     for (int q = tid; q < (int)L::pcr(P, levels); q += blockDim.x) spcr[q] = tab[5 * (size_t)nzp + q];
     __syncthreads();
 
+    const uint64_t pol = l2_policy_evict_first(); // every tile is read once
     auto fetch = [&](int t) {
         const int f = t / tiles_per_field, tt = t - f * tiles_per_field, col0 = tt * kTX;
         mbar_arrive_expect_tx(bar, tile_bytes);
@@ -99,7 +101,8 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, Limits<M>::kMinBlocks)
                 tma_load_2d(tile + (size_t)b * box_rows * 32, &args.map[f], (tt >> 1) * 32, (tt & 1) * (nzp / 2) + b * box_rows, bar);
             return;
         }
-        for (int b = 0; b < nbox; ++b) tma_load_2d(tile + (size_t)b * box_rows * kTX, &args.map[f], col0, b * box_rows, bar);
+        for (int b = 0; b < nbox; ++b)
+            tma_load_2d_hint(tile + (size_t)b * box_rows * kTX, &args.map[f], col0, b * box_rows, bar, pol);
     };
 
     int t = blockIdx.x;
@@ -134,7 +137,7 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, Limits<M>::kMinBlocks)
             double *up = args.u[f] + (size_t)(t - f * tiles_per_field) * kTX + c2 + (size_t)k0 * plane;
 #pragma unroll
             for (int i = 0; i < M; ++i)
-                if (FULL || k0 + i < nz) st2(up + (size_t)i * plane, make_double2(da[i], db[i]));
+                if (FULL || k0 + i < nz) st2g(up + (size_t)i * plane, make_double2(da[i], db[i]));
             continue;
         }
         // Step 2: runtime reduction, d only (forward i = 2..M-1, backward i = M-3..0)
@@ -211,8 +214,8 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, Limits<M>::kMinBlocks)
                 w.x = fma(-qc.y, x1.x, fma(-qa.y, x0.x, qb.y * da[i + 1]));
                 w.y = fma(-qc.y, x1.y, fma(-qa.y, x0.y, qb.y * db[i + 1]));
             }
-            if (FULL || k0 + i < nz) st2(up + (size_t)i * plane, v);
-            if (FULL || k0 + i + 1 < nz) st2(up + (size_t)(i + 1) * plane, w);
+            if (FULL || k0 + i < nz) st2g(up + (size_t)i * plane, v);
+            if (FULL || k0 + i + 1 < nz) st2g(up + (size_t)(i + 1) * plane, w);
         }
     }
 }
