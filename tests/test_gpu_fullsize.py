@@ -1,0 +1,117 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (default
+options, fields resident in HBM, in-place solves).
+
+* c2 (512^3): element by element against the oracle, Poisson and all three Helmholtz fields.
+* c4 (1024^3): Helmholtz on one field; the oracle solves 8192 sampled columns one by one
+  (columns are independent, so sampled columns are exact parity for those columns), spread over
+  every tile position, plus the maximum principle on the whole field.
+* c3 (2048x1024x512): Poisson; the oracle's operator is applied to the GPU solution on the host:
+  the solution is unique, so a small normwise backward error plus the zero weighted mean pin it
+  (readings R3, R11); and linearity, solve(f) + solve(g) == solve(f + g) to rounding,
+  a property that holds at any size.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+
+    import oracle
+    from paper_2502_06296_b200 import binding as pz
+    from paper_2502_06296_b200 import workloads as wl
+
+    assert torch.cuda.is_available()
+    pz.lib()
+    return torch, pz, wl, oracle
+
+
+def rel_err(got, ref):
+    return float(np.abs(got - ref).max() / np.abs(ref).max())
+
+
+def test_c2_full_poisson_and_three_helmholtz_fields(env):
+    torch, pz, wl, oracle = env
+    w = wl.CONFIGS["c2"]
+    zc, zf = wl.grid(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    f = wl.poisson_rhs(w)
+    p = torch.from_numpy(f).cuda()
+    pz.poisson_solve(plan, p)
+    got = p.cpu().numpy()
+    del p
+    ref = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)
+    assert rel_err(got, ref) <= TOL
+    dzf = np.diff(zf)
+    wm = np.dot(dzf, got.mean(axis=(1, 2))) / dzf.sum()
+    assert abs(wm) <= 1e-13 * np.abs(got).max()
+    del f, got, ref
+    pz.helmholtz_z_setup(plan, w.a)
+    rs = [wl.helmholtz_rhs(w, c) for c in range(w.n_helmholtz)]
+    us = [torch.from_numpy(r).cuda() for r in rs]
+    pz.helmholtz_z_solve_n(plan, us)                      # the call bench.py times
+    torch.cuda.synchronize()
+    for r, u in zip(rs, us):
+        assert rel_err(u.cpu().numpy(), oracle.helmholtz_z_solve(zc, zf, w.a, r)) <= TOL
+    pz.poisson_plan_destroy(plan)
+
+
+def test_c4_helmholtz_sampled_columns(env):
+    torch, pz, wl, oracle = env
+    w = wl.CONFIGS["c4"]
+    zc, zf = wl.grid(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    pz.helmholtz_z_setup(plan, w.a)
+    u = wl.device_field(w, w.helmholtz_seeds[0])          # seeded device generator, as in bench.py
+    rng = np.random.default_rng(4)
+    cols = np.unique(np.concatenate([rng.integers(0, w.nx * w.ny, 8192),
+                                     np.arange(0, 64), np.arange(w.nx * w.ny - 64, w.nx * w.ny)]))
+    idx = torch.from_numpy(cols).cuda()
+    flat = u.view(w.nz, w.nx * w.ny)
+    r_cols = flat[:, idx].t().contiguous().cpu().numpy()  # [ncols][nz], before the solve
+    r_max = float(u.abs().max())
+    pz.helmholtz_z_solve(plan, u)
+    torch.cuda.synchronize()
+    got = flat[:, idx].t().contiguous().cpu().numpy()
+    ref = oracle.helmholtz_z_solve_columns(zc, zf, w.a, r_cols)
+    assert rel_err(got, ref) <= TOL
+    assert float(u.abs().max()) <= r_max * (1 + 1e-12)    # maximum principle (M-matrix, row sums >= 1)
+    pz.poisson_plan_destroy(plan)
+
+
+def test_c3_poisson_backward_error_and_linearity(env):
+    torch, pz, wl, oracle = env
+    w = wl.CONFIGS["c3"]
+    zc, zf = wl.grid(w)
+    dzf, dzc = np.diff(zf), np.diff(zc)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    p = wl.device_remove_weighted_mean(wl.device_field(w, w.poisson_seed), zf)
+    f = p.cpu().numpy()
+    pz.poisson_solve(plan, p)
+    torch.cuda.synchronize()
+    phi = p.cpu().numpy()
+    # zero volume mean
+    wm = np.dot(dzf, phi.mean(axis=(1, 2))) / dzf.sum()
+    assert abs(wm) <= 1e-13 * np.abs(phi).max()
+    # normwise backward error with the ORACLE's operator
+    res = f - oracle.apply_poisson_operator(w.lx, w.ly, zc, zf, phi)
+    normL = 4 / (w.lx / w.nx) ** 2 + 4 / (w.ly / w.ny) ** 2 + 4 / (dzf.min() * dzc.min())
+    assert np.abs(res).max() <= 1e-13 * (normL * np.abs(phi).max() + np.abs(f).max())
+    del res, f
+    # linearity on the device: solve(f) + solve(g) == solve(f + g)
+    g = wl.device_remove_weighted_mean(wl.device_field(w, w.poisson_seed + 1), zf)
+    fg = torch.from_numpy(phi).cuda()                     # reuse: fg := f + g is rebuilt below
+    fg.copy_(wl.device_remove_weighted_mean(wl.device_field(w, w.poisson_seed), zf))
+    fg += g
+    pz.poisson_solve(plan, g)
+    pz.poisson_solve(plan, fg)
+    torch.cuda.synchronize()
+    fg -= g
+    fg -= torch.from_numpy(phi).cuda()
+    assert float(fg.abs().max()) <= 1e-11 * np.abs(phi).max()
+    pz.poisson_plan_destroy(plan)
