@@ -35,6 +35,14 @@ struct XchgX {
         return make_double2(re[q], im[q]);
     }
     __device__ __forceinline__ void sync() const { __syncthreads(); }
+    // unpadded access for the split exchange: written ascending, read descending, both contiguous
+    // (the Stockham padding would put positions q and q-15 of a 16-lane group into the same bank)
+    __device__ __forceinline__ void put_lin(int pos, double2 v) const
+    {
+        re[pos] = v.x;
+        im[pos] = v.y;
+    }
+    __device__ __forceinline__ double2 get_lin(int pos) const { return make_double2(re[pos], im[pos]); }
 };
 
 template <int M, int LPB, bool INV>
@@ -58,7 +66,7 @@ __global__ void __launch_bounds__(FftPlan<M>::T *LPB)
         fft_line<M, 2, 1>(v, tid, tw, xc);
         if constexpr (P::R2 > 1) xc.sync();
 #pragma unroll
-        for (int e = 0; e < E; ++e) xc.put(tid + e * T, v[e]);
+        for (int e = 0; e < E; ++e) xc.put_lin(tid + e * T, v[e]);
         xc.sync();
 #pragma unroll
         for (int e = 0; e < E; ++e) {
@@ -67,7 +75,7 @@ __global__ void __launch_bounds__(FftPlan<M>::T *LPB)
             if (k == 0) {
                 out = make_double2(v[e].x + v[e].y, v[e].x - v[e].y);
             } else {
-                const double2 zm = cconj(xc.get(M - k));
+                const double2 zm = cconj(xc.get_lin(M - k));
                 const double2 w = __ldg(&tw[k]);
                 const double2 ev = make_double2(0.5 * (v[e].x + zm.x), 0.5 * (v[e].y + zm.y));
                 const double2 d = csub(v[e], zm);
