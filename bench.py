@@ -298,15 +298,18 @@ def main():
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
     if not args.no_e2e:
-        host = torch.empty(w.n, dtype=torch.float64).pin_memory()
-        host.copy_((p if p is not None else us[0]).flatten())
+        # one pinned host buffer per field of the step; pz_solve_host_batch pipelines upload,
+        # solve and download of consecutive fields (full-duplex PCIe)
+        src = (p if p is not None else us[0]).flatten()
+        hosts = []
+        for _ in range(fields):
+            h = torch.empty(w.n, dtype=torch.float64).pin_memory()
+            h.copy_(src)
+            hosts.append(h)
         torch.cuda.synchronize()
 
         def e2e_step():
-            if w.poisson:
-                pz.poisson_solve_host(plan, host)
-            for _ in range(w.n_helmholtz):
-                pz.helmholtz_z_solve_host(plan, host)
+            pz.pz_solve_host_batch(plan, hosts[0] if w.poisson else None, hosts[1:] if w.poisson else hosts)
 
         e2e_step()
         barrier()
@@ -322,8 +325,8 @@ def main():
         e2e = {"value": fields * w.n * world * args.e2e_steps / (e_ms * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": fields * w.n * 8, "d2h_bytes_per_step": fields * w.n * 8,
                "steps": args.e2e_steps, "ms_per_step": e_ms / args.e2e_steps,
-               "api": "poisson_solve_host + helmholtz_z_solve_host (pinned host buffers)"}
-        del host
+               "api": "pz_solve_host_batch (pinned host buffers, one per field; upload / solve / download pipelined)"}
+        del hosts
 
     if rank != 0:
         if dist is not None:

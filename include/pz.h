@@ -109,6 +109,17 @@ PZ_API int helmholtz_z_solve_n(pz_plan *plan, double *const *u, int n, void *str
 PZ_API int poisson_solve_host(pz_plan *plan, double *p_host, void *stream);
 PZ_API int helmholtz_z_solve_host(pz_plan *plan, double *u_host, void *stream);
 
+/*
+ * One time step's worth of solves on HOST buffers, pipelined: the Poisson field p_host (may be
+ * NULL) and the n_u Helmholtz fields u_host[0..n_u-1] go through three device staging fields
+ * (owned by the plan, allocated on first use) so that the upload of field f+1, the solve of field
+ * f and the download of field f-1 overlap (two internal copy streams; the PCIe link is full
+ * duplex).  Ordered after prior work on `stream`; when `stream` has been synchronised every
+ * host buffer holds its solution.  Pinned host memory is needed for the copies to overlap.
+ * Errors: as the single-field calls; PZ_ENOTSETUP if n_u > 0 before helmholtz_z_setup.
+ */
+PZ_API int pz_solve_host_batch(pz_plan *plan, double *p_host, double *const *u_host, int n_u, void *stream);
+
 /* Frees every device and host resource of the plan.  NULL is accepted. */
 PZ_API int poisson_plan_destroy(pz_plan *plan);
 

@@ -33,6 +33,7 @@ SIGNATURES = {
     "helmholtz_z_solve_n": (_i, [_vp, ctypes.POINTER(_vp), _i, _vp]),
     "poisson_solve_host": (_i, [_vp, _vp, _vp]),
     "helmholtz_z_solve_host": (_i, [_vp, _vp, _vp]),
+    "pz_solve_host_batch": (_i, [_vp, _vp, ctypes.POINTER(_vp), ctypes.c_int, _vp]),
     "poisson_plan_destroy": (_i, [_vp]),
     "pz_last_error": (ctypes.c_char_p, []),
     "pz_poisson_stage": (_i, [_vp, _vp, _i, _vp]),
@@ -160,6 +161,14 @@ def helmholtz_z_solve_n(plan: Plan, fields, stream=None) -> None:
 
 def poisson_solve_host(plan: Plan, p_host, stream=None) -> None:
     _check(lib().poisson_solve_host(plan.handle, _host_ptr(p_host, plan.n), _stream_ptr(stream)))
+
+
+def pz_solve_host_batch(plan: Plan, p_host, u_hosts, stream=None) -> None:
+    """p_host: pinned host tensor or None; u_hosts: sequence of pinned host tensors."""
+    n = len(u_hosts)
+    arr = (_vp * max(n, 1))(*[_host_ptr(u, plan.n) for u in u_hosts])
+    _check(lib().pz_solve_host_batch(plan.handle, _host_ptr(p_host, plan.n) if p_host is not None else None,
+                                     arr, n, _stream_ptr(stream)))
 
 
 def helmholtz_z_solve_host(plan: Plan, u_host, stream=None) -> None:

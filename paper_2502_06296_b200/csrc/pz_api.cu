@@ -276,6 +276,11 @@ int poisson_plan_destroy(pz_plan *pl)
     if (pl->d_zwork) cudaFree(pl->d_zwork);
     if (pl->d_host_stage) cudaFree(pl->d_host_stage);
     if (pl->d_xyctr) cudaFree(pl->d_xyctr);
+    for (int b = 0; b < 3; ++b)
+        if (pl->d_batch_stage[b]) cudaFree(pl->d_batch_stage[b]);
+    if (pl->h2d_stream) cudaStreamDestroy(pl->h2d_stream);
+    if (pl->d2h_stream) cudaStreamDestroy(pl->d2h_stream);
+    for (auto e : pl->batch_events) cudaEventDestroy(e);
     for (int b = 0; b < 2; ++b) {
         if (pl->helm[b].dev) cudaFree(pl->helm[b].dev);
         if (pl->helm[b].uploaded) cudaEventDestroy(pl->helm[b].uploaded);
@@ -380,6 +385,51 @@ int helmholtz_z_solve_host(pz_plan *pl, double *u_host, void *stream)
     PZ_CUDA(cudaMemcpyAsync(pl->d_host_stage, u_host, pl->n * sizeof(double), cudaMemcpyHostToDevice, st));
     if ((rc = helmholtz_z_solve(pl, pl->d_host_stage, stream)) != PZ_OK) return rc;
     PZ_CUDA(cudaMemcpyAsync(u_host, pl->d_host_stage, pl->n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    return PZ_OK;
+}
+
+int pz_solve_host_batch(pz_plan *pl, double *p_host, double *const *u_host, int n_u, void *stream)
+{
+    if (!pl || n_u < 0 || (n_u > 0 && !u_host)) { set_error("pz_solve_host_batch: bad argument"); return PZ_EINVAL; }
+    for (int c = 0; c < n_u; ++c)
+        if (!u_host[c]) { set_error("pz_solve_host_batch: field %d is NULL", c); return PZ_EINVAL; }
+    if (n_u > 0 && pl->helm_cur < 0) { set_error("pz_solve_host_batch: call helmholtz_z_setup first"); return PZ_ENOTSETUP; }
+    const int nf = (p_host ? 1 : 0) + n_u;
+    if (nf == 0) return PZ_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = pl->n * sizeof(double);
+    for (int b = 0; b < 3 && b < nf; ++b)
+        if (!pl->d_batch_stage[b]) {
+            cudaError_t e = cudaMalloc(&pl->d_batch_stage[b], bytes);
+            if (e != cudaSuccess) { cudaGetLastError(); set_error("batch staging field: %s", cudaGetErrorString(e)); return PZ_ENOMEM; }
+        }
+    if (!pl->h2d_stream) PZ_CUDA(cudaStreamCreateWithFlags(&pl->h2d_stream, cudaStreamNonBlocking));
+    if (!pl->d2h_stream) PZ_CUDA(cudaStreamCreateWithFlags(&pl->d2h_stream, cudaStreamNonBlocking));
+    // events: [0] start, then per field (uploaded, solved, downloaded)
+    while ((int)pl->batch_events.size() < 1 + 3 * nf) {
+        cudaEvent_t e = nullptr;
+        PZ_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        pl->batch_events.push_back(e);
+    }
+    auto ev = [&](int f, int which) { return pl->batch_events[1 + 3 * f + which]; };
+    PZ_CUDA(cudaEventRecord(pl->batch_events[0], st));
+    PZ_CUDA(cudaStreamWaitEvent(pl->h2d_stream, pl->batch_events[0], 0));
+    for (int f = 0; f < nf; ++f) {
+        const bool is_p = (p_host && f == 0);
+        double *host = is_p ? p_host : u_host[f - (p_host ? 1 : 0)];
+        double *dev = pl->d_batch_stage[f % 3];
+        if (f >= 3) PZ_CUDA(cudaStreamWaitEvent(pl->h2d_stream, ev(f - 3, 2), 0)); // staging field free again
+        PZ_CUDA(cudaMemcpyAsync(dev, host, bytes, cudaMemcpyHostToDevice, pl->h2d_stream));
+        PZ_CUDA(cudaEventRecord(ev(f, 0), pl->h2d_stream));
+        PZ_CUDA(cudaStreamWaitEvent(st, ev(f, 0), 0));
+        const int rc = is_p ? poisson_solve(pl, dev, stream) : helmholtz_z_solve(pl, dev, stream);
+        if (rc != PZ_OK) return rc;
+        PZ_CUDA(cudaEventRecord(ev(f, 1), st));
+        PZ_CUDA(cudaStreamWaitEvent(pl->d2h_stream, ev(f, 1), 0));
+        PZ_CUDA(cudaMemcpyAsync(host, dev, bytes, cudaMemcpyDeviceToHost, pl->d2h_stream));
+        PZ_CUDA(cudaEventRecord(ev(f, 2), pl->d2h_stream));
+    }
+    PZ_CUDA(cudaStreamWaitEvent(st, ev(nf - 1, 2), 0)); // downloads are in order on one stream
     return PZ_OK;
 }
 

@@ -66,6 +66,10 @@ struct pz_plan {
     // optional workspaces (allocated on first use)
     double *d_zwork = nullptr;       // variant-0 z solve: N doubles
     double *d_host_stage = nullptr;  // *_host calls: N doubles
+    // pz_solve_host_batch: staging fields, copy streams, events (created on first use)
+    double *d_batch_stage[3] = {nullptr, nullptr, nullptr};
+    cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
+    std::vector<cudaEvent_t> batch_events;
     int *d_xyctr = nullptr;          // fused x/y kernels: 2 x (1 + nz) ticket / per-plane counters
 
     // Helmholtz

@@ -361,6 +361,34 @@ def test_host_buffer_entry_points(torch, pz, wl, oracle):
     assert rel_err(hb.numpy(), oracle.helmholtz_z_solve(zc, zf, w.a, r)) <= TOL
 
 
+def test_host_batch_pipeline(torch, pz, wl, oracle):
+    """pz_solve_host_batch: Poisson + several Helmholtz fields on pinned host buffers, more fields
+    than staging buffers, twice in a row on a side stream."""
+    w = wl.scaled(wl.CONFIGS["c1"], 64, 32, 48)
+    zc, zf = wl.grid(w)
+    f = wl.poisson_rhs(w)
+    rs = [np.random.default_rng(40 + c).standard_normal((w.nz, w.ny, w.nx)) for c in range(5)]
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    pz.helmholtz_z_setup(plan, w.a)
+    ref_p = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)
+    ref_u = [oracle.helmholtz_z_solve(zc, zf, w.a, r) for r in rs]
+    s = torch.cuda.Stream()
+    for _ in range(2):
+        hp = torch.from_numpy(f.copy()).pin_memory()
+        hu = [torch.from_numpy(r.copy()).pin_memory() for r in rs]
+        with torch.cuda.stream(s):
+            pz.pz_solve_host_batch(plan, hp, hu)
+        s.synchronize()
+        assert rel_err(hp.numpy(), ref_p) <= TOL
+        for h, ref in zip(hu, ref_u):
+            assert rel_err(h.numpy(), ref) <= TOL
+    hu = [torch.from_numpy(rs[0].copy()).pin_memory()]
+    pz.pz_solve_host_batch(plan, None, hu)               # Helmholtz only, default stream
+    torch.cuda.synchronize()
+    assert rel_err(hu[0].numpy(), ref_u[0]) <= TOL
+    pz.poisson_plan_destroy(plan)
+
+
 # ------------------------------------------------------- BASELINE configs 1 and 2 in full
 
 def test_config1_poisson_and_helmholtz_full(torch, pz, wl, oracle):
