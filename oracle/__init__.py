@@ -27,4 +27,6 @@ from .cpu import (  # noqa: F401
     poisson_solve,
     helmholtz_z_solve,
     helmholtz_z_solve_columns,
+    apply_helmholtz3d_operator,
+    helmholtz3d_solve,
 )

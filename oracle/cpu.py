@@ -189,3 +189,29 @@ def helmholtz_z_solve_columns(zc, zf, a: float, rcols: np.ndarray) -> np.ndarray
     if rc != 0:
         raise MemoryError("orc_helmholtz_z_solve_columns: allocation failed")
     return ucols
+
+
+def apply_helmholtz3d_operator(lx: float, ly: float, zc, zf, a: float, u: np.ndarray) -> np.ndarray:
+    """u[nz][ny][nx] -> (I - a L_h) u, definition O-H3 (periodic x, y; Dirichlet walls in z)."""
+    u = _c(u)
+    nz, ny, nx = u.shape
+    zc, zf = _c(zc), _c(zf)
+    out = np.empty_like(u)
+    lib().orc_apply_helmholtz3d_operator(ctypes.c_int(nx), ctypes.c_int(ny), ctypes.c_int(nz),
+                                         ctypes.c_double(lx), ctypes.c_double(ly), _p(zc), _p(zf),
+                                         ctypes.c_double(a), _p(u), _p(out))
+    return out
+
+
+def helmholtz3d_solve(lx: float, ly: float, zc, zf, a: float, r: np.ndarray, variant: int = 1) -> np.ndarray:
+    """r[nz][ny][nx] -> u with (I - a L_h) u = r (Eq. 8).  variant as poisson_solve."""
+    r = _c(r)
+    nz, ny, nx = r.shape
+    zc, zf = _c(zc), _c(zf)
+    u = np.empty_like(r)
+    rc = lib().orc_helmholtz3d_solve(ctypes.c_int(nx), ctypes.c_int(ny), ctypes.c_int(nz),
+                                     ctypes.c_double(lx), ctypes.c_double(ly), _p(zc), _p(zf),
+                                     ctypes.c_double(a), _p(r), _p(u), ctypes.c_int(variant))
+    if rc != 0:
+        raise MemoryError("orc_helmholtz3d_solve: allocation failed")
+    return u

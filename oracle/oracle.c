@@ -400,3 +400,89 @@ int orc_helmholtz_z_solve_columns(int nz, const double *zc, const double *zf, do
     free(m);
     return 0;
 }
+
+/* ------------------------------------------- fully implicit diffusion, Eq. (8) */
+
+/* u -> (I - a L_h) u with periodic x, y and Dirichlet walls in z (definition O-H3):
+ *   u - a [ (u_{i+1} - 2u + u_{i-1})/dx^2 + (u_{j+1} - 2u + u_{j-1})/dy^2
+ *           + A_k (u_{k-1} - u) + C_k (u_{k+1} - u) - W_k u ],
+ * W_k as in orc_helmholtz_matrix (reading R7).  PAPER.md:63 (Eq. 8): "a Helmholtz equation for
+ * the prediction velocity, implicit in the three spatial directions". */
+void orc_apply_helmholtz3d_operator(int nx, int ny, int nz, double lx, double ly,
+                                    const double *zc, const double *zf, double a,
+                                    const double *u, double *out)
+{
+    double *dzf = (double *)malloc(sizeof(double) * 4 * (size_t)nz);
+    double *dzc = dzf + nz, *A = dzf + 2 * nz, *C = dzf + 3 * nz;
+    orc_z_tables(nz, zc, zf, dzf, dzc, A, C);
+    const double dx = lx / nx, dy = ly / ny;
+    const double rdx2 = 1.0 / (dx * dx), rdy2 = 1.0 / (dy * dy);
+    const double W0 = 2.0 / (dzf[0] * (2.0 * (zc[0] - zf[0])));
+    const double W1 = 2.0 / (dzf[nz - 1] * (2.0 * (zf[nz] - zc[nz - 1])));
+    const size_t plane = (size_t)nx * ny;
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const size_t c = (size_t)k * plane + (size_t)j * nx + i;
+                const int ip = (i + 1) % nx, im = (i + nx - 1) % nx;
+                const int jp = (j + 1) % ny, jm = (j + ny - 1) % ny;
+                const double pc = u[c];
+                double v = (u[c - i + ip] - 2.0 * pc + u[c - i + im]) * rdx2
+                         + (u[c - (size_t)j * nx + (size_t)jp * nx] - 2.0 * pc
+                            + u[c - (size_t)j * nx + (size_t)jm * nx]) * rdy2;
+                if (k > 0)      v += A[k] * (u[c - plane] - pc);
+                if (k + 1 < nz) v += C[k] * (u[c + plane] - pc);
+                if (k == 0)      v -= W0 * pc;
+                if (k == nz - 1) v -= W1 * pc;
+                out[c] = pc - a * v;
+            }
+    free(dzf);
+}
+
+/* 3-D Helmholtz solve, out of place: r[N] -> u[N], (I - a L_h) u = r.  The same eigenfunction
+ * expansion as the Poisson solve ("Poisson/Helmholtz equation"): transforms
+ * along x and y, then per (qx, qy) one plain Thomas solve of
+ *   -a A_k u_{k-1} + (1 + a (A_k + C_k + W_k + sigma)) u_k - a C_k u_{k+1} = r~_k,
+ * sigma = -(lambda_x + lambda_y) >= 0, inverse transforms.  The matrix is strictly diagonally
+ * dominant with positive diagonal: no cancellation, no pin. */
+int orc_helmholtz3d_solve(int nx, int ny, int nz, double lx, double ly,
+                          const double *zc, const double *zf, double a,
+                          const double *r, double *u, int variant)
+{
+    const size_t plane = (size_t)nx * ny, N = plane * (size_t)nz;
+    double *re = (double *)malloc(sizeof(double) * N);
+    double *im = (double *)calloc(N, sizeof(double));
+    double *tab = (double *)malloc(sizeof(double) * (3 * (size_t)nz + nx + ny));
+    if (!re || !im || !tab) { free(re); free(im); free(tab); return 1; }
+    double *lo = tab, *di = tab + nz, *up = tab + 2 * nz;
+    double *lamx = tab + 3 * nz, *lamy = lamx + nx;
+    orc_helmholtz_matrix(nz, zc, zf, a, lo, di, up);
+    orc_lambda(nx, lx, lamx);
+    orc_lambda(ny, ly, lamy);
+    memcpy(re, r, sizeof(double) * N);
+
+    orc_dft_xy(nx, ny, nz, -1, variant, re, im);
+
+#pragma omp parallel
+    {
+        double *work = (double *)malloc(sizeof(double) * 3 * (size_t)nz);
+        double *dk = work + 2 * nz;
+#pragma omp for schedule(static)
+        for (long long c = 0; c < (long long)plane; ++c) {
+            const int qy = (int)(c / nx), qx = (int)(c % nx);
+            const double sigma = -(lamx[qx] + lamy[qy]);
+            for (int k = 0; k < nz; ++k) dk[k] = di[k] + a * sigma;
+            orc_thomas(nz, lo, dk, up, re + c, re + c, plane, work);
+            orc_thomas(nz, lo, dk, up, im + c, im + c, plane, work);
+        }
+        free(work);
+    }
+
+    orc_dft_xy(nx, ny, nz, +1, variant, re, im);
+    const double scale = 1.0 / ((double)nx * (double)ny);
+#pragma omp parallel for schedule(static)
+    for (long long c = 0; c < (long long)N; ++c) u[c] = re[c] * scale;
+    free(re); free(im); free(tab);
+    return 0;
+}
