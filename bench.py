@@ -295,6 +295,23 @@ def main():
     t_max = ranks.max_over_ranks(ms_total, dist, "cuda")
     value = ranks.whole_job_rate(fields * w.n * steps, world, t_max)
 
+    # ---- next-row capability, outside the timed region: the fully implicit Helmholtz solve of Eq. (8)
+    h3 = None
+    if w.poisson and w.nz <= 1024:
+        pz.helmholtz3d_setup(plan, w.a if w.a > 0 else 2.5e-5)
+        for _ in range(2):
+            pz.helmholtz3d_solve(plan, p)
+        h0, h1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        h0.record()
+        for _ in range(5):
+            pz.helmholtz3d_solve(plan, p)
+        h1.record()
+        torch.cuda.synchronize()
+        h3_ms = h0.elapsed_time(h1) / 5
+        h3 = {"ms_per_solve": h3_ms, "points_per_s": w.n / (h3_ms * 1e-3),
+              "hbm_frac_48B_per_point": 48.0 * w.n / (h3_ms * 1e-3) / 1e9 / measured_peak()[0]}
+
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -382,6 +399,8 @@ def main():
                               "strict_16B_poisson_frac": ((16.0 * fields) * w.n * steps / (ms_total * 1e-3) / 1e9 / peak)},
         "kernels": per_kernel,
     }
+    if h3 is not None:
+        line["helmholtz3d"] = h3
     if e2e is not None:
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:

@@ -102,6 +102,23 @@ PZ_API int helmholtz_z_solve(pz_plan *plan, double *u, void *stream);
 PZ_API int helmholtz_z_solve_n(pz_plan *plan, double *const *u, int n, void *stream);
 
 /*
+ * Fully implicit diffusion, Eq. (8), PAPER.md:63-72 ("a Helmholtz equation for the prediction
+ * velocity, implicit in the three spatial directions", solved "using the fast direct methods" of
+ * the Poisson solve): for a = gamma_k nu dt / 2 >= 0 solves, in place,
+ *   (I - a L_h) u = r,   L_h = the 7-point Laplacian of poisson_solve in x, y (periodic) and
+ *   A_k (u_{k-1}-u_k) + C_k (u_{k+1}-u_k) - W_k u_k in z (u = 0 on the wall faces, W as above).
+ * Same pipeline as poisson_solve: transforms along x and y, one tridiagonal solve per (kx,ky)
+ * with diagonal 1 + a (A_k + C_k + W_k - lambda_x - lambda_y), inverse transforms.  The systems
+ * are non-singular for every mode (no pinned column).  helmholtz3d_setup only records a (the
+ * coefficient tables are scaled inside the kernel), so it may be called between any two solves.
+ *   u  device, nx*ny*nz doubles, 16-byte aligned, in place.  nz <= 1024.
+ * Errors: PZ_ENOTSETUP before the first setup; PZ_EINVAL for a < 0 or null pointers;
+ * PZ_EUNSUPPORTED for nz > 1024.
+ */
+PZ_API int helmholtz3d_setup(pz_plan *plan, double a);
+PZ_API int helmholtz3d_solve(pz_plan *plan, double *u, void *stream);
+
+/*
  * End-to-end variants with HOST buffers: copy host -> device workspace (owned by the plan,
  * allocated on first use: nx*ny*nz doubles), solve, copy back, all asynchronously on
  * `stream`.  The host buffer must stay valid until the stream has been synchronised.

@@ -33,6 +33,8 @@ SIGNATURES = {
     "helmholtz_z_solve_n": (_i, [_vp, ctypes.POINTER(_vp), _i, _vp]),
     "poisson_solve_host": (_i, [_vp, _vp, _vp]),
     "helmholtz_z_solve_host": (_i, [_vp, _vp, _vp]),
+    "helmholtz3d_setup": (_i, [_vp, ctypes.c_double]),
+    "helmholtz3d_solve": (_i, [_vp, _vp, _vp]),
     "pz_solve_host_batch": (_i, [_vp, _vp, ctypes.POINTER(_vp), ctypes.c_int, _vp]),
     "poisson_plan_destroy": (_i, [_vp]),
     "pz_last_error": (ctypes.c_char_p, []),
@@ -161,6 +163,14 @@ def helmholtz_z_solve_n(plan: Plan, fields, stream=None) -> None:
 
 def poisson_solve_host(plan: Plan, p_host, stream=None) -> None:
     _check(lib().poisson_solve_host(plan.handle, _host_ptr(p_host, plan.n), _stream_ptr(stream)))
+
+
+def helmholtz3d_setup(plan: Plan, a: float) -> None:
+    _check(lib().helmholtz3d_setup(plan.handle, float(a)))
+
+
+def helmholtz3d_solve(plan: Plan, u, stream=None) -> None:
+    _check(lib().helmholtz3d_solve(plan.handle, _dev_ptr(u, plan.n), _stream_ptr(stream)))
 
 
 def pz_solve_host_batch(plan: Plan, p_host, u_hosts, stream=None) -> None:

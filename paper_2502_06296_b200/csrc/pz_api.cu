@@ -227,6 +227,8 @@ int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double
         pl->C[k] = (k + 1 < nz) ? 1.0 / (pl->dzf[k] * pl->dzc[k]) : 0.0;
     }
     pl->inv_lz = 1.0 / lz;
+    pl->wall_w0 = 2.0 / (pl->dzf[0] * (2.0 * (zc[0] - zf[0])));
+    pl->wall_w1 = 2.0 / (pl->dzf[nz - 1] * (2.0 * (zf[nz] - zc[nz - 1])));
 
     // one device allocation for all tables
     const size_t ndbl = 3 * (size_t)nz + (size_t)nx + 2 * (size_t)ny + 2 * (size_t)nx + 2 * (size_t)ny + 8;
@@ -329,6 +331,27 @@ int poisson_solve(pz_plan *pl, double *p, void *stream)
     if ((rc = forward_xy(pl, p, st)) != PZ_OK) return rc;
     if ((rc = launch_zsolve(pl, p, st)) != PZ_OK) return rc;
     return inverse_xy(pl, p, st);
+}
+
+int helmholtz3d_setup(pz_plan *pl, double a)
+{
+    if (!pl) { set_error("helmholtz3d_setup: plan is NULL"); return PZ_EINVAL; }
+    if (!(a >= 0.0) || !std::isfinite(a)) { set_error("helmholtz3d_setup: a must be finite and >= 0"); return PZ_EINVAL; }
+    pl->h3_a = a; // the coefficient tables are scaled inside the kernel: nothing to upload
+    return PZ_OK;
+}
+
+int helmholtz3d_solve(pz_plan *pl, double *u, void *stream)
+{
+    if (!pl || !u) { set_error("helmholtz3d_solve: NULL argument"); return PZ_EINVAL; }
+    if (((uintptr_t)u & 15) != 0) { set_error("helmholtz3d_solve: u must be 16-byte aligned"); return PZ_EINVAL; }
+    if (pl->h3_a < 0.0) { set_error("helmholtz3d_solve: call helmholtz3d_setup first"); return PZ_ENOTSETUP; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 1) * sizeof(int), st));
+    if ((rc = forward_xy(pl, u, st)) != PZ_OK) return rc;
+    if ((rc = launch_zsolve(pl, u, st, pl->h3_a)) != PZ_OK) return rc;
+    return inverse_xy(pl, u, st);
 }
 
 int helmholtz_z_setup(pz_plan *pl, double a)

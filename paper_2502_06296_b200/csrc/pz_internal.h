@@ -62,6 +62,8 @@ struct pz_plan {
     double2 *d_twx = nullptr;        // nx: exp(-2 pi i k / nx)
     double2 *d_twy = nullptr;        // ny: exp(-2 pi i k / ny)
     double inv_lz = 0;               // 1 / sum dzf
+    double wall_w0 = 0, wall_w1 = 0; // Dirichlet wall terms W_0, W_{nz-1} of the Helmholtz operators
+    double h3_a = -1.0;              // helmholtz3d_setup: a of the fully implicit Helmholtz solve
 
     // optional workspaces (allocated on first use)
     double *d_zwork = nullptr;       // variant-0 z solve: N doubles
@@ -115,7 +117,7 @@ struct ProfScope {
 int launch_fft_x(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
 int launch_fft_y(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
 int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
-int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st);
+int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a = -1.0); // helm_a >= 0: Eq. (8) systems
 int launch_fft_xy_fwd(pz_plan *pl, double *p, cudaStream_t st);
 int launch_fft_xy_inv(pz_plan *pl, double *p, cudaStream_t st);
 int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st);

@@ -18,8 +18,8 @@
 
 namespace pz {
 
-int launch_zsolve_cr(pz_plan *pl, double *p, cudaStream_t st);
-int launch_zsolve_tma(pz_plan *pl, double *p, cudaStream_t st);
+int launch_zsolve_cr(pz_plan *pl, double *p, cudaStream_t st, double helm_a);
+int launch_zsolve_tma(pz_plan *pl, double *p, cudaStream_t st, double helm_a);
 
 namespace {
 
@@ -75,10 +75,14 @@ __global__ void __launch_bounds__(128)
 
 } // namespace
 
-int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st)
+int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
 {
-    if (pl->opt.zsolve_variant == 1) return launch_zsolve_cr(pl, p, st);
-    if (pl->opt.zsolve_variant == 2) return launch_zsolve_tma(pl, p, st);
+    if (pl->opt.zsolve_variant == 1) return launch_zsolve_cr(pl, p, st, helm_a);
+    if (pl->opt.zsolve_variant == 2) return launch_zsolve_tma(pl, p, st, helm_a);
+    if (helm_a >= 0.0) {
+        set_error("helmholtz3d_solve needs z-solve variant 1 or 2 (nz <= 1024)");
+        return PZ_EUNSUPPORTED;
+    }
     if (!pl->d_zwork) {
         cudaError_t e = cudaMalloc(&pl->d_zwork, pl->n * sizeof(double));
         if (e != cudaSuccess) {

@@ -29,12 +29,12 @@ struct RowAcc {
     __device__ __forceinline__ double2 &operator()(int i) const { return d[i * (kTX / 2)]; }
 };
 
-template <int M>
+template <int M, bool HELM>
 __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 1))
     zsolve_cr_kernel(double *__restrict__ p, const double *__restrict__ A, const double *__restrict__ C,
                      const double *__restrict__ dzf, const double *__restrict__ lamx,
                      const double *__restrict__ lamy_nat, const double *__restrict__ lamy_pk, int nx, int ny,
-                     int nz, double inv_lz)
+                     int nz, double inv_lz, double ha, double hw0, double hw1)
 {
     constexpr int CH = M * kTX + 2;  // doubles per sub-domain in the tile (+2: bank spread, 16-B aligned)
     constexpr int CS = M + 1;        // coefficient stride per lane (bank spread)
@@ -42,6 +42,7 @@ __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 
     double *tile = smem_z;                     // kLanes * CH
     double *s_al = tile + kLanes * CH;         // kLanes * CS
     double *s_ga = s_al + kLanes * CS;
+    double *s_e0 = s_ga + kLanes * CS;
 
     const size_t plane = (size_t)nx * ny;
     const size_t col0 = (size_t)blockIdx.x * kTX;
@@ -54,8 +55,10 @@ __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 
             *reinterpret_cast<double2 *>(tile + (k / M) * CH + (k % M) * kTX + c2) = v;
         }
         for (int k = threadIdx.x; k < kLanes * M; k += blockDim.x) {
-            s_al[(k / M) * CS + (k % M)] = (k < nz) ? A[k] : 0.0;
-            s_ga[(k / M) * CS + (k % M)] = (k < nz) ? C[k] : 0.0;
+            const double sc = HELM ? ha : 1.0;
+            s_al[(k / M) * CS + (k % M)] = (k < nz) ? sc * A[k] : 0.0;
+            s_ga[(k / M) * CS + (k % M)] = (k < nz) ? sc * C[k] : 0.0;
+            s_e0[(k / M) * CS + (k % M)] = 1.0 + ha * ((k == 0 ? hw0 : 0.0) + (k == nz - 1 ? hw1 : 0.0));
         }
     }
     __syncthreads();
@@ -69,7 +72,15 @@ __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 
         const RowAcc d{reinterpret_cast<double2 *>(tile + lane * CH + 2 * q)};
         const double *al = s_al + lane * CS, *ga = s_ga + lane * CS;
         const int k0 = lane * M;
-        if (sig0 == sig1) {
+        if constexpr (HELM) {
+            const double *e0 = s_e0 + lane * CS;
+            if (sig0 == sig1) {
+                solve_pair<M, 3, false, false, true>(d, al, ga, ha * sig0, k0, nz, dzf, inv_lz, e0);
+            } else {
+                solve_pair<M, 1, false, false, true>(d, al, ga, ha * sig0, k0, nz, dzf, inv_lz, e0);
+                solve_pair<M, 2, false, false, true>(d, al, ga, ha * sig1, k0, nz, dzf, inv_lz, e0);
+            }
+        } else if (sig0 == sig1) {
             solve_pair<M, 3, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
         } else {
             // pair 0 of a row: x-modes 0 and nx/2 have different eigenvalues; (0,0) is singular
@@ -91,21 +102,21 @@ __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 
     }
 }
 
-template <int M>
-int launch_m(pz_plan *pl, double *p, cudaStream_t st)
+template <int M, bool HELM>
+int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha)
 {
-    constexpr size_t smem = ((size_t)kLanes * (M * kTX + 2) + 2 * (size_t)kLanes * (M + 1)) * sizeof(double);
+    constexpr size_t smem = ((size_t)kLanes * (M * kTX + 2) + 3 * (size_t)kLanes * (M + 1)) * sizeof(double);
     static bool attr_done = false;
     if (smem > 48 * 1024 && !attr_done) {
-        PZ_CUDA(cudaFuncSetAttribute(zsolve_cr_kernel<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PZ_CUDA(cudaFuncSetAttribute(zsolve_cr_kernel<M, HELM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
     }
     const size_t plane = (size_t)pl->nx * pl->ny;
     const unsigned blocks = (unsigned)(plane / kTX);
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
-    zsolve_cr_kernel<M><<<blocks, kPairs * kLanes, smem, st>>>(p, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
-                                                                pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny,
-                                                                pl->nz, pl->inv_lz);
+    zsolve_cr_kernel<M, HELM><<<blocks, kPairs * kLanes, smem, st>>>(p, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
+                                                                      pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny,
+                                                                      pl->nz, pl->inv_lz, ha, pl->wall_w0, pl->wall_w1);
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
@@ -113,13 +124,15 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st)
 
 } // namespace
 
-int launch_zsolve_cr(pz_plan *pl, double *p, cudaStream_t st)
+int launch_zsolve_cr(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
 {
     const int nz = pl->nz;
-    if (nz <= 32 * 4) return launch_m<4>(pl, p, st);
-    if (nz <= 32 * 8) return launch_m<8>(pl, p, st);
-    if (nz <= 32 * 16) return launch_m<16>(pl, p, st);
-    if (nz <= 32 * 32) return launch_m<32>(pl, p, st);
+#define PZ_ZC(MM) (helm_a >= 0.0 ? launch_m<MM, true>(pl, p, st, helm_a) : launch_m<MM, false>(pl, p, st, 0.0))
+    if (nz <= 32 * 4) return PZ_ZC(4);
+    if (nz <= 32 * 8) return PZ_ZC(8);
+    if (nz <= 32 * 16) return PZ_ZC(16);
+    if (nz <= 32 * 32) return PZ_ZC(32);
+#undef PZ_ZC
     set_error("z-solve variant 1 supports nz <= 1024 (got %d); use zsolve_variant = 0", nz);
     return PZ_EUNSUPPORTED;
 }

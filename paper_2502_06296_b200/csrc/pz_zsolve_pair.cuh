@@ -38,15 +38,21 @@ __device__ __forceinline__ double shfl_down(double v, int d) { return __shfl_dow
 //   C  rows 1..M-2 forward: g_i = (r_i + alpha_i g_{i-1}) rb_i with g_0 := x_0  (overwrites the tile)
 //   D  rows M-2..1 backward: x_i = g_i + gamma_i rb_i x_{i+1}
 // FULL: nz == 32 M and the column is not the pinned one: no padding rows, no row tests.
-template <int M, int MASK, bool pin, bool FULL = false, class Acc>
+// HELM: the fully implicit Helmholtz system of Eq. (8), in the same M-matrix form:
+//   -a A_k x_{k-1} + (a A_k + a C_k + ex0_k + a sigma) x_k - a C_k x_{k+1} = +d_k,
+// al/ga hold a A_k / a C_k, ex0_k = 1 + a W_k (Dirichlet wall term), sigma is passed pre-scaled.
+template <int M, int MASK, bool pin, bool FULL = false, bool HELM = false, class Acc>
 __device__ __forceinline__ void solve_pair(const Acc d, const double *al, const double *ga, double sigma,
-                                           int k0, int nz, const double *__restrict__ dzf, double inv_lz)
+                                           int k0, int nz, const double *__restrict__ dzf, double inv_lz,
+                                           const double *ex0 = nullptr)
 {
+    static_assert(!(HELM && (pin || FULL)), "the Helmholtz system has no pinned column and takes the general path");
     // row coefficients: real rows have excess sigma, padding rows (k >= nz) are x = 0,
     // the pinned row (gauge of the singular column) likewise.
     static_assert(!(FULL && pin), "the pinned column takes the general path");
     auto eps_of = [&](int i) {
         if constexpr (FULL) return sigma;
+        else if constexpr (HELM) return (k0 + i < nz) ? ex0[i] + sigma : 1.0;
         else return (k0 + i < nz && !(pin && k0 + i == nz - 1)) ? sigma : 1.0;
     };
     auto alpha_of = [&](int i) { return (pin && k0 + i == nz - 1) ? 0.0 : al[i]; };
@@ -56,7 +62,8 @@ __device__ __forceinline__ void solve_pair(const Acc d, const double *al, const 
             return make_double2(-v.x, -v.y);
         } else {
             const bool live = (k0 + i < nz) && !(pin && k0 + i == nz - 1);
-            return live ? make_double2(-v.x, -v.y) : make_double2(0.0, 0.0);
+            if constexpr (HELM) return live ? v : make_double2(0.0, 0.0);
+            else return live ? make_double2(-v.x, -v.y) : make_double2(0.0, 0.0);
         }
     };
 

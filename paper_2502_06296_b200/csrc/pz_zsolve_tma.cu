@@ -49,16 +49,19 @@ template <int M> struct Geo {
     static constexpr int SLOT = M + 1;                       // rows per sub-domain slot
     static constexpr size_t STAGE = (size_t)kLanes * SLOT * 128;
     static constexpr int CS = M + 1;                         // coefficient stride per lane
-    static constexpr size_t COEF = (size_t)2 * kLanes * CS * sizeof(double);
+    static constexpr size_t COEF = (size_t)3 * kLanes * CS * sizeof(double);   // alpha, gamma, e0
     __host__ __device__ static size_t bytes(int stages) { return 1024 + stages * STAGE + COEF + 64; }
 };
 
-template <int M>
+// HELM = false: the Poisson systems (diagonal excess sigma = -(lambda_x + lambda_y), rhs -d, (0,0)
+// pinned).  HELM = true: the fully implicit Helmholtz systems of Eq. (8) with a = ha and the
+// Dirichlet wall terms hw0, hw1 (solve_pair, HELM).
+template <int M, bool HELM>
 __global__ void __launch_bounds__(kThreads, 1)
     zsolve_tma_kernel(const __grid_constant__ CUtensorMap map, const double *__restrict__ A,
                       const double *__restrict__ C, const double *__restrict__ dzf, const double *__restrict__ lamx,
                       const double *__restrict__ lamy_nat, const double *__restrict__ lamy_pk, int nx, int ny, int nz,
-                      double inv_lz, int ntiles, int stages)
+                      double inv_lz, int ntiles, int stages, double ha, double hw0, double hw1)
 {
     using G = Geo<M>;
     extern __shared__ unsigned char smem_zt[];
@@ -66,7 +69,8 @@ __global__ void __launch_bounds__(kThreads, 1)
     unsigned char *base = smem_zt + ((1024u - (smem_u32(smem_zt) & 1023u)) & 1023u);
     double *s_al = reinterpret_cast<double *>(base + stages * G::STAGE);
     double *s_ga = s_al + kLanes * G::CS;
-    uint64_t *full = reinterpret_cast<uint64_t *>(s_ga + kLanes * G::CS);
+    double *s_e0 = s_ga + kLanes * G::CS;
+    uint64_t *full = reinterpret_cast<uint64_t *>(s_e0 + kLanes * G::CS);
     uint64_t *done = full + 4;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -78,8 +82,10 @@ __global__ void __launch_bounds__(kThreads, 1)
         mbar_fence_init();
     }
     for (int k = threadIdx.x; k < kLanes * M; k += blockDim.x) {
-        s_al[(k / M) * G::CS + (k % M)] = (k < nz) ? A[k] : 0.0;
-        s_ga[(k / M) * G::CS + (k % M)] = (k < nz) ? C[k] : 0.0;
+        const double sc = HELM ? ha : 1.0;
+        s_al[(k / M) * G::CS + (k % M)] = (k < nz) ? sc * A[k] : 0.0;
+        s_ga[(k / M) * G::CS + (k % M)] = (k < nz) ? sc * C[k] : 0.0;
+        s_e0[(k / M) * G::CS + (k % M)] = 1.0 + ha * ((k == 0 ? hw0 : 0.0) + (k == nz - 1 ? hw1 : 0.0));
     }
     __syncthreads();
 
@@ -129,7 +135,15 @@ __global__ void __launch_bounds__(kThreads, 1)
         const double sig0 = -(lamx[i] + ly), sig1 = -(lamx[i + 1] + ly);
         d.slot = base + b * G::STAGE + (size_t)R0 * 128;
         mbar_wait(&full[b], (it / stages) & 1);
-        if (sig0 == sig1) {
+        if constexpr (HELM) {
+            const double *e0 = s_e0 + lane * G::CS;
+            if (sig0 == sig1) {
+                solve_pair<M, 3, false, false, true>(d, al, ga, ha * sig0, k0, nz, dzf, inv_lz, e0);
+            } else {
+                solve_pair<M, 1, false, false, true>(d, al, ga, ha * sig0, k0, nz, dzf, inv_lz, e0);
+                solve_pair<M, 2, false, false, true>(d, al, ga, ha * sig1, k0, nz, dzf, inv_lz, e0);
+            }
+        } else if (sig0 == sig1) {
             if (no_pad) solve_pair<M, 3, false, true>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
             else solve_pair<M, 3, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
         } else {
@@ -146,8 +160,8 @@ __global__ void __launch_bounds__(kThreads, 1)
     }
 }
 
-template <int M>
-int launch_m(pz_plan *pl, double *p, cudaStream_t st)
+template <int M, bool HELM>
+int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha)
 {
     using G = Geo<M>;
     int stages = (int)((227 * 1024 - 1024 - G::COEF - 64) / G::STAGE);
@@ -157,7 +171,7 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st)
     const size_t smem = G::bytes(stages);
     static bool attr_done = false;
     if (!attr_done) {
-        PZ_CUDA(cudaFuncSetAttribute(zsolve_tma_kernel<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        PZ_CUDA(cudaFuncSetAttribute(zsolve_tma_kernel<M, HELM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         attr_done = true;
     }
     const size_t plane = (size_t)pl->nx * pl->ny;
@@ -166,13 +180,14 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st)
     if (rc != PZ_OK) return rc;
     const int ntiles = (int)(plane / kTX);
     int occ = 1;
-    if (smem * 2 <= 227 * 1024) PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, zsolve_tma_kernel<M>, kThreads, smem));
+    if (smem * 2 <= 227 * 1024) PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, zsolve_tma_kernel<M, HELM>, kThreads, smem));
     if (occ < 1) occ = 1;
     int blocks = pl->num_sms * occ;
     if (blocks > ntiles) blocks = ntiles;
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
-    zsolve_tma_kernel<M><<<blocks, kThreads, smem, st>>>(map, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx, pl->d_lamy_nat,
-                                                          pl->d_lamy_pk, pl->nx, pl->ny, pl->nz, pl->inv_lz, ntiles, stages);
+    zsolve_tma_kernel<M, HELM><<<blocks, kThreads, smem, st>>>(map, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
+                                                                pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, pl->nz,
+                                                                pl->inv_lz, ntiles, stages, ha, pl->wall_w0, pl->wall_w1);
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
@@ -180,13 +195,16 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st)
 
 } // namespace
 
-int launch_zsolve_tma(pz_plan *pl, double *p, cudaStream_t st)
+// helm_a < 0: the Poisson systems; helm_a >= 0: the fully implicit Helmholtz systems with a = helm_a.
+int launch_zsolve_tma(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
 {
     const int nz = pl->nz;
-    if (nz <= 32 * 4) return launch_m<4>(pl, p, st);
-    if (nz <= 32 * 8) return launch_m<8>(pl, p, st);
-    if (nz <= 32 * 16) return launch_m<16>(pl, p, st);
-    if (nz <= 32 * 32) return launch_m<32>(pl, p, st);
+#define PZ_ZT(MM) (helm_a >= 0.0 ? launch_m<MM, true>(pl, p, st, helm_a) : launch_m<MM, false>(pl, p, st, 0.0))
+    if (nz <= 32 * 4) return PZ_ZT(4);
+    if (nz <= 32 * 8) return PZ_ZT(8);
+    if (nz <= 32 * 16) return PZ_ZT(16);
+    if (nz <= 32 * 32) return PZ_ZT(32);
+#undef PZ_ZT
     set_error("z-solve variant 2 supports nz <= 1024 (got %d); use zsolve_variant = 0", nz);
     return PZ_EUNSUPPORTED;
 }

@@ -61,6 +61,21 @@ def test_c2_full_poisson_and_three_helmholtz_fields(env):
     pz.poisson_plan_destroy(plan)
 
 
+def test_c2_full_helmholtz3d(env):
+    """Fully implicit Helmholtz (Eq. 8) at 512^3, element by element."""
+    torch, pz, wl, oracle = env
+    w = wl.CONFIGS["c2"]
+    zc, zf = wl.grid(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    pz.helmholtz3d_setup(plan, w.a)
+    r = np.random.default_rng(12).standard_normal((w.nz, w.ny, w.nx))
+    u = torch.from_numpy(r).cuda()
+    pz.helmholtz3d_solve(plan, u)
+    torch.cuda.synchronize()
+    assert rel_err(u.cpu().numpy(), oracle.helmholtz3d_solve(w.lx, w.ly, zc, zf, w.a, r, 1)) <= TOL
+    pz.poisson_plan_destroy(plan)
+
+
 def test_c4_helmholtz_sampled_columns(env):
     torch, pz, wl, oracle = env
     w = wl.CONFIGS["c4"]

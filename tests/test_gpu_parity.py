@@ -361,6 +361,69 @@ def test_host_buffer_entry_points(torch, pz, wl, oracle):
     assert rel_err(hb.numpy(), oracle.helmholtz_z_solve(zc, zf, w.a, r)) <= TOL
 
 
+# ------------------------------------------- fully implicit (3-D) Helmholtz, Eq. (8)
+
+H3_CASES = [
+    # (base config, nx, ny, nz, a)
+    ("c0", 8, 8, 4, 0.1),
+    ("c0", 64, 64, 64, 5e-5),
+    ("c1", 32, 64, 48, 5e-5),
+    ("c1", 128, 32, 100, 1e-2),
+    ("c1", 64, 128, 129, 5e-5),
+    ("c3", 256, 64, 96, 2.5e-5),
+    ("c3", 32, 256, 33, 1.0),
+    ("c2", 64, 64, 512, 5e-5),
+    ("c1", 16, 16, 1024, 2.5e-5),
+]
+
+
+@pytest.mark.parametrize("base,nx,ny,nz,a", H3_CASES)
+@pytest.mark.parametrize("variant", [1, 2])
+def test_helmholtz3d_matches_oracle(torch, pz, wl, oracle, base, nx, ny, nz, a, variant):
+    w = wl.scaled(wl.CONFIGS[base], nx, ny, nz)
+    zc, zf = wl.grid(w)
+    r = np.random.default_rng(nx + 5 * ny + 11 * nz).standard_normal((nz, ny, nx))
+    ref = oracle.helmholtz3d_solve(w.lx, w.ly, zc, zf, a, r, 0 if nx * ny <= 64 * 64 else 1)
+    plan = pz.poisson_plan_create(nx, ny, nz, w.lx, w.ly, zc, zf)
+    pz.pz_set_option(plan, "zsolve_variant", variant)
+    u = torch.from_numpy(r).cuda()
+    with pytest.raises(pz.PzError) as ei:
+        pz.helmholtz3d_solve(plan, u)
+    assert ei.value.status == pz.PZ_ENOTSETUP
+    pz.helmholtz3d_setup(plan, a)
+    pz.helmholtz3d_solve(plan, u)
+    torch.cuda.synchronize()
+    assert rel_err(u.cpu().numpy(), ref) <= TOL
+    # a second a on the same plan (a changes every Runge-Kutta sub-step), and a = 0 is the identity
+    pz.helmholtz3d_setup(plan, 2 * a)
+    v = torch.from_numpy(r).cuda()
+    pz.helmholtz3d_solve(plan, v)
+    assert rel_err(v.cpu().numpy(), oracle.helmholtz3d_solve(w.lx, w.ly, zc, zf, 2 * a, r, 1)) <= TOL
+    pz.helmholtz3d_setup(plan, 0.0)
+    v = torch.from_numpy(r).cuda()
+    pz.helmholtz3d_solve(plan, v)
+    assert rel_err(v.cpu().numpy(), r) <= 1e-13
+    pz.poisson_plan_destroy(plan)
+
+
+def test_helmholtz3d_config1_full_and_fused_transforms(torch, pz, wl, oracle):
+    w = wl.CONFIGS["c1"]
+    zc, zf = wl.grid(w)
+    r = wl.helmholtz_rhs(w)
+    ref = oracle.helmholtz3d_solve(w.lx, w.ly, zc, zf, w.a, r, 1)
+    outs = []
+    for fused in (0, 1):
+        plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+        pz.pz_set_option(plan, "fft_fused", fused)
+        pz.helmholtz3d_setup(plan, w.a)
+        u = torch.from_numpy(r).cuda()
+        pz.helmholtz3d_solve(plan, u)
+        outs.append(u.cpu().numpy())
+        pz.poisson_plan_destroy(plan)
+    assert rel_err(outs[0], ref) <= TOL
+    assert np.array_equal(outs[0], outs[1])
+
+
 def test_host_batch_pipeline(torch, pz, wl, oracle):
     """pz_solve_host_batch: Poisson + several Helmholtz fields on pinned host buffers, more fields
     than staging buffers, twice in a row on a side stream."""
