@@ -500,6 +500,7 @@ static int *option_slot(pz_plan *pl, const char *key)
     if (!std::strcmp(key, "helm_tx")) return &pl->opt.helm_tx;
     if (!std::strcmp(key, "helm_m")) return &pl->opt.helm_m;
     if (!std::strcmp(key, "fft_y_tc")) return &pl->opt.fft_y_tc;
+    if (!std::strcmp(key, "fft_y_p0")) return &pl->opt.fft_y_p0;
     if (!std::strcmp(key, "fft_x_lpb")) return &pl->opt.fft_x_lpb;
     return nullptr;
 }

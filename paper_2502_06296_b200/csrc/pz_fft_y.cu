@@ -26,7 +26,7 @@ struct XchgY {
     __device__ __forceinline__ void sync() const { __syncthreads(); }
 };
 
-template <int L, int TC, bool INV>
+template <int L, int TC, bool INV, bool FUSE_P0>
 __global__ void __launch_bounds__(FftPlan<L>::T *TC, (FftPlan<L>::T * TC <= 256) ? 2 : 1)
     fft_y_kernel(double *__restrict__ p, const double2 *__restrict__ tw, int nx)
 {
@@ -39,16 +39,72 @@ __global__ void __launch_bounds__(FftPlan<L>::T *TC, (FftPlan<L>::T * TC <= 256)
     double *base = p + (size_t)blockIdx.y * L * nx + 2 * pair;
     XchgY<TC> xc{smem_y, c};
 
+    // The CTA that owns pair 0 (x-modes 0 and nx/2: two real sequences) also converts between
+    // W_r = A_r + i B_r and the packed spectra of the two real columns (rows (2r, 2r+1) hold
+    // (Re A_r, Re B_r), (Im A_r, Im B_r); rows 0, 1 hold r = 0, ny/2) -- see pair0_kernel below,
+    // which does the same as a separate pass (fft_y_p0 = 0).
+    const bool p0 = FUSE_P0 && blockIdx.x == 0;
+    constexpr int h = L / 2;
     double2 v[E];
+    if (INV && p0) {
+        if (c == 0)
 #pragma unroll
-    for (int e = 0; e < E; ++e) {
-        const double2 t = *reinterpret_cast<const double2 *>(base + (size_t)(tid + e * T) * nx);
-        v[e] = INV ? cconj(t) : t;
+            for (int e = 0; e < E; ++e)
+                smem_y[tid + e * T] = *reinterpret_cast<const double2 *>(base + (size_t)(tid + e * T) * nx);
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int r = tid + e * T;
+            if (c == 0) {
+                double2 w;
+                if (r == 0 || r == h) {
+                    w = smem_y[r == 0 ? 0 : 1];
+                } else {
+                    const int rr = r < h ? r : L - r;
+                    const double2 lo = smem_y[2 * rr], hi = smem_y[2 * rr + 1];
+                    w = r < h ? make_double2(lo.x - hi.y, hi.x + lo.y) : make_double2(lo.x + hi.y, lo.y - hi.x);
+                }
+                v[e] = cconj(w);
+            } else {
+                v[e] = cconj(*reinterpret_cast<const double2 *>(base + (size_t)r * nx));
+            }
+        }
+        __syncthreads(); // the merge buffer is the exchange buffer
+    } else {
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const double2 t = *reinterpret_cast<const double2 *>(base + (size_t)(tid + e * T) * nx);
+            v[e] = INV ? cconj(t) : t;
+        }
     }
     fft_line<L, 1, 0>(v, tid, tw, xc);
+    if (!INV && p0) {
+        __syncthreads();
+        if (c == 0)
 #pragma unroll
-    for (int e = 0; e < E; ++e)
-        *reinterpret_cast<double2 *>(base + (size_t)(tid + e * T) * nx) = INV ? cconj(v[e]) : v[e];
+            for (int e = 0; e < E; ++e) smem_y[tid + e * T] = v[e];
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int r = tid + e * T;
+            if (c != 0) {
+                *reinterpret_cast<double2 *>(base + (size_t)r * nx) = v[e];
+            } else if (r == 0 || r == h) {
+                *reinterpret_cast<double2 *>(base + (size_t)(r == 0 ? 0 : 1) * nx) = v[e];
+            } else if (r < h) {
+                const double2 w = v[e], wm = cconj(smem_y[L - r]);
+                const double2 a = make_double2(0.5 * (w.x + wm.x), 0.5 * (w.y + wm.y));
+                const double2 d = csub(w, wm);
+                const double2 b = make_double2(0.5 * d.y, -0.5 * d.x);
+                *reinterpret_cast<double2 *>(base + (size_t)(2 * r) * nx) = make_double2(a.x, b.x);
+                *reinterpret_cast<double2 *>(base + (size_t)(2 * r + 1) * nx) = make_double2(a.y, b.y);
+            }
+        }
+    } else {
+#pragma unroll
+        for (int e = 0; e < E; ++e)
+            *reinterpret_cast<double2 *>(base + (size_t)(tid + e * T) * nx) = INV ? cconj(v[e]) : v[e];
+    }
 }
 
 // Pair q = 0: W_r = A_r + i B_r with A, B the spectra of the real sequences in columns 0 and 1.
@@ -99,15 +155,20 @@ int launch_ltc(const pz_plan *pl, double *p, int nk, cudaStream_t st)
 {
     using P = FftPlan<L>;
     constexpr int threads = P::T * TC;
-    constexpr size_t smem = (P::R2 > 1) ? (size_t)L * TC * sizeof(double2) : 0;
+    // exchange tile; at least one column pair for the pair-0 conversion of single-pass lengths
+    constexpr size_t smem = (P::R2 > 1) ? (size_t)L * TC * sizeof(double2) : (size_t)L * sizeof(double2);
     static bool attr_done = false;
     if (smem > 48 * 1024 && !attr_done) {
-        PZ_CUDA(cudaFuncSetAttribute(fft_y_kernel<L, TC, INV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PZ_CUDA(cudaFuncSetAttribute(fft_y_kernel<L, TC, INV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PZ_CUDA(cudaFuncSetAttribute(fft_y_kernel<L, TC, INV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
     }
     dim3 grid((unsigned)(pl->nx / 2 / TC), (unsigned)nk);
     ProfScope prof(pl, INV ? PZ_K_FFT_Y_INV : PZ_K_FFT_Y_FWD, st);
-    fft_y_kernel<L, TC, INV><<<grid, threads, smem, st>>>(p, pl->d_twy, pl->nx);
+    if (pl->opt.fft_y_p0 != 0)
+        fft_y_kernel<L, TC, INV, true><<<grid, threads, smem, st>>>(p, pl->d_twy, pl->nx);
+    else
+        fft_y_kernel<L, TC, INV, false><<<grid, threads, smem, st>>>(p, pl->d_twy, pl->nx);
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
@@ -171,6 +232,7 @@ int launch_fft_y(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cud
 
 int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st)
 {
+    if (pl->opt.fft_y_p0 != 0) return PZ_OK; // done inside fft_y_kernel
     double *base = p + (size_t)k0 * pl->nx * pl->ny;
     const size_t smem = (size_t)pl->ny * sizeof(double2);
     const int threads = pl->ny / 2 >= 256 ? 256 : (pl->ny / 2 < 32 ? 32 : pl->ny / 2);

@@ -37,6 +37,7 @@ struct Options {
     int helm_probe = 0;       // diagnostic (variant 1): 1 = no stores, 2 = no arithmetic (results are wrong)
     int helm_tx = 0;          // 0 = auto: columns per CTA in the Helmholtz kernel (variant 0)
     int helm_m = 0;           // 0 = auto: rows per sub-domain in the Helmholtz kernel
+    int fft_y_p0 = 1;         // 1 = pair-0 conversion inside the y-FFT kernel, 0 = separate small kernel
     int fft_y_tc = 0;         // 0 = auto: complex column pairs per CTA in the y FFT
     int fft_x_lpb = 0;        // 0 = auto: lines per CTA in the x FFT
 };

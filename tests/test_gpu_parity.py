@@ -225,6 +225,26 @@ def test_fused_xy_transform_equals_the_separate_kernels(torch, pz, wl, nx, ny, n
     pz.poisson_plan_destroy(plan)
 
 
+@pytest.mark.parametrize("nx,ny,nz", [(8, 8, 4), (16, 32, 5), (64, 16, 6), (128, 512, 4), (32, 1024, 4), (8, 4096, 4)])
+def test_pair0_conversion_inside_the_y_kernel_equals_the_separate_kernel(torch, pz, wl, nx, ny, nz):
+    w = wl.scaled(wl.CONFIGS["c0"], nx, ny, nz)
+    zc, zf = wl.grid(w)
+    f = np.random.default_rng(nx + ny).standard_normal((nz, ny, nx))
+    outs = []
+    for p0 in (0, 1):
+        plan = pz.poisson_plan_create(nx, ny, nz, w.lx, w.ly, zc, zf)
+        pz.pz_set_option(plan, "fft_y_p0", p0)
+        a = torch.from_numpy(f).cuda()
+        pz.pz_poisson_stage(plan, a, pz.PZ_STAGE_FFT_X_FWD)
+        pz.pz_poisson_stage(plan, a, pz.PZ_STAGE_FFT_Y_FWD)
+        spec = a.clone()
+        pz.pz_poisson_stage(plan, a, pz.PZ_STAGE_FFT_Y_INV)
+        pz.pz_poisson_stage(plan, a, pz.PZ_STAGE_FFT_X_INV)
+        outs.append((spec, a))
+        pz.poisson_plan_destroy(plan)
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+
+
 def test_poisson_fused_and_separate_transforms_agree_with_the_oracle(torch, pz, wl, oracle):
     w = wl.scaled(wl.CONFIGS["c3"], 512, 256, 48)
     zc, zf = wl.grid(w)
