@@ -25,6 +25,7 @@ struct Options {
     int zsolve_variant = 0;   // 0 = thread-per-column Thomas through global memory (2 sweeps)
                               // 1 = chunked cyclic reduction in shared memory
                               // 2 = the same solve inside a TMA load / solve / TMA store pipeline
+    int zsolve_probe = 0;     // diagnostic (variant 2): 2 = no arithmetic (results are wrong)
     int zsolve_stages = 0;    // variant 2: shared-memory stages (0 = as many as fit, at most 3)
     int fft_fused = -1;       // -1 = auto (currently the separate kernels); 0 = separate kernels; 1 = fused x/y kernel
                               // (nx, ny in {256, 512, 1024, 2048})

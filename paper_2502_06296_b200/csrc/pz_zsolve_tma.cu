@@ -61,7 +61,7 @@ __global__ void __launch_bounds__(kThreads, 1)
     zsolve_tma_kernel(const __grid_constant__ CUtensorMap map, const double *__restrict__ A,
                       const double *__restrict__ C, const double *__restrict__ dzf, const double *__restrict__ lamx,
                       const double *__restrict__ lamy_nat, const double *__restrict__ lamy_pk, int nx, int ny, int nz,
-                      double inv_lz, int ntiles, int stages, double ha, double hw0, double hw1)
+                      double inv_lz, int ntiles, int stages, double ha, double hw0, double hw1, int probe)
 {
     using G = Geo<M>;
     extern __shared__ unsigned char smem_zt[];
@@ -135,7 +135,9 @@ __global__ void __launch_bounds__(kThreads, 1)
         const double sig0 = -(lamx[i] + ly), sig1 = -(lamx[i + 1] + ly);
         d.slot = base + b * G::STAGE + (size_t)R0 * 128;
         mbar_wait(&full[b], (it / stages) & 1);
-        if constexpr (HELM) {
+        if (probe == 2) {
+            // diagnostic: pipeline skeleton only (TMA load, TMA store), no arithmetic
+        } else if constexpr (HELM) {
             const double *e0 = s_e0 + lane * G::CS;
             if (sig0 == sig1) {
                 solve_pair<M, 3, false, false, true>(d, al, ga, ha * sig0, k0, nz, dzf, inv_lz, e0);
@@ -187,7 +189,8 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha)
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
     zsolve_tma_kernel<M, HELM><<<blocks, kThreads, smem, st>>>(map, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
                                                                 pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, pl->nz,
-                                                                pl->inv_lz, ntiles, stages, ha, pl->wall_w0, pl->wall_w1);
+                                                                pl->inv_lz, ntiles, stages, ha, pl->wall_w0, pl->wall_w1,
+                                                                pl->opt.zsolve_probe);
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
