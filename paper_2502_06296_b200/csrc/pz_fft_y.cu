@@ -196,7 +196,7 @@ int launch_l(const pz_plan *pl, double *p, int nk, cudaStream_t st)
 {
     const int npairs = pl->nx / 2;
     int tc = pl->opt.fft_y_tc;
-    if (tc == 0) tc = (L <= 512) ? 8 : 4;
+    if (tc == 0) tc = (L <= 256) ? 16 : (L <= 512) ? 8 : 4; // 256 threads and <= 64 KB of exchange tile per CTA
     if (tc > npairs) tc = npairs;
     if (tc >= 16 && tc_valid<L, 16>()) return try_ltc<L, 16, INV>(pl, p, nk, st);
     if (tc >= 8 && tc_valid<L, 8>()) return try_ltc<L, 8, INV>(pl, p, nk, st);
