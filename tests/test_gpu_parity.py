@@ -444,6 +444,32 @@ def test_helmholtz3d_config1_full_and_fused_transforms(torch, pz, wl, oracle):
     assert np.array_equal(outs[0], outs[1])
 
 
+def test_error_paths_of_the_widened_entry_points(torch, pz, wl):
+    zf = wl.z_faces(1100, 2.0, 1.8)
+    plan = pz.poisson_plan_create(16, 16, 1100, 1.0, 1.0, wl.z_centres(zf), zf)
+    assert pz.pz_get_option(plan, "zsolve_variant") == 0          # thread-per-column fallback above nz = 1024
+    with pytest.raises(pz.PzError) as ei:
+        pz.helmholtz3d_setup(plan, -1e-3)
+    assert ei.value.status == pz.PZ_EINVAL
+    pz.helmholtz3d_setup(plan, 1e-3)
+    u = torch.zeros(1100, 16, 16, dtype=torch.float64, device="cuda")
+    with pytest.raises(pz.PzError) as ei:
+        pz.helmholtz3d_solve(plan, u)                              # needs a shared-memory z-solve variant
+    assert ei.value.status == pz.PZ_EUNSUPPORTED
+    with pytest.raises(pz.PzError) as ei:
+        pz.pz_set_option(plan, "zsolve_variant", 2)
+    assert ei.value.status == pz.PZ_EUNSUPPORTED
+    h = torch.zeros(1100 * 256, dtype=torch.float64).pin_memory()
+    with pytest.raises(pz.PzError) as ei:
+        pz.pz_solve_host_batch(plan, None, [h])                    # Helmholtz field before helmholtz_z_setup
+    assert ei.value.status == pz.PZ_ENOTSETUP
+    pz.pz_solve_host_batch(plan, None, [])                         # nothing to do
+    with pytest.raises(pz.PzError) as ei:
+        pz.pz_set_option(plan, "no_such_option", 1)
+    assert ei.value.status == pz.PZ_EUNSUPPORTED
+    pz.poisson_plan_destroy(plan)
+
+
 def test_host_batch_pipeline(torch, pz, wl, oracle):
     """pz_solve_host_batch: Poisson + several Helmholtz fields on pinned host buffers, more fields
     than staging buffers, twice in a row on a side stream."""
