@@ -68,6 +68,9 @@ POISSON_SHAPES = [
     ("c3", 256, 64, 96),      # beta = 2.0, long x
     ("c3", 32, 256, 33),
     ("c2", 64, 64, 128),      # few-mode right-hand side
+    ("c1", 16, 16, 1024),     # one shared-memory stage (m = 32)
+    ("c3", 32, 16, 700),      # ragged, m = 32
+    ("c1", 16, 32, 300),      # ragged, m = 16
 ]
 
 
