@@ -119,6 +119,27 @@ PZ_API int helmholtz3d_setup(pz_plan *plan, double a);
 PZ_API int helmholtz3d_solve(pz_plan *plan, double *u, void *stream);
 
 /*
+ * The steps either side of the Poisson solve in the pressure-correction scheme,
+ * on the staggered grid: u[k][j][i] on the x-face between cells i and i+1, v on the y-face between
+ * j and j+1 (periodic), w on the z-face zf[k+1] (the bottom wall face carries w = 0 and is not
+ * stored; w[nz-1] is the top wall face and should be 0), p and Phi at cell centres.
+ *   pz_divergence_rhs      rhs = D u* / (gamma dt), Eq. (4):
+ *                          (u_i-u_{i-1})/dx + (v_j-v_{j-1})/dy + (w_k-w_{k-1})/dzf_k, times inv_gdt
+ *   pz_project             u -= gamma dt G Phi (Eq. 5), p += Phi (Eq. 6); the top wall face of w
+ *                          is left untouched (zero wall-normal gradient of Phi)
+ *   pz_pressure_correction both around poisson_solve: work <- rhs, solved in place, then the
+ *                          correction; afterwards D u = 0 to rounding (D G is the operator of
+ *                          poisson_solve exactly).  work: device, nx*ny*nz doubles, holds Phi on return.
+ * All fields: device, nx*ny*nz doubles, 16-byte aligned; in place where written.
+ */
+PZ_API int pz_divergence_rhs(pz_plan *plan, const double *u, const double *v, const double *w, double *rhs,
+                             double inv_gdt, void *stream);
+PZ_API int pz_project(pz_plan *plan, double *u, double *v, double *w, double *p, const double *phi, double gdt,
+                      void *stream);
+PZ_API int pz_pressure_correction(pz_plan *plan, double *u, double *v, double *w, double *p, double *work, double gdt,
+                                  void *stream);
+
+/*
  * End-to-end variants with HOST buffers: copy host -> device workspace (owned by the plan,
  * allocated on first use: nx*ny*nz doubles), solve, copy back, all asynchronously on
  * `stream`.  The host buffer must stay valid until the stream has been synchronised.

@@ -35,6 +35,9 @@ SIGNATURES = {
     "helmholtz_z_solve_host": (_i, [_vp, _vp, _vp]),
     "helmholtz3d_setup": (_i, [_vp, ctypes.c_double]),
     "helmholtz3d_solve": (_i, [_vp, _vp, _vp]),
+    "pz_divergence_rhs": (_i, [_vp, _vp, _vp, _vp, _vp, ctypes.c_double, _vp]),
+    "pz_project": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_double, _vp]),
+    "pz_pressure_correction": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_double, _vp]),
     "pz_solve_host_batch": (_i, [_vp, _vp, ctypes.POINTER(_vp), ctypes.c_int, _vp]),
     "poisson_plan_destroy": (_i, [_vp]),
     "pz_last_error": (ctypes.c_char_p, []),
@@ -171,6 +174,24 @@ def helmholtz3d_setup(plan: Plan, a: float) -> None:
 
 def helmholtz3d_solve(plan: Plan, u, stream=None) -> None:
     _check(lib().helmholtz3d_solve(plan.handle, _dev_ptr(u, plan.n), _stream_ptr(stream)))
+
+
+def pz_divergence_rhs(plan: Plan, u, v, w, rhs, inv_gdt: float, stream=None) -> None:
+    n = plan.n
+    _check(lib().pz_divergence_rhs(plan.handle, _dev_ptr(u, n), _dev_ptr(v, n), _dev_ptr(w, n), _dev_ptr(rhs, n),
+                                   float(inv_gdt), _stream_ptr(stream)))
+
+
+def pz_project(plan: Plan, u, v, w, p, phi, gdt: float, stream=None) -> None:
+    n = plan.n
+    _check(lib().pz_project(plan.handle, _dev_ptr(u, n), _dev_ptr(v, n), _dev_ptr(w, n), _dev_ptr(p, n),
+                            _dev_ptr(phi, n), float(gdt), _stream_ptr(stream)))
+
+
+def pz_pressure_correction(plan: Plan, u, v, w, p, work, gdt: float, stream=None) -> None:
+    n = plan.n
+    _check(lib().pz_pressure_correction(plan.handle, _dev_ptr(u, n), _dev_ptr(v, n), _dev_ptr(w, n), _dev_ptr(p, n),
+                                        _dev_ptr(work, n), float(gdt), _stream_ptr(stream)))
 
 
 def pz_solve_host_batch(plan: Plan, p_host, u_hosts, stream=None) -> None:

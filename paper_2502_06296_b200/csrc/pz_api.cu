@@ -231,13 +231,13 @@ int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double
     pl->wall_w1 = 2.0 / (pl->dzf[nz - 1] * (2.0 * (zf[nz] - zc[nz - 1])));
 
     // one device allocation for all tables
-    const size_t ndbl = 3 * (size_t)nz + (size_t)nx + 2 * (size_t)ny + 2 * (size_t)nx + 2 * (size_t)ny + 8;
+    const size_t ndbl = 4 * (size_t)nz + (size_t)nx + 2 * (size_t)ny + 2 * (size_t)nx + 2 * (size_t)ny + 10;
     std::vector<double> host(ndbl, 0.0);
     size_t off = 0;
     auto take = [&](size_t cnt) { size_t o = off; off += (cnt + 1) & ~(size_t)1; return o; }; // keep 16-B alignment
-    const size_t oA = take(nz), oC = take(nz), oD = take(nz), oLx = take(nx), oLyn = take(ny), oLyp = take(ny);
+    const size_t oA = take(nz), oC = take(nz), oD = take(nz), oZc = take(nz), oLx = take(nx), oLyn = take(ny), oLyp = take(ny);
     const size_t oTx = take(2 * (size_t)nx), oTy = take(2 * (size_t)ny);
-    for (int k = 0; k < nz; ++k) { host[oA + k] = pl->A[k]; host[oC + k] = pl->C[k]; host[oD + k] = pl->dzf[k]; }
+    for (int k = 0; k < nz; ++k) { host[oA + k] = pl->A[k]; host[oC + k] = pl->C[k]; host[oD + k] = pl->dzf[k]; host[oZc + k] = zc[k]; }
     // modified wavenumbers re-ordered for the packed layout
     for (int i = 0; i < nx; ++i) host[oLx + i] = lambda(i == 0 ? 0 : (i == 1 ? nx / 2 : i / 2), nx, lx);
     for (int j = 0; j < ny; ++j) {
@@ -251,7 +251,7 @@ int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double
     if (ce != cudaSuccess) { cudaGetLastError(); set_error("plan tables: %s", cudaGetErrorString(ce)); return fail(PZ_ENOMEM); }
     ce = cudaMemcpy(pl->tables, host.data(), off * sizeof(double), cudaMemcpyHostToDevice);
     if (ce != cudaSuccess) return fail(cuda_fail(ce, "cudaMemcpy(tables)"));
-    pl->d_A = pl->tables + oA; pl->d_C = pl->tables + oC; pl->d_dzf = pl->tables + oD;
+    pl->d_A = pl->tables + oA; pl->d_C = pl->tables + oC; pl->d_dzf = pl->tables + oD; pl->d_zc = pl->tables + oZc;
     pl->d_lamx = pl->tables + oLx; pl->d_lamy_nat = pl->tables + oLyn; pl->d_lamy_pk = pl->tables + oLyp;
     pl->d_twx = reinterpret_cast<double2 *>(pl->tables + oTx);
     pl->d_twy = reinterpret_cast<double2 *>(pl->tables + oTy);
@@ -332,6 +332,33 @@ int poisson_solve(pz_plan *pl, double *p, void *stream)
     if ((rc = forward_xy(pl, p, st)) != PZ_OK) return rc;
     if ((rc = launch_zsolve(pl, p, st)) != PZ_OK) return rc;
     return inverse_xy(pl, p, st);
+}
+
+static bool misaligned(const void *q) { return ((uintptr_t)q & 15) != 0; }
+
+int pz_divergence_rhs(pz_plan *pl, const double *u, const double *v, const double *w, double *rhs, double inv_gdt, void *stream)
+{
+    if (!pl || !u || !v || !w || !rhs) { set_error("pz_divergence_rhs: NULL argument"); return PZ_EINVAL; }
+    if (misaligned(u) || misaligned(v) || misaligned(w) || misaligned(rhs)) { set_error("pz_divergence_rhs: fields must be 16-byte aligned"); return PZ_EINVAL; }
+    if (!std::isfinite(inv_gdt)) { set_error("pz_divergence_rhs: 1/(gamma dt) must be finite"); return PZ_EINVAL; }
+    return launch_divergence_rhs(pl, u, v, w, rhs, inv_gdt, (cudaStream_t)stream);
+}
+
+int pz_project(pz_plan *pl, double *u, double *v, double *w, double *p, const double *phi, double gdt, void *stream)
+{
+    if (!pl || !u || !v || !w || !p || !phi) { set_error("pz_project: NULL argument"); return PZ_EINVAL; }
+    if (misaligned(u) || misaligned(v) || misaligned(w) || misaligned(p) || misaligned(phi)) { set_error("pz_project: fields must be 16-byte aligned"); return PZ_EINVAL; }
+    if (!std::isfinite(gdt)) { set_error("pz_project: gamma dt must be finite"); return PZ_EINVAL; }
+    return launch_project(pl, u, v, w, p, phi, gdt, (cudaStream_t)stream);
+}
+
+int pz_pressure_correction(pz_plan *pl, double *u, double *v, double *w, double *p, double *work, double gdt, void *stream)
+{
+    if (!(gdt > 0.0) || !std::isfinite(gdt)) { set_error("pz_pressure_correction: gamma dt must be positive and finite"); return PZ_EINVAL; }
+    int rc;
+    if ((rc = pz_divergence_rhs(pl, u, v, w, work, 1.0 / gdt, stream)) != PZ_OK) return rc;
+    if ((rc = poisson_solve(pl, work, stream)) != PZ_OK) return rc;
+    return pz_project(pl, u, v, w, p, work, gdt, stream);
 }
 
 int helmholtz3d_setup(pz_plan *pl, double a)

@@ -57,7 +57,7 @@ struct pz_plan {
 
     // device tables (one allocation, freed as `tables`)
     double *tables = nullptr;
-    double *d_A = nullptr, *d_C = nullptr, *d_dzf = nullptr;   // nz each
+    double *d_A = nullptr, *d_C = nullptr, *d_dzf = nullptr, *d_zc = nullptr;   // nz each
     double *d_lamx = nullptr;        // nx: lambda_x per real column i in packed order
     double *d_lamy_nat = nullptr;    // ny: lambda_y, natural order (complex pairs i >= 2)
     double *d_lamy_pk = nullptr;     // ny: lambda_y, packed order (columns i = 0, 1)
@@ -120,6 +120,9 @@ int launch_fft_x(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cud
 int launch_fft_y(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
 int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
 int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a = -1.0); // helm_a >= 0: Eq. (8) systems
+int launch_divergence_rhs(pz_plan *pl, const double *u, const double *v, const double *w, double *out, double inv_gdt,
+                          cudaStream_t st);
+int launch_project(pz_plan *pl, double *u, double *v, double *w, double *p, const double *phi, double gdt, cudaStream_t st);
 int launch_fft_xy_fwd(pz_plan *pl, double *p, cudaStream_t st);
 int launch_fft_xy_inv(pz_plan *pl, double *p, cudaStream_t st);
 int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st);

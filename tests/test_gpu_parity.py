@@ -447,6 +447,62 @@ def test_helmholtz3d_config1_full_and_fused_transforms(torch, pz, wl, oracle):
     assert np.array_equal(outs[0], outs[1])
 
 
+# --------------------------------- the steps either side of the Poisson solve, Eqs. (4)-(6)
+
+@pytest.mark.parametrize("base,nx,ny,nz", [("c0", 8, 8, 4), ("c1", 32, 16, 48), ("c3", 64, 32, 33), ("c1", 128, 64, 96)])
+def test_divergence_rhs_and_projection_match_oracle(torch, pz, wl, oracle, base, nx, ny, nz):
+    from oracle import projection as proj
+
+    w_ = wl.scaled(wl.CONFIGS[base], nx, ny, nz)
+    zc, zf = wl.grid(w_)
+    rng = np.random.default_rng(nx + 3 * nz)
+    u, v, w = (rng.standard_normal((nz, ny, nx)) for _ in range(3))
+    w[-1] = 0.0
+    p, phi = rng.standard_normal((nz, ny, nx)), rng.standard_normal((nz, ny, nx))
+    gdt = 2.5e-3
+    plan = pz.poisson_plan_create(nx, ny, nz, w_.lx, w_.ly, zc, zf)
+    du, dv, dw, dp, dphi = (torch.from_numpy(a).cuda() for a in (u, v, w, p, phi))
+    rhs = torch.empty_like(du)
+    pz.pz_divergence_rhs(plan, du, dv, dw, rhs, 1.0 / gdt)
+    ref = proj.divergence_rhs(w_.lx, w_.ly, zf, u, v, w, 1.0 / gdt)
+    scale = (np.abs(u).max() / (w_.lx / nx) + np.abs(v).max() / (w_.ly / ny) + np.abs(w).max() / np.diff(zf).min()) / gdt
+    assert np.abs(rhs.cpu().numpy() - ref).max() <= 1e-14 * scale       # cancellation-aware bound
+    pz.pz_project(plan, du, dv, dw, dp, dphi, gdt)
+    ru, rv, rw, rp = proj.project(w_.lx, w_.ly, zc, u, v, w, p, phi, gdt)
+    for got, want in ((du, ru), (dv, rv), (dw, rw), (dp, rp)):
+        assert rel_err(got.cpu().numpy(), want) <= 1e-13
+    assert torch.equal(dw[-1], torch.from_numpy(w[-1]).cuda())          # top wall face untouched
+    pz.poisson_plan_destroy(plan)
+
+
+@pytest.mark.parametrize("base,nx,ny,nz", [("c0", 64, 64, 64), ("c1", 64, 32, 96), ("c3", 128, 64, 129)])
+def test_pressure_correction_step_is_divergence_free_and_matches_oracle(torch, pz, wl, oracle, base, nx, ny, nz):
+    from oracle import projection as proj
+
+    w_ = wl.scaled(wl.CONFIGS[base], nx, ny, nz)
+    zc, zf = wl.grid(w_)
+    rng = np.random.default_rng(7 * nx + nz)
+    u, v, w = (rng.standard_normal((nz, ny, nx)) for _ in range(3))
+    w[-1] = 0.0
+    p = rng.standard_normal((nz, ny, nx))
+    gdt = 1e-3
+    plan = pz.poisson_plan_create(nx, ny, nz, w_.lx, w_.ly, zc, zf)
+    du, dv, dw, dp = (torch.from_numpy(a).cuda() for a in (u, v, w, p))
+    work = torch.empty_like(du)
+    pz.pz_pressure_correction(plan, du, dv, dw, dp, work, gdt)
+    torch.cuda.synchronize()
+    gu, gv, gw, gp = (t.cpu().numpy() for t in (du, dv, dw, dp))
+    div0 = np.abs(proj.divergence(w_.lx, w_.ly, zf, u, v, w)).max()
+    assert np.abs(proj.divergence(w_.lx, w_.ly, zf, gu, gv, gw)).max() <= 1e-11 * div0
+    # the oracle's own step
+    phi = oracle.poisson_solve(w_.lx, w_.ly, zc, zf, proj.divergence_rhs(w_.lx, w_.ly, zf, u, v, w, 1.0 / gdt), 1)
+    assert rel_err(work.cpu().numpy(), phi) <= TOL
+    ru, rv, rw, rp = proj.project(w_.lx, w_.ly, zc, u, v, w, p, phi, gdt)
+    for got, want in ((gu, ru), (gv, rv), (gw, rw), (gp, rp)):
+        assert rel_err(got, want) <= TOL
+    pz.poisson_plan_destroy(plan)
+
+
 def test_error_paths_of_the_widened_entry_points(torch, pz, wl):
     zf = wl.z_faces(1100, 2.0, 1.8)
     plan = pz.poisson_plan_create(16, 16, 1100, 1.0, 1.0, wl.z_centres(zf), zf)
