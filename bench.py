@@ -312,6 +312,30 @@ def main():
         h3 = {"ms_per_solve": h3_ms, "points_per_s": w.n / (h3_ms * 1e-3),
               "hbm_frac_48B_per_point": 48.0 * w.n / (h3_ms * 1e-3) / 1e9 / measured_peak()[0]}
 
+    # ---- next-row capability, outside the timed region: the pressure-correction step of Eqs. (4)-(6)
+    pc = None
+    if w.poisson and len(us) >= 3:
+        work = torch.empty_like(p)
+        gdt = 1e-3
+        for _ in range(2):
+            pz.pz_pressure_correction(plan, us[0], us[1], us[2], p, work, gdt)
+        pz.pz_profile_enable(plan, True)
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        c0.record()
+        for _ in range(5):
+            pz.pz_pressure_correction(plan, us[0], us[1], us[2], p, work, gdt)
+        c1.record()
+        torch.cuda.synchronize()
+        pz.pz_profile_enable(plan, False)
+        pc_ms = c0.elapsed_time(c1) / 5
+        div_ms, nd = pz.pz_profile_read(plan, pz.KERNEL_CLASSES.index("div_rhs"))
+        prj_ms, npj = pz.pz_profile_read(plan, pz.KERNEL_CLASSES.index("project"))
+        pc = {"ms_per_step": pc_ms, "points_per_s": w.n / (pc_ms * 1e-3),
+              "div_rhs": {"ms": div_ms / max(nd, 1), "GBps_algorithmic": 32.0 * w.n / (div_ms / max(nd, 1) * 1e-3) / 1e9},
+              "project": {"ms": prj_ms / max(npj, 1), "GBps_algorithmic": 72.0 * w.n / (prj_ms / max(npj, 1) * 1e-3) / 1e9}}
+        del work
+
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -401,6 +425,8 @@ def main():
     }
     if h3 is not None:
         line["helmholtz3d"] = h3
+    if pc is not None:
+        line["pressure_correction"] = pc
     if e2e is not None:
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:

@@ -196,7 +196,9 @@ enum pz_kernel_class {
     PZ_K_PAIR0_INV = 4, PZ_K_FFT_Y_INV = 5, PZ_K_FFT_X_INV = 6, PZ_K_HELMHOLTZ = 7,
     PZ_K_FFT_XY_FWD = 8, /* a1+a2 in one kernel (second trip of the plane through L2 only) */
     PZ_K_FFT_XY_INV = 9, /* a4+a5 in one kernel */
-    PZ_K_COUNT = 10
+    PZ_K_DIV_RHS = 10,   /* pz_divergence_rhs */
+    PZ_K_PROJECT = 11,   /* pz_project */
+    PZ_K_COUNT = 12
 };
 PZ_API int pz_profile_enable(pz_plan *plan, int on);
 PZ_API int pz_profile_read(pz_plan *plan, int kernel_class, double *total_ms, long long *launches);

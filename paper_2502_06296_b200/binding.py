@@ -221,7 +221,7 @@ def pz_get_option(plan: Plan, key: str) -> int:
 
 
 KERNEL_CLASSES = ("fft_x_fwd", "fft_y_fwd", "pair0_fwd", "z_solve", "pair0_inv", "fft_y_inv", "fft_x_inv", "helmholtz",
-                  "fft_xy_fwd", "fft_xy_inv")
+                  "fft_xy_fwd", "fft_xy_inv", "div_rhs", "project")
 
 
 def pz_profile_enable(plan: Plan, on: bool) -> None:

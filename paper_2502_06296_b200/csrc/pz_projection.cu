@@ -95,6 +95,7 @@ int launch_divergence_rhs(pz_plan *pl, const double *u, const double *v, const d
                           cudaStream_t st)
 {
     const double dx = pl->lx / pl->nx, dy = pl->ly / pl->ny;
+    ProfScope prof(pl, PZ_K_DIV_RHS, st);
     divergence_rhs_kernel<<<grid_for(pl), 256, 0, st>>>(u, v, w, out, pl->d_dzf, pl->nx, pl->ny, pl->nz, 1.0 / dx, 1.0 / dy,
                                                         inv_gdt);
     count_launch();
@@ -105,6 +106,7 @@ int launch_divergence_rhs(pz_plan *pl, const double *u, const double *v, const d
 int launch_project(pz_plan *pl, double *u, double *v, double *w, double *p, const double *phi, double gdt, cudaStream_t st)
 {
     const double dx = pl->lx / pl->nx, dy = pl->ly / pl->ny;
+    ProfScope prof(pl, PZ_K_PROJECT, st);
     project_kernel<<<grid_for(pl), 256, 0, st>>>(u, v, w, p, phi, pl->d_zc, pl->nx, pl->ny, pl->nz, gdt / dx, gdt / dy, gdt);
     count_launch();
     PZ_CUDA(cudaGetLastError());

@@ -76,6 +76,29 @@ def test_c2_full_helmholtz3d(env):
     pz.poisson_plan_destroy(plan)
 
 
+def test_c2_pressure_correction_is_divergence_free(env):
+    """Eqs. (4)-(6) around the Poisson solve at 512^3: the corrected velocity is divergence free to
+    rounding (D G is exactly the operator of the solve), checked with the oracle's divergence."""
+    from oracle import projection as proj
+
+    torch, pz, wl, oracle = env
+    w_ = wl.CONFIGS["c2"]
+    zc, zf = wl.grid(w_)
+    plan = pz.poisson_plan_create(w_.nx, w_.ny, w_.nz, w_.lx, w_.ly, zc, zf)
+    g = torch.Generator(device="cuda")
+    g.manual_seed(31)
+    u, v, w, p = (torch.randn(w_.nz, w_.ny, w_.nx, dtype=torch.float64, device="cuda", generator=g) for _ in range(4))
+    w[-1] = 0.0
+    u0, v0, w0 = u.cpu().numpy(), v.cpu().numpy(), w.cpu().numpy()
+    work = torch.empty_like(u)
+    pz.pz_pressure_correction(plan, u, v, w, p, work, 1e-3)
+    torch.cuda.synchronize()
+    div0 = np.abs(proj.divergence(w_.lx, w_.ly, zf, u0, v0, w0)).max()
+    div1 = np.abs(proj.divergence(w_.lx, w_.ly, zf, u.cpu().numpy(), v.cpu().numpy(), w.cpu().numpy())).max()
+    assert div1 <= 1e-11 * div0
+    pz.poisson_plan_destroy(plan)
+
+
 def test_c4_helmholtz_sampled_columns(env):
     torch, pz, wl, oracle = env
     w = wl.CONFIGS["c4"]
