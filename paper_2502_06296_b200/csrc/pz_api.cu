@@ -356,6 +356,20 @@ int pz_pressure_correction(pz_plan *pl, double *u, double *v, double *w, double 
 {
     if (!(gdt > 0.0) || !std::isfinite(gdt)) { set_error("pz_pressure_correction: gamma dt must be positive and finite"); return PZ_EINVAL; }
     int rc;
+    if (pl && u && v && w && work && pl->opt.div_fused != 0 && !use_fused(pl) && pl->opt.slab_planes == 0 &&
+        !misaligned(u) && !misaligned(v) && !misaligned(w) && !misaligned(work)) {
+        // Eq. (4)'s right-hand side is formed inside the forward x transform: it never touches HBM
+        cudaStream_t st = (cudaStream_t)stream;
+        DivSrc ds;
+        ds.u = u; ds.v = v; ds.w = w; ds.dzf = pl->d_dzf;
+        ds.rdx = 1.0 / (pl->lx / pl->nx); ds.rdy = 1.0 / (pl->ly / pl->ny); ds.scale = 1.0 / gdt; ds.ny = pl->ny;
+        if ((rc = launch_fft_x(pl, work, 0, pl->nz, false, st, &ds)) != PZ_OK) return rc;
+        if ((rc = launch_fft_y(pl, work, 0, pl->nz, false, st)) != PZ_OK) return rc;
+        if ((rc = launch_pair0(pl, work, 0, pl->nz, false, st)) != PZ_OK) return rc;
+        if ((rc = launch_zsolve(pl, work, st)) != PZ_OK) return rc;
+        if ((rc = inverse_xy(pl, work, st)) != PZ_OK) return rc;
+        return pz_project(pl, u, v, w, p, work, gdt, stream);
+    }
     if ((rc = pz_divergence_rhs(pl, u, v, w, work, 1.0 / gdt, stream)) != PZ_OK) return rc;
     if ((rc = poisson_solve(pl, work, stream)) != PZ_OK) return rc;
     return pz_project(pl, u, v, w, p, work, gdt, stream);
@@ -529,6 +543,7 @@ static int *option_slot(pz_plan *pl, const char *key)
     if (!std::strcmp(key, "helm_tx")) return &pl->opt.helm_tx;
     if (!std::strcmp(key, "helm_m")) return &pl->opt.helm_m;
     if (!std::strcmp(key, "fft_y_tc")) return &pl->opt.fft_y_tc;
+    if (!std::strcmp(key, "div_fused")) return &pl->opt.div_fused;
     if (!std::strcmp(key, "fft_y_p0")) return &pl->opt.fft_y_p0;
     if (!std::strcmp(key, "fft_x_lpb")) return &pl->opt.fft_x_lpb;
     return nullptr;

@@ -45,10 +45,15 @@ struct XchgX {
     __device__ __forceinline__ double2 get_lin(int pos) const { return make_double2(re[pos], im[pos]); }
 };
 
-template <int M, int LPB, bool INV>
+// DIV (forward only): the lines are not read from p but formed on the fly as the right-hand side of
+// Eq. (4), D u* / (gamma dt), from the staggered velocity (pz_projection.cu, same arithmetic in the
+// same order, so the result is bitwise the one of pz_divergence_rhs followed by this kernel); the
+// 16 B/point round trip of the right-hand side through HBM disappears.
+template <int M, int LPB, bool INV, bool DIV>
 __global__ void __launch_bounds__(FftPlan<M>::T *LPB)
-    fft_x_kernel(double *__restrict__ p, const double2 *__restrict__ tw, long long nlines, double scale)
+    fft_x_kernel(double *__restrict__ p, const double2 *__restrict__ tw, long long nlines, double scale, const DivSrc ds)
 {
+    static_assert(!(INV && DIV), "the divergence is fused into the forward transform only");
     using P = FftPlan<M>;
     constexpr int E = P::E, T = P::T, LD = line_ld(M);
     extern __shared__ double smem_x[];
@@ -61,8 +66,33 @@ __global__ void __launch_bounds__(FftPlan<M>::T *LPB)
 
     double2 v[E];
     if constexpr (!INV) {
+        if constexpr (DIV) {
+            const long long ln = active ? line : 0;
+            const int j = (int)(ln % ds.ny), k = (int)(ln / ds.ny);
+            const size_t c0 = (size_t)ln * (2 * (size_t)M);
+            const double *ul = ds.u + c0;
+            const double2 *vl = reinterpret_cast<const double2 *>(ds.v + c0);
+            const double2 *vp = reinterpret_cast<const double2 *>(ds.v + (j == 0 ? c0 + (size_t)(ds.ny - 1) * 2 * M : c0 - 2 * (size_t)M));
+            const double2 *wl = reinterpret_cast<const double2 *>(ds.w + c0);
+            const double2 *wp = reinterpret_cast<const double2 *>(ds.w + (k > 0 ? c0 - (size_t)ds.ny * 2 * M : c0));
+            const double rdz = 1.0 / ds.dzf[k];
 #pragma unroll
-        for (int e = 0; e < E; ++e) v[e] = active ? lp[tid + e * T] : make_double2(0.0, 0.0);
+            for (int e = 0; e < E; ++e) {
+                const int m = tid + e * T;
+                const double2 uc = reinterpret_cast<const double2 *>(ul)[m], vc = vl[m], wc = wl[m];
+                const double um = ul[m == 0 ? 2 * M - 1 : 2 * m - 1];
+                const double2 vm = vp[m];
+                double2 wm = make_double2(0.0, 0.0);
+                if (k > 0) wm = wp[m];
+                double2 d;
+                d.x = ((uc.x - um) * ds.rdx + (vc.x - vm.x) * ds.rdy + (wc.x - wm.x) * rdz) * ds.scale;
+                d.y = ((uc.y - uc.x) * ds.rdx + (vc.y - vm.y) * ds.rdy + (wc.y - wm.y) * rdz) * ds.scale;
+                v[e] = active ? d : make_double2(0.0, 0.0);
+            }
+        } else {
+#pragma unroll
+            for (int e = 0; e < E; ++e) v[e] = active ? lp[tid + e * T] : make_double2(0.0, 0.0);
+        }
         fft_line<M, 2, 1>(v, tid, tw, xc);
         if constexpr (P::R2 > 1) xc.sync();
 #pragma unroll
@@ -115,7 +145,7 @@ __global__ void __launch_bounds__(FftPlan<M>::T *LPB)
 }
 
 template <int M, bool INV>
-int launch_m(const pz_plan *pl, double *p, long long nlines, cudaStream_t st)
+int launch_m(const pz_plan *pl, double *p, long long nlines, cudaStream_t st, const DivSrc *div)
 {
     using P = FftPlan<M>;
     constexpr int LPB = (P::T >= 128) ? 1 : 128 / P::T;
@@ -125,26 +155,34 @@ int launch_m(const pz_plan *pl, double *p, long long nlines, cudaStream_t st)
     const long long blocks = (nlines + LPB - 1) / LPB;
     const double scale = 1.0 / ((double)pl->nx * (double)pl->ny);
     ProfScope prof(pl, INV ? PZ_K_FFT_X_INV : PZ_K_FFT_X_FWD, st);
-    fft_x_kernel<M, LPB, INV><<<(unsigned)blocks, threads, smem, st>>>(p, pl->d_twx, nlines, scale);
+    if constexpr (!INV) {
+        if (div) {
+            fft_x_kernel<M, LPB, false, true><<<(unsigned)blocks, threads, smem, st>>>(p, pl->d_twx, nlines, scale, *div);
+            count_launch();
+            PZ_CUDA(cudaGetLastError());
+            return PZ_OK;
+        }
+    }
+    fft_x_kernel<M, LPB, INV, false><<<(unsigned)blocks, threads, smem, st>>>(p, pl->d_twx, nlines, scale, DivSrc{});
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
 }
 
 template <bool INV>
-int dispatch(const pz_plan *pl, double *p, long long nlines, cudaStream_t st)
+int dispatch(const pz_plan *pl, double *p, long long nlines, cudaStream_t st, const DivSrc *div)
 {
     switch (pl->nx / 2) {
-    case 4: return launch_m<4, INV>(pl, p, nlines, st);
-    case 8: return launch_m<8, INV>(pl, p, nlines, st);
-    case 16: return launch_m<16, INV>(pl, p, nlines, st);
-    case 32: return launch_m<32, INV>(pl, p, nlines, st);
-    case 64: return launch_m<64, INV>(pl, p, nlines, st);
-    case 128: return launch_m<128, INV>(pl, p, nlines, st);
-    case 256: return launch_m<256, INV>(pl, p, nlines, st);
-    case 512: return launch_m<512, INV>(pl, p, nlines, st);
-    case 1024: return launch_m<1024, INV>(pl, p, nlines, st);
-    case 2048: return launch_m<2048, INV>(pl, p, nlines, st);
+    case 4: return launch_m<4, INV>(pl, p, nlines, st, div);
+    case 8: return launch_m<8, INV>(pl, p, nlines, st, div);
+    case 16: return launch_m<16, INV>(pl, p, nlines, st, div);
+    case 32: return launch_m<32, INV>(pl, p, nlines, st, div);
+    case 64: return launch_m<64, INV>(pl, p, nlines, st, div);
+    case 128: return launch_m<128, INV>(pl, p, nlines, st, div);
+    case 256: return launch_m<256, INV>(pl, p, nlines, st, div);
+    case 512: return launch_m<512, INV>(pl, p, nlines, st, div);
+    case 1024: return launch_m<1024, INV>(pl, p, nlines, st, div);
+    case 2048: return launch_m<2048, INV>(pl, p, nlines, st, div);
     default: set_error("fft_x: unsupported nx = %d", pl->nx); return PZ_EUNSUPPORTED;
     }
 }
@@ -152,11 +190,13 @@ int dispatch(const pz_plan *pl, double *p, long long nlines, cudaStream_t st)
 } // namespace
 
 // Transform the x lines of planes k0 .. k0+nk-1, in place.
-int launch_fft_x(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st)
+// div != NULL (forward, whole field only): transform the right-hand side of Eq. (4) formed from *div
+int launch_fft_x(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st, const DivSrc *div)
 {
     double *base = p + (size_t)k0 * pl->nx * pl->ny;
     const long long nlines = (long long)nk * pl->ny;
-    return inverse ? dispatch<true>(pl, base, nlines, st) : dispatch<false>(pl, base, nlines, st);
+    if (div && (inverse || k0 != 0 || nk != pl->nz)) { set_error("fft_x: the fused divergence needs the whole field, forward"); return PZ_EINVAL; }
+    return inverse ? dispatch<true>(pl, base, nlines, st, nullptr) : dispatch<false>(pl, base, nlines, st, div);
 }
 
 } // namespace pz

@@ -39,6 +39,7 @@ struct Options {
     int helm_tx = 0;          // 0 = auto: columns per CTA in the Helmholtz kernel (variant 0)
     int helm_m = 0;           // 0 = auto: rows per sub-domain in the Helmholtz kernel
     int fft_y_p0 = 1;         // 1 = pair-0 conversion inside the y-FFT kernel, 0 = separate small kernel
+    int div_fused = 1;        // pz_pressure_correction: 1 = divergence formed inside the forward x transform
     int fft_y_tc = 0;         // 0 = auto: complex column pairs per CTA in the y FFT
     int fft_x_lpb = 0;        // 0 = auto: lines per CTA in the x FFT
 };
@@ -116,7 +117,13 @@ struct ProfScope {
 };
 
 // kernels (each returns a pz_status)
-int launch_fft_x(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
+// velocity source of the fused divergence (forward x transform, pz_fft_x.cu)
+struct DivSrc {
+    const double *u = nullptr, *v = nullptr, *w = nullptr, *dzf = nullptr;
+    double rdx = 0, rdy = 0, scale = 0;
+    int ny = 0;
+};
+int launch_fft_x(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st, const DivSrc *div = nullptr);
 int launch_fft_y(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
 int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st);
 int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a = -1.0); // helm_a >= 0: Eq. (8) systems
