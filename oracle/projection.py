@@ -51,3 +51,18 @@ def project(lx, ly, zc, u, v, w, p, phi, gdt: float):
     """Eqs. (5)-(6): returns (u - gdt G Phi, v - ..., w - ..., p + Phi), gdt = gamma_k dt."""
     gx, gy, gz = gradient(lx, ly, zc, phi)
     return u - gdt * gx, v - gdt * gy, w - gdt * gz, p + phi
+
+
+def helmholtz_z_rhs(zc, zf, a: float, ustar2: np.ndarray, uk: np.ndarray) -> np.ndarray:
+    """Right-hand side of Eq. (11): u** - a L_z u^k with a = gamma_k nu dt / 2 and L_z
+    the wall-normal operator of definition O-H (Dirichlet walls, reading R7):
+    (L_z q)_k = A_k (q_{k-1} - q_k) + C_k (q_{k+1} - q_k) - W_k q_k."""
+    zc, zf = np.asarray(zc, dtype=np.float64), np.asarray(zf, dtype=np.float64)
+    dzf, dzc = np.diff(zf), np.diff(zc)
+    nz = zc.size
+    lz = np.zeros_like(uk)
+    lz[1:] += (1.0 / (dzf[1:] * dzc))[:, None, None] * (uk[:-1] - uk[1:])
+    lz[:-1] += (1.0 / (dzf[:-1] * dzc))[:, None, None] * (uk[1:] - uk[:-1])
+    lz[0] -= 2.0 / (dzf[0] * (2.0 * (zc[0] - zf[0]))) * uk[0]
+    lz[nz - 1] -= 2.0 / (dzf[nz - 1] * (2.0 * (zf[nz] - zc[nz - 1]))) * uk[nz - 1]
+    return ustar2 - a * lz

@@ -74,3 +74,31 @@ def test_projection_step_makes_the_field_divergence_free(shape, beta):
     assert np.abs(proj.divergence(lx, ly, zf, un, vn, wn)).max() <= 1e-11 * div0
     assert np.abs(wn[-1]).max() == 0.0                       # the wall face is not touched
     assert np.array_equal(pn, p + phi)
+
+
+@pytest.mark.parametrize("beta", [0.0, 1.8])
+def test_helmholtz_z_rhs_against_the_helmholtz_matrix_and_eigenfunctions(beta):
+    """u** - a L_z u^k = u** - u^k + (I - a L_z) u^k, with (I - a L_z) the tridiagonal matrix of the
+    oracle's Helmholtz solve (oracle.c); on a uniform grid sin(pi q (k+1/2)/nz) is an eigenfunction of
+    L_z with eigenvalue mu, so the right-hand side of u** = u^k = f is (1 - a mu) f and Eq. (11) returns
+    f itself (the implicit and the explicit half of the wall-normal diffusion cancel)."""
+    nx, ny, nz, a = 4, 6, 24, 3e-3
+    zc, zf = grid(nz, beta)
+    rng = np.random.default_rng(3)
+    u2, uk = rng.standard_normal((nz, ny, nx)), rng.standard_normal((nz, ny, nx))
+    lo, di, up = oracle.helmholtz_matrix(zc, zf, a)
+    muk = di[:, None, None] * uk
+    muk[1:] += lo[1:, None, None] * uk[:-1]
+    muk[:-1] += up[:-1, None, None] * uk[1:]
+    ref = u2 - uk + muk
+    got = proj.helmholtz_z_rhs(zc, zf, a, u2, uk)
+    assert np.abs(got - ref).max() <= 1e-13 * np.abs(ref).max()
+    if beta == 0.0:
+        q = 5
+        mode = np.sin(np.pi * q * (np.arange(nz) + 0.5) / nz)
+        f = np.broadcast_to(mode[:, None, None], (nz, ny, nx)).copy()
+        mu = -4 * np.sin(np.pi * q / (2 * nz)) ** 2 / (2.0 / nz) ** 2
+        r = proj.helmholtz_z_rhs(zc, zf, a, f, f)
+        assert np.abs(r - (1 - a * mu) * f).max() <= 1e-13
+        unew = oracle.helmholtz_z_solve(zc, zf, a, r)
+        assert np.abs(unew - f).max() <= 1e-13
