@@ -102,6 +102,16 @@ PZ_API int helmholtz_z_solve(pz_plan *plan, double *u, void *stream);
 PZ_API int helmholtz_z_solve_n(pz_plan *plan, double *const *u, int n, void *stream);
 
 /*
+ * The whole of Eq. (11):  u* - a L_z u* = u** - a L_z u^k  with the a of the last
+ * helmholtz_z_setup.  helmholtz_z_rhs overwrites ustar2 (on entry u**) with the right-hand side
+ * u** - a L_z u^k, L_z the operator above; helmholtz_z_step does that and then helmholtz_z_solve:
+ * on return ustar2 holds u*.  uk is only read.  Both device, nx*ny*nz doubles, 16-byte aligned.
+ * Errors: PZ_ENOTSETUP before the first setup; PZ_EINVAL for null or misaligned pointers.
+ */
+PZ_API int helmholtz_z_rhs(pz_plan *plan, double *ustar2, const double *uk, void *stream);
+PZ_API int helmholtz_z_step(pz_plan *plan, double *ustar2, const double *uk, void *stream);
+
+/*
  * Fully implicit diffusion, Eq. (8), PAPER.md:63-72 ("a Helmholtz equation for the prediction
  * velocity, implicit in the three spatial directions", solved "using the fast direct methods" of
  * the Poisson solve): for a = gamma_k nu dt / 2 >= 0 solves, in place,
@@ -198,7 +208,8 @@ enum pz_kernel_class {
     PZ_K_FFT_XY_INV = 9, /* a4+a5 in one kernel */
     PZ_K_DIV_RHS = 10,   /* pz_divergence_rhs */
     PZ_K_PROJECT = 11,   /* pz_project */
-    PZ_K_COUNT = 12
+    PZ_K_HELM_RHS = 12,  /* helmholtz_z_rhs */
+    PZ_K_COUNT = 13
 };
 PZ_API int pz_profile_enable(pz_plan *plan, int on);
 PZ_API int pz_profile_read(pz_plan *plan, int kernel_class, double *total_ms, long long *launches);

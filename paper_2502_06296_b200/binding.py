@@ -33,6 +33,8 @@ SIGNATURES = {
     "helmholtz_z_solve_n": (_i, [_vp, ctypes.POINTER(_vp), _i, _vp]),
     "poisson_solve_host": (_i, [_vp, _vp, _vp]),
     "helmholtz_z_solve_host": (_i, [_vp, _vp, _vp]),
+    "helmholtz_z_rhs": (_i, [_vp, _vp, _vp, _vp]),
+    "helmholtz_z_step": (_i, [_vp, _vp, _vp, _vp]),
     "helmholtz3d_setup": (_i, [_vp, ctypes.c_double]),
     "helmholtz3d_solve": (_i, [_vp, _vp, _vp]),
     "pz_divergence_rhs": (_i, [_vp, _vp, _vp, _vp, _vp, ctypes.c_double, _vp]),
@@ -168,6 +170,14 @@ def poisson_solve_host(plan: Plan, p_host, stream=None) -> None:
     _check(lib().poisson_solve_host(plan.handle, _host_ptr(p_host, plan.n), _stream_ptr(stream)))
 
 
+def helmholtz_z_rhs(plan: Plan, ustar2, uk, stream=None) -> None:
+    _check(lib().helmholtz_z_rhs(plan.handle, _dev_ptr(ustar2, plan.n), _dev_ptr(uk, plan.n), _stream_ptr(stream)))
+
+
+def helmholtz_z_step(plan: Plan, ustar2, uk, stream=None) -> None:
+    _check(lib().helmholtz_z_step(plan.handle, _dev_ptr(ustar2, plan.n), _dev_ptr(uk, plan.n), _stream_ptr(stream)))
+
+
 def helmholtz3d_setup(plan: Plan, a: float) -> None:
     _check(lib().helmholtz3d_setup(plan.handle, float(a)))
 
@@ -221,7 +231,7 @@ def pz_get_option(plan: Plan, key: str) -> int:
 
 
 KERNEL_CLASSES = ("fft_x_fwd", "fft_y_fwd", "pair0_fwd", "z_solve", "pair0_inv", "fft_y_inv", "fft_x_inv", "helmholtz",
-                  "fft_xy_fwd", "fft_xy_inv", "div_rhs", "project")
+                  "fft_xy_fwd", "fft_xy_inv", "div_rhs", "project", "helm_rhs")
 
 
 def pz_profile_enable(plan: Plan, on: bool) -> None:

@@ -375,6 +375,21 @@ int pz_pressure_correction(pz_plan *pl, double *u, double *v, double *w, double 
     return pz_project(pl, u, v, w, p, work, gdt, stream);
 }
 
+int helmholtz_z_rhs(pz_plan *pl, double *ustar2, const double *uk, void *stream)
+{
+    if (!pl || !ustar2 || !uk) { set_error("helmholtz_z_rhs: NULL argument"); return PZ_EINVAL; }
+    if (misaligned(ustar2) || misaligned(uk)) { set_error("helmholtz_z_rhs: fields must be 16-byte aligned"); return PZ_EINVAL; }
+    if (pl->helm_cur < 0) { set_error("helmholtz_z_rhs: call helmholtz_z_setup first"); return PZ_ENOTSETUP; }
+    return launch_helmholtz_z_rhs(pl, ustar2, uk, pl->helm_a, (cudaStream_t)stream);
+}
+
+int helmholtz_z_step(pz_plan *pl, double *ustar2, const double *uk, void *stream)
+{
+    const int rc = helmholtz_z_rhs(pl, ustar2, uk, stream);
+    if (rc != PZ_OK) return rc;
+    return helmholtz_z_solve(pl, ustar2, stream);
+}
+
 int helmholtz3d_setup(pz_plan *pl, double a)
 {
     if (!pl) { set_error("helmholtz3d_setup: plan is NULL"); return PZ_EINVAL; }

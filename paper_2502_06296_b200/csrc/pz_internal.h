@@ -129,6 +129,7 @@ int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cud
 int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a = -1.0); // helm_a >= 0: Eq. (8) systems
 int launch_divergence_rhs(pz_plan *pl, const double *u, const double *v, const double *w, double *out, double inv_gdt,
                           cudaStream_t st);
+int launch_helmholtz_z_rhs(pz_plan *pl, double *u2, const double *uk, double a, cudaStream_t st);
 int launch_project(pz_plan *pl, double *u, double *v, double *w, double *p, const double *phi, double gdt, cudaStream_t st);
 int launch_fft_xy_fwd(pz_plan *pl, double *p, cudaStream_t st);
 int launch_fft_xy_inv(pz_plan *pl, double *p, cudaStream_t st);

@@ -81,6 +81,41 @@ __global__ void __launch_bounds__(256)
     }
 }
 
+// Right-hand side of Eq. (11): r = u** - a L_z u^k, in place in u**, with
+// (L_z q)_k = A_k (q_{k-1} - q_k) + C_k (q_{k+1} - q_k) - W_k q_k (Dirichlet walls, reading R7).
+// Streaming z stencil: 24 algorithmic bytes per point (u**, u^k read; r written).
+__global__ void __launch_bounds__(256)
+    helmholtz_z_rhs_kernel(double *__restrict__ u2, const double *__restrict__ uk, const double *__restrict__ A,
+                           const double *__restrict__ C, int nx, int ny, int nz, double a, double w0, double w1)
+{
+    const size_t plane = (size_t)nx * ny, npairs = plane * nz / 2;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < npairs; q += (size_t)gridDim.x * blockDim.x) {
+        const size_t c = 2 * q;
+        const int k = (int)(c / plane);
+        const double2 qc = ld2(uk + c);
+        double2 lz = make_double2(0.0, 0.0);
+        if (k > 0) {
+            const double2 qm = ld2(uk + c - plane);
+            const double ak = A[k];
+            lz.x += ak * (qm.x - qc.x);
+            lz.y += ak * (qm.y - qc.y);
+        }
+        if (k + 1 < nz) {
+            const double2 qp = ld2(uk + c + plane);
+            const double ck = C[k];
+            lz.x += ck * (qp.x - qc.x);
+            lz.y += ck * (qp.y - qc.y);
+        }
+        const double wk = (k == 0 ? w0 : 0.0) + (k == nz - 1 ? w1 : 0.0);
+        lz.x -= wk * qc.x;
+        lz.y -= wk * qc.y;
+        double2 r = ld2(u2 + c);
+        r.x -= a * lz.x;
+        r.y -= a * lz.y;
+        st2(u2 + c, r);
+    }
+}
+
 int grid_for(const pz_plan *pl)
 {
     const size_t npairs = pl->n / 2;
@@ -98,6 +133,16 @@ int launch_divergence_rhs(pz_plan *pl, const double *u, const double *v, const d
     ProfScope prof(pl, PZ_K_DIV_RHS, st);
     divergence_rhs_kernel<<<grid_for(pl), 256, 0, st>>>(u, v, w, out, pl->d_dzf, pl->nx, pl->ny, pl->nz, 1.0 / dx, 1.0 / dy,
                                                         inv_gdt);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+int launch_helmholtz_z_rhs(pz_plan *pl, double *u2, const double *uk, double a, cudaStream_t st)
+{
+    ProfScope prof(pl, PZ_K_HELM_RHS, st);
+    helmholtz_z_rhs_kernel<<<grid_for(pl), 256, 0, st>>>(u2, uk, pl->d_A, pl->d_C, pl->nx, pl->ny, pl->nz, a, pl->wall_w0,
+                                                         pl->wall_w1);
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;

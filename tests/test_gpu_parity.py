@@ -510,6 +510,34 @@ def test_pressure_correction_step_is_divergence_free_and_matches_oracle(torch, p
     pz.poisson_plan_destroy(plan)
 
 
+@pytest.mark.parametrize("nx,ny,nz,beta,a", [(8, 8, 4, 0.0, 0.1), (32, 16, 100, 1.8, 5e-5), (64, 32, 512, 1.8, 5e-5),
+                                            (16, 16, 1100, 2.0, 2.5e-5)])
+def test_helmholtz_z_rhs_and_step_match_oracle(torch, pz, wl, oracle, nx, ny, nz, beta, a):
+    """Eq. (11) whole: r = u** - a L_z u^k (helmholtz_z_rhs), then the solve (helmholtz_z_step)."""
+    from oracle import projection as proj
+
+    zf = wl.z_faces(nz, 2.0, beta)
+    zc = wl.z_centres(zf)
+    rng = np.random.default_rng(nz + nx)
+    u2, uk = rng.standard_normal((nz, ny, nx)), rng.standard_normal((nz, ny, nx))
+    plan = pz.poisson_plan_create(nx, ny, nz, 1.0, 1.0, zc, zf)
+    d2, dk = torch.from_numpy(u2).cuda(), torch.from_numpy(uk).cuda()
+    with pytest.raises(pz.PzError) as ei:
+        pz.helmholtz_z_rhs(plan, d2, dk)
+    assert ei.value.status == pz.PZ_ENOTSETUP
+    pz.helmholtz_z_setup(plan, a)
+    pz.helmholtz_z_rhs(plan, d2, dk)
+    ref_r = proj.helmholtz_z_rhs(zc, zf, a, u2, uk)
+    bound = np.abs(u2).max() + 4 * a * np.abs(uk).max() / (np.diff(zf).min() * np.diff(zc).min())
+    assert np.abs(d2.cpu().numpy() - ref_r).max() <= 1e-14 * bound     # cancellation-aware bound
+    e2 = torch.from_numpy(u2).cuda()
+    pz.helmholtz_z_step(plan, e2, dk)
+    torch.cuda.synchronize()
+    assert rel_err(e2.cpu().numpy(), oracle.helmholtz_z_solve(zc, zf, a, ref_r)) <= TOL
+    assert torch.equal(dk, torch.from_numpy(uk).cuda())                 # u^k is only read
+    pz.poisson_plan_destroy(plan)
+
+
 def test_error_paths_of_the_widened_entry_points(torch, pz, wl):
     zf = wl.z_faces(1100, 2.0, 1.8)
     plan = pz.poisson_plan_create(16, 16, 1100, 1.0, 1.0, wl.z_centres(zf), zf)
