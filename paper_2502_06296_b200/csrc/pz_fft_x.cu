@@ -50,7 +50,7 @@ struct XchgX {
 // same order, so the result is bitwise the one of pz_divergence_rhs followed by this kernel); the
 // 16 B/point round trip of the right-hand side through HBM disappears.
 template <int M, int LPB, bool INV, bool DIV>
-__global__ void __launch_bounds__(FftPlan<M>::T *LPB)
+__global__ void __launch_bounds__(FftPlan<M>::T *LPB, (FftPlan<M>::T * LPB <= 128) ? 5 : 1)
     fft_x_kernel(double *__restrict__ p, const double2 *__restrict__ tw, long long nlines, double scale, const DivSrc ds)
 {
     static_assert(!(INV && DIV), "the divergence is fused into the forward transform only");
