@@ -385,6 +385,10 @@ int helmholtz_z_rhs(pz_plan *pl, double *ustar2, const double *uk, void *stream)
 
 int helmholtz_z_step(pz_plan *pl, double *ustar2, const double *uk, void *stream)
 {
+    if (pl && ustar2 && uk && !misaligned(ustar2) && !misaligned(uk) && pl->helm_cur >= 0) {
+        const int fused = launch_helmholtz_step(pl, ustar2, uk, (cudaStream_t)stream);
+        if (fused != PZ_EUNSUPPORTED) return fused;
+    }
     const int rc = helmholtz_z_rhs(pl, ustar2, uk, stream);
     if (rc != PZ_OK) return rc;
     return helmholtz_z_solve(pl, ustar2, stream);
@@ -559,6 +563,7 @@ static int *option_slot(pz_plan *pl, const char *key)
     if (!std::strcmp(key, "helm_m")) return &pl->opt.helm_m;
     if (!std::strcmp(key, "fft_y_tc")) return &pl->opt.fft_y_tc;
     if (!std::strcmp(key, "div_fused")) return &pl->opt.div_fused;
+    if (!std::strcmp(key, "step_fused")) return &pl->opt.step_fused;
     if (!std::strcmp(key, "fft_y_p0")) return &pl->opt.fft_y_p0;
     if (!std::strcmp(key, "fft_x_lpb")) return &pl->opt.fft_x_lpb;
     return nullptr;

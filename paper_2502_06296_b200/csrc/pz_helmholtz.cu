@@ -259,6 +259,25 @@ int helmholtz_build_tables(pz_plan *pl, double a)
     return PZ_OK;
 }
 
+// Eq. (11) in one kernel where the variant-1 pipeline can hold the tiles of u** and u^k;
+// PZ_EUNSUPPORTED otherwise (no launch made).
+int launch_helmholtz_step(pz_plan *pl, double *u2, const double *uk, cudaStream_t st)
+{
+    if (pl->helm_variant != 1 || pl->opt.step_fused == 0) return PZ_EUNSUPPORTED;
+    HelmTables &t = pl->helm[pl->helm_cur];
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    PZ_CUDA(cudaStreamIsCapturing(st, &cap));
+    const bool capturing = (cap != cudaStreamCaptureStatusNone);
+    if (!capturing && cudaEventQuery(t.uploaded) != cudaSuccess) PZ_CUDA(cudaStreamWaitEvent(st, t.uploaded, 0));
+    int rc;
+    {
+        ProfScope prof(pl, PZ_K_HELMHOLTZ, st);
+        rc = launch_helmholtz_tma_cn(pl, u2, uk, t.dev, st);
+    }
+    if (rc == PZ_OK && !capturing) PZ_CUDA(cudaEventRecord(t.last_use, st));
+    return rc;
+}
+
 int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st)
 {
     if (n == 0) return PZ_OK;

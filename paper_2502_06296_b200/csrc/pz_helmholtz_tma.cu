@@ -35,6 +35,10 @@ constexpr int kMaxFields = 4;  // fields per launch
 struct HelmArgs {
     CUtensorMap map[kMaxFields];
     double *u[kMaxFields];
+    // CN mode (helmholtz_z_step, one field): tiles of u^k and what the operator L_z needs
+    CUtensorMap qmap;
+    const double *A, *C;
+    double a, w0, w1;
 };
 
 template <int M> struct Limits {
@@ -55,15 +59,18 @@ template <int M> struct Smem {
     __host__ __device__ static size_t xch(int P) { return (size_t)2 * 2 * P * kTX; }
     __host__ __device__ static size_t tab(int P) { return (size_t)5 * P * TS; }
     __host__ __device__ static size_t pcr(int P, int levels) { return (size_t)levels * 4 * P + 2 * P; }
-    __host__ __device__ static size_t bytes(int P, int levels)
+    __host__ __device__ static size_t bytes(int P, int levels, bool cn = false)
     {
-        return (tile(P) + xch(P) + tab(P) + pcr(P, levels)) * sizeof(double) + 16;
+        return ((cn ? 2 : 1) * tile(P) + xch(P) + tab(P) + pcr(P, levels)) * sizeof(double) + 16;
     }
 };
 
 // Thread (cp, s): columns (2cp, 2cp+1) of the tile, sub-domain s (rows s*M .. s*M+M-1).
-template <int M, bool FULL>
-__global__ void __launch_bounds__(Limits<M>::kMaxThreads, Limits<M>::kMinBlocks)
+// CN: the whole of Eq. (11), PAPER.md:76 -- a second tile holds u^k and the right-hand side
+// u** - a L_z u^k is formed in registers while the rows are copied out (the separate pass of
+// helmholtz_z_rhs and its 16 B/point round trip disappear); one CTA per SM.
+template <int M, bool FULL, bool CN>
+__global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN ? 1 : Limits<M>::kMinBlocks)
     helmholtz_tma_kernel(const __grid_constant__ HelmArgs args, const double *__restrict__ tab, size_t plane, int nz,
                          int P, int levels, int tiles_per_field, int total_tiles, int probe, int box_rows, int nbox, int csz)
 {
@@ -72,14 +79,15 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, Limits<M>::kMinBlocks)
     constexpr int TS = L::TS;
     const int nzp = P * M, n2 = 2 * P;
     double *tile = reinterpret_cast<double *>(smem_raw);   // rows x 16
-    double *xch = tile + L::tile(P);                       // [buffer][first/last][s][16]
+    double *qtile = tile + L::tile(P);                     // CN only: rows x 16 of u^k
+    double *xch = qtile + (CN ? L::tile(P) : 0);           // [buffer][first/last][s][16]
     double *stab = xch + L::xch(P);                        // [table][s][TS]
     double *spcr = stab + L::tab(P);                       // [level][s][4], then [s][2]
     uint64_t *bar = reinterpret_cast<uint64_t *>(spcr + L::pcr(P, levels));
 
     const int tid = threadIdx.x, c2 = 2 * (tid & 7), s = tid >> 3;
     const int k0 = s * M;
-    const unsigned tile_bytes = (unsigned)(L::tile(P) * sizeof(double));
+    const unsigned tile_bytes = (unsigned)((CN ? 2 : 1) * L::tile(P) * sizeof(double));
 
     if (tid == 0) {
         mbar_init(bar, 1);
@@ -103,6 +111,9 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, Limits<M>::kMinBlocks)
         }
         for (int b = 0; b < nbox; ++b)
             tma_load_2d_hint(tile + (size_t)b * box_rows * kTX, &args.map[f], col0, b * box_rows, bar, pol);
+        if constexpr (CN)
+            for (int b = 0; b < nbox; ++b)
+                tma_load_2d_hint(qtile + (size_t)b * box_rows * kTX, &args.qmap, col0, b * box_rows, bar, pol);
     };
 
     int t = blockIdx.x;
@@ -121,6 +132,38 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, Limits<M>::kMinBlocks)
             const double2 v = ld2(tile + (k0 + i) * kTX + c2);
             da[i] = v.x;
             db[i] = v.y;
+        }
+        if constexpr (CN) {
+            // d <- u** - a L_z u^k, (L_z q)_k = A_k (q_{k-1} - q_k) + C_k (q_{k+1} - q_k) - W_k q_k
+            const double *qt = qtile + c2;
+            double2 qm = make_double2(0.0, 0.0), qc = ld2(qt + k0 * kTX);
+            if (k0 > 0) qm = ld2(qt + (k0 - 1) * kTX);
+#pragma unroll
+            for (int i = 0; i < M; ++i) {
+                const int k = k0 + i;
+                double2 qn = make_double2(0.0, 0.0);
+                if (k + 1 < nz) qn = ld2(qt + (k + 1) * kTX);
+                if (FULL || k < nz) {
+                    double2 lz = make_double2(0.0, 0.0);
+                    if (k > 0) {
+                        const double ak = __ldg(args.A + k);
+                        lz.x += ak * (qm.x - qc.x);
+                        lz.y += ak * (qm.y - qc.y);
+                    }
+                    if (k + 1 < nz) {
+                        const double ck = __ldg(args.C + k);
+                        lz.x += ck * (qn.x - qc.x);
+                        lz.y += ck * (qn.y - qc.y);
+                    }
+                    const double wk = (k == 0 ? args.w0 : 0.0) + (k == nz - 1 ? args.w1 : 0.0);
+                    lz.x -= wk * qc.x;
+                    lz.y -= wk * qc.y;
+                    da[i] -= args.a * lz.x;
+                    db[i] -= args.a * lz.y;
+                }
+                qm = qc;
+                qc = qn;
+            }
         }
         // every thread holds its rows: the buffer is free again.  With a cluster (csz > 1) the
         // CTAs of the cluster, which own neighbouring tiles, also meet here, so that their next
@@ -224,7 +267,7 @@ template <int M, bool FULL>
 int prepare_mf(pz_plan *pl)
 {
     const size_t smem = Smem<M>::bytes(pl->helm_P, pl->helm_levels);
-    auto kern = helmholtz_tma_kernel<M, FULL>;
+    auto kern = helmholtz_tma_kernel<M, FULL, false>;
     if (smem > 227 * 1024) { set_error("helmholtz (TMA variant): tile of %zu bytes does not fit shared memory", smem); return PZ_EUNSUPPORTED; }
     PZ_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     int bps = 0;
@@ -280,20 +323,63 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
     if (csz > 1) {
         cfg.gridDim = dim3((unsigned)(blocks / csz * csz));
         int nclusters = 0;
-        PZ_CUDA(cudaOccupancyMaxActiveClusters(&nclusters, helmholtz_tma_kernel<M, FULL>, &cfg));
+        PZ_CUDA(cudaOccupancyMaxActiveClusters(&nclusters, helmholtz_tma_kernel<M, FULL, false>, &cfg));
         if (nclusters < 1) { set_error("helmholtz (TMA variant): no cluster of %d CTAs fits", csz); return PZ_ECUDA; }
         if ((long long)nclusters * csz < blocks) blocks = (long long)nclusters * csz;
     }
     blocks = blocks / csz * csz;
     cfg.gridDim = dim3((unsigned)blocks);
-    PZ_CUDA(cudaLaunchKernelEx(&cfg, helmholtz_tma_kernel<M, FULL>, args, tab, plane, pl->nz, P, pl->helm_levels,
+    PZ_CUDA(cudaLaunchKernelEx(&cfg, helmholtz_tma_kernel<M, FULL, false>, args, tab, plane, pl->nz, P, pl->helm_levels,
                                tiles_per_field, (int)total, probe, box_rows, nbox, csz));
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
 }
 
+// helmholtz_z_step: one field, u** in u2 (in place), u^k in uk.  Returns PZ_EUNSUPPORTED when the two
+// tiles do not fit shared memory (the caller then runs the right-hand side as a separate pass).
+template <int M, bool FULL>
+int launch_cn_mf(pz_plan *pl, double *u2, const double *uk, const double *tab, cudaStream_t st)
+{
+    const int P = pl->helm_P;
+    const size_t plane = (size_t)pl->nx * pl->ny;
+    const size_t smem = Smem<M>::bytes(P, pl->helm_levels, true);
+    if (smem > 227 * 1024) return PZ_EUNSUPPORTED;
+    auto kern = helmholtz_tma_kernel<M, FULL, true>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        PZ_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        attr_done = true;
+    }
+    const int box_rows = Smem<M>::box_rows(P), nbox = Smem<M>::nbox(P);
+    HelmArgs args;
+    int rc = encode_column_tile_map(&args.map[0], u2, plane, pl->nz, kTX, box_rows, pl->opt.helm_l2promo);
+    if (rc != PZ_OK) return rc;
+    if ((rc = encode_column_tile_map(&args.qmap, uk, plane, pl->nz, kTX, box_rows, pl->opt.helm_l2promo)) != PZ_OK) return rc;
+    for (int f = 0; f < kMaxFields; ++f) { args.map[f] = args.map[0]; args.u[f] = u2; }
+    args.A = pl->d_A; args.C = pl->d_C; args.a = pl->helm_a; args.w0 = pl->wall_w0; args.w1 = pl->wall_w1;
+    const int tiles = (int)(plane / kTX);
+    int blocks = pl->num_sms < tiles ? pl->num_sms : tiles;
+    kern<<<blocks, (kTX / 2) * P, smem, st>>>(args, tab, plane, pl->nz, P, pl->helm_levels, tiles, tiles, 0, box_rows, nbox, 1);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
 } // namespace
+
+int launch_helmholtz_tma_cn(pz_plan *pl, double *u2, const double *uk, const double *tab, cudaStream_t st)
+{
+    const bool full = (pl->helm_P * pl->helm_m == pl->nz);
+#define PZ_HC(MM) (full ? launch_cn_mf<MM, true>(pl, u2, uk, tab, st) : launch_cn_mf<MM, false>(pl, u2, uk, tab, st))
+    switch (pl->helm_m) {
+    case 4: return PZ_HC(4);
+    case 8: return PZ_HC(8);
+    case 16: return PZ_HC(16);
+    default: return PZ_EUNSUPPORTED;
+    }
+#undef PZ_HC
+}
 
 // Called when the launch geometry (m, P) changes: shared-memory opt-in and resident CTAs per SM.
 int helmholtz_tma_prepare(pz_plan *pl)

@@ -39,6 +39,7 @@ struct Options {
     int helm_tx = 0;          // 0 = auto: columns per CTA in the Helmholtz kernel (variant 0)
     int helm_m = 0;           // 0 = auto: rows per sub-domain in the Helmholtz kernel
     int fft_y_p0 = 1;         // 1 = pair-0 conversion inside the y-FFT kernel, 0 = separate small kernel
+    int step_fused = 1;       // helmholtz_z_step: 1 = right-hand side of Eq. (11) formed inside the solve kernel
     int div_fused = 1;        // pz_pressure_correction: 1 = divergence formed inside the forward x transform
     int fft_y_tc = 0;         // 0 = auto: complex column pairs per CTA in the y FFT
     int fft_x_lpb = 0;        // 0 = auto: lines per CTA in the x FFT
@@ -136,6 +137,8 @@ int launch_fft_xy_inv(pz_plan *pl, double *p, cudaStream_t st);
 int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st);
 int launch_helmholtz_tma(pz_plan *pl, double *const *u, int n, const double *tab, cudaStream_t st);
 int helmholtz_tma_prepare(pz_plan *pl);
+int launch_helmholtz_tma_cn(pz_plan *pl, double *u2, const double *uk, const double *tab, cudaStream_t st);
+int launch_helmholtz_step(pz_plan *pl, double *u2, const double *uk, cudaStream_t st);
 int helmholtz_build_tables(pz_plan *pl, double a);
 
 } // namespace pz

@@ -84,27 +84,35 @@ __global__ void __launch_bounds__(256)
 // Right-hand side of Eq. (11): r = u** - a L_z u^k, in place in u**, with
 // (L_z q)_k = A_k (q_{k-1} - q_k) + C_k (q_{k+1} - q_k) - W_k q_k (Dirichlet walls, reading R7).
 // Streaming z stencil: 24 algorithmic bytes per point (u**, u^k read; r written).
+// Each thread owns one pair of x-neighbours and marches over kZChunk rows with u^k in a rolling
+// window, so every value of u^k is read once (plus two halo rows per chunk).
+constexpr int kZChunk = 32;
+
 __global__ void __launch_bounds__(256)
     helmholtz_z_rhs_kernel(double *__restrict__ u2, const double *__restrict__ uk, const double *__restrict__ A,
                            const double *__restrict__ C, int nx, int ny, int nz, double a, double w0, double w1)
 {
-    const size_t plane = (size_t)nx * ny, npairs = plane * nz / 2;
-    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < npairs; q += (size_t)gridDim.x * blockDim.x) {
-        const size_t c = 2 * q;
-        const int k = (int)(c / plane);
-        const double2 qc = ld2(uk + c);
+    const size_t plane = (size_t)nx * ny, ppairs = plane / 2;
+    const size_t pr = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pr >= ppairs) return;
+    const int kb = blockIdx.y * kZChunk, ke = min(kb + kZChunk, nz);
+    const size_t c0 = 2 * pr;
+    double2 qm = make_double2(0.0, 0.0), qc = ld2(uk + (size_t)kb * plane + c0);
+    if (kb > 0) qm = ld2(uk + (size_t)(kb - 1) * plane + c0);
+    for (int k = kb; k < ke; ++k) {
+        const size_t c = (size_t)k * plane + c0;
+        double2 qn = make_double2(0.0, 0.0);
+        if (k + 1 < nz) qn = ld2(uk + c + plane);
         double2 lz = make_double2(0.0, 0.0);
         if (k > 0) {
-            const double2 qm = ld2(uk + c - plane);
             const double ak = A[k];
             lz.x += ak * (qm.x - qc.x);
             lz.y += ak * (qm.y - qc.y);
         }
         if (k + 1 < nz) {
-            const double2 qp = ld2(uk + c + plane);
             const double ck = C[k];
-            lz.x += ck * (qp.x - qc.x);
-            lz.y += ck * (qp.y - qc.y);
+            lz.x += ck * (qn.x - qc.x);
+            lz.y += ck * (qn.y - qc.y);
         }
         const double wk = (k == 0 ? w0 : 0.0) + (k == nz - 1 ? w1 : 0.0);
         lz.x -= wk * qc.x;
@@ -113,6 +121,8 @@ __global__ void __launch_bounds__(256)
         r.x -= a * lz.x;
         r.y -= a * lz.y;
         st2(u2 + c, r);
+        qm = qc;
+        qc = qn;
     }
 }
 
@@ -141,7 +151,9 @@ int launch_divergence_rhs(pz_plan *pl, const double *u, const double *v, const d
 int launch_helmholtz_z_rhs(pz_plan *pl, double *u2, const double *uk, double a, cudaStream_t st)
 {
     ProfScope prof(pl, PZ_K_HELM_RHS, st);
-    helmholtz_z_rhs_kernel<<<grid_for(pl), 256, 0, st>>>(u2, uk, pl->d_A, pl->d_C, pl->nx, pl->ny, pl->nz, a, pl->wall_w0,
+    const size_t ppairs = (size_t)pl->nx * pl->ny / 2;
+    const dim3 grid((unsigned)((ppairs + 255) / 256), (unsigned)((pl->nz + kZChunk - 1) / kZChunk));
+    helmholtz_z_rhs_kernel<<<grid, 256, 0, st>>>(u2, uk, pl->d_A, pl->d_C, pl->nx, pl->ny, pl->nz, a, pl->wall_w0,
                                                          pl->wall_w1);
     count_launch();
     PZ_CUDA(cudaGetLastError());

@@ -530,10 +530,13 @@ def test_helmholtz_z_rhs_and_step_match_oracle(torch, pz, wl, oracle, nx, ny, nz
     ref_r = proj.helmholtz_z_rhs(zc, zf, a, u2, uk)
     bound = np.abs(u2).max() + 4 * a * np.abs(uk).max() / (np.diff(zf).min() * np.diff(zc).min())
     assert np.abs(d2.cpu().numpy() - ref_r).max() <= 1e-14 * bound     # cancellation-aware bound
-    e2 = torch.from_numpy(u2).cuda()
-    pz.helmholtz_z_step(plan, e2, dk)
-    torch.cuda.synchronize()
-    assert rel_err(e2.cpu().numpy(), oracle.helmholtz_z_solve(zc, zf, a, ref_r)) <= TOL
+    ref_u = oracle.helmholtz_z_solve(zc, zf, a, ref_r)
+    for fused in (1, 0):   # right-hand side formed inside the solve kernel (where two tiles fit) / as a separate pass
+        pz.pz_set_option(plan, "step_fused", fused)
+        e2 = torch.from_numpy(u2).cuda()
+        pz.helmholtz_z_step(plan, e2, dk)
+        torch.cuda.synchronize()
+        assert rel_err(e2.cpu().numpy(), ref_u) <= TOL
     assert torch.equal(dk, torch.from_numpy(uk).cuda())                 # u^k is only read
     pz.poisson_plan_destroy(plan)
 
