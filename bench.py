@@ -341,6 +341,22 @@ def main():
                                            if "project" in pc_kernels else None)}
         del work
 
+    # ---- next-row capability, outside the timed region: the whole of Eq. (11) for one component
+    hs = None
+    if len(us) >= 2:
+        for _ in range(2):
+            pz.helmholtz_z_step(plan, us[0], us[1])
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        s0.record()
+        for _ in range(5):
+            pz.helmholtz_z_step(plan, us[0], us[1])
+        s1.record()
+        torch.cuda.synchronize()
+        hs_ms = s0.elapsed_time(s1) / 5
+        hs = {"ms_per_field": hs_ms, "points_per_s": w.n / (hs_ms * 1e-3),
+              "GBps_algorithmic_24B_per_point": 24.0 * w.n / (hs_ms * 1e-3) / 1e9}
+
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -432,6 +448,8 @@ def main():
         line["helmholtz3d"] = h3
     if pc is not None:
         line["pressure_correction"] = pc
+    if hs is not None:
+        line["helmholtz_z_step"] = hs
     if e2e is not None:
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:
