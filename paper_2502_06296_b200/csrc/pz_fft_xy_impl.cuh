@@ -164,7 +164,7 @@ __device__ __forceinline__ void y_item(double *__restrict__ plane_base, const do
             v[e] = INV ? cconj(t) : t;
         }
     }
-    fft_line<L, 1, 0>(v, tid, tw, xc);
+    fft_line<L, 1, (L >= 1024) ? 1 : 0>(v, tid, tw, xc);
     if (!INV && p0) {
         // split W_r = A_r + i B_r into the packed spectra of the two real columns
         __syncthreads();
