@@ -37,6 +37,7 @@ struct HelmArgs {
     double *u[kMaxFields];
     // CN mode (helmholtz_z_step, one field): tiles of u^k and what the operator L_z needs
     CUtensorMap qmap;
+    const double *q;
     const double *A, *C;
     double a, w0, w1;
 };
@@ -69,8 +70,8 @@ template <int M> struct Smem {
 // CN: the whole of Eq. (11), PAPER.md:76 -- a second tile holds u^k and the right-hand side
 // u** - a L_z u^k is formed in registers while the rows are copied out (the separate pass of
 // helmholtz_z_rhs and its 16 B/point round trip disappear); one CTA per SM.
-template <int M, bool FULL, bool CN>
-__global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN ? 1 : Limits<M>::kMinBlocks)
+template <int M, bool FULL, int CN>
+__global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M>::kMinBlocks)
     helmholtz_tma_kernel(const __grid_constant__ HelmArgs args, const double *__restrict__ tab, size_t plane, int nz,
                          int P, int levels, int tiles_per_field, int total_tiles, int probe, int box_rows, int nbox, int csz)
 {
@@ -80,14 +81,14 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN ? 1 : Limits<M>::kM
     const int nzp = P * M, n2 = 2 * P;
     double *tile = reinterpret_cast<double *>(smem_raw);   // rows x 16
     double *qtile = tile + L::tile(P);                     // CN only: rows x 16 of u^k
-    double *xch = qtile + (CN ? L::tile(P) : 0);           // [buffer][first/last][s][16]
+    double *xch = qtile + (CN == 1 ? L::tile(P) : 0);           // [buffer][first/last][s][16]
     double *stab = xch + L::xch(P);                        // [table][s][TS]
     double *spcr = stab + L::tab(P);                       // [level][s][4], then [s][2]
     uint64_t *bar = reinterpret_cast<uint64_t *>(spcr + L::pcr(P, levels));
 
     const int tid = threadIdx.x, c2 = 2 * (tid & 7), s = tid >> 3;
     const int k0 = s * M;
-    const unsigned tile_bytes = (unsigned)((CN ? 2 : 1) * L::tile(P) * sizeof(double));
+    const unsigned tile_bytes = (unsigned)((CN == 1 ? 2 : 1) * L::tile(P) * sizeof(double));
 
     if (tid == 0) {
         mbar_init(bar, 1);
@@ -111,7 +112,7 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN ? 1 : Limits<M>::kM
         }
         for (int b = 0; b < nbox; ++b)
             tma_load_2d_hint(tile + (size_t)b * box_rows * kTX, &args.map[f], col0, b * box_rows, bar, pol);
-        if constexpr (CN)
+        if constexpr (CN == 1)
             for (int b = 0; b < nbox; ++b)
                 tma_load_2d_hint(qtile + (size_t)b * box_rows * kTX, &args.qmap, col0, b * box_rows, bar, pol);
     };
@@ -133,16 +134,20 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN ? 1 : Limits<M>::kM
             da[i] = v.x;
             db[i] = v.y;
         }
-        if constexpr (CN) {
-            // d <- u** - a L_z u^k, (L_z q)_k = A_k (q_{k-1} - q_k) + C_k (q_{k+1} - q_k) - W_k q_k
-            const double *qt = qtile + c2;
-            double2 qm = make_double2(0.0, 0.0), qc = ld2(qt + k0 * kTX);
-            if (k0 > 0) qm = ld2(qt + (k0 - 1) * kTX);
+        if constexpr (CN != 0) {
+            // d <- u** - a L_z u^k, (L_z q)_k = A_k (q_{k-1} - q_k) + C_k (q_{k+1} - q_k) - W_k q_k.
+            // CN == 1: u^k from the second shared-memory tile; CN == 2 (the tile pair does not fit):
+            // straight from global memory, row stride `plane`.
+            const size_t qs = (CN == 1) ? (size_t)kTX : plane;
+            const double *qt = (CN == 1) ? qtile + c2 : args.q + (size_t)t * kTX + c2;
+            double2 qm = make_double2(0.0, 0.0), qc = make_double2(0.0, 0.0);
+            if (FULL || k0 < nz) qc = ld2(qt + k0 * qs);
+            if (k0 > 0 && (FULL || k0 - 1 < nz)) qm = ld2(qt + (k0 - 1) * qs);
 #pragma unroll
             for (int i = 0; i < M; ++i) {
                 const int k = k0 + i;
                 double2 qn = make_double2(0.0, 0.0);
-                if (k + 1 < nz) qn = ld2(qt + (k + 1) * kTX);
+                if (k + 1 < nz) qn = ld2(qt + (k + 1) * qs);
                 if (FULL || k < nz) {
                     double2 lz = make_double2(0.0, 0.0);
                     if (k > 0) {
@@ -267,7 +272,7 @@ template <int M, bool FULL>
 int prepare_mf(pz_plan *pl)
 {
     const size_t smem = Smem<M>::bytes(pl->helm_P, pl->helm_levels);
-    auto kern = helmholtz_tma_kernel<M, FULL, false>;
+    auto kern = helmholtz_tma_kernel<M, FULL, 0>;
     if (smem > 227 * 1024) { set_error("helmholtz (TMA variant): tile of %zu bytes does not fit shared memory", smem); return PZ_EUNSUPPORTED; }
     PZ_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     int bps = 0;
@@ -323,13 +328,13 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
     if (csz > 1) {
         cfg.gridDim = dim3((unsigned)(blocks / csz * csz));
         int nclusters = 0;
-        PZ_CUDA(cudaOccupancyMaxActiveClusters(&nclusters, helmholtz_tma_kernel<M, FULL, false>, &cfg));
+        PZ_CUDA(cudaOccupancyMaxActiveClusters(&nclusters, helmholtz_tma_kernel<M, FULL, 0>, &cfg));
         if (nclusters < 1) { set_error("helmholtz (TMA variant): no cluster of %d CTAs fits", csz); return PZ_ECUDA; }
         if ((long long)nclusters * csz < blocks) blocks = (long long)nclusters * csz;
     }
     blocks = blocks / csz * csz;
     cfg.gridDim = dim3((unsigned)blocks);
-    PZ_CUDA(cudaLaunchKernelEx(&cfg, helmholtz_tma_kernel<M, FULL, false>, args, tab, plane, pl->nz, P, pl->helm_levels,
+    PZ_CUDA(cudaLaunchKernelEx(&cfg, helmholtz_tma_kernel<M, FULL, 0>, args, tab, plane, pl->nz, P, pl->helm_levels,
                                tiles_per_field, (int)total, probe, box_rows, nbox, csz));
     count_launch();
     PZ_CUDA(cudaGetLastError());
@@ -338,14 +343,13 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
 
 // helmholtz_z_step: one field, u** in u2 (in place), u^k in uk.  Returns PZ_EUNSUPPORTED when the two
 // tiles do not fit shared memory (the caller then runs the right-hand side as a separate pass).
-template <int M, bool FULL>
-int launch_cn_mf(pz_plan *pl, double *u2, const double *uk, const double *tab, cudaStream_t st)
+template <int M, bool FULL, int CN>
+int launch_cn_mfc(pz_plan *pl, double *u2, const double *uk, const double *tab, cudaStream_t st)
 {
     const int P = pl->helm_P;
     const size_t plane = (size_t)pl->nx * pl->ny;
-    const size_t smem = Smem<M>::bytes(P, pl->helm_levels, true);
-    if (smem > 227 * 1024) return PZ_EUNSUPPORTED;
-    auto kern = helmholtz_tma_kernel<M, FULL, true>;
+    const size_t smem = Smem<M>::bytes(P, pl->helm_levels, CN == 1);
+    auto kern = helmholtz_tma_kernel<M, FULL, CN>;
     static bool attr_done = false;
     if (!attr_done) {
         PZ_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
@@ -357,6 +361,7 @@ int launch_cn_mf(pz_plan *pl, double *u2, const double *uk, const double *tab, c
     if (rc != PZ_OK) return rc;
     if ((rc = encode_column_tile_map(&args.qmap, uk, plane, pl->nz, kTX, box_rows, pl->opt.helm_l2promo)) != PZ_OK) return rc;
     for (int f = 0; f < kMaxFields; ++f) { args.map[f] = args.map[0]; args.u[f] = u2; }
+    args.q = uk;
     args.A = pl->d_A; args.C = pl->d_C; args.a = pl->helm_a; args.w0 = pl->wall_w0; args.w1 = pl->wall_w1;
     const int tiles = (int)(plane / kTX);
     int blocks = pl->num_sms < tiles ? pl->num_sms : tiles;
@@ -364,6 +369,17 @@ int launch_cn_mf(pz_plan *pl, double *u2, const double *uk, const double *tab, c
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
+}
+
+// helmholtz_z_step: one field, u** in u2 (in place), u^k in uk.  u^k comes through a second
+// shared-memory tile where the pair fits, from global memory otherwise.
+template <int M, bool FULL>
+int launch_cn_mf(pz_plan *pl, double *u2, const double *uk, const double *tab, cudaStream_t st)
+{
+    if (Smem<M>::bytes(pl->helm_P, pl->helm_levels, true) <= 227 * 1024 && pl->opt.step_fused != 2)
+        return launch_cn_mfc<M, FULL, 1>(pl, u2, uk, tab, st);
+    if (Smem<M>::bytes(pl->helm_P, pl->helm_levels, false) > 227 * 1024) return PZ_EUNSUPPORTED;
+    return launch_cn_mfc<M, FULL, 2>(pl, u2, uk, tab, st);
 }
 
 } // namespace

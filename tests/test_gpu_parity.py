@@ -511,7 +511,7 @@ def test_pressure_correction_step_is_divergence_free_and_matches_oracle(torch, p
 
 
 @pytest.mark.parametrize("nx,ny,nz,beta,a", [(8, 8, 4, 0.0, 0.1), (32, 16, 100, 1.8, 5e-5), (64, 32, 512, 1.8, 5e-5),
-                                            (16, 16, 1100, 2.0, 2.5e-5)])
+                                            (16, 16, 1100, 2.0, 2.5e-5), (32, 16, 1024, 1.8, 2.5e-5), (16, 16, 700, 1.8, 2.5e-5)])
 def test_helmholtz_z_rhs_and_step_match_oracle(torch, pz, wl, oracle, nx, ny, nz, beta, a):
     """Eq. (11) whole: r = u** - a L_z u^k (helmholtz_z_rhs), then the solve (helmholtz_z_step)."""
     from oracle import projection as proj
@@ -531,7 +531,7 @@ def test_helmholtz_z_rhs_and_step_match_oracle(torch, pz, wl, oracle, nx, ny, nz
     bound = np.abs(u2).max() + 4 * a * np.abs(uk).max() / (np.diff(zf).min() * np.diff(zc).min())
     assert np.abs(d2.cpu().numpy() - ref_r).max() <= 1e-14 * bound     # cancellation-aware bound
     ref_u = oracle.helmholtz_z_solve(zc, zf, a, ref_r)
-    for fused in (1, 0):   # right-hand side formed inside the solve kernel (where two tiles fit) / as a separate pass
+    for fused in (1, 2, 0):   # formed inside the solve kernel (u^k through shared memory where two tiles fit; 2: u^k from global memory) / separate pass
         pz.pz_set_option(plan, "step_fused", fused)
         e2 = torch.from_numpy(u2).cuda()
         pz.helmholtz_z_step(plan, e2, dk)
