@@ -9,16 +9,16 @@ namespace pz {
 
 constexpr int kLanes = 32; // sub-domains per column = lanes of the warp that owns it
 
-// 1/x to ~1 ulp: hardware seed + two Newton steps (x is a positive, normal pivot).
+// 1/x to ~1 ulp: hardware seed r0 (relative error e0 <= ~2^-20: rcp.approx.ftz.f64 reads only the
+// upper 32 bits of x) and one cubic step r0 (1 + e + e^2), e = 1 - x r0, which leaves e0^3 < 2^-59.
+// x is a positive, normal pivot.
 __device__ __forceinline__ double fast_rcp(double x)
 {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    double e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    return r;
+    const double e = fma(-x, r, 1.0);
+    const double t = fma(e, e, e);
+    return fma(r, t, r);
 }
 
 __device__ __forceinline__ double shfl_up(double v, int d) { return __shfl_up_sync(0xffffffffu, v, d); }
