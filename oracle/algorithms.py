@@ -13,7 +13,8 @@ Pure-Python loops in the paper's order and notation, for small cases only:
 * ``pack_halfcomplex`` / ``unpack_halfcomplex``  Appendix A's n-reals-in / n-reals-out layout
   (the format equation itself is missing from the text, reading R8).
 
-All of them are pinned in tests/test_oracle_algorithms.py against dense LU
+All of them are pinned in tests/test_oracle_helmholtz.py (and tests/test_oracle_dft.py for the
+packed layout) against dense LU
 (numpy.linalg.solve) -- the paper's own verification style.
 """
 from __future__ import annotations

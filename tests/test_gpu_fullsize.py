@@ -5,10 +5,12 @@ options, fields resident in HBM, in-place solves).
 * c4 (1024^3): Helmholtz on one field; the oracle solves 8192 sampled columns one by one
   (columns are independent, so sampled columns are exact parity for those columns), spread over
   every tile position, plus the maximum principle on the whole field.
-* c3 (2048x1024x512): Poisson; the oracle's operator is applied to the GPU solution on the host:
-  the solution is unique, so a small normwise backward error plus the zero weighted mean pin it
-  (readings R3, R11); and linearity, solve(f) + solve(g) == solve(f + g) to rounding,
-  a property that holds at any size.
+* c3 (2048x1024x512): Poisson; element by element against the oracle on the c3 recipe at
+  2048x1024x128 (the transform kernels of c3: nx = 2048, ny = 1024) and at 64x64x512 with beta = 2.0
+  (c3's z-solve template: 16 rows per sub-domain, no padding rows), and on the full grid when the
+  box has the host memory for the oracle's work arrays; beside them, at the full size, the
+  oracle's operator applied to the GPU solution on the host (normwise backward error plus the
+  zero weighted mean, readings R3, R11) and linearity, a property that holds at any size.
 """
 import numpy as np
 import pytest
@@ -153,3 +155,53 @@ def test_c3_poisson_backward_error_and_linearity(env):
     fg -= torch.from_numpy(phi).cuda()
     assert float(fg.abs().max()) <= 1e-11 * np.abs(phi).max()
     pz.poisson_plan_destroy(plan)
+
+
+def _c3_like(wl, nx, ny, nz):
+    return wl.scaled(wl.CONFIGS["c3"], nx, ny, nz)
+
+
+@pytest.mark.parametrize("shape", [(2048, 1024, 128), (64, 64, 512), (2048, 64, 512), (64, 1024, 512)])
+def test_c3_templates_element_by_element(env, shape):
+    """The kernels c3 runs (x transform of 2048 reals, y transform of 1024 points, z-solve with
+    16-row sub-domains on the beta = 2.0 grid), whole solves compared with the oracle element by
+    element (Eq. 12; verification style PAPER.md:256)."""
+    torch, pz, wl, oracle = env
+    w = _c3_like(wl, *shape)
+    zc, zf = wl.grid(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    f = wl.poisson_rhs(w)
+    p = torch.from_numpy(f).cuda()
+    pz.poisson_solve(plan, p)
+    torch.cuda.synchronize()
+    got = p.cpu().numpy()
+    del p
+    ref = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)
+    assert rel_err(got, ref) <= TOL
+    pz.poisson_plan_destroy(plan)
+
+
+def test_c3_full_element_by_element_when_host_memory_allows(env):
+    """The full 2048x1024x512 solve against the oracle, element by element.  The oracle needs about
+    five field-sized host arrays (43 GB); the test is skipped, saying so, on a box without them."""
+    import psutil
+
+    torch, pz, wl, oracle = env
+    w = wl.CONFIGS["c3"]
+    need = 7 * w.n * 8
+    if psutil.virtual_memory().available < need:
+        pytest.skip(f"host has {psutil.virtual_memory().available / 2**30:.0f} GiB available, the oracle at c3 needs {need / 2**30:.0f}")
+    zc, zf = wl.grid(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    p = wl.device_remove_weighted_mean(wl.device_field(w, w.poisson_seed), zf)
+    f = p.cpu().numpy()
+    pz.poisson_solve(plan, p)
+    torch.cuda.synchronize()
+    got = p.cpu().numpy()
+    del p
+    pz.poisson_plan_destroy(plan)
+    ref = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)
+    del f
+    scale = np.abs(ref).max()
+    np.subtract(got, ref, out=got)
+    assert float(np.abs(got).max()) / scale <= TOL

@@ -251,3 +251,21 @@ def test_z_tables_uniform_reduce_to_textbook():
     assert np.allclose(dzf, dz, rtol=0, atol=1e-15) and np.allclose(dzc, dz, rtol=0, atol=1e-15)
     assert A[0] == 0.0 and C[-1] == 0.0
     assert np.allclose(A[1:], 1 / dz ** 2, rtol=1e-13) and np.allclose(C[:-1], 1 / dz ** 2, rtol=1e-13)
+
+
+@pytest.mark.parametrize("shape,beta", [((8, 4, 6), 1.8), ((4, 8, 7), 2.0), ((6, 4, 5), 0.0)])
+def test_apply_operator_matches_independent_stencil_on_stretched_grid(shape, beta):
+    """oracle.apply_poisson_operator (the checker of the full-size c3 GPU test) against the two
+    independent statements of O-P in this file: the dense matrix assembled entry by entry and
+    the long-double difference-form stencil (Eq. 12)."""
+    nx, ny, nz = shape
+    lx, ly = 8 * np.pi, 3 * np.pi
+    zf = wl.z_faces(nz, 2.0, beta)
+    zc = wl.z_centres(zf)
+    M, _ = dense_poisson_matrix(nx, ny, nz, lx, ly, zc, zf)
+    phi = np.random.default_rng(91 + nz).standard_normal((nz, ny, nx))
+    got = oracle.apply_poisson_operator(lx, ly, zc, zf, phi)
+    scale = np.abs(M).sum(axis=1).max() * np.abs(phi).max()
+    assert np.abs(got.reshape(-1) - M @ phi.reshape(-1)).max() <= 1e-14 * scale
+    ref_ld = apply_stencil_longdouble(phi, lx, ly, zc, zf)
+    assert np.abs(got - ref_ld.astype(np.float64)).max() <= 1e-14 * scale
