@@ -184,7 +184,7 @@ enum pz_stage {
     PZ_STAGE_Z_SOLVE = 2,   /* a3: tridiagonal solves in spectral space                   */
     PZ_STAGE_FFT_Y_INV = 3, /* a4                                                         */
     PZ_STAGE_FFT_X_INV = 4, /* a5: C2R along x and 1/(nx ny) scaling                      */
-    PZ_STAGE_FFT_XY_FWD = 5, /* a1+a2 by the fused kernel (nx, ny in {256,512,1024,2048})  */
+    PZ_STAGE_FFT_XY_FWD = 5, /* a1+a2 by the fused kernel (nx in {256,..,2048}, ny in {256,512,1024}) */
     PZ_STAGE_FFT_XY_INV = 6  /* a4+a5 by the fused kernel                                  */
 };
 PZ_API int pz_poisson_stage(pz_plan *plan, double *p, int stage, void *stream);

@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libpz_b200.so")
 SOURCES = ["pz_api.cu", "pz_fft_x.cu", "pz_fft_y.cu", "pz_fft_xy_fwd.cu", "pz_fft_xy_inv.cu", "pz_zsolve.cu", "pz_zsolve_cr.cu", "pz_zsolve_tma.cu", "pz_helmholtz.cu", "pz_helmholtz_tma.cu", "pz_projection.cu", "pz_tma.cu"]
-HEADERS = ["pz_internal.h", "pz_fft.cuh", "pz_tma.cuh", "pz_zsolve_pair.cuh", "pz_fft_xy_impl.cuh", os.path.join("..", "..", "include", "pz.h")]
+HEADERS = ["pz_internal.h", "pz_fft.cuh", "pz_tma.cuh", "pz_zsolve_pair.cuh", "pz_fft_xy_impl.cuh", "pz_fft2.cuh", os.path.join("..", "..", "include", "pz.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--fmad=true"]
 
@@ -57,7 +57,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
                 if r.returncode != 0:
                     raise RuntimeError("nvcc failed for " + cmd[-3])
     objs = [os.path.join(OBJ, s.replace(".cu", ".o")) for s in SOURCES]
-    if jobs or not os.path.exists(LIB):
+    if jobs or not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(o) for o in objs):
         cmd = [_nvcc(), "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a",
                "-Xcompiler", "-fPIC"]
         r = subprocess.run(cmd, capture_output=True, text=True)

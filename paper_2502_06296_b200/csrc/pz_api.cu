@@ -122,8 +122,8 @@ int slab_planes(const pz_plan *pl)
 
 bool fused_sizes(const pz_plan *pl)
 {
-    auto ok = [](int n) { return n == 256 || n == 512 || n == 1024 || n == 2048; };
-    return ok(pl->nx) && ok(pl->ny);
+    const int nx = pl->nx, ny = pl->ny;
+    return (nx == 256 || nx == 512 || nx == 1024 || nx == 2048) && (ny == 256 || ny == 512 || ny == 1024);
 }
 
 bool use_fused(const pz_plan *pl)
@@ -262,7 +262,7 @@ int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double
         if ((ce = cudaEventCreateWithFlags(&pl->helm[b].uploaded, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
         if ((ce = cudaEventCreateWithFlags(&pl->helm[b].last_use, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
     }
-    ce = cudaMalloc(&pl->d_xyctr, 2 * (size_t)(nz + 1) * sizeof(int));
+    ce = cudaMalloc(&pl->d_xyctr, 2 * (size_t)(nz + 64) * sizeof(int));
     if (ce != cudaSuccess) { cudaGetLastError(); set_error("plan counters: %s", cudaGetErrorString(ce)); return fail(PZ_ENOMEM); }
     // measured at 512 x 512 x nz: variant 2 wins from nz = 256 up to 1024, variant 1 below
     pl->opt.zsolve_variant = (nz <= 128) ? 1 : (nz <= 1024) ? 2 : 0;
@@ -315,8 +315,8 @@ int pz_poisson_stage(pz_plan *pl, double *p, int stage, void *stream)
     case PZ_STAGE_FFT_X_INV: return launch_fft_x(pl, p, 0, pl->nz, true, st);
     case PZ_STAGE_FFT_XY_FWD:
     case PZ_STAGE_FFT_XY_INV:
-        if (!fused_sizes(pl)) { set_error("pz_poisson_stage: the fused x/y kernel needs nx, ny in {256, 512, 1024, 2048}"); return PZ_EUNSUPPORTED; }
-        PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 1) * sizeof(int), st));
+        if (!fused_sizes(pl)) { set_error("pz_poisson_stage: the fused x/y kernel needs nx in {256, 512, 1024, 2048}, ny in {256, 512, 1024}"); return PZ_EUNSUPPORTED; }
+        PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 64) * sizeof(int), st));
         return stage == PZ_STAGE_FFT_XY_FWD ? launch_fft_xy_fwd(pl, p, st) : launch_fft_xy_inv(pl, p, st);
     default: set_error("pz_poisson_stage: unknown stage %d", stage); return PZ_EINVAL;
     }
@@ -328,7 +328,7 @@ int poisson_solve(pz_plan *pl, double *p, void *stream)
     if (((uintptr_t)p & 15) != 0) { set_error("poisson_solve: p must be 16-byte aligned"); return PZ_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
-    if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 1) * sizeof(int), st));
+    if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 64) * sizeof(int), st));
     if ((rc = forward_xy(pl, p, st)) != PZ_OK) return rc;
     if ((rc = launch_zsolve(pl, p, st)) != PZ_OK) return rc;
     return inverse_xy(pl, p, st);
@@ -409,7 +409,7 @@ int helmholtz3d_solve(pz_plan *pl, double *u, void *stream)
     if (pl->h3_a < 0.0) { set_error("helmholtz3d_solve: call helmholtz3d_setup first"); return PZ_ENOTSETUP; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
-    if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 1) * sizeof(int), st));
+    if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 64) * sizeof(int), st));
     if ((rc = forward_xy(pl, u, st)) != PZ_OK) return rc;
     if ((rc = launch_zsolve(pl, u, st, pl->h3_a)) != PZ_OK) return rc;
     return inverse_xy(pl, u, st);
@@ -554,6 +554,9 @@ static int *option_slot(pz_plan *pl, const char *key)
     if (!std::strcmp(key, "slab_planes")) return &pl->opt.slab_planes;
     if (!std::strcmp(key, "fft_fused")) return &pl->opt.fft_fused;
     if (!std::strcmp(key, "xy_lag")) return &pl->opt.xy_lag;
+    if (!std::strcmp(key, "xy_bps")) return &pl->opt.xy_bps;
+    if (!std::strcmp(key, "xy_prefetch")) return &pl->opt.xy_prefetch;
+    if (!std::strcmp(key, "xy_xshare")) return &pl->opt.xy_xshare;
     if (!std::strcmp(key, "helm_variant")) return &pl->opt.helm_variant;
     if (!std::strcmp(key, "helm_probe")) return &pl->opt.helm_probe;
     if (!std::strcmp(key, "helm_cluster")) return &pl->opt.helm_cluster;

@@ -1,0 +1,119 @@
+// pz_fft2.cuh -- two-pass register-resident FFT items (32 complex points per thread) for the fused
+// x/y transform (pz_fft_xy.cu), steps a1+a2 / a4+a5 of the hot path (
+// packed half-complex layout of Appendix A, reading R8).
+//
+// Why a second FFT core next to pz_fft.cuh.  With 16 points per thread a line of 512 complex points
+// takes three register passes (two shared-memory exchanges) and the real-to-complex split of an x
+// line a third exchange; at 512^3 that is 96 bytes per grid point through the 128 B/clk
+// shared-memory / L1 path per transform direction, 0.35 ms of a 0.33 ms DRAM budget.  Here a
+// thread keeps 32 complex points: every length up to 1024 is TWO passes (L = R1 R2, one exchange),
+// and on the x lines a thread owns the residue classes +-t of the spectral index, so the split
+// X_k <- (Z_k, Z_{M-k}) (and the merge of the inverse) pairs values the thread already holds: no
+// exchange.  64 bytes per point per direction instead of 96.
+//
+// Index convention (Stockham, decimation in frequency, as pz_fft.cuh), L = R1 R2:
+//   pass 1, butterfly j1 < R2:  y[j1 R1 + r'] = sum_r x[j1 + r R2] w_R1^{r r'}
+//   twiddle:                    y[j1 R1 + r'] *= w_L^{j1 r'}
+//   pass 2, butterfly j2 < R1:  X[j2 + r' R1] = sum_r y[j2 + r R1] w_R2^{r r'}
+// The twiddle is applied on the radix-32 side, where a thread holds ONE butterfly and every
+// factor is a power of a single base.
+#pragma once
+#include "pz_fft.cuh"
+
+namespace pz {
+
+constexpr int kE2 = 32; // complex points per thread
+
+// result r' of an in-register butterfly of radix R (dif<R, 1>) sits in slot bitrev(r')
+template <int R> __host__ __device__ constexpr int slot_of(int rp) { return bitrev(rp, ilog2(R)); }
+
+// v[slot(r)] *= w^r, r = 1..31, for the radix-32 side of a transform, w a single base per thread.  Only w, w^2, w^4, w^8, w^16 are looked
+// up; every other power is a product of at most two factors w^{4a} w^{b} (the table look-ups of a
+// 16-byte twiddle cost as many L1 wavefronts as the data they multiply, ncu r02: the transforms are
+// bound by the L1 / shared-memory data pipe, not by FP64).
+// BITREV: value r sits in slot bitrev(r) (outputs of a butterfly) or in slot r (inputs).
+// The five looked-up powers come from a small table base[m * pitch] = w^(2^m) of this thread
+// (staged in shared memory once per CTA: the thread's base never changes).
+template <bool BITREV>
+__device__ __forceinline__ void apply_twiddles32(double2 *v, const double2 *base, int pitch)
+{
+    auto slot = [](int r) { return BITREV ? slot_of<32>(r) : r; };
+    double2 wl[4], wh[8];
+    wl[1] = base[0];
+    wl[2] = base[pitch];
+    wl[3] = cmul(wl[1], wl[2]);
+    wh[1] = base[2 * pitch];
+    wh[2] = base[3 * pitch];
+    wh[4] = base[4 * pitch];
+    wh[3] = cmul(wh[1], wh[2]);
+    wh[5] = cmul(wh[4], wh[1]);
+    wh[6] = cmul(wh[4], wh[2]);
+    wh[7] = cmul(wh[4], wh[3]);
+#pragma unroll
+    for (int r = 1; r < 32; ++r) {
+        const int a = r / 4, b = r % 4;
+        double2 x = v[slot(r)];
+        if (a) x = cmul(x, wh[a]);
+        if (b) x = cmul(x, wl[b]);
+        v[slot(r)] = x;
+    }
+}
+
+// d * conj(w_R^r)
+template <int R, int r>
+__device__ __forceinline__ double2 mul_wc(double2 d) { return cconj(mul_w<R, r>(cconj(d))); }
+
+// ---- exchange buffers
+// x lines: one line per T threads, 16-byte elements, indexed (pos / R1)(R1 + 1) + pos % R1: lanes of
+// pass 1 (consecutive j1 = pos / R1) write with stride R1 + 1, lanes of pass 2 (consecutive
+// j2 = pos % R1) read consecutive elements; both are conflict-free (8 lanes x 16 B per wavefront).
+template <int R1>
+struct Xchg2X {
+    double2 *buf;
+    __device__ __forceinline__ static int idx(int pos) { return (pos / R1) * (R1 + 1) + (pos % R1); }
+    __device__ __forceinline__ void put(int pos, double2 v) const { buf[idx(pos)] = v; }
+    __device__ __forceinline__ double2 get(int pos) const { return buf[idx(pos)]; }
+};
+template <int L, int R1> __host__ __device__ constexpr int xline_elems() { return (L / R1) * (R1 + 1); }
+
+// y columns: TC neighbouring complex columns side by side, c fastest: 8 lanes = 128 contiguous bytes
+template <int TC>
+struct Xchg2Y {
+    double2 *buf;
+    int c;
+    __device__ __forceinline__ void put(int pos, double2 v) const { buf[pos * TC + c] = v; }
+    __device__ __forceinline__ double2 get(int pos) const { return buf[pos * TC + c]; }
+};
+
+// Residue classes mod 32 closed under negation for thread t of T (x lines): 32 / T classes per
+// thread in pairs (ja, jb = -ja mod 32).
+//   t >= 1: pair p = (t + 2 T p, 32 - t - 2 T p)
+//   t == 0: pair 0 = (0, 16), the two self-paired classes; pair p >= 1 = (T p, 32 - T p)
+template <int T> __device__ __forceinline__ int sym_ja(int t, int p) { return t ? t + 2 * T * p : T * p; }
+template <int T> __device__ __forceinline__ int sym_jb(int t, int p) { return t ? 32 - t - 2 * T * p : (p ? 32 - T * p : 16); }
+
+// split of the real-to-complex transform: X_k from Z_k, Z_{M-k} and w_n^k, n = 2M,
+//   X_k = (Z_k + conj Z_{M-k})/2 - (i/2) w_n^k (Z_k - conj Z_{M-k}),
+// with k = j + 32 r': w_n^k = w_n^j w_{n/32}^{r'}; wj = w_n^j is one look-up per residue class and
+// the second factor a compile-time constant (R2X = n / 32 <= 32) or, for n = 2048, wj itself is
+// the full twiddle (ROT = 0).
+template <int R2X, int ROT>
+__device__ __forceinline__ double2 r2c_split(double2 zk, double2 zmk, double2 wj)
+{
+    const double2 zm = cconj(zmk);
+    const double2 ev = make_double2(0.5 * (zk.x + zm.x), 0.5 * (zk.y + zm.y));
+    const double2 d = csub(zk, zm);
+    const double2 od = make_double2(0.5 * d.y, -0.5 * d.x);
+    return cadd(ev, cmul(mul_w<R2X, ROT>(od), wj));
+}
+// merge of the complex-to-real transform: conj(Z'_k), Z'_k = (X_k + conj X_{M-k}) + i conj(w_n^k)(X_k - conj X_{M-k})
+template <int R2X, int ROT>
+__device__ __forceinline__ double2 c2r_merge_conj(double2 xk, double2 xmk, double2 wj)
+{
+    const double2 xm = cconj(xmk);
+    const double2 s = cadd(xk, xm);
+    const double2 c = cmul_conj(mul_wc<R2X, ROT>(csub(xk, xm)), wj);
+    return make_double2(s.x - c.y, -(s.y + c.x));
+}
+
+} // namespace pz

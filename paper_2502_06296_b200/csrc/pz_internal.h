@@ -30,6 +30,9 @@ struct Options {
     int fft_fused = -1;       // -1 = auto (currently the separate kernels); 0 = separate kernels; 1 = fused x/y kernel
                               // (nx, ny in {256, 512, 1024, 2048})
     int xy_lag = 0;           // fused kernel: planes by which the first phase runs ahead (0 = auto)
+    int xy_bps = 0;           // fused kernel: resident CTAs per SM (0 = as many as fit)
+    int xy_xshare = 0;        // fused kernel: sixteenths of the SMs that prefer the first phase (0 = auto)
+    int xy_prefetch = 0;      // fused kernel: planes by which first-phase inputs are prefetched into L2 (0 = auto)
     int slab_planes = 0;      // 0 = auto: z-planes per L2-resident slab for the fused x/y FFT passes
     int helm_variant = -1;    // -1 = auto; 1 = persistent TMA-fed pipeline (nz <= 1024); 0 = register tile, direct loads
     int helm_box_rows = 0;    // diagnostic (variant 1): rows per TMA box (0 = 256)
@@ -76,7 +79,8 @@ struct pz_plan {
     double *d_batch_stage[3] = {nullptr, nullptr, nullptr};
     cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
     std::vector<cudaEvent_t> batch_events;
-    int *d_xyctr = nullptr;          // fused x/y kernels: 2 x (1 + nz) ticket / per-plane counters
+    int *d_xyctr = nullptr;          // fused x/y kernels: 2 x (64 + nz) ticket / per-plane counters
+    int xy_bps[2] = {0, 0};          // fused x/y kernels: resident CTAs per SM (forward, inverse), 0 = not yet queried
 
     // Helmholtz
     double helm_a = -1.0;
