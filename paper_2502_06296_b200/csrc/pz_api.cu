@@ -128,11 +128,13 @@ bool fused_sizes(const pz_plan *pl)
 
 bool use_fused(const pz_plan *pl)
 {
-    if (pl->opt.slab_planes > 0) return false;
-    // auto = separate kernels: the fused kernel halves the DRAM traffic of the transforms (ncu r01d:
-    // 16 instead of 32 B/point) but is bound by the on-SM work of the two transforms, which the
-    // separate kernels overlap with their own HBM time just as well (0.85 vs 0.72 ms at 512^3)
-    return pl->opt.fft_fused == 1 && fused_sizes(pl);
+    if (pl->opt.slab_planes > 0 || pl->opt.fft_fused == 0 || !fused_sizes(pl)) return false;
+    if (pl->opt.fft_fused == 1) return true;
+    // auto: the fused kernel hands a plane from the x to the y transform through L2 (16 instead of
+    // 32 DRAM bytes per point, ncu r02); that needs a few planes in flight to stay L2-resident, which
+    // holds up to 4 MB per plane (512^3: 0.62 + 0.57 ms against 0.71 + 0.72 ms for the separate
+    // kernels; 2048 x 1024 planes of 16 MB fall out of L2 and the separate kernels win)
+    return (size_t)pl->nx * pl->ny * sizeof(double) <= (size_t)4 << 20;
 }
 
 int forward_xy(pz_plan *pl, double *p, cudaStream_t st)
@@ -356,7 +358,7 @@ int pz_pressure_correction(pz_plan *pl, double *u, double *v, double *w, double 
 {
     if (!(gdt > 0.0) || !std::isfinite(gdt)) { set_error("pz_pressure_correction: gamma dt must be positive and finite"); return PZ_EINVAL; }
     int rc;
-    if (pl && u && v && w && work && pl->opt.div_fused != 0 && !use_fused(pl) && pl->opt.slab_planes == 0 &&
+    if (pl && u && v && w && work && pl->opt.div_fused != 0 && pl->opt.slab_planes == 0 &&
         !misaligned(u) && !misaligned(v) && !misaligned(w) && !misaligned(work)) {
         // Eq. (4)'s right-hand side is formed inside the forward x transform: it never touches HBM
         cudaStream_t st = (cudaStream_t)stream;
@@ -367,6 +369,7 @@ int pz_pressure_correction(pz_plan *pl, double *u, double *v, double *w, double 
         if ((rc = launch_fft_y(pl, work, 0, pl->nz, false, st)) != PZ_OK) return rc;
         if ((rc = launch_pair0(pl, work, 0, pl->nz, false, st)) != PZ_OK) return rc;
         if ((rc = launch_zsolve(pl, work, st)) != PZ_OK) return rc;
+        if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 64) * sizeof(int), st));
         if ((rc = inverse_xy(pl, work, st)) != PZ_OK) return rc;
         return pz_project(pl, u, v, w, p, work, gdt, stream);
     }
@@ -557,6 +560,7 @@ static int *option_slot(pz_plan *pl, const char *key)
     if (!std::strcmp(key, "xy_bps")) return &pl->opt.xy_bps;
     if (!std::strcmp(key, "xy_prefetch")) return &pl->opt.xy_prefetch;
     if (!std::strcmp(key, "xy_xshare")) return &pl->opt.xy_xshare;
+    if (!std::strcmp(key, "xy_group")) return &pl->opt.xy_group;
     if (!std::strcmp(key, "helm_variant")) return &pl->opt.helm_variant;
     if (!std::strcmp(key, "helm_probe")) return &pl->opt.helm_probe;
     if (!std::strcmp(key, "helm_cluster")) return &pl->opt.helm_cluster;

@@ -362,7 +362,7 @@ struct XYArgs {
     int n1, n2;    // first- / second-phase items per plane
     int D;         // planes by which the first phase may run ahead of the second
     int pf;        // planes by which first-phase inputs are prefetched into L2
-    int xshare;    // SMs with (index mod 16) < xshare prefer the first phase
+    int xshare, group; // SMs with (index mod 2 group) < xshare prefer the first phase
     double scale;
 };
 constexpr int kC1 = 0, kC2 = 32, kPub = 64; // counters on separate 128-byte lines
@@ -421,6 +421,7 @@ __global__ void __launch_bounds__(kThreads, 3) fft_xy_kernel(const __grid_consta
     double2 *smem = reinterpret_cast<double2 *>(smem_raw_xy + ((128u - (smem_u32(smem_raw_xy) & 127u)) & 127u));
     __shared__ double2 s_tw[TT::COUNT];
     __shared__ Item s_item;
+    __shared__ int s_deferred;
     __shared__ __align__(8) uint64_t s_bar;
     const size_t plane_sz = (size_t)a.nx * a.ny;
 
@@ -439,7 +440,7 @@ __global__ void __launch_bounds__(kThreads, 3) fft_xy_kernel(const __grid_consta
     const uint64_t pol_keep = l2_policy_evict_last(), pol_stream = l2_policy_evict_first();
     unsigned smid;
     asm("mov.u32 %0, %%smid;" : "=r"(smid));
-    int role = ((int)(smid % 16u) < a.xshare) ? 1 : 2; // thread 0's current phase preference
+    int role = ((int)(smid % (2u * a.group)) < a.xshare) ? 1 : 2; // thread 0's current phase preference
     Item pend;                                          // thread 0: ticket drawn but not started yet
     pend.phase = -1; pend.k = 0; pend.idx = 0;
 
@@ -502,11 +503,13 @@ __global__ void __launch_bounds__(kThreads, 3) fft_xy_kernel(const __grid_consta
     while (it.phase != 0) {
         double *pb = a.p + (size_t)it.k * plane_sz;
         // Called by every thread when its last read of the buffer is done: after the barrier the
-        // buffer is free and thread 0 takes the next item, if one can start right now.
-        bool deferred = false;
+        // buffer is free and thread 0 draws the next item and, if it can start right now, starts
+        // its fetch; otherwise the fetch is deferred to the end of this item.  (Drawing tickets
+        // earlier hides the L2 round trips but leaves the last items of a plane waiting in CTAs
+        // that are still busy, which stalls the second phase: measured slower.)
         auto next = [&]() {
             __syncthreads();
-            if (threadIdx.x == 0) deferred = !acquire(false);
+            if (threadIdx.x == 0) s_deferred = acquire(false) ? 0 : 1;
         };
         mbar_wait(&s_bar, parity);
         parity ^= 1;
@@ -519,16 +522,20 @@ __global__ void __launch_bounds__(kThreads, 3) fft_xy_kernel(const __grid_consta
             if (it.idx == 0) y_item<LY, INV, true>(pb, s_tw + TT::YP, it.idx, a.nx, smem, pol, next);
             else y_item<LY, INV, false>(pb, s_tw + TT::YP, it.idx, a.nx, smem, pol, next);
         }
-        __syncthreads(); // every store of this item precedes its publication
-        if (threadIdx.x == 0) {
-            if (it.phase == 1) {
-                __threadfence();
-                atomicAdd(&a.ctr[kPub + it.k], 1);
-            }
-            if (deferred) acquire(true);
+        __syncthreads(); // every store of this item precedes its publication; s_item / s_deferred are visible
+        const Item done = it;
+        const bool deferred = s_deferred != 0;
+        if (!deferred) it = s_item;
+        if (threadIdx.x == 0 && done.phase == 1) {
+            // publication; the fence overlaps the wait for the next item's data
+            __threadfence();
+            atomicAdd(&a.ctr[kPub + done.k], 1);
         }
-        __syncthreads(); // s_item of the next item is visible
-        it = s_item;
+        if (deferred) {
+            if (threadIdx.x == 0) acquire(true);
+            __syncthreads();
+            it = s_item;
+        }
     }
 }
 
@@ -567,7 +574,8 @@ int launch_xy(pz_plan *pl, double *p, cudaStream_t st)
     if (D > pl->nz) D = pl->nz;
     a.D = D;
     a.pf = pl->opt.xy_prefetch > 0 ? pl->opt.xy_prefetch : 3;
-    a.xshare = (pl->opt.xy_xshare > 0 && pl->opt.xy_xshare < 16) ? pl->opt.xy_xshare : 8;
+    a.group = pl->opt.xy_group > 0 ? pl->opt.xy_group : 2; // the two SMs of a TPC share an instruction-cache level: same role
+    a.xshare = (pl->opt.xy_xshare > 0 && pl->opt.xy_xshare < 2 * a.group) ? pl->opt.xy_xshare : a.group;
     ProfScope prof(pl, INV ? PZ_K_FFT_XY_INV : PZ_K_FFT_XY_FWD, st);
     kern<<<(unsigned)blocks, kThreads, G::SMEM, st>>>(ymap, a);
     count_launch();

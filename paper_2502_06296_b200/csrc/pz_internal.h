@@ -32,6 +32,7 @@ struct Options {
     int xy_lag = 0;           // fused kernel: planes by which the first phase runs ahead (0 = auto)
     int xy_bps = 0;           // fused kernel: resident CTAs per SM (0 = as many as fit)
     int xy_xshare = 0;        // fused kernel: sixteenths of the SMs that prefer the first phase (0 = auto)
+    int xy_group = 0;         // fused kernel: SMs per role group (0 = auto)
     int xy_prefetch = 0;      // fused kernel: planes by which first-phase inputs are prefetched into L2 (0 = auto)
     int slab_planes = 0;      // 0 = auto: z-planes per L2-resident slab for the fused x/y FFT passes
     int helm_variant = -1;    // -1 = auto; 1 = persistent TMA-fed pipeline (nz <= 1024); 0 = register tile, direct loads

@@ -203,10 +203,12 @@ def test_fft_roundtrip_and_spectrum_every_size(torch, pz, wl, nx, ny):
 
 @pytest.mark.parametrize("nx,ny,nz,lag", [(256, 256, 5, 0), (512, 256, 4, 0), (256, 512, 40, 0), (256, 256, 40, 1),
                                           (256, 256, 40, 3), (1024, 256, 4, 0), (256, 1024, 4, 0), (2048, 256, 4, 0),
-                                          (256, 2048, 4, 0)])
+                                          (512, 512, 70, 0), (512, 512, 70, 2), (1024, 512, 9, 0), (2048, 1024, 5, 0)])
 def test_fused_xy_transform_equals_the_separate_kernels(torch, pz, wl, nx, ny, nz, lag):
-    """The fused x/y kernel (ticket-ordered items, plane handed from phase one to phase two through
-    L2) runs the same arithmetic as the separate kernels: bitwise equal spectra and round trips."""
+    """The fused x/y kernel (two-pass 32-point items fed by TMA, plane handed from phase one to
+    phase two through L2, per-phase ticket counters) computes the same packed spectrum as the
+    separate kernels (another factorisation of the same transforms: equal to rounding, and bitwise
+    equal from one call to the next) and the same round trip."""
     w = wl.scaled(wl.CONFIGS["c0"], nx, ny, nz)
     zc, zf = wl.grid(w)
     f = np.random.default_rng(nx + 3 * ny + nz).standard_normal((nz, ny, nx))
@@ -216,14 +218,27 @@ def test_fused_xy_transform_equals_the_separate_kernels(torch, pz, wl, nx, ny, n
     b = torch.from_numpy(f).cuda()
     pz.pz_poisson_stage(plan, a, pz.PZ_STAGE_FFT_X_FWD)
     pz.pz_poisson_stage(plan, a, pz.PZ_STAGE_FFT_Y_FWD)
-    for _ in range(2):  # twice: the counters are reset per call
+    first = None
+    for _ in range(3):  # repeated: the counters are reset per call, the result does not depend on the item order
         b.copy_(torch.from_numpy(f))
         pz.pz_poisson_stage(plan, b, pz.PZ_STAGE_FFT_XY_FWD)
-        assert torch.equal(a, b)
+        assert float((a - b).abs().max()) <= 1e-13 * float(a.abs().max())
+        if first is None:
+            first = b.clone()
+        assert torch.equal(first, b)
+    # independent check of the fused spectrum against a library transform
+    g = b.cpu().numpy()
+    F = np.fft.fft(np.fft.rfft(f, axis=2), axis=1)   # [k][qy][qx], qx = 0..nx/2
+    scale = np.abs(F).max()
+    for q in (1, 2, nx // 4, nx // 2 - 1):
+        got = g[:, :, 2 * q] + 1j * g[:, :, 2 * q + 1]
+        assert np.abs(got - F[:, :, q]).max() <= 1e-12 * scale, q
+    assert np.abs(g[:, 0, 0] - F[:, 0, 0].real).max() <= 1e-12 * scale
+    assert np.abs(g[:, 1, 1] - F[:, ny // 2, nx // 2].real).max() <= 1e-12 * scale
     pz.pz_poisson_stage(plan, a, pz.PZ_STAGE_FFT_Y_INV)
     pz.pz_poisson_stage(plan, a, pz.PZ_STAGE_FFT_X_INV)
     pz.pz_poisson_stage(plan, b, pz.PZ_STAGE_FFT_XY_INV)
-    assert torch.equal(a, b)
+    assert float((a - b).abs().max()) <= 1e-13 * float(a.abs().max())
     assert np.abs(b.cpu().numpy() - f).max() <= 1e-13 * np.abs(f).max()
     pz.poisson_plan_destroy(plan)
 
@@ -255,8 +270,8 @@ def test_poisson_fused_and_separate_transforms_agree_with_the_oracle(torch, pz, 
     ref = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)
     fused = gpu_poisson(torch, pz, w, zc, zf, f, [("fft_fused", 1)])
     separate = gpu_poisson(torch, pz, w, zc, zf, f, [("fft_fused", 0)])
-    assert rel_err(fused, ref) <= TOL
-    assert np.array_equal(fused, separate)
+    assert rel_err(fused, ref) <= TOL and rel_err(separate, ref) <= TOL
+    assert rel_err(fused, separate) <= 1e-12
 
 
 # ---------------------------------------------------------------------- Helmholtz
@@ -443,8 +458,8 @@ def test_helmholtz3d_config1_full_and_fused_transforms(torch, pz, wl, oracle):
         pz.helmholtz3d_solve(plan, u)
         outs.append(u.cpu().numpy())
         pz.poisson_plan_destroy(plan)
-    assert rel_err(outs[0], ref) <= TOL
-    assert np.array_equal(outs[0], outs[1])
+    assert rel_err(outs[0], ref) <= TOL and rel_err(outs[1], ref) <= TOL
+    assert rel_err(outs[0], outs[1]) <= 1e-12
 
 
 # --------------------------------- the steps either side of the Poisson solve, Eqs. (4)-(6)
