@@ -133,8 +133,9 @@ bool use_fused(const pz_plan *pl)
     // auto: the fused kernel hands a plane from the x to the y transform through L2 (16 instead of
     // 32 DRAM bytes per point, ncu r02); that needs a few planes in flight to stay L2-resident, which
     // holds up to 4 MB per plane (512^3: 0.62 + 0.57 ms against 0.71 + 0.72 ms for the separate
-    // kernels; 2048 x 1024 planes of 16 MB fall out of L2 and the separate kernels win)
-    return (size_t)pl->nx * pl->ny * sizeof(double) <= (size_t)4 << 20;
+    // kernels; 2048 x 1024 planes of 16 MB fall out of L2 and the separate kernels win; a 256^3 field
+    // is L2-sized as a whole and the separate kernels already hit L2: 0.30 against 0.32 ms)
+    return (size_t)pl->nx * pl->ny * sizeof(double) <= ((size_t)4 << 20) && pl->n * sizeof(double) >= ((size_t)512 << 20);
 }
 
 int forward_xy(pz_plan *pl, double *p, cudaStream_t st)

@@ -313,16 +313,6 @@ __device__ __forceinline__ void y_item(double *__restrict__ plane_base, const do
 #pragma unroll
                 for (int rp = 0; rp < R2; ++rp) smem[t + b * T + 32 * rp] = v[b * R2 + slot_of<R2>(rp)];
         __syncthreads();
-        double2 wm[kE2];
-        if (c == 0)
-#pragma unroll
-            for (int b = 0; b < NB; ++b)
-#pragma unroll
-                for (int rp = 0; rp < R2; ++rp) {
-                    const int row = t + b * T + 32 * rp;
-                    wm[b * R2 + rp] = smem[(L - row) % L];
-                }
-        next();
 #pragma unroll
         for (int b = 0; b < NB; ++b)
 #pragma unroll
@@ -334,7 +324,7 @@ __device__ __forceinline__ void y_item(double *__restrict__ plane_base, const do
                 } else if (row == 0 || row == h) {
                     st2h(reinterpret_cast<double2 *>(base + (size_t)(row == 0 ? 0 : 1) * nx), w, pol);
                 } else if (row < h) {
-                    const double2 wc = cconj(wm[b * R2 + rp]);
+                    const double2 wc = cconj(smem[L - row]);
                     const double2 a = make_double2(0.5 * (w.x + wc.x), 0.5 * (w.y + wc.y));
                     const double2 d = csub(w, wc);
                     const double2 bb = make_double2(0.5 * d.y, -0.5 * d.x);
@@ -342,6 +332,7 @@ __device__ __forceinline__ void y_item(double *__restrict__ plane_base, const do
                     st2h(reinterpret_cast<double2 *>(base + (size_t)(2 * row + 1) * nx), make_double2(a.y, bb.y), pol);
                 }
             }
+        next(); // one item in ny / TC: the buffer is released after the stores
     } else {
 #pragma unroll
         for (int b = 0; b < NB; ++b)
