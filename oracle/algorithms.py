@@ -148,14 +148,19 @@ def _split(n, p):
     return bounds
 
 
-def solve_chunked(lo, di, up, d, p, algorithm=2):
+def solve_chunked(lo, di, up, d, p, algorithm=2, bounds=None):
     """Solve lo_k x_{k-1} + di_k x_k + up_k x_{k+1} = d_k with p sub-domains, following
-    PAPER.md:124-131 steps 4-6 with Algorithm 1 or Algorithm 2 inside each sub-domain."""
+    PAPER.md:124-131 steps 4-6 with Algorithm 1 or Algorithm 2 inside each sub-domain.
+
+    bounds: optional list of (start, end) row ranges of the sub-domains (the z-slabs owned by the
+    ranks of a distributed solve), contiguous, each of at least 3 rows (reading
+    R9); default: p sub-domains of sizes differing by at most one."""
     lo, di, up, d = (np.array(v, dtype=np.float64) for v in (lo, di, up, d))
     n = d.size
     lo[0] = 0.0
     up[n - 1] = 0.0
-    chunks = _split(n, p)
+    chunks = _split(n, p) if bounds is None else [tuple(b) for b in bounds]
+    assert chunks[0][0] == 0 and chunks[-1][1] == n and all(chunks[s][1] == chunks[s + 1][0] for s in range(len(chunks) - 1))
     red, state = [], []
     for (s0, s1) in chunks:
         if algorithm == 1:

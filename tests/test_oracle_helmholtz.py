@@ -112,6 +112,28 @@ def test_chunked_algorithms_match_dense_lu(n, p, algorithm):
     assert np.abs(oracle.thomas(lo, di, up, d) - ref).max() <= 1e-13 * np.abs(ref).max()
 
 
+@pytest.mark.parametrize("bounds", [[(0, 3), (3, 6)], [(0, 3), (3, 40), (40, 43), (43, 64)], [(0, 34), (34, 67), (67, 100)],
+                                    [(0, 5), (5, 8), (8, 11), (11, 14), (14, 17), (17, 20), (20, 23), (23, 26)]])
+@pytest.mark.parametrize("algorithm", [1, 2])
+def test_uneven_slabs_match_dense_lu(bounds, algorithm):
+    """The z-slabs of a distributed solve need not be equal: any contiguous
+    partition with at least 3 rows per slab (reading R9) reproduces the serial solve, also on the
+    Poisson systems of a low mode of a stretched grid (diagonal -(A+C) - sigma)."""
+    n = bounds[-1][1]
+    rng = np.random.default_rng(7 * n + len(bounds))
+    lo, di, up, d, ref = _random_system(n, rng)
+    got = alg.solve_chunked(lo, di, up, d, len(bounds), algorithm, bounds=bounds)
+    assert np.abs(got - ref).max() <= 1e-13 * np.abs(ref).max()
+    zf = wl.z_faces(n, 2.0, 1.8)
+    zc = wl.z_centres(zf)
+    A, C = oracle.z_tables(zc, zf)[2:]
+    sigma = 0.37
+    lo2, up2, di2 = A.copy(), C.copy(), -(A + C) - sigma
+    ref2 = oracle.thomas(lo2, di2, up2, d)
+    got2 = alg.solve_chunked(lo2, di2, up2, d, len(bounds), algorithm, bounds=bounds)
+    assert np.abs(got2 - ref2).max() <= 1e-10 * np.abs(ref2).max()
+
+
 @pytest.mark.parametrize("algorithm", [1, 2])
 def test_two_row_subdomains_are_not_supported(algorithm):
     """Reading R9: the algorithms as printed need m >= 3 rows per sub-domain."""
