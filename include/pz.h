@@ -80,6 +80,37 @@ PZ_API int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx,
 PZ_API int poisson_solve(pz_plan *plan, double *p, void *stream);
 
 /*
+ * ONE Poisson problem spread over several ranks (GPUs) by z-slabs: the paper's parallel tridiagonal
+ * solver, PAPER.md:120-135 (steps 1-8 of section 2.2.3) and :139-155, with GPUs for its "MPI tasks".
+ * Rank `slab` of `n_slabs` owns the planes [kbounds[slab], kbounds[slab+1]) of the global grid of nz
+ * planes (kbounds: host, n_slabs + 1 ints, from 0 to nz, at least 3 and at most 1024 planes per slab,
+ * PAPER.md:284; n_slabs <= 16); x and y transforms are plane-local.  zc, zf describe the GLOBAL grid.
+ * Plan creation also computes, on the device, the right-hand-side-independent coefficients of the
+ * reduced boundary systems of ALL slabs ("only once as an initialization step"; every
+ * rank computes them itself, so creating the plans needs no communication).
+ *
+ * A solve is two calls around ONE collective that the caller performs (e.g. NCCL all-gather):
+ *   poisson_solve_reduce   p (device, this rank's nx*ny*nk doubles, in place): forward transforms,
+ *                          slab-local reduction; writes this rank's boundary values into
+ *                          boundary_out (device, poisson_slab_boundary_doubles(plan) doubles:
+ *                          2 nx ny values "packed" as in PAPER.md:127 plus the slab's rows of the
+ *                          singular (0,0) column).
+ *   [all-gather boundary_out of every rank, in rank order, into boundary_all]
+ *   poisson_solve_finish   solves the reduced systems of size 2 n_slabs for every column
+ *                          (redundantly on every rank), reconstructs the slab and
+ *                          applies the inverse transforms: p holds this rank's planes of phi, the
+ *                          same solution poisson_solve gives on one GPU (zero volume mean).
+ * Errors: PZ_EINVAL (bad bounds, NULL, not a slab plan), PZ_EUNSUPPORTED (slab thickness), PZ_ENOMEM,
+ * PZ_ECUDA.  poisson_solve, helmholtz_* and helmholtz3d_* refuse a slab plan.
+ */
+PZ_API int poisson_slab_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double ly,
+                             const double *zc, const double *zf, int bc, int n_slabs, int slab,
+                             const int *kbounds);
+PZ_API long long poisson_slab_boundary_doubles(const pz_plan *plan);
+PZ_API int poisson_solve_reduce(pz_plan *plan, double *p, double *boundary_out, void *stream);
+PZ_API int poisson_solve_finish(pz_plan *plan, double *p, const double *boundary_all, void *stream);
+
+/*
  * Wall-normal implicit diffusion, Eq. (11), with the paper's split of the
  * cyclic-reduction solver into pre-processing and runtime (Algorithm 2).
  *

@@ -28,6 +28,10 @@ _dp = ctypes.POINTER(ctypes.c_double)
 SIGNATURES = {
     "poisson_plan_create": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _d, _d, _dp, _dp, _i]),
     "poisson_solve": (_i, [_vp, _vp, _vp]),
+    "poisson_slab_plan_create": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _d, _d, _dp, _dp, _i, _i, _i, ctypes.POINTER(_i)]),
+    "poisson_slab_boundary_doubles": (ctypes.c_longlong, [_vp]),
+    "poisson_solve_reduce": (_i, [_vp, _vp, _vp, _vp]),
+    "poisson_solve_finish": (_i, [_vp, _vp, _vp, _vp]),
     "helmholtz_z_setup": (_i, [_vp, _d]),
     "helmholtz_z_solve": (_i, [_vp, _vp, _vp]),
     "helmholtz_z_solve_n": (_i, [_vp, ctypes.POINTER(_vp), _i, _vp]),
@@ -93,12 +97,12 @@ def _stream_ptr(stream) -> int:
     return stream.cuda_stream
 
 
-def _dev_ptr(t, n: int) -> int:
+def _dev_ptr(t, n) -> int:
     import torch
 
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
         raise TypeError("field must be a contiguous float64 CUDA tensor")
-    if t.numel() != n:
+    if n is not None and t.numel() != n:
         raise ValueError(f"field has {t.numel()} elements, plan expects {n}")
     return t.data_ptr()
 
@@ -141,6 +145,35 @@ def poisson_plan_create(nx: int, ny: int, nz: int, lx: float, ly: float, zc, zf,
     _check(lib().poisson_plan_create(ctypes.byref(out), nx, ny, nz, float(lx), float(ly),
                                      zc.ctypes.data_as(_dp), zf.ctypes.data_as(_dp), bc))
     return Plan(out.value, nx, ny, nz)
+
+
+def poisson_slab_plan_create(nx: int, ny: int, nz: int, lx: float, ly: float, zc, zf, n_slabs: int, slab: int, kbounds,
+                             bc: int = PZ_BC_PERIODIC_XY_NEUMANN_P_DIRICHLET_U) -> Plan:
+    """Plan of rank `slab` of a Poisson problem cut into `n_slabs` z-slabs; the
+    plan's field is the slab's planes [kbounds[slab], kbounds[slab+1]) of the global grid zc, zf."""
+    zc = np.ascontiguousarray(zc, dtype=np.float64)
+    zf = np.ascontiguousarray(zf, dtype=np.float64)
+    kb = np.ascontiguousarray(kbounds, dtype=np.int32)
+    if zc.size != nz or zf.size != nz + 1 or kb.size != n_slabs + 1:
+        raise ValueError("zc must have nz entries, zf nz+1 and kbounds n_slabs+1")
+    out = _vp()
+    _check(lib().poisson_slab_plan_create(ctypes.byref(out), nx, ny, nz, float(lx), float(ly), zc.ctypes.data_as(_dp),
+                                          zf.ctypes.data_as(_dp), bc, n_slabs, slab,
+                                          kb.ctypes.data_as(ctypes.POINTER(_i))))
+    return Plan(out.value, nx, ny, int(kb[slab + 1] - kb[slab]))
+
+
+def poisson_slab_boundary_doubles(plan: Plan) -> int:
+    return int(lib().poisson_slab_boundary_doubles(plan.handle))
+
+
+def poisson_solve_reduce(plan: Plan, p, boundary_out, stream=None) -> None:
+    _check(lib().poisson_solve_reduce(plan.handle, _dev_ptr(p, plan.n), _dev_ptr(boundary_out, poisson_slab_boundary_doubles(plan)),
+                                      _stream_ptr(stream)))
+
+
+def poisson_solve_finish(plan: Plan, p, boundary_all, stream=None) -> None:
+    _check(lib().poisson_solve_finish(plan.handle, _dev_ptr(p, plan.n), _dev_ptr(boundary_all, None), _stream_ptr(stream)))
 
 
 def poisson_plan_destroy(plan: Plan) -> None:

@@ -181,8 +181,9 @@ const char *pz_last_error(void) { return g_err; }
 long long pz_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 int pz_version(void) { return 100; }
 
-int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double ly, const double *zc,
-                        const double *zf, int bc)
+// kb0 / nk: the planes [kb0, kb0 + nk) this plan transforms and owns (the whole grid for an ordinary plan)
+static int plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double ly, const double *zc, const double *zf,
+                       int bc, int kb0, int nk)
 {
     g_err[0] = 0;
     if (!out) { set_error("poisson_plan_create: out is NULL"); return PZ_EINVAL; }
@@ -211,8 +212,9 @@ int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double
 
     pz_plan *pl = new (std::nothrow) pz_plan();
     if (!pl) { set_error("poisson_plan_create: out of host memory"); return PZ_ENOMEM; }
-    pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->lx = lx; pl->ly = ly;
-    pl->n = (size_t)nx * ny * nz;
+    pl->nx = nx; pl->ny = ny; pl->nz = nk; pl->nz_glob = nz; pl->lx = lx; pl->ly = ly;
+    pl->n = (size_t)nx * ny * nk;
+    (void)kb0;
     int rc = PZ_OK;
     auto fail = [&](int code) { poisson_plan_destroy(pl); return code; };
     if (cudaGetDevice(&pl->device) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaGetDevice"));
@@ -265,13 +267,88 @@ int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double
         if ((ce = cudaEventCreateWithFlags(&pl->helm[b].uploaded, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
         if ((ce = cudaEventCreateWithFlags(&pl->helm[b].last_use, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
     }
-    ce = cudaMalloc(&pl->d_xyctr, 2 * (size_t)(nz + 64) * sizeof(int));
+    ce = cudaMalloc(&pl->d_xyctr, 2 * (size_t)(nk + 64) * sizeof(int));
     if (ce != cudaSuccess) { cudaGetLastError(); set_error("plan counters: %s", cudaGetErrorString(ce)); return fail(PZ_ENOMEM); }
     // measured at 512 x 512 x nz: variant 2 wins from nz = 256 up to 1024, variant 1 below
     pl->opt.zsolve_variant = (nz <= 128) ? 1 : (nz <= 1024) ? 2 : 0;
-    if (pl->opt.zsolve_variant == 0 && (rc = ensure_zwork(pl)) != PZ_OK) return fail(rc);
+    if (nk == nz && pl->opt.zsolve_variant == 0 && (rc = ensure_zwork(pl)) != PZ_OK) return fail(rc);
     *out = pl;
     return PZ_OK;
+}
+
+int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double ly, const double *zc,
+                        const double *zf, int bc)
+{
+    return plan_create(out, nx, ny, nz, lx, ly, zc, zf, bc, 0, nz);
+}
+
+int poisson_slab_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double ly, const double *zc,
+                             const double *zf, int bc, int n_slabs, int slab, const int *kbounds)
+{
+    if (out) *out = nullptr;
+    if (!kbounds || n_slabs < 1 || n_slabs > 16 || slab < 0 || slab >= n_slabs) {
+        set_error("poisson_slab_plan_create: need 1 <= n_slabs <= 16, 0 <= slab < n_slabs and the plane bounds");
+        return PZ_EINVAL;
+    }
+    if (kbounds[0] != 0 || kbounds[n_slabs] != nz) { set_error("poisson_slab_plan_create: kbounds must run from 0 to nz"); return PZ_EINVAL; }
+    int nkmax = 0;
+    for (int j = 0; j < n_slabs; ++j) {
+        const int nk = kbounds[j + 1] - kbounds[j];
+        // Algorithms 1 and 2 need three rows per sub-domain (reading R9)
+        if (nk < 3 || nk > 1024) { set_error("poisson_slab_plan_create: slab %d has %d planes (3..1024 supported)", j, nk); return PZ_EUNSUPPORTED; }
+        if (nk > nkmax) nkmax = nk;
+    }
+    pz_plan *pl = nullptr;
+    int rc = plan_create(&pl, nx, ny, nz, lx, ly, zc, zf, bc, kbounds[slab], kbounds[slab + 1] - kbounds[slab]);
+    if (rc != PZ_OK) return rc;
+    auto fail = [&](int code) { poisson_plan_destroy(pl); return code; };
+    pl->slab_G = n_slabs; pl->slab_g = slab;
+    pl->slab_kb.assign(kbounds, kbounds + n_slabs + 1);
+    const size_t plane = (size_t)nx * ny;
+    pl->slab_bstride = 2 * plane + (size_t)((nkmax + 1) & ~1);
+    cudaError_t ce;
+    if ((ce = cudaMalloc(&pl->d_slab_kb, (n_slabs + 1) * sizeof(int))) != cudaSuccess ||
+        (ce = cudaMalloc(&pl->slab_coef, (size_t)n_slabs * 6 * plane * sizeof(double))) != cudaSuccess ||
+        (ce = cudaMalloc(&pl->slab_phi, 2 * plane * sizeof(double))) != cudaSuccess) {
+        cudaGetLastError();
+        set_error("poisson_slab_plan_create: %s", cudaGetErrorString(ce));
+        return fail(PZ_ENOMEM);
+    }
+    if ((ce = cudaMemcpy(pl->d_slab_kb, kbounds, (n_slabs + 1) * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(cuda_fail(ce, "cudaMemcpy(kbounds)"));
+    // every rank computes the interface coefficients of ALL slabs itself: no collective
+    if ((rc = launch_slab_coefficients(pl, nullptr)) != PZ_OK) return fail(rc);
+    if ((ce = cudaDeviceSynchronize()) != cudaSuccess) return fail(cuda_fail(ce, "slab coefficients"));
+    *out = pl;
+    return PZ_OK;
+}
+
+long long poisson_slab_boundary_doubles(const pz_plan *pl)
+{
+    return (pl && pl->slab_G > 0) ? (long long)pl->slab_bstride : 0;
+}
+
+int poisson_solve_reduce(pz_plan *pl, double *p, double *boundary_out, void *stream)
+{
+    if (!pl || !p || !boundary_out) { set_error("poisson_solve_reduce: NULL argument"); return PZ_EINVAL; }
+    if (pl->slab_G < 1) { set_error("poisson_solve_reduce: the plan is not a slab plan"); return PZ_EINVAL; }
+    if ((((uintptr_t)p | (uintptr_t)boundary_out) & 15) != 0) { set_error("poisson_solve_reduce: buffers must be 16-byte aligned"); return PZ_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 64) * sizeof(int), st));
+    if ((rc = forward_xy(pl, p, st)) != PZ_OK) return rc;
+    return launch_slab_reduce(pl, p, boundary_out, st);
+}
+
+int poisson_solve_finish(pz_plan *pl, double *p, const double *boundary_all, void *stream)
+{
+    if (!pl || !p || !boundary_all) { set_error("poisson_solve_finish: NULL argument"); return PZ_EINVAL; }
+    if (pl->slab_G < 1) { set_error("poisson_solve_finish: the plan is not a slab plan"); return PZ_EINVAL; }
+    if ((((uintptr_t)p | (uintptr_t)boundary_all) & 15) != 0) { set_error("poisson_solve_finish: buffers must be 16-byte aligned"); return PZ_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if ((rc = launch_slab_finish(pl, p, boundary_all, st)) != PZ_OK) return rc;
+    if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 64) * sizeof(int), st));
+    return inverse_xy(pl, p, st);
 }
 
 int poisson_plan_destroy(pz_plan *pl)
@@ -282,6 +359,9 @@ int poisson_plan_destroy(pz_plan *pl)
     if (pl->d_zwork) cudaFree(pl->d_zwork);
     if (pl->d_host_stage) cudaFree(pl->d_host_stage);
     if (pl->d_xyctr) cudaFree(pl->d_xyctr);
+    if (pl->d_slab_kb) cudaFree(pl->d_slab_kb);
+    if (pl->slab_coef) cudaFree(pl->slab_coef);
+    if (pl->slab_phi) cudaFree(pl->slab_phi);
     for (int b = 0; b < 3; ++b)
         if (pl->d_batch_stage[b]) cudaFree(pl->d_batch_stage[b]);
     if (pl->h2d_stream) cudaStreamDestroy(pl->h2d_stream);
@@ -328,6 +408,7 @@ int pz_poisson_stage(pz_plan *pl, double *p, int stage, void *stream)
 int poisson_solve(pz_plan *pl, double *p, void *stream)
 {
     if (!pl || !p) { set_error("poisson_solve: NULL argument"); return PZ_EINVAL; }
+    if (pl->slab_G > 0) { set_error("poisson_solve: a slab plan solves through poisson_solve_reduce / poisson_solve_finish"); return PZ_EINVAL; }
     if (((uintptr_t)p & 15) != 0) { set_error("poisson_solve: p must be 16-byte aligned"); return PZ_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
@@ -411,6 +492,7 @@ int helmholtz3d_solve(pz_plan *pl, double *u, void *stream)
     if (!pl || !u) { set_error("helmholtz3d_solve: NULL argument"); return PZ_EINVAL; }
     if (((uintptr_t)u & 15) != 0) { set_error("helmholtz3d_solve: u must be 16-byte aligned"); return PZ_EINVAL; }
     if (pl->h3_a < 0.0) { set_error("helmholtz3d_solve: call helmholtz3d_setup first"); return PZ_ENOTSETUP; }
+    if (pl->slab_G > 0) { set_error("helmholtz3d_solve: not available on a z-slab plan"); return PZ_EUNSUPPORTED; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
     if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 64) * sizeof(int), st));
@@ -423,6 +505,7 @@ int helmholtz_z_setup(pz_plan *pl, double a)
 {
     if (!pl) { set_error("helmholtz_z_setup: plan is NULL"); return PZ_EINVAL; }
     if (!(a >= 0.0) || !std::isfinite(a)) { set_error("helmholtz_z_setup: a must be finite and >= 0"); return PZ_EINVAL; }
+    if (pl->slab_G > 0) { set_error("helmholtz_z_setup: not available on a z-slab plan (columns are cut; shard Helmholtz solves in y)"); return PZ_EUNSUPPORTED; }
     return helmholtz_build_tables(pl, a);
 }
 

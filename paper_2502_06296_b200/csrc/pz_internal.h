@@ -94,6 +94,15 @@ struct pz_plan {
     double *helm_host = nullptr;     // pinned staging for uploads, 2 halves
     size_t helm_host_bytes = 0;
 
+    // z-slab of a distributed Poisson solve (poisson_slab_plan_create): nz above is the slab's own
+    // number of planes; the z tables (d_A, d_C, d_dzf, d_zc) cover the global grid
+    int slab_G = 0, slab_g = 0, nz_glob = 0;
+    std::vector<int> slab_kb;        // G + 1 plane bounds
+    int *d_slab_kb = nullptr;
+    double *slab_coef = nullptr;     // [G][6][nx ny] interface coefficients of every slab
+    double *slab_phi = nullptr;      // [2][nx ny] phi_prev, phi_next of this rank's slab
+    size_t slab_bstride = 0;         // doubles per rank in the gathered boundary buffer
+
     pz::Options opt;
 
     // optional per-launch event timing (pz_profile_enable)
@@ -139,6 +148,9 @@ int launch_helmholtz_z_rhs(pz_plan *pl, double *u2, const double *uk, double a, 
 int launch_project(pz_plan *pl, double *u, double *v, double *w, double *p, const double *phi, double gdt, cudaStream_t st);
 int launch_fft_xy_fwd(pz_plan *pl, double *p, cudaStream_t st);
 int launch_fft_xy_inv(pz_plan *pl, double *p, cudaStream_t st);
+int launch_slab_coefficients(pz_plan *pl, cudaStream_t st);
+int launch_slab_reduce(pz_plan *pl, const double *p, double *bout, cudaStream_t st);
+int launch_slab_finish(pz_plan *pl, double *p, const double *ball, cudaStream_t st);
 int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st);
 int launch_helmholtz_tma(pz_plan *pl, double *const *u, int n, const double *tab, cudaStream_t st);
 int helmholtz_tma_prepare(pz_plan *pl);

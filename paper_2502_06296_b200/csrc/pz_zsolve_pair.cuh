@@ -41,18 +41,24 @@ __device__ __forceinline__ double shfl_down(double v, int d) { return __shfl_dow
 // HELM: the fully implicit Helmholtz system of Eq. (8), in the same M-matrix form:
 //   -a A_k x_{k-1} + (a A_k + a C_k + ex0_k + a sigma) x_k - a C_k x_{k+1} = +d_k,
 // al/ga hold a A_k / a C_k, ex0_k = 1 + a W_k (Dirichlet wall term), sigma is passed pre-scaled.
-template <int M, int MASK, bool pin, bool FULL = false, bool HELM = false, class Acc>
+// OPEN: the rows of ONE z-slab of a distributed solve once the neighbouring
+//   slabs' boundary values are known: the couplings of the first and last row to the rows outside
+//   are on the right-hand side (bprev = A_first phi_prev, bnext = C_last phi_next, added to rows
+//   0 and nz-1 of the slab), al / ga hold 0 there and ex0_k the diagonal excess they leave behind.
+template <int M, int MASK, bool pin, bool FULL = false, bool HELM = false, bool OPEN = false, class Acc>
 __device__ __forceinline__ void solve_pair(const Acc d, const double *al, const double *ga, double sigma,
                                            int k0, int nz, const double *__restrict__ dzf, double inv_lz,
-                                           const double *ex0 = nullptr)
+                                           const double *ex0 = nullptr, double2 bprev = make_double2(0.0, 0.0),
+                                           double2 bnext = make_double2(0.0, 0.0))
 {
     static_assert(!(HELM && (pin || FULL)), "the Helmholtz system has no pinned column and takes the general path");
+    static_assert(!(OPEN && (pin || FULL || HELM)), "a slab takes the general path");
     // row coefficients: real rows have excess sigma, padding rows (k >= nz) are x = 0,
     // the pinned row (gauge of the singular column) likewise.
     static_assert(!(FULL && pin), "the pinned column takes the general path");
     auto eps_of = [&](int i) {
         if constexpr (FULL) return sigma;
-        else if constexpr (HELM) return (k0 + i < nz) ? ex0[i] + sigma : 1.0;
+        else if constexpr (HELM || OPEN) return (k0 + i < nz) ? ex0[i] + sigma : 1.0;
         else return (k0 + i < nz && !(pin && k0 + i == nz - 1)) ? sigma : 1.0;
     };
     auto alpha_of = [&](int i) { return (pin && k0 + i == nz - 1) ? 0.0 : al[i]; };
@@ -62,8 +68,16 @@ __device__ __forceinline__ void solve_pair(const Acc d, const double *al, const 
             return make_double2(-v.x, -v.y);
         } else {
             const bool live = (k0 + i < nz) && !(pin && k0 + i == nz - 1);
-            if constexpr (HELM) return live ? v : make_double2(0.0, 0.0);
-            else return live ? make_double2(-v.x, -v.y) : make_double2(0.0, 0.0);
+            if constexpr (HELM) {
+                return live ? v : make_double2(0.0, 0.0);
+            } else if constexpr (OPEN) {
+                double2 r = live ? make_double2(-v.x, -v.y) : make_double2(0.0, 0.0);
+                if (k0 + i == 0) { r.x += bprev.x; r.y += bprev.y; }
+                if (k0 + i == nz - 1) { r.x += bnext.x; r.y += bnext.y; }
+                return r;
+            } else {
+                return live ? make_double2(-v.x, -v.y) : make_double2(0.0, 0.0);
+            }
         }
     };
 
