@@ -1,15 +1,17 @@
-"""One process per GPU: how the hot path shards, and the rank plumbing bench.py uses.
+"""One process per GPU: how the hot path shards, and the rank plumbing bench.py and sharded.py use.
 
-The path shards without any data-path collective:
+
 
 * Helmholtz: every (i, j) column is an independent tridiagonal system (Eq. 11),
   so a field splits into y-slabs ``[:, j0:j1, :]``, one per rank, each solved by an ordinary plan
-  with ``ny = j1 - j0``.
-* Poisson on one GPU per problem: independent fields (time steps of independent simulations,
-  ensemble members) are dealt round-robin to the ranks.
+  with ``ny = j1 - j0``; no collective.
+* ONE Poisson problem: z-slabs ``[k0:k1, :, :]`` and the paper's parallel tridiagonal solver
+  (PAPER.md:120-135): one all-gather of 2 nx ny boundary values per rank and solve
+  (:func:`gather_boundaries`).
+* Independent Poisson problems (replicas): dealt round-robin, no collective.
 
-Only timing (max over ranks) and bookkeeping use ``torch.distributed``; this module holds no
-arithmetic of the method and works with the ``gloo`` backend on CPU (tests) and ``nccl`` on GPUs.
+This module holds no arithmetic of the method and works with the ``gloo`` backend on CPU (tests)
+and ``nccl`` on GPUs.
 """
 from __future__ import annotations
 
@@ -35,6 +37,39 @@ def y_slab(ny: int, rank: int, world: int, align: int = 1) -> Tuple[int, int]:
     j0 = rank * base + min(rank, extra)
     j1 = j0 + base + (1 if rank < extra else 0)
     return j0 * align, j1 * align
+
+
+def y_slab_pow2(ny: int, rank: int, world: int) -> Tuple[int, int]:
+    """y-slab of a Helmholtz field for a plan: the plan's transforms want ny' a multiple of 8, and
+    equal slabs keep every rank's work the same; needs world | ny and ny / world >= 8."""
+    if world < 1 or ny % world or (ny // world) % 8:
+        raise ValueError(f"ny = {ny} does not split into {world} y-slabs of a multiple of 8 rows")
+    return y_slab(ny, rank, world, align=ny // world)
+
+
+def z_slab_bounds(nz: int, world: int) -> List[int]:
+    """Plane bounds kb[0..world] of the z-slabs of one Poisson problem: contiguous, sizes differing
+    by at most one, at least 3 planes each (Algorithms 1 and 2 need three rows per sub-domain,
+    PAPER.md:284, reading R9)."""
+    if world < 1 or nz < 3 * world:
+        raise ValueError(f"nz = {nz} cannot be cut into {world} slabs of at least 3 planes")
+    base, extra = divmod(nz, world)
+    kb = [0]
+    for g in range(world):
+        kb.append(kb[-1] + base + (1 if g < extra else 0))
+    return kb
+
+
+def gather_boundaries(ball, bout, dist=None) -> None:
+    """The ONE collective of a z-slab Poisson solve: every rank's boundary
+    buffer ``bout`` (stride doubles) lands at ``ball[rank * stride : (rank + 1) * stride]`` on every
+    rank.  Without a process group (single rank) it is a copy."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        ball[: bout.numel()].copy_(bout)
+        return
+    if ball.numel() != bout.numel() * dist.get_world_size():
+        raise ValueError("gather_boundaries: ball must hold world_size buffers of bout's size")
+    dist.all_gather_into_tensor(ball, bout)
 
 
 def deal_fields(n_fields: int, rank: int, world: int) -> List[int]:

@@ -79,3 +79,75 @@ def test_two_gloo_ranks_shard_helmholtz_by_y_slabs(tmp_path):
     ok, ms = np.load(tmp_path / "ok.npy")
     assert ok == 1.0
     assert ms == 10.0 + world - 1
+
+
+def test_z_slab_bounds_and_pow2_y_slabs():
+    for nz, world in ((12, 4), (512, 8), (100, 3), (1594, 4), (30, 1)):
+        kb = ranks.z_slab_bounds(nz, world)
+        sizes = np.diff(kb)
+        assert kb[0] == 0 and kb[-1] == nz and len(kb) == world + 1
+        assert sizes.min() >= 3 and sizes.max() - sizes.min() <= 1
+    with pytest.raises(ValueError):
+        ranks.z_slab_bounds(8, 3)
+    assert [ranks.y_slab_pow2(64, r, 4) for r in range(4)] == [(0, 16), (16, 32), (32, 48), (48, 64)]
+    with pytest.raises(ValueError):
+        ranks.y_slab_pow2(64, 0, 16)    # 4 rows per rank: below a plan's minimum
+    with pytest.raises(ValueError):
+        ranks.y_slab_pow2(64, 0, 3)
+
+
+def _ptdma_worker(rank, world, port, out_dir):
+    """The z-slab plumbing of sharded.SlabPoisson on CPU: every rank reduces ITS rows of a batch of
+    tridiagonal systems with the oracle's Algorithm 1, the boundary rows go through
+    ranks.gather_boundaries (the product's ONE collective), every rank solves the reduced systems
+    of size 2 world redundantly and reconstructs its rows."""
+    import torch
+    import torch.distributed as dist
+
+    from oracle import algorithms as alg
+
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        nz, ncol = 23, 5
+        rng = np.random.default_rng(3)                      # same systems on every rank
+        lo, up = -rng.uniform(0.5, 1.5, (ncol, nz)), -rng.uniform(0.5, 1.5, (ncol, nz))
+        di = np.abs(lo) + np.abs(up) + rng.uniform(0.01, 0.5, (ncol, nz))
+        lo[:, 0] = 0.0
+        up[:, -1] = 0.0
+        d = rng.standard_normal((ncol, nz))
+        kb = ranks.z_slab_bounds(nz, world)
+        k0, k1 = kb[rank], kb[rank + 1]
+        state, bout = [], torch.zeros(6 * ncol, dtype=torch.float64)
+        for q in range(ncol):
+            a, c, dd = alg.algorithm1_reduce(lo[q, k0:k1], di[q, k0:k1], up[q, k0:k1], d[q, k0:k1])
+            state.append((a, c, dd))
+            bout[6 * q:6 * q + 6] = torch.tensor([a[0], c[0], dd[0], a[-1], c[-1], dd[-1]])
+        ball = torch.zeros(6 * ncol * world, dtype=torch.float64)
+        ranks.gather_boundaries(ball, bout, dist)
+        rows = ball.numpy().reshape(world, ncol, 6)
+        mine = np.empty((ncol, k1 - k0))
+        for q in range(ncol):
+            red = [((rows[g, q, 0], 1.0, rows[g, q, 1], rows[g, q, 2]), (rows[g, q, 3], 1.0, rows[g, q, 4], rows[g, q, 5]))
+                   for g in range(world)]
+            xb = alg._dense_tridiag_solve(*alg.reduced_system(red))
+            a, c, dd = state[q]
+            mine[q] = alg.algorithm1_reconstruct(a, c, dd, xb[2 * rank], xb[2 * rank + 1])
+        parts = [None] * world
+        dist.all_gather_object(parts, (k0, k1, mine))
+        if rank == 0:
+            full = np.empty((ncol, nz))
+            for b0, b1, part in parts:
+                full[:, b0:b1] = part
+            ref = np.stack([alg._dense_tridiag_solve(lo[q], di[q], up[q], d[q]) for q in range(ncol)])
+            np.save(os.path.join(out_dir, "err.npy"), np.array([np.abs(full - ref).max() / np.abs(ref).max()]))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_gloo_ranks_solve_z_slabs_through_gather_boundaries(tmp_path, world):
+    import torch.multiprocessing as mp
+
+    mp.spawn(_ptdma_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    assert np.load(tmp_path / "err.npy")[0] <= 1e-13
