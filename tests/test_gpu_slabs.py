@@ -123,7 +123,7 @@ def test_slab_driver_single_rank_and_error_paths(env):
     with pytest.raises(RuntimeError):
         pz.poisson_slab_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf, 2, 0, [0, 20, 39])  # not to nz
     plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
-    with pytest.raises(RuntimeError):
+    with pytest.raises((RuntimeError, ValueError)):
         pz.poisson_solve_reduce(plan, p, p)          # not a slab plan
     pz.poisson_plan_destroy(plan)
 
