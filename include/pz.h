@@ -44,7 +44,7 @@ typedef struct pz_plan pz_plan; /* opaque */
 enum pz_status {
     PZ_OK = 0,
     PZ_EINVAL = 1,       /* null pointer, non-positive size, non-monotone grid, a < 0, ... */
-    PZ_EUNSUPPORTED = 2, /* nx or ny not a power of two in [8, 4096], nz < 4, unknown bc/option */
+    PZ_EUNSUPPORTED = 2, /* nx or ny outside the supported lengths, nz < 4, unknown bc/option */
     PZ_ENOMEM = 3,       /* host or device allocation failed */
     PZ_ECUDA = 4,        /* CUDA runtime error (message in pz_last_error) */
     PZ_ENOTSETUP = 5     /* helmholtz_z_solve before helmholtz_z_setup */
@@ -117,8 +117,12 @@ PZ_API int poisson_solve_finish(pz_plan *plan, double *p, const double *boundary
  * helmholtz_z_setup: pre-processing for (I - a L_z), a = gamma_k nu dt / 2 >= 0.  Computes the
  * k-only coefficient sub-arrays of Algorithm 2 Step 1 for every sub-domain, and the per-level
  * multipliers of the cyclic reduction of the boundary system, on the host (O(nz) work), and
- * uploads them into the table set not used by solves still in flight.  May be called once
- * per Runge-Kutta sub-step ("time-dependent").
+ * uploads them into a table set that no solve still in flight and no captured CUDA graph reads.
+ * May be called once per Runge-Kutta sub-step ("time-dependent").
+ * CUDA graphs: a helmholtz_z_solve / _solve_n / helmholtz_z_step captured into a graph keeps the
+ * table set (and so the coefficient a) that was current at capture time; that set stays untouched
+ * until poisson_plan_destroy, so replays remain valid across any number of later set-ups or
+ * geometry options, and solve with the captured a.  Capture after the set-up for that a.
  *
  * helmholtz_z_solve: runtime.  For every (i,j) column solves
  *   u_k - a [A_k (u_{k-1}-u_k) + C_k (u_{k+1}-u_k) - W_k u_k] = r_k,

@@ -1,6 +1,6 @@
 """Build libpz_b200.so (hand-written CUDA for sm_100a + the C ABI of include/pz.h) in-tree.
 
-    python -m paper_2502_06296_b200.build [--force] [--verbose]
+    python -m paper_2502_06296_b200.build [--force] [--verbose] [--probes]
 
 nvcc cross-compiles without a GPU.  Objects go to csrc/build/, the library next to this file.
 """
@@ -32,15 +32,17 @@ def _newest_header() -> float:
     return max(os.path.getmtime(os.path.join(CSRC, h)) for h in HEADERS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, probes: bool = False) -> str:
+    """probes: compile the timing-only diagnostics (-DPZ_PROBES; wrong results) in; forces a rebuild."""
     os.makedirs(OBJ, exist_ok=True)
+    force = force or probes
     hdr = _newest_header()
     jobs = []
     for src in SOURCES:
         s = os.path.join(CSRC, src)
         o = os.path.join(OBJ, src.replace(".cu", ".o"))
         if force or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), hdr):
-            cmd = [_nvcc(), *NVCC_FLAGS, "-c", s, "-o", o]
+            cmd = [_nvcc(), *NVCC_FLAGS, *(["-DPZ_PROBES"] if probes else []), "-c", s, "-o", o]
             if verbose:
                 cmd.insert(1, "-Xptxas=-v")
             jobs.append(cmd)
@@ -68,4 +70,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, probes="--probes" in sys.argv))

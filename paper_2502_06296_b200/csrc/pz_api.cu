@@ -30,6 +30,15 @@ int cuda_fail(cudaError_t e, const char *what)
 
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+int ensure_smem_optin(pz_plan *pl, const void *kernel, int bytes)
+{
+    for (const void *k : pl->smem_optin)
+        if (k == kernel) return PZ_OK;
+    PZ_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    pl->smem_optin.push_back(kernel);
+    return PZ_OK;
+}
+
 static cudaEvent_t prof_event(pz_plan *pl)
 {
     cudaEvent_t e = nullptr;
@@ -263,10 +272,6 @@ static int plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double 
 
     ce = cudaStreamCreateWithFlags(&pl->upload_stream, cudaStreamNonBlocking);
     if (ce != cudaSuccess) return fail(cuda_fail(ce, "cudaStreamCreate"));
-    for (int b = 0; b < 2; ++b) {
-        if ((ce = cudaEventCreateWithFlags(&pl->helm[b].uploaded, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
-        if ((ce = cudaEventCreateWithFlags(&pl->helm[b].last_use, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(ce, "cudaEventCreate"));
-    }
     ce = cudaMalloc(&pl->d_xyctr, 2 * (size_t)(nk + 64) * sizeof(int));
     if (ce != cudaSuccess) { cudaGetLastError(); set_error("plan counters: %s", cudaGetErrorString(ce)); return fail(PZ_ENOMEM); }
     // measured at 512 x 512 x nz: variant 2 wins from nz = 256 up to 1024, variant 1 below
@@ -367,12 +372,12 @@ int poisson_plan_destroy(pz_plan *pl)
     if (pl->h2d_stream) cudaStreamDestroy(pl->h2d_stream);
     if (pl->d2h_stream) cudaStreamDestroy(pl->d2h_stream);
     for (auto e : pl->batch_events) cudaEventDestroy(e);
-    for (int b = 0; b < 2; ++b) {
-        if (pl->helm[b].dev) cudaFree(pl->helm[b].dev);
-        if (pl->helm[b].uploaded) cudaEventDestroy(pl->helm[b].uploaded);
-        if (pl->helm[b].last_use) cudaEventDestroy(pl->helm[b].last_use);
+    for (auto &t : pl->helm) {
+        if (t.dev) cudaFree(t.dev);
+        if (t.host) cudaFreeHost(t.host);
+        if (t.uploaded) cudaEventDestroy(t.uploaded);
+        if (t.last_use) cudaEventDestroy(t.last_use);
     }
-    if (pl->helm_host) cudaFreeHost(pl->helm_host);
     if (pl->upload_stream) cudaStreamDestroy(pl->upload_stream);
     for (auto &r : pl->prof_recs) { cudaEventDestroy(r.start); cudaEventDestroy(r.stop); }
     for (auto e : pl->prof_pool) cudaEventDestroy(e);
@@ -637,7 +642,7 @@ static int *option_slot(pz_plan *pl, const char *key)
 {
     if (!std::strcmp(key, "zsolve_variant")) return &pl->opt.zsolve_variant;
     if (!std::strcmp(key, "zsolve_stages")) return &pl->opt.zsolve_stages;
-    if (!std::strcmp(key, "zsolve_probe")) return &pl->opt.zsolve_probe;
+    if (kProbes && !std::strcmp(key, "zsolve_probe")) return &pl->opt.zsolve_probe;
     if (!std::strcmp(key, "slab_planes")) return &pl->opt.slab_planes;
     if (!std::strcmp(key, "fft_fused")) return &pl->opt.fft_fused;
     if (!std::strcmp(key, "xy_lag")) return &pl->opt.xy_lag;
@@ -646,7 +651,7 @@ static int *option_slot(pz_plan *pl, const char *key)
     if (!std::strcmp(key, "xy_xshare")) return &pl->opt.xy_xshare;
     if (!std::strcmp(key, "xy_group")) return &pl->opt.xy_group;
     if (!std::strcmp(key, "helm_variant")) return &pl->opt.helm_variant;
-    if (!std::strcmp(key, "helm_probe")) return &pl->opt.helm_probe;
+    if (kProbes && !std::strcmp(key, "helm_probe")) return &pl->opt.helm_probe;
     if (!std::strcmp(key, "helm_cluster")) return &pl->opt.helm_cluster;
     if (!std::strcmp(key, "helm_box_rows")) return &pl->opt.helm_box_rows;
     if (!std::strcmp(key, "helm_l2promo")) return &pl->opt.helm_l2promo;

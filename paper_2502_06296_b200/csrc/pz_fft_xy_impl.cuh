@@ -543,7 +543,7 @@ int launch_xy(pz_plan *pl, double *p, cudaStream_t st)
     auto kern = fft_xy_kernel<MX, LY, INV>;
     int &bps = pl->xy_bps[INV ? 1 : 0];
     if (bps == 0) {
-        PZ_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
+        { const int rc = smem_optin(pl, kern, G::SMEM); if (rc != PZ_OK) return rc; }
         PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, kThreads, G::SMEM));
         if (bps < 1) { bps = 0; set_error("fft_xy: kernel does not fit an SM"); return PZ_ECUDA; }
     }

@@ -157,11 +157,10 @@ int launch_ltc(const pz_plan *pl, double *p, int nk, cudaStream_t st)
     constexpr int threads = P::T * TC;
     // exchange tile; at least one column pair for the pair-0 conversion of single-pass lengths
     constexpr size_t smem = (P::R2 > 1) ? (size_t)L * TC * sizeof(double2) : (size_t)L * sizeof(double2);
-    static bool attr_done = false;
-    if (smem > 48 * 1024 && !attr_done) {
-        PZ_CUDA(cudaFuncSetAttribute(fft_y_kernel<L, TC, INV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        PZ_CUDA(cudaFuncSetAttribute(fft_y_kernel<L, TC, INV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
+    if (smem > 48 * 1024) {
+        int rc;
+        if ((rc = smem_optin(pl, fft_y_kernel<L, TC, INV, true>, smem)) != PZ_OK) return rc;
+        if ((rc = smem_optin(pl, fft_y_kernel<L, TC, INV, false>, smem)) != PZ_OK) return rc;
     }
     dim3 grid((unsigned)(pl->nx / 2 / TC), (unsigned)nk);
     ProfScope prof(pl, INV ? PZ_K_FFT_Y_INV : PZ_K_FFT_Y_FWD, st);
@@ -236,11 +235,10 @@ int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cud
     double *base = p + (size_t)k0 * pl->nx * pl->ny;
     const size_t smem = (size_t)pl->ny * sizeof(double2);
     const int threads = pl->ny / 2 >= 256 ? 256 : (pl->ny / 2 < 32 ? 32 : pl->ny / 2);
-    static bool attr_done = false;
-    if (smem > 48 * 1024 && !attr_done) {
-        PZ_CUDA(cudaFuncSetAttribute(pair0_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
-        PZ_CUDA(cudaFuncSetAttribute(pair0_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
-        attr_done = true;
+    if (smem > 48 * 1024) {
+        int rc;
+        if ((rc = smem_optin(pl, pair0_kernel<false>, 64 * 1024)) != PZ_OK) return rc;
+        if ((rc = smem_optin(pl, pair0_kernel<true>, 64 * 1024)) != PZ_OK) return rc;
     }
     ProfScope prof(pl, inverse ? PZ_K_PAIR0_INV : PZ_K_PAIR0_FWD, st);
     if (inverse)

@@ -227,32 +227,42 @@ int helmholtz_build_tables(pz_plan *pl, double a)
         for (int r = 0; r < n2; ++r) rbr[r] = (double)((ld)1 / rbd[r]);
     }
 
-    // upload into the table set that no in-flight solve reads (double buffering)
-    const int nb = (pl->helm_cur < 0) ? 0 : 1 - pl->helm_cur;
+    // upload into a table set that no in-flight solve reads and no captured graph refers to (a
+    // captured helmholtz_z_solve keeps the address of the set that was current at capture time: such
+    // a set is never rewritten or freed before the plan is destroyed, so replays stay valid -- and
+    // keep solving with the coefficient of capture time -- across any number of later set-ups)
+    int nb = -1;
+    for (int i = 0; i < (int)pl->helm.size(); ++i)
+        if (i != pl->helm_cur && !pl->helm[i].captured) { nb = i; break; }
+    if (nb < 0) {
+        HelmTables fresh;
+        PZ_CUDA(cudaEventCreateWithFlags(&fresh.uploaded, cudaEventDisableTiming));
+        PZ_CUDA(cudaEventCreateWithFlags(&fresh.last_use, cudaEventDisableTiming));
+        pl->helm.push_back(fresh);
+        nb = (int)pl->helm.size() - 1;
+    }
     HelmTables &t = pl->helm[nb];
+    if (t.used) PZ_CUDA(cudaEventSynchronize(t.uploaded)); // this set's previous upload has left its staging buffer
     if (t.bytes < bytes) {
+        if (t.used) PZ_CUDA(cudaEventSynchronize(t.last_use));
         if (t.dev) PZ_CUDA(cudaFree(t.dev));
         t.dev = nullptr;
         cudaError_t e = cudaMalloc(&t.dev, bytes);
-        if (e != cudaSuccess) { set_error("helmholtz tables: %s", cudaGetErrorString(e)); return PZ_ENOMEM; }
+        if (e != cudaSuccess) { cudaGetLastError(); set_error("helmholtz tables: %s", cudaGetErrorString(e)); return PZ_ENOMEM; }
         t.bytes = bytes;
     }
-    if (pl->helm_host_bytes < 2 * bytes) {
-        PZ_CUDA(cudaStreamSynchronize(pl->upload_stream));
-        if (pl->helm_host) PZ_CUDA(cudaFreeHost(pl->helm_host));
-        pl->helm_host = nullptr;
-        cudaError_t e = cudaMallocHost(&pl->helm_host, 2 * bytes);
-        if (e != cudaSuccess) { set_error("helmholtz staging: %s", cudaGetErrorString(e)); return PZ_ENOMEM; }
-        pl->helm_host_bytes = 2 * bytes;
+    if (t.host_bytes < bytes) {
+        if (t.host) PZ_CUDA(cudaFreeHost(t.host));
+        t.host = nullptr;
+        cudaError_t e = cudaMallocHost(&t.host, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); set_error("helmholtz staging: %s", cudaGetErrorString(e)); return PZ_ENOMEM; }
+        t.host_bytes = bytes;
     }
     if (t.used) PZ_CUDA(cudaStreamWaitEvent(pl->upload_stream, t.last_use, 0)); // old readers done
-    // the staging half was last read by the upload two setups ago: that copy has completed
-    // because its event has been waited on by every later solve's stream; be safe and sync it
-    if (t.used) PZ_CUDA(cudaEventSynchronize(t.uploaded));
-    double *stage = pl->helm_host + (size_t)nb * (pl->helm_host_bytes / 2 / sizeof(double));
-    std::memcpy(stage, host.data(), bytes);
-    PZ_CUDA(cudaMemcpyAsync(t.dev, stage, bytes, cudaMemcpyHostToDevice, pl->upload_stream));
+    std::memcpy(t.host, host.data(), bytes);
+    PZ_CUDA(cudaMemcpyAsync(t.dev, t.host, bytes, cudaMemcpyHostToDevice, pl->upload_stream));
     PZ_CUDA(cudaEventRecord(t.uploaded, pl->upload_stream));
+    t.upload_seen = false;
     t.used = true;
     pl->helm_cur = nb;
     pl->helm_a = a;
@@ -261,14 +271,47 @@ int helmholtz_build_tables(pz_plan *pl, double a)
 
 // Eq. (11) in one kernel where the variant-1 pipeline can hold the tiles of u** and u^k;
 // PZ_EUNSUPPORTED otherwise (no launch made).
+// Orders a solve on `st` after the upload of table set t.  While `st` is being captured into a
+// graph the set is pinned for the plan's lifetime (see helmholtz_build_tables) and the upload,
+// a few kilobytes on another stream, is waited for on the host, so the graph needs no dependency
+// on it.
+static int order_after_upload(HelmTables &t, cudaStream_t st, bool *capturing)
+{
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    PZ_CUDA(cudaStreamIsCapturing(st, &cap));
+    *capturing = (cap != cudaStreamCaptureStatusNone);
+    if (*capturing) {
+        t.captured = true;
+        if (!t.upload_seen) {
+            // event calls on another stream are "potentially unsafe" under global capture mode:
+            // make this one in relaxed mode (the upload stream is not part of the capture)
+            cudaStreamCaptureMode mode = cudaStreamCaptureModeRelaxed;
+            PZ_CUDA(cudaThreadExchangeStreamCaptureMode(&mode));
+            const cudaError_t q = cudaEventSynchronize(t.uploaded);
+            cudaThreadExchangeStreamCaptureMode(&mode);
+            if (q != cudaSuccess) return cuda_fail(q, "helmholtz table upload");
+            t.upload_seen = true;
+        }
+    } else if (t.upload_seen) {
+        // nothing to order
+    } else if (cudaEventQuery(t.uploaded) == cudaSuccess) {
+        t.upload_seen = true;
+    } else {
+        cudaGetLastError();
+        PZ_CUDA(cudaStreamWaitEvent(st, t.uploaded, 0));
+    }
+    return PZ_OK;
+}
+
 int launch_helmholtz_step(pz_plan *pl, double *u2, const double *uk, cudaStream_t st)
 {
     if (pl->helm_variant != 1 || pl->opt.step_fused == 0) return PZ_EUNSUPPORTED;
     HelmTables &t = pl->helm[pl->helm_cur];
-    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-    PZ_CUDA(cudaStreamIsCapturing(st, &cap));
-    const bool capturing = (cap != cudaStreamCaptureStatusNone);
-    if (!capturing && cudaEventQuery(t.uploaded) != cudaSuccess) PZ_CUDA(cudaStreamWaitEvent(st, t.uploaded, 0));
+    bool capturing = false;
+    {
+        const int rc0 = order_after_upload(t, st, &capturing);
+        if (rc0 != PZ_OK) return rc0;
+    }
     int rc;
     {
         ProfScope prof(pl, PZ_K_HELMHOLTZ, st);
@@ -282,12 +325,11 @@ int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st)
 {
     if (n == 0) return PZ_OK;
     HelmTables &t = pl->helm[pl->helm_cur];
-    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-    PZ_CUDA(cudaStreamIsCapturing(st, &cap));
-    const bool capturing = (cap != cudaStreamCaptureStatusNone);
-    // order after the table upload unless it is known to have completed (always the case when
-    // capturing a graph after a warm-up solve)
-    if (!capturing && cudaEventQuery(t.uploaded) != cudaSuccess) PZ_CUDA(cudaStreamWaitEvent(st, t.uploaded, 0));
+    bool capturing = false;
+    {
+        const int rc0 = order_after_upload(t, st, &capturing);
+        if (rc0 != PZ_OK) return rc0;
+    }
     const size_t plane = (size_t)pl->nx * pl->ny;
     const int tx = pl->helm_tx, P = pl->helm_P;
     if (pl->helm_variant == 1) {

@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
     auto fetch = [&](int t) {
         const int f = t / tiles_per_field, tt = t - f * tiles_per_field, col0 = tt * kTX;
         mbar_arrive_expect_tx(bar, tile_bytes);
-        if (probe == 3) { // diagnostic: same bytes fetched as 32-column boxes (256-byte rows)
+        if (kProbes && probe == 3) { // diagnostic: same bytes fetched as 32-column boxes (256-byte rows)
             for (int b = 0; b < nbox; ++b)
                 tma_load_2d(tile + (size_t)b * box_rows * 32, &args.map[f], (tt >> 1) * 32, (tt & 1) * (nzp / 2) + b * box_rows, bar);
             return;
@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
         }
         if (tid == 0 && t + (int)gridDim.x < total_tiles) fetch(t + gridDim.x);
 
-        if (probe == 2) { // diagnostic: pipeline skeleton only (load, store)
+        if (kProbes && probe == 2) { // diagnostic: pipeline skeleton only (load, store)
             const int f = t / tiles_per_field;
             double *up = args.u[f] + (size_t)(t - f * tiles_per_field) * kTX + c2 + (size_t)k0 * plane;
 #pragma unroll
@@ -243,7 +243,7 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
         }
 
         // Step 4: reconstruct and store
-        if ((probe == 1 || probe == 3) && x0.x != 1.2345e300) continue; // diagnostic: no stores
+        if (kProbes && (probe == 1 || probe == 3) && x0.x != 1.2345e300) continue; // diagnostic: no stores
         const int f = t / tiles_per_field;
         double *up = args.u[f] + (size_t)(t - f * tiles_per_field) * kTX + c2 + (size_t)k0 * plane;
 #pragma unroll
@@ -274,11 +274,15 @@ int prepare_mf(pz_plan *pl)
     const size_t smem = Smem<M>::bytes(pl->helm_P, pl->helm_levels);
     auto kern = helmholtz_tma_kernel<M, FULL, 0>;
     if (smem > 227 * 1024) { set_error("helmholtz (TMA variant): tile of %zu bytes does not fit shared memory", smem); return PZ_EUNSUPPORTED; }
-    PZ_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    {
+        const int rc = smem_optin(pl, kern, 227 * 1024);
+        if (rc != PZ_OK) return rc;
+    }
     int bps = 0;
     PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, (kTX / 2) * pl->helm_P, smem));
     if (bps < 1) { set_error("helmholtz (TMA variant): kernel does not fit an SM"); return PZ_ECUDA; }
     pl->helm_bps = bps;
+    pl->helm_nclusters[0] = pl->helm_nclusters[1] = pl->helm_nclusters[2] = 0;
     return PZ_OK;
 }
 
@@ -297,8 +301,10 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
     if (wide) { box_rows = 256; nbox = P * M / 512; }
     HelmArgs args;
     for (int f = 0; f < n; ++f) {
-        const int rc = encode_column_tile_map(&args.map[f], u[f], plane, pl->nz, wide ? 32 : kTX, box_rows, pl->opt.helm_l2promo);
+        const CUtensorMap *mf = nullptr;
+        const int rc = cached_column_map(pl, &mf, u[f], plane, pl->nz, wide ? 32 : kTX, box_rows, pl->opt.helm_l2promo, false);
         if (rc != PZ_OK) return rc;
+        args.map[f] = *mf;
         args.u[f] = u[f];
     }
     for (int f = n; f < kMaxFields; ++f) { args.map[f] = args.map[0]; args.u[f] = u[0]; }
@@ -326,10 +332,15 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     if (csz > 1) {
-        cfg.gridDim = dim3((unsigned)(blocks / csz * csz));
-        int nclusters = 0;
-        PZ_CUDA(cudaOccupancyMaxActiveClusters(&nclusters, helmholtz_tma_kernel<M, FULL, 0>, &cfg));
-        if (nclusters < 1) { set_error("helmholtz (TMA variant): no cluster of %d CTAs fits", csz); return PZ_ECUDA; }
+        // resident clusters: queried once per geometry (helmholtz_tma_prepare resets it)
+        if (pl->helm_nclusters[csz == 2 ? 0 : csz == 4 ? 1 : 2] == 0) {
+            cfg.gridDim = dim3((unsigned)((long long)pl->num_sms * pl->helm_bps / csz * csz));
+            int nclusters = 0;
+            PZ_CUDA(cudaOccupancyMaxActiveClusters(&nclusters, helmholtz_tma_kernel<M, FULL, 0>, &cfg));
+            if (nclusters < 1) { set_error("helmholtz (TMA variant): no cluster of %d CTAs fits", csz); return PZ_ECUDA; }
+            pl->helm_nclusters[csz == 2 ? 0 : csz == 4 ? 1 : 2] = nclusters;
+        }
+        const int nclusters = pl->helm_nclusters[csz == 2 ? 0 : csz == 4 ? 1 : 2];
         if ((long long)nclusters * csz < blocks) blocks = (long long)nclusters * csz;
     }
     blocks = blocks / csz * csz;
@@ -350,16 +361,15 @@ int launch_cn_mfc(pz_plan *pl, double *u2, const double *uk, const double *tab, 
     const size_t plane = (size_t)pl->nx * pl->ny;
     const size_t smem = Smem<M>::bytes(P, pl->helm_levels, CN == 1);
     auto kern = helmholtz_tma_kernel<M, FULL, CN>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        PZ_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        attr_done = true;
-    }
+    int rc = smem_optin(pl, kern, 227 * 1024);
+    if (rc != PZ_OK) return rc;
     const int box_rows = Smem<M>::box_rows(P), nbox = Smem<M>::nbox(P);
     HelmArgs args;
-    int rc = encode_column_tile_map(&args.map[0], u2, plane, pl->nz, kTX, box_rows, pl->opt.helm_l2promo);
-    if (rc != PZ_OK) return rc;
-    if ((rc = encode_column_tile_map(&args.qmap, uk, plane, pl->nz, kTX, box_rows, pl->opt.helm_l2promo)) != PZ_OK) return rc;
+    const CUtensorMap *m0 = nullptr, *m1 = nullptr;
+    if ((rc = cached_column_map(pl, &m0, u2, plane, pl->nz, kTX, box_rows, pl->opt.helm_l2promo, false)) != PZ_OK) return rc;
+    args.map[0] = *m0;
+    if ((rc = cached_column_map(pl, &m1, uk, plane, pl->nz, kTX, box_rows, pl->opt.helm_l2promo, false)) != PZ_OK) return rc;
+    args.qmap = *m1;
     for (int f = 0; f < kMaxFields; ++f) { args.map[f] = args.map[0]; args.u[f] = u2; }
     args.q = uk;
     args.A = pl->d_A; args.C = pl->d_C; args.a = pl->helm_a; args.w0 = pl->wall_w0; args.w1 = pl->wall_w1;

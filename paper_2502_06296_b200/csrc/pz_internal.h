@@ -1,6 +1,7 @@
 // pz_internal.h -- plan object and launch declarations shared by the translation units of
 // libpz_b200.so.  Not installed; the public boundary is include/pz.h.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cstddef>
 #include <cstdint>
@@ -18,7 +19,11 @@ struct HelmTables {
     size_t bytes = 0;
     cudaEvent_t uploaded = nullptr;   // recorded on the upload stream after the H2D copy
     cudaEvent_t last_use = nullptr;   // recorded on the caller's stream after each solve
+    double *host = nullptr;           // pinned staging of this set's upload
+    size_t host_bytes = 0;
     bool used = false;
+    bool upload_seen = false;         // host has observed the upload's completion: solves need no ordering
+    bool captured = false;            // a CUDA graph holds this set's address: never rewritten or freed before destroy
 };
 
 struct Options {
@@ -88,11 +93,10 @@ struct pz_plan {
     int helm_m = 0, helm_P = 0, helm_tx = 0, helm_levels = 0;
     int helm_variant = 0;            // variant the current tables were built for
     int helm_bps = 0;                // variant 1: resident CTAs per SM
-    pz::HelmTables helm[2];
+    int helm_nclusters[3] = {0, 0, 0}; // variant 1: resident clusters of 2 / 4 / 8 CTAs (0 = not yet queried)
+    std::vector<pz::HelmTables> helm; // table sets: the current one, one being uploaded, and any a captured graph reads
     int helm_cur = -1;
     cudaStream_t upload_stream = nullptr;
-    double *helm_host = nullptr;     // pinned staging for uploads, 2 halves
-    size_t helm_host_bytes = 0;
 
     // z-slab of a distributed Poisson solve (poisson_slab_plan_create): nz above is the slab's own
     // number of planes; the z tables (d_A, d_C, d_dzf, d_zc) cover the global grid
@@ -102,6 +106,20 @@ struct pz_plan {
     double *slab_coef = nullptr;     // [G][6][nx ny] interface coefficients of every slab
     double *slab_phi = nullptr;      // [2][nx ny] phi_prev, phi_next of this rank's slab
     size_t slab_bstride = 0;         // doubles per rank in the gathered boundary buffer
+
+    // z-solve variant 2: launch geometry per (sub-domain rows M, HELM), queried once per plan (= per device)
+    struct ZtGeo { int blocks = 0, stages = 0; };
+    ZtGeo zt[4][2];
+
+    // tensor maps of the column-tile kernels, keyed by (field pointer, geometry): a solve that sees the
+    // same field again encodes nothing
+    struct MapEntry { const void *ptr; size_t ncols; int nz, tx, box_rows, l2promo, swz; CUtensorMap map; };
+    std::vector<MapEntry> maps;
+    size_t maps_next = 0;
+
+    // kernels whose dynamic shared-memory limit has been raised on THIS plan's device (function
+    // attributes are per device: no process-wide statics)
+    std::vector<const void *> smem_optin;
 
     pz::Options opt;
 
@@ -113,6 +131,14 @@ struct pz_plan {
 };
 
 namespace pz {
+
+// Timing-only diagnostics that skip arithmetic or stores (results are WRONG): compiled in only with
+// -DPZ_PROBES (python -m paper_2502_06296_b200.build --probes); the shipped library has none.
+#ifdef PZ_PROBES
+constexpr bool kProbes = true;
+#else
+constexpr bool kProbes = false;
+#endif
 
 void set_error(const char *fmt, ...);
 int cuda_fail(cudaError_t e, const char *what);
@@ -157,5 +183,14 @@ int helmholtz_tma_prepare(pz_plan *pl);
 int launch_helmholtz_tma_cn(pz_plan *pl, double *u2, const double *uk, const double *tab, cudaStream_t st);
 int launch_helmholtz_step(pz_plan *pl, double *u2, const double *uk, cudaStream_t st);
 int helmholtz_build_tables(pz_plan *pl, double a);
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (plan, kernel)
+int ensure_smem_optin(pz_plan *pl, const void *kernel, int bytes);
+template <class K> int smem_optin(const pz_plan *pl, K kernel, size_t bytes)
+{
+    return ensure_smem_optin(const_cast<pz_plan *>(pl), reinterpret_cast<const void *>(kernel), (int)bytes);
+}
+// encode_column_tile_map (pz_tma.cuh) through the plan's small cache (at most 16 maps, round robin)
+int cached_column_map(pz_plan *pl, const CUtensorMap **out, const double *field, size_t ncols, int nz, int tx, int box_rows,
+                      int l2promo, bool swizzle128);
 
 } // namespace pz

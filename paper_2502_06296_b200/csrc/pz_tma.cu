@@ -55,4 +55,30 @@ int encode_column_tile_map(CUtensorMap *map, const double *field, size_t ncols, 
     return PZ_OK;
 }
 
+int cached_column_map(pz_plan *pl, const CUtensorMap **out, const double *field, size_t ncols, int nz, int tx, int box_rows,
+                      int l2promo, bool swizzle128)
+{
+    const int swz = swizzle128 ? 1 : 0;
+    for (auto &e : pl->maps)
+        if (e.ptr == field && e.ncols == ncols && e.nz == nz && e.tx == tx && e.box_rows == box_rows && e.l2promo == l2promo &&
+            e.swz == swz) {
+            *out = &e.map;
+            return PZ_OK;
+        }
+    pz_plan::MapEntry e;
+    e.ptr = field; e.ncols = ncols; e.nz = nz; e.tx = tx; e.box_rows = box_rows; e.l2promo = l2promo; e.swz = swz;
+    const int rc = encode_column_tile_map(&e.map, field, ncols, nz, tx, box_rows, l2promo, swizzle128);
+    if (rc != PZ_OK) return rc;
+    if (pl->maps.size() < 16) {
+        pl->maps.reserve(16);   // entries never move: callers keep the pointer until their launch returns
+        pl->maps.push_back(e);
+        *out = &pl->maps.back().map;
+    } else {
+        pl->maps[pl->maps_next % 16] = e;
+        *out = &pl->maps[pl->maps_next % 16].map;
+        ++pl->maps_next;
+    }
+    return PZ_OK;
+}
+
 } // namespace pz

@@ -437,7 +437,7 @@ int launch_slab_reduce(pz_plan *pl, const double *p, double *bout, cudaStream_t 
     const int kb = pl->slab_kb[pl->slab_g], nk = pl->nz;
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
     PZ_SLAB_DISPATCH(nk, {
-        PZ_CUDA(cudaFuncSetAttribute(slab_reduce_kernel<MM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)slab_smem<MM>()));
+        { const int rc = smem_optin(pl, slab_reduce_kernel<MM>, slab_smem<MM>()); if (rc != PZ_OK) return rc; }
         slab_reduce_kernel<MM><<<blocks, kPairs * kLanes, slab_smem<MM>(), st>>>(p, bout, pl->d_A, pl->d_C, pl->d_lamx, pl->d_lamy_nat,
                                                                                  pl->d_lamy_pk, pl->nx, plane, kb, nk);
     });
@@ -457,7 +457,7 @@ int launch_slab_finish(pz_plan *pl, double *p, const double *ball, cudaStream_t 
     count_launch();
     PZ_CUDA(cudaGetLastError());
     PZ_SLAB_DISPATCH(nk, {
-        PZ_CUDA(cudaFuncSetAttribute(slab_finish_kernel<MM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)slab_smem<MM>()));
+        { const int rc = smem_optin(pl, slab_finish_kernel<MM>, slab_smem<MM>()); if (rc != PZ_OK) return rc; }
         slab_finish_kernel<MM><<<blocks, kPairs * kLanes, slab_smem<MM>(), st>>>(p, pl->slab_phi, pl->slab_phi + plane, pl->d_A, pl->d_C,
                                                                                  pl->d_lamx, pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, plane, kb, nk);
     });

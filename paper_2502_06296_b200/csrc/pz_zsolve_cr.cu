@@ -106,10 +106,9 @@ template <int M, bool HELM>
 int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha)
 {
     constexpr size_t smem = ((size_t)kLanes * (M * kTX + 2) + 3 * (size_t)kLanes * (M + 1)) * sizeof(double);
-    static bool attr_done = false;
-    if (smem > 48 * 1024 && !attr_done) {
-        PZ_CUDA(cudaFuncSetAttribute(zsolve_cr_kernel<M, HELM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
+    if (smem > 48 * 1024) {
+        const int rc = smem_optin(pl, zsolve_cr_kernel<M, HELM>, smem);
+        if (rc != PZ_OK) return rc;
     }
     const size_t plane = (size_t)pl->nx * pl->ny;
     const unsigned blocks = (unsigned)(plane / kTX);

@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(kThreads, 1)
         const double sig0 = -(lamx[i] + ly), sig1 = -(lamx[i + 1] + ly);
         d.slot = base + b * G::STAGE + (size_t)R0 * 128;
         mbar_wait(&full[b], (it / stages) & 1);
-        if (probe == 2) {
+        if (kProbes && probe == 2) {
             // diagnostic: pipeline skeleton only (TMA load, TMA store), no arithmetic
         } else if constexpr (HELM) {
             const double *e0 = s_e0 + lane * G::CS;
@@ -171,21 +171,25 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha)
     if (pl->opt.zsolve_stages > 0 && pl->opt.zsolve_stages < stages) stages = pl->opt.zsolve_stages;
     if (stages < 1) { set_error("z-solve variant 2: nz = %d does not fit shared memory", pl->nz); return PZ_EUNSUPPORTED; }
     const size_t smem = G::bytes(stages);
-    static bool attr_done = false;
-    if (!attr_done) {
-        PZ_CUDA(cudaFuncSetAttribute(zsolve_tma_kernel<M, HELM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        attr_done = true;
-    }
     const size_t plane = (size_t)pl->nx * pl->ny;
-    CUtensorMap map;
-    const int rc = encode_column_tile_map(&map, p, plane, pl->nz, kTX, M, 1, /*swizzle128=*/true);
-    if (rc != PZ_OK) return rc;
     const int ntiles = (int)(plane / kTX);
-    int occ = 1;
-    if (smem * 2 <= 227 * 1024) PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, zsolve_tma_kernel<M, HELM>, kThreads, smem));
-    if (occ < 1) occ = 1;
-    int blocks = pl->num_sms * occ;
+    // per plan (= per device): shared-memory opt-in and resident CTAs, queried once
+    constexpr int mi = (M == 4) ? 0 : (M == 8) ? 1 : (M == 16) ? 2 : 3;
+    pz_plan::ZtGeo &g = pl->zt[mi][HELM ? 1 : 0];
+    if (g.blocks == 0 || g.stages != stages) {
+        { const int rc = smem_optin(pl, zsolve_tma_kernel<M, HELM>, 227 * 1024); if (rc != PZ_OK) return rc; }
+        int occ = 1;
+        if (smem * 2 <= 227 * 1024) PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, zsolve_tma_kernel<M, HELM>, kThreads, smem));
+        if (occ < 1) occ = 1;
+        g.blocks = pl->num_sms * occ;
+        g.stages = stages;
+    }
+    int blocks = g.blocks;
     if (blocks > ntiles) blocks = ntiles;
+    const CUtensorMap *mapp = nullptr;
+    const int rc = cached_column_map(pl, &mapp, p, plane, pl->nz, kTX, M, 1, /*swizzle128=*/true);
+    if (rc != PZ_OK) return rc;
+    const CUtensorMap &map = *mapp;
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
     zsolve_tma_kernel<M, HELM><<<blocks, kThreads, smem, st>>>(map, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
                                                                 pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, pl->nz,

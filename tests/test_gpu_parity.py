@@ -381,6 +381,46 @@ def test_helmholtz_graph_capture_and_determinism(torch, pz, wl):
     pz.poisson_plan_destroy(plan)
 
 
+@pytest.mark.parametrize("nz,variant", [(512, 1), (96, 1), (1100, 0)])
+def test_helmholtz_graph_replay_survives_later_setups(torch, pz, wl, oracle, nz, variant):
+    """A captured helmholtz_z_solve keeps the coefficient tables of capture time: set-ups made after
+    the capture (one per Runge-Kutta sub-step) go to other table sets, so a replay is
+    still ordered correctly and solves with the captured coefficient, whatever was set up since; the
+    step of Eq. (11) in one kernel likewise.  Eager solves use the newest set-up."""
+    nx, ny = 32, 16
+    zf = wl.z_faces(nz, 2.0, 1.8)
+    zc = wl.z_centres(zf)
+    plan = pz.poisson_plan_create(nx, ny, nz, 1.0, 1.0, zc, zf)
+    pz.pz_set_option(plan, "helm_variant", variant)
+    a1, a2, a3 = 5e-5, 3e-4, 1e-3
+    r = np.random.default_rng(77).standard_normal((nz, ny, nx))
+    uk = np.random.default_rng(78).standard_normal((nz, ny, nx))
+    ref1 = oracle.helmholtz_z_solve(zc, zf, a1, r)
+    pz.helmholtz_z_setup(plan, a1)
+    static, ukd, step = torch.from_numpy(r).cuda(), torch.from_numpy(uk).cuda(), torch.from_numpy(r).cuda()
+    g = torch.cuda.CUDAGraph()
+    torch.cuda.synchronize()
+    with torch.cuda.graph(g):
+        pz.helmholtz_z_solve(plan, static)
+        pz.helmholtz_z_step(plan, step, ukd)
+    g.replay()
+    torch.cuda.synchronize()
+    first, first_step = static.clone(), step.clone()
+    assert rel_err(first.cpu().numpy(), ref1) <= TOL
+    for a in (a2, a3, a2, a3, a1 * 7):          # more set-ups than there are spare table sets
+        pz.helmholtz_z_setup(plan, a)
+        static.copy_(torch.from_numpy(r))
+        step.copy_(torch.from_numpy(r))
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(static, first) and torch.equal(step, first_step)
+    eager = torch.from_numpy(r).cuda()
+    pz.helmholtz_z_solve(plan, eager)
+    torch.cuda.synchronize()
+    assert rel_err(eager.cpu().numpy(), oracle.helmholtz_z_solve(zc, zf, a1 * 7, r)) <= TOL
+    pz.poisson_plan_destroy(plan)
+
+
 def test_host_buffer_entry_points(torch, pz, wl, oracle):
     w = wl.scaled(wl.CONFIGS["c1"], 32, 32, 48)
     zc, zf = wl.grid(w)
