@@ -330,6 +330,30 @@ def sub_c4(torch, pz, wl, peak, local):
     return rec
 
 
+def sub_paper_shape(torch, pz, wl, peak, local):
+    """The paper's per-GPU weak-scaling grid 3456 x 3072 x 30: mixed-radix transforms
+    (3456 = 2^7 27, 3072 = 2^10 3).  Poisson, 10 solves with one plan."""
+    w = wl.scaled(wl.CONFIGS["c3"], 3456, 3072, 30, name="paper_weak_3456x3072x30")
+    zc, zf = wl.grid(w)
+    plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
+    p = wl.device_remove_weighted_mean(wl.device_field(w, w.poisson_seed), zf)
+    for _ in range(3):
+        pz.poisson_solve(plan, p)
+    torch.cuda.synchronize()
+    pz.pz_profile_enable(plan, True)
+    ms = event_times(torch, lambda: pz.poisson_solve(plan, p), 10)
+    pz.pz_profile_enable(plan, False)
+    med = statistics.median(ms)
+    rec = {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "solves": 10, "ms_per_solve": med,
+           "points_per_s": w.n / (med * 1e-3), "frac_48B": 48.0 * w.n / (med * 1e-3) / 1e9 / peak,
+           "frac_80B_five_passes": 80.0 * w.n / (med * 1e-3) / 1e9 / peak, "kernels": kernel_table(pz, plan, 10),
+           "note": "mixed-radix kernels (pz_fft_generic.cu), five HBM passes"}
+    pz.poisson_plan_destroy(plan)
+    del p
+    torch.cuda.empty_cache()
+    return rec
+
+
 def bench_strong(args, w, torch, pz, ranks, wl, rank, world, local, dist):
     """ONE problem of the workload over all ranks: Poisson by z-slabs around one all-gather
     (sharded.SlabPoisson), Helmholtz by y-slabs without a collective (sharded.YSlabHelmholtz)."""
@@ -676,7 +700,7 @@ def main():
         return 0
 
     # ---- the other roofline targets of BASELINE.json (c3, c4), outside the timed region, own clock samples
-    c3rec = c4rec = None
+    c3rec = c4rec = wkrec = None
     if extras and world == 1 and args.workload == "c2":
         pz.poisson_plan_destroy(plan)
         p = None
@@ -684,6 +708,7 @@ def main():
         torch.cuda.empty_cache()
         c3rec = sub_c3(torch, pz, wl, measured_peak()[0], local)
         c4rec = sub_c4(torch, pz, wl, measured_peak()[0], local)
+        wkrec = sub_paper_shape(torch, pz, wl, measured_peak()[0], local)
 
     # ---- roofline of the dominant kernel (largest share of the step), live event timings
     peak, peak_src = measured_peak()
@@ -728,6 +753,8 @@ def main():
         line["c3"] = c3rec
     if c4rec is not None:
         line["c4"] = c4rec
+    if wkrec is not None:
+        line["paper_weak_shape"] = wkrec
     if h3 is not None:
         line["helmholtz3d"] = h3
     if pc is not None:

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libpz_b200.so")
-SOURCES = ["pz_api.cu", "pz_fft_x.cu", "pz_fft_y.cu", "pz_fft_xy_fwd.cu", "pz_fft_xy_inv.cu", "pz_zsolve.cu", "pz_zsolve_cr.cu", "pz_zsolve_tma.cu", "pz_zslab.cu", "pz_helmholtz.cu", "pz_helmholtz_tma.cu", "pz_projection.cu", "pz_tma.cu"]
+SOURCES = ["pz_api.cu", "pz_fft_x.cu", "pz_fft_y.cu", "pz_fft_generic.cu", "pz_fft_xy_fwd.cu", "pz_fft_xy_inv.cu", "pz_zsolve.cu", "pz_zsolve_cr.cu", "pz_zsolve_tma.cu", "pz_zslab.cu", "pz_helmholtz.cu", "pz_helmholtz_tma.cu", "pz_projection.cu", "pz_tma.cu"]
 HEADERS = ["pz_internal.h", "pz_fft.cuh", "pz_tma.cuh", "pz_zsolve_pair.cuh", "pz_fft_xy_impl.cuh", "pz_fft2.cuh", os.path.join("..", "..", "include", "pz.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--fmad=true"]

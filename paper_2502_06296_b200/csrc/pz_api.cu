@@ -63,7 +63,7 @@ ProfScope::~ProfScope()
 
 namespace {
 
-bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
 
 typedef long double ld;
 const ld kPi = 3.141592653589793238462643383279502884L;
@@ -80,8 +80,8 @@ double lambda(int q, int n, double length)
 // exp(-2 pi i k / n) with the argument folded into the first octant
 void twiddle(int k, int n, double *re, double *im)
 {
-    // angle = 2 pi k / n, k in [0, n); use symmetries about multiples of pi/4 (n is a power of two >= 8)
-    const int e = n / 8;
+    // angle = 2 pi k / n, k in [0, n); use symmetries about multiples of pi/4 where n is a multiple of 8
+    const int e = (n % 8 == 0) ? n / 8 : 0;
     int oct = (e > 0) ? k / e : 0;
     int rem = (e > 0) ? k % e : 0;
     ld c, s;
@@ -201,8 +201,9 @@ static int plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double 
     if (nx <= 0 || ny <= 0 || nz <= 0) { set_error("poisson_plan_create: non-positive size %d x %d x %d", nx, ny, nz); return PZ_EINVAL; }
     if (!(lx > 0.0) || !(ly > 0.0) || !std::isfinite(lx) || !std::isfinite(ly)) { set_error("poisson_plan_create: lx, ly must be positive and finite"); return PZ_EINVAL; }
     if (bc != PZ_BC_PERIODIC_XY_NEUMANN_P_DIRICHLET_U) { set_error("poisson_plan_create: unsupported bc %d", bc); return PZ_EUNSUPPORTED; }
-    if (!is_pow2(nx) || !is_pow2(ny) || nx < 8 || ny < 8 || nx > 4096 || ny > 4096) {
-        set_error("poisson_plan_create: nx, ny must be powers of two in [8, 4096] (got %d, %d)", nx, ny);
+    if (!(fast_fft_len(nx) || generic_fft_x_ok(nx)) || !(fast_fft_len(ny) || generic_fft_y_ok(ny)) || ((long long)nx * ny) % 16 != 0) {
+        set_error("poisson_plan_create: nx, ny must be even with nx / 2 and ny products of 2, 3, 5, 7 (nx <= 16384, ny <= 8192) and "
+                  "nx ny a multiple of 16 (got %d, %d)", nx, ny);
         return PZ_EUNSUPPORTED;
     }
     if (nz < 4) { set_error("poisson_plan_create: nz must be >= 4 (got %d)", nz); return PZ_EUNSUPPORTED; }
@@ -445,7 +446,7 @@ int pz_pressure_correction(pz_plan *pl, double *u, double *v, double *w, double 
 {
     if (!(gdt > 0.0) || !std::isfinite(gdt)) { set_error("pz_pressure_correction: gamma dt must be positive and finite"); return PZ_EINVAL; }
     int rc;
-    if (pl && u && v && w && work && pl->opt.div_fused != 0 && pl->opt.slab_planes == 0 &&
+    if (pl && u && v && w && work && pl->opt.div_fused != 0 && pl->opt.slab_planes == 0 && fast_fft_len(pl->nx) &&
         !misaligned(u) && !misaligned(v) && !misaligned(w) && !misaligned(work)) {
         // Eq. (4)'s right-hand side is formed inside the forward x transform: it never touches HBM
         cudaStream_t st = (cudaStream_t)stream;

@@ -1,0 +1,291 @@
+// pz_fft_generic.cu -- steps a1/a2/a4/a5 for lengths that are not powers of two: mixed-radix
+// (2, 3, 4, 5, 7, 8) Stockham transforms.  The paper's in-house FFT is mixed-radix
+// and every grid it runs has such lengths: 7168 = 2^10 7, 3200 x 3456 (:278),
+// 3456 x 3072 (:280).  Same data layout as the power-of-two kernels (pz_fft_x.cu, pz_fft_y.cu):
+// real-to-complex along x through one complex transform of length M = nx / 2 plus the split,
+// output packed into the nx reals of the line (Appendix A, reading R8);
+// along y one complex transform of length ny per packed pair, TC neighbouring pairs per CTA.
+//
+// One pass of radix R (Ns = product of the earlier radices, butterfly j < L / R), as in pz_fft.cuh:
+//     in : x[j + r L/R] w_{Ns R}^{r (j mod Ns)},   r < R
+//     out: y[(j div Ns) Ns R + (j mod Ns) + r' Ns] = sum_r in_r exp(-2 pi i r r' / R)
+// The lines of a CTA live in ONE shared-memory buffer; a pass reads all its butterflies' inputs into
+// registers (at most kE points per thread), synchronises, and writes the results back in place, so
+// the buffer is as large as shared memory allows (8192 points) and rows stay as wide as possible.
+#include "pz_internal.h"
+#include "pz_fft.cuh"
+
+namespace pz {
+
+namespace {
+
+constexpr int kT = 512;   // threads per CTA
+constexpr int kE = 16;    // complex points per thread, at most
+constexpr int kPts = kT * kE;
+
+struct Radices { int n; int r[20]; };
+
+// ---- small DFTs, forward sign, natural order in and out
+__device__ __forceinline__ double2 mul_mi(double2 a) { return make_double2(a.y, -a.x); } // a * (-i)
+__device__ __forceinline__ double2 axpy(double c, double2 x, double2 y) { return make_double2(fma(c, x.x, y.x), fma(c, x.y, y.y)); }
+__device__ __forceinline__ double2 scal(double c, double2 x) { return make_double2(c * x.x, c * x.y); }
+
+template <int R> __device__ __forceinline__ void dft(double2 (&v)[R]);
+
+template <> __device__ __forceinline__ void dft<2>(double2 (&v)[2])
+{
+    const double2 a = v[0], b = v[1];
+    v[0] = cadd(a, b);
+    v[1] = csub(a, b);
+}
+template <> __device__ __forceinline__ void dft<4>(double2 (&v)[4])
+{
+    dif<4, 1>(v); // result r' in slot bitrev(r')
+    const double2 t = v[1];
+    v[1] = v[2];
+    v[2] = t;
+}
+template <> __device__ __forceinline__ void dft<8>(double2 (&v)[8])
+{
+    dif<8, 1>(v);
+    double2 t[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) t[i] = v[i];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = t[bitrev(i, 3)];
+}
+template <> __device__ __forceinline__ void dft<3>(double2 (&v)[3])
+{
+    constexpr double s = 0.86602540378443864676; // sin(2 pi / 3)
+    const double2 t1 = cadd(v[1], v[2]), d = mul_mi(scal(s, csub(v[1], v[2])));
+    const double2 m1 = axpy(-0.5, t1, v[0]);
+    v[0] = cadd(v[0], t1);
+    v[1] = cadd(m1, d);
+    v[2] = csub(m1, d);
+}
+template <> __device__ __forceinline__ void dft<5>(double2 (&v)[5])
+{
+    constexpr double c1 = 0.30901699437494742410, c2 = -0.80901699437494742410; // cos(2 pi/5), cos(4 pi/5)
+    constexpr double s1 = 0.95105651629515357212, s2 = 0.58778525229247312917;  // sin(2 pi/5), sin(4 pi/5)
+    const double2 a1 = cadd(v[1], v[4]), a2 = cadd(v[2], v[3]), b1 = csub(v[1], v[4]), b2 = csub(v[2], v[3]);
+    const double2 e1 = axpy(c2, a2, axpy(c1, a1, v[0])), e2 = axpy(c1, a2, axpy(c2, a1, v[0]));
+    const double2 d1 = mul_mi(axpy(s2, b2, scal(s1, b1))), d2 = mul_mi(axpy(-s1, b2, scal(s2, b1)));
+    v[0] = cadd(v[0], cadd(a1, a2));
+    v[1] = cadd(e1, d1);
+    v[4] = csub(e1, d1);
+    v[2] = cadd(e2, d2);
+    v[3] = csub(e2, d2);
+}
+template <> __device__ __forceinline__ void dft<7>(double2 (&v)[7])
+{
+    constexpr double c1 = 0.62348980185873353053, c2 = -0.22252093395631440429, c3 = -0.90096886790241912624;
+    constexpr double s1 = 0.78183148246802980871, s2 = 0.97492791218182360702, s3 = 0.43388373911755812048;
+    const double2 a1 = cadd(v[1], v[6]), a2 = cadd(v[2], v[5]), a3 = cadd(v[3], v[4]);
+    const double2 b1 = csub(v[1], v[6]), b2 = csub(v[2], v[5]), b3 = csub(v[3], v[4]);
+    // X_m = v0 + sum_k cos(2 pi m k / 7) a_k - i sum_k sin(2 pi m k / 7) b_k
+    const double2 e1 = axpy(c3, a3, axpy(c2, a2, axpy(c1, a1, v[0])));
+    const double2 e2 = axpy(c1, a3, axpy(c3, a2, axpy(c2, a1, v[0])));   // m = 2: k = 1, 2, 3 -> angles 2, 4, 6 -> c2, c3, c1
+    const double2 e3 = axpy(c2, a3, axpy(c1, a2, axpy(c3, a1, v[0])));   // m = 3: angles 3, 6, 9 = 2 -> c3, c1, c2
+    const double2 d1 = mul_mi(axpy(s3, b3, axpy(s2, b2, scal(s1, b1))));
+    const double2 d2 = mul_mi(axpy(-s1, b3, axpy(-s3, b2, scal(s2, b1)))); // sin(4) = -s3, sin(6) = -s1 (units of 2 pi / 7)
+    const double2 d3 = mul_mi(axpy(s2, b3, axpy(-s1, b2, scal(s3, b1))));  // sin(6) = -s1, sin(9 = 2) = s2
+    v[0] = cadd(v[0], cadd(a1, cadd(a2, a3)));
+    v[1] = cadd(e1, d1); v[6] = csub(e1, d1);
+    v[2] = cadd(e2, d2); v[5] = csub(e2, d2);
+    v[3] = cadd(e3, d3); v[4] = csub(e3, d3);
+}
+
+// One in-place pass over `nlines` lines of complex length L in shared memory; element pos of line
+// ln sits at s[ln * sl + pos * sp].  tw[k * tws] = exp(-2 pi i k / L).
+template <int R>
+__device__ __forceinline__ void pass(double2 *s, int L, int Ns, int nlines, int sl, int sp, const double2 *__restrict__ tw, int tws)
+{
+    constexpr int Q = (kE + R - 1) / R;
+    const int nb = L / R, W = nlines * nb, step = (L / (Ns * R)) * tws;
+    double2 v[Q][R];
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+        const int w = threadIdx.x + q * kT;
+        if (w < W) {
+            // lines fastest when they are interleaved in memory (sl == 1), butterflies fastest otherwise
+            const int ln = (sl == 1) ? w % nlines : w / nb, j = (sl == 1) ? w / nlines : w % nb;
+            const double2 *x = s + (size_t)ln * sl + (size_t)j * sp;
+            const int jm = j % Ns;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                double2 t = x[(size_t)r * nb * sp];
+                if (r > 0 && Ns > 1) t = cmul(t, __ldg(&tw[(size_t)r * jm * step]));
+                v[q][r] = t;
+            }
+            dft<R>(v[q]);
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+        const int w = threadIdx.x + q * kT;
+        if (w < W) {
+            const int ln = (sl == 1) ? w % nlines : w / nb, j = (sl == 1) ? w / nlines : w % nb;
+            double2 *y = s + (size_t)ln * sl + (size_t)((j / Ns) * Ns * R + (j % Ns)) * sp;
+#pragma unroll
+            for (int r = 0; r < R; ++r) y[(size_t)r * Ns * sp] = v[q][r];
+        }
+    }
+    __syncthreads();
+}
+
+__device__ __forceinline__ void all_passes(double2 *s, int L, int nlines, int sl, int sp, const double2 *__restrict__ tw, int tws,
+                                           const Radices &rl)
+{
+    int Ns = 1;
+    for (int i = 0; i < rl.n; ++i) {
+        switch (rl.r[i]) {
+        case 2: pass<2>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        case 3: pass<3>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        case 4: pass<4>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        case 5: pass<5>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        case 7: pass<7>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        default: pass<8>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        }
+        Ns *= rl.r[i];
+    }
+}
+
+// x lines: lpb lines of n = 2M reals per CTA.  twx[k] = exp(-2 pi i k / n).
+template <bool INV>
+__global__ void __launch_bounds__(kT, 1) gen_fft_x_kernel(double *__restrict__ p, const double2 *__restrict__ twx, int M, long long nlines,
+                                                        int lpb, Radices rl, double scale)
+{
+    extern __shared__ double2 smem_gx[];
+    const long long l0 = (long long)blockIdx.x * lpb;
+    const int nl = (int)((nlines - l0 < lpb) ? nlines - l0 : lpb);
+    double2 *g = reinterpret_cast<double2 *>(p) + (size_t)l0 * M;
+    for (int q = threadIdx.x; q < nl * M; q += kT) {
+        const int ln = q / M, k = q - ln * M;
+        double2 z = g[q];
+        if constexpr (INV) {
+            // merge of the complex-to-real transform, conjugated (inverse through the forward passes)
+            if (k == 0) {
+                z = make_double2(z.x + z.y, -(z.x - z.y));
+            } else {
+                const double2 xm = cconj(g[(size_t)ln * M + (M - k)]);
+                const double2 sm = cadd(z, xm), c = cmul_conj(csub(z, xm), __ldg(&twx[k]));
+                z = make_double2(sm.x - c.y, -(sm.y + c.x));
+            }
+        }
+        smem_gx[q] = z;
+    }
+    __syncthreads();
+    all_passes(smem_gx, M, nl, M, 1, twx, 2, rl);
+    for (int q = threadIdx.x; q < nl * M; q += kT) {
+        const int ln = q / M, k = q - ln * M;
+        const double2 z = smem_gx[q];
+        double2 o;
+        if constexpr (INV) {
+            o = make_double2(z.x * scale, -z.y * scale);
+        } else if (k == 0) {
+            o = make_double2(z.x + z.y, z.x - z.y); // Re X_0, Re X_{n/2}
+        } else {
+            // split: X_k = (Z_k + conj Z_{M-k}) / 2 - (i/2) w_n^k (Z_k - conj Z_{M-k})
+            const double2 zm = cconj(smem_gx[ln * M + (M - k)]);
+            const double2 ev = make_double2(0.5 * (z.x + zm.x), 0.5 * (z.y + zm.y));
+            const double2 d = csub(z, zm);
+            o = cadd(ev, cmul(make_double2(0.5 * d.y, -0.5 * d.x), __ldg(&twx[k])));
+        }
+        g[q] = o;
+    }
+}
+
+// y columns: TC neighbouring packed pairs x all ny rows of one plane per CTA.  twy[k] = exp(-2 pi i k / ny).
+template <bool INV>
+__global__ void __launch_bounds__(kT, 1) gen_fft_y_kernel(double *__restrict__ p, const double2 *__restrict__ twy, int nx, int ny, int tc,
+                                                        Radices rl)
+{
+    extern __shared__ double2 smem_gy[];
+    double *base = p + (size_t)blockIdx.y * nx * ny + 2 * (size_t)blockIdx.x * tc;
+    for (int q = threadIdx.x; q < ny * tc; q += kT) {
+        const int row = q / tc, c = q - row * tc;
+        const double2 t = *reinterpret_cast<const double2 *>(base + (size_t)row * nx + 2 * c);
+        smem_gy[q] = INV ? cconj(t) : t;
+    }
+    __syncthreads();
+    all_passes(smem_gy, ny, tc, 1, tc, twy, 1, rl);
+    for (int q = threadIdx.x; q < ny * tc; q += kT) {
+        const int row = q / tc, c = q - row * tc;
+        const double2 t = smem_gy[q];
+        *reinterpret_cast<double2 *>(base + (size_t)row * nx + 2 * c) = INV ? cconj(t) : t;
+    }
+}
+
+bool factor(int n, Radices *out)
+{
+    out->n = 0;
+    // odd radices first: their strided writes of the first pass are free of bank conflicts
+    for (int f : {7, 5, 3})
+        while (n % f == 0) { out->r[out->n++] = f; n /= f; }
+    while (n % 8 == 0) { out->r[out->n++] = 8; n /= 8; }
+    if (n % 4 == 0) { out->r[out->n++] = 4; n /= 4; }
+    if (n % 2 == 0) { out->r[out->n++] = 2; n /= 2; }
+    return n == 1 && out->n <= 20;
+}
+
+} // namespace
+
+// lengths the mixed-radix kernels take: even, 7-smooth (nx / 2 resp. ny), a line within the
+// 8192-point shared-memory buffer
+bool generic_fft_x_ok(int nx)
+{
+    Radices r;
+    return nx >= 8 && !(nx & 1) && nx / 2 <= kPts && factor(nx / 2, &r);
+}
+bool generic_fft_y_ok(int ny)
+{
+    Radices r;
+    return ny >= 8 && !(ny & 1) && ny <= kPts && factor(ny, &r);
+}
+
+int launch_fft_x_generic(const pz_plan *pl, double *p, long long nlines, bool inverse, cudaStream_t st)
+{
+    const int M = pl->nx / 2;
+    Radices rl;
+    if (!factor(M, &rl)) { set_error("fft_x: nx / 2 = %d has a prime factor above 7", M); return PZ_EUNSUPPORTED; }
+    int lpb = kPts / M;
+    if (lpb > 64) lpb = 64;
+    // keep the grid a few waves deep on small fields
+    while (lpb > 1 && (nlines + lpb - 1) / lpb < 4LL * pl->num_sms) lpb /= 2;
+    const size_t smem = (size_t)lpb * M * sizeof(double2);
+    const long long blocks = (nlines + lpb - 1) / lpb;
+    const double scale = 1.0 / ((double)pl->nx * (double)pl->ny);
+    int rc;
+    if ((rc = smem_optin(pl, gen_fft_x_kernel<false>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
+    if ((rc = smem_optin(pl, gen_fft_x_kernel<true>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
+    ProfScope prof(pl, inverse ? PZ_K_FFT_X_INV : PZ_K_FFT_X_FWD, st);
+    if (inverse) gen_fft_x_kernel<true><<<(unsigned)blocks, kT, smem, st>>>(p, pl->d_twx, M, nlines, lpb, rl, scale);
+    else gen_fft_x_kernel<false><<<(unsigned)blocks, kT, smem, st>>>(p, pl->d_twx, M, nlines, lpb, rl, scale);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+int launch_fft_y_generic(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_t st)
+{
+    const int L = pl->ny, npairs = pl->nx / 2;
+    Radices rl;
+    if (!factor(L, &rl)) { set_error("fft_y: ny = %d has a prime factor above 7", L); return PZ_EUNSUPPORTED; }
+    int tc = 8;
+    while (tc > 1 && (npairs % tc != 0 || tc * L > kPts)) tc /= 2;
+    if (tc * L > kPts) { set_error("fft_y: ny = %d exceeds the %d-point buffer", L, kPts); return PZ_EUNSUPPORTED; }
+    const size_t smem = (size_t)tc * L * sizeof(double2);
+    int rc;
+    if ((rc = smem_optin(pl, gen_fft_y_kernel<false>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
+    if ((rc = smem_optin(pl, gen_fft_y_kernel<true>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
+    dim3 grid((unsigned)(npairs / tc), (unsigned)nk);
+    ProfScope prof(pl, inverse ? PZ_K_FFT_Y_INV : PZ_K_FFT_Y_FWD, st);
+    if (inverse) gen_fft_y_kernel<true><<<grid, kT, smem, st>>>(p, pl->d_twy, pl->nx, L, tc, rl);
+    else gen_fft_y_kernel<false><<<grid, kT, smem, st>>>(p, pl->d_twy, pl->nx, L, tc, rl);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+} // namespace pz

@@ -197,9 +197,10 @@ int launch_l(const pz_plan *pl, double *p, int nk, cudaStream_t st)
     int tc = pl->opt.fft_y_tc;
     if (tc == 0) tc = (L <= 256) ? 16 : (L <= 512) ? 8 : 4; // 256 threads and <= 64 KB of exchange tile per CTA
     if (tc > npairs) tc = npairs;
-    if (tc >= 16 && tc_valid<L, 16>()) return try_ltc<L, 16, INV>(pl, p, nk, st);
-    if (tc >= 8 && tc_valid<L, 8>()) return try_ltc<L, 8, INV>(pl, p, nk, st);
-    if (tc >= 4 && tc_valid<L, 4>()) return try_ltc<L, 4, INV>(pl, p, nk, st);
+    // the pairs of a row must split evenly over the CTAs (nx / 2 need not be a power of two)
+    if (tc >= 16 && npairs % 16 == 0 && tc_valid<L, 16>()) return try_ltc<L, 16, INV>(pl, p, nk, st);
+    if (tc >= 8 && npairs % 8 == 0 && tc_valid<L, 8>()) return try_ltc<L, 8, INV>(pl, p, nk, st);
+    if (tc >= 4 && npairs % 4 == 0 && tc_valid<L, 4>()) return try_ltc<L, 4, INV>(pl, p, nk, st);
     return try_ltc<L, 2, INV>(pl, p, nk, st);
 }
 
@@ -226,19 +227,20 @@ int dispatch(const pz_plan *pl, double *p, int nk, cudaStream_t st)
 int launch_fft_y(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st)
 {
     double *base = p + (size_t)k0 * pl->nx * pl->ny;
+    if (!fast_fft_len(pl->ny) || (pl->nx / 2) % 2 != 0) return launch_fft_y_generic(pl, base, nk, inverse, st);
     return inverse ? dispatch<true>(pl, base, nk, st) : dispatch<false>(pl, base, nk, st);
 }
 
 int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st)
 {
-    if (pl->opt.fft_y_p0 != 0) return PZ_OK; // done inside fft_y_kernel
+    if (pl->opt.fft_y_p0 != 0 && fast_fft_len(pl->ny) && (pl->nx / 2) % 2 == 0) return PZ_OK; // done inside fft_y_kernel
     double *base = p + (size_t)k0 * pl->nx * pl->ny;
     const size_t smem = (size_t)pl->ny * sizeof(double2);
     const int threads = pl->ny / 2 >= 256 ? 256 : (pl->ny / 2 < 32 ? 32 : pl->ny / 2);
     if (smem > 48 * 1024) {
         int rc;
-        if ((rc = smem_optin(pl, pair0_kernel<false>, 64 * 1024)) != PZ_OK) return rc;
-        if ((rc = smem_optin(pl, pair0_kernel<true>, 64 * 1024)) != PZ_OK) return rc;
+        if ((rc = smem_optin(pl, pair0_kernel<false>, 128 * 1024)) != PZ_OK) return rc;
+        if ((rc = smem_optin(pl, pair0_kernel<true>, 128 * 1024)) != PZ_OK) return rc;
     }
     ProfScope prof(pl, inverse ? PZ_K_PAIR0_INV : PZ_K_PAIR0_FWD, st);
     if (inverse)

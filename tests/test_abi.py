@@ -47,9 +47,12 @@ def test_argument_validation_needs_no_gpu(built):
     zf = wl.z_faces(16)
     zc = wl.z_centres(zf)
     cases = [
-        (dict(nx=12, ny=16, nz=16), pz.PZ_EUNSUPPORTED),   # nx not a power of two
+        (dict(nx=22, ny=16, nz=16), pz.PZ_EUNSUPPORTED),   # nx / 2 = 11: a prime factor above 7
+        (dict(nx=16, ny=26, nz=16), pz.PZ_EUNSUPPORTED),   # ny = 2 * 13
+        (dict(nx=18, ny=12, nz=16), pz.PZ_EUNSUPPORTED),   # nx ny = 216 is not a multiple of 16 (column tiles)
+        (dict(nx=15, ny=16, nz=16), pz.PZ_EUNSUPPORTED),   # odd
         (dict(nx=16, ny=4, nz=16), pz.PZ_EUNSUPPORTED),    # ny < 8
-        (dict(nx=8192, ny=16, nz=16), pz.PZ_EUNSUPPORTED),
+        (dict(nx=32768, ny=16, nz=16), pz.PZ_EUNSUPPORTED),
         (dict(nx=0, ny=16, nz=16), pz.PZ_EINVAL),
         (dict(nx=16, ny=16, nz=16, lx=-1.0), pz.PZ_EINVAL),
         (dict(nx=16, ny=16, nz=16, bc=7), pz.PZ_EUNSUPPORTED),
