@@ -658,6 +658,7 @@ static int *option_slot(pz_plan *pl, const char *key)
     if (!std::strcmp(key, "helm_l2promo")) return &pl->opt.helm_l2promo;
     if (!std::strcmp(key, "helm_tx")) return &pl->opt.helm_tx;
     if (!std::strcmp(key, "helm_m")) return &pl->opt.helm_m;
+    if (!std::strcmp(key, "helm_zsplit")) return &pl->opt.helm_zsplit;
     if (!std::strcmp(key, "fft_y_tc")) return &pl->opt.fft_y_tc;
     if (!std::strcmp(key, "div_fused")) return &pl->opt.div_fused;
     if (!std::strcmp(key, "step_fused")) return &pl->opt.step_fused;
@@ -680,7 +681,7 @@ int pz_set_option(pz_plan *pl, const char *key, int value)
         return PZ_EUNSUPPORTED;
     }
     *slot = value;
-    if ((slot == &pl->opt.helm_tx || slot == &pl->opt.helm_m || slot == &pl->opt.helm_variant) && pl->helm_cur >= 0)
+    if ((slot == &pl->opt.helm_tx || slot == &pl->opt.helm_m || slot == &pl->opt.helm_variant || slot == &pl->opt.helm_zsplit) && pl->helm_cur >= 0)
         return helmholtz_build_tables(pl, pl->helm_a); // geometry changed: rebuild the tables
     return PZ_OK;
 }
@@ -694,6 +695,7 @@ int pz_get_option(const pz_plan *pl, const char *key, int *value)
         if (!std::strcmp(key, "helm_variant_actual")) { *value = pl->helm_variant; return PZ_OK; }
         if (!std::strcmp(key, "helm_tx_actual")) { *value = pl->helm_tx; return PZ_OK; }
         if (!std::strcmp(key, "helm_p_actual")) { *value = pl->helm_P; return PZ_OK; }
+        if (!std::strcmp(key, "helm_zsplit_actual")) { *value = pl->helm_zs; return PZ_OK; }
         if (!std::strcmp(key, "slab_planes_actual")) { *value = slab_planes(pl); return PZ_OK; }
         set_error("pz_get_option: unknown key '%s'", key);
         return PZ_EUNSUPPORTED;

@@ -114,18 +114,34 @@ int ilog2_ceil(int n)
 static void helm_geometry(pz_plan *pl)
 {
     int variant = pl->opt.helm_variant;
-    if (variant != 0 && variant != 1) variant = (pl->nz <= 1024) ? 1 : 0;
-    if (variant == 1 && pl->nz > 1024) variant = 0;
+    // variant 1 up to nz = 1920: beyond, the tile of a chunk plus the tables exceed shared memory
+    if (variant != 0 && variant != 1) variant = (pl->nz <= 1920) ? 1 : 0;
+    if (variant == 1 && (pl->nz > 1920 || (pl->nz > 1024 && pl->opt.helm_zsplit == 1))) variant = 0;
     pl->helm_variant = variant;
     int m = pl->opt.helm_m;
+    pl->helm_zs = 1;
     if (variant == 1) {
-        // 8 column pairs x P sub-domains per CTA, P <= 64, m in {4, 8, 16}
+        // TX / 2 column pairs x P sub-domains per CTA, at most 512 threads, m in {4, 8, 16}
         if (m != 4 && m != 8 && m != 16) m = (pl->nz <= 128) ? 4 : (pl->nz <= 256 ? 8 : 16);
         while (m < 16 && (pl->nz + m - 1) / m > 64) m *= 2;
         pl->helm_m = m;
-        pl->helm_P = (pl->nz + m - 1) / m;
-        pl->helm_tx = 16;
-        pl->helm_levels = ilog2_ceil(2 * pl->helm_P);
+        int P = (pl->nz + m - 1) / m;
+        const bool even64 = ((size_t)pl->nx * pl->ny) % 64 == 0;
+        // m = 16 (nz > 256): the column is cut in two chunks owned by the two CTAs of a cluster (the
+        // paper's own decomposition, with CTAs for its MPI tasks): half the rows per
+        // tile leave room for 256-byte rows up to nz = 1024, for two resident CTAs per SM up to
+        // nz = 512 and for nz up to 1920 at all.  Measured, 3 fields: 512^3 5.96 TB/s against 5.73
+        // (whole columns, 32-column tiles) and 5.45 (16-column tiles); 1024^3 5.80 against 5.13 TB/s.
+        int zs = pl->opt.helm_zsplit;
+        if (zs != 1 && zs != 2) zs = (m == 16) ? 2 : 1;
+        if (zs == 2 && (m != 16 || pl->nz < 4 * m)) zs = 1;
+        if (zs == 2) P = (P + 1) / 2;            // sub-domains per chunk
+        pl->helm_zs = zs;
+        pl->helm_P = P;
+        // wide tiles (32 columns, 256-byte rows) where one of them fits shared memory and 512 threads
+        // (measured: 5.76 against 5.45 TB/s at 512^3 x 3 fields, 5.81 against 5.17 TB/s at 1024 x 1024 x 512 x 3)
+        pl->helm_tx = (pl->opt.helm_tx != 16 && m == 16 && P <= 32 && even64) ? 32 : 16;
+        pl->helm_levels = ilog2_ceil(2 * P);
         return;
     }
     if (m != 4 && m != 8 && m != 16 && m != 32) m = (pl->nz <= 128) ? 4 : (pl->nz <= 256) ? 8 : (pl->nz <= 512 ? 16 : 32);
@@ -141,40 +157,22 @@ static void helm_geometry(pz_plan *pl)
     pl->helm_levels = ilog2_ceil(2 * P);
 }
 
-// Algorithm 2 Step 1 on the host, plus the precomputed PCR of the boundary system.
-int helmholtz_build_tables(pz_plan *pl, double a)
-{
-    typedef long double ld;
-    helm_geometry(pl);
-    const int nz = pl->nz, m = pl->helm_m, P = pl->helm_P, nzp = P * m, n2 = 2 * P, LV = pl->helm_levels;
-    if (pl->helm_variant == 1) {
-        const int rc = helmholtz_tma_prepare(pl);
-        if (rc != PZ_OK) return rc;
-    } else if (pl->helm_tx * P > ((m >= 32) ? 256 : 512)) {
-        set_error("helmholtz: nz = %d is too large for the register-tile kernel (P = %d sub-domains)", nz, P);
-        return PZ_EUNSUPPORTED;
-    }
-    const size_t ndbl = 5 * (size_t)nzp + (size_t)LV * 2 * n2 + n2;
-    const size_t bytes = ndbl * sizeof(double);
+namespace {
 
-    // matrix of I - a L_z with Dirichlet walls, padded with identity rows
-    std::vector<ld> A(nzp, 0), B(nzp, 1), C(nzp, 0);
-    for (int k = 0; k < nz; ++k) {
-        ld W = 0;
-        if (k == 0) W += (ld)2 / ((ld)pl->dzf[0] * ((ld)2 * ((ld)pl->zc[0] - (ld)pl->zf[0])));
-        if (k == nz - 1) W += (ld)2 / ((ld)pl->dzf[nz - 1] * ((ld)2 * ((ld)pl->zf[nz] - (ld)pl->zc[nz - 1])));
-        A[k] = -(ld)a * (ld)pl->A[k];
-        C[k] = -(ld)a * (ld)pl->C[k];
-        B[k] = (ld)1 + (ld)a * ((ld)pl->A[k] + (ld)pl->C[k] + W);
-    }
-    std::vector<double> host(ndbl, 0.0);
-    double *fA = host.data(), *bC = fA + nzp, *rb = bC + nzp, *ra = rb + nzp, *rc = ra + nzp;
+typedef long double ld;
+
+// Algorithm 2 Step 1 for the P sub-domains of m rows of ONE tridiagonal matrix
+// (A, B, C: sub-diagonal, diagonal, super-diagonal of P*m rows), plus the precomputed parallel
+// cyclic reduction of its boundary system.  out: [fA | bC | rb | ra | rc] (5 P m) + LV*2*2P + 2P.
+void build_chunk_tables(const ld *A, const ld *B, const ld *C, int m, int P, int LV, double *out)
+{
+    const int nzp = P * m, n2 = 2 * P;
+    double *fA = out, *bC = fA + nzp, *rb = bC + nzp, *ra = rb + nzp, *rc = ra + nzp;
     double *pcr = rc + nzp;
     std::vector<ld> ra2(n2), rbd(n2), rc2(n2); // boundary system
     std::vector<ld> ca(m), cb(m), cc(m);
     for (int s = 0; s < P; ++s) {
         const ld *As = &A[s * m], *Bs = &B[s * m], *Cs = &C[s * m];
-        // Algorithm 2, Step 1
         for (int i = 0; i < m; ++i) ca[i] = cb[i] = cc[i] = 0;
         ca[1] = As[1];
         cb[1] = Bs[1];
@@ -195,6 +193,7 @@ int helmholtz_build_tables(pz_plan *pl, double a)
             const int k = s * m + i;
             fA[k] = (i >= 2) ? (double)(As[i] / cb[i - 1]) : 0.0;
             bC[k] = (i <= m - 3) ? (double)(Cs[i] / cb[i + 1]) : 0.0;
+            rb[k] = ra[k] = rc[k] = 0.0;
             if (i >= 1 && i <= m - 2) {
                 rb[k] = (double)((ld)1 / cb[i]);
                 ra[k] = (double)(ca[i] / cb[i]);
@@ -207,24 +206,116 @@ int helmholtz_build_tables(pz_plan *pl, double a)
     ra2[0] = 0;
     rc2[n2 - 1] = 0;
     // PCR of the boundary system with the multipliers recorded per level
-    {
-        std::vector<ld> na(n2), nb(n2), nc(n2);
-        int h = 1;
-        for (int l = 0; l < LV; ++l, h *= 2) {
-            double *kk = pcr + (size_t)l * 2 * n2;
-            for (int r = 0; r < n2; ++r) {
-                ld k1 = 0, k2 = 0;
-                ld b = rbd[r], an = 0, cn = 0;
-                if (r - h >= 0) { k1 = ra2[r] / rbd[r - h]; b -= k1 * rc2[r - h]; an = -k1 * ra2[r - h]; }
-                if (r + h < n2) { k2 = rc2[r] / rbd[r + h]; b -= k2 * ra2[r + h]; cn = -k2 * rc2[r + h]; }
-                kk[2 * r] = (double)(-k1);
-                kk[2 * r + 1] = (double)(-k2);
-                na[r] = an; nb[r] = b; nc[r] = cn;
-            }
-            ra2 = na; rbd = nb; rc2 = nc;
+    std::vector<ld> na(n2), nb(n2), nc(n2);
+    int h = 1;
+    for (int l = 0; l < LV; ++l, h *= 2) {
+        double *kk = pcr + (size_t)l * 2 * n2;
+        for (int r = 0; r < n2; ++r) {
+            ld k1 = 0, k2 = 0;
+            ld b = rbd[r], an = 0, cn = 0;
+            if (r - h >= 0) { k1 = ra2[r] / rbd[r - h]; b -= k1 * rc2[r - h]; an = -k1 * ra2[r - h]; }
+            if (r + h < n2) { k2 = rc2[r] / rbd[r + h]; b -= k2 * ra2[r + h]; cn = -k2 * rc2[r + h]; }
+            kk[2 * r] = (double)(-k1);
+            kk[2 * r + 1] = (double)(-k2);
+            na[r] = an; nb[r] = b; nc[r] = cn;
         }
-        double *rbr = pcr + (size_t)LV * 2 * n2;
-        for (int r = 0; r < n2; ++r) rbr[r] = (double)((ld)1 / rbd[r]);
+        ra2 = na; rbd = nb; rc2 = nc;
+    }
+    double *rbr = pcr + (size_t)LV * 2 * n2;
+    for (int r = 0; r < n2; ++r) rbr[r] = (double)((ld)1 / rbd[r]);
+}
+
+// x = T^{-1} e_j by plain elimination in long double (T diagonally dominant: no pivoting)
+void unit_response(const ld *A, const ld *B, const ld *C, int n, int j, std::vector<ld> &x)
+{
+    std::vector<ld> cp(n), dp(n);
+    for (int k = 0; k < n; ++k) {
+        const ld rhs = (k == j) ? (ld)1 : (ld)0;
+        const ld den = (k == 0) ? B[0] : B[k] - A[k] * cp[k - 1];
+        cp[k] = C[k] / den;
+        dp[k] = (k == 0) ? rhs / den : (rhs - A[k] * dp[k - 1]) / den;
+    }
+    x.assign(n, 0);
+    x[n - 1] = dp[n - 1];
+    for (int k = n - 2; k >= 0; --k) x[k] = dp[k] - cp[k] * x[k + 1];
+}
+
+} // namespace
+
+// Doubles of one chunk's table block: [5 nzc | PCR | corr (nzc) | wOwn, wPeer]
+static size_t chunk_doubles(int nzc, int P, int LV) { return 6 * (size_t)nzc + (size_t)LV * 4 * P + 2 * P + 2; }
+
+// Algorithm 2 Step 1 on the host, plus the precomputed PCR of the boundary system.
+int helmholtz_build_tables(pz_plan *pl, double a)
+{
+    helm_geometry(pl);
+    const int nz = pl->nz, m = pl->helm_m, P = pl->helm_P, ZS = pl->helm_zs, nzc = P * m, LV = pl->helm_levels;
+    const int nzp = ZS * nzc;
+    if (pl->helm_variant == 1) {
+        const int rc = helmholtz_tma_prepare(pl);
+        if (rc != PZ_OK) return rc;
+    } else if (pl->helm_tx * P > ((m >= 32) ? 256 : 512)) {
+        set_error("helmholtz: nz = %d is too large for the register-tile kernel (P = %d sub-domains)", nz, P);
+        return PZ_EUNSUPPORTED;
+    }
+    const size_t cstride = chunk_doubles(nzc, P, LV);
+    // the one-kernel step of Eq. (11) (helmholtz_z_step) takes whole columns: its own table block
+    // behind the chunks' where the columns are cut and a whole one still fits the kernel (nz <= 1024)
+    pl->helm_cn_P = 0; pl->helm_cn_levels = 0; pl->helm_cn_off = 0;
+    size_t cn_doubles = 0;
+    if (pl->helm_variant == 1) {
+        if (ZS == 1) { pl->helm_cn_P = P; pl->helm_cn_levels = LV; }
+        else if ((nz + m - 1) / m <= 64) {
+            pl->helm_cn_P = (nz + m - 1) / m;
+            pl->helm_cn_levels = ilog2_ceil(2 * pl->helm_cn_P);
+            pl->helm_cn_off = ZS * cstride;
+            cn_doubles = chunk_doubles(pl->helm_cn_P * m, pl->helm_cn_P, pl->helm_cn_levels);
+        }
+    }
+    const size_t ndbl = ZS * cstride + cn_doubles;
+    const size_t bytes = ndbl * sizeof(double);
+
+    // matrix of I - a L_z with Dirichlet walls, padded with identity rows
+    const int nzw = (cn_doubles > 0 && pl->helm_cn_P * m > nzp) ? pl->helm_cn_P * m : nzp;
+    std::vector<ld> A(nzw, 0), B(nzw, 1), C(nzw, 0);
+    for (int k = 0; k < nz; ++k) {
+        ld W = 0;
+        if (k == 0) W += (ld)2 / ((ld)pl->dzf[0] * ((ld)2 * ((ld)pl->zc[0] - (ld)pl->zf[0])));
+        if (k == nz - 1) W += (ld)2 / ((ld)pl->dzf[nz - 1] * ((ld)2 * ((ld)pl->zf[nz] - (ld)pl->zc[nz - 1])));
+        A[k] = -(ld)a * (ld)pl->A[k];
+        C[k] = -(ld)a * (ld)pl->C[k];
+        B[k] = (ld)1 + (ld)a * ((ld)pl->A[k] + (ld)pl->C[k] + W);
+    }
+    std::vector<double> host(ndbl, 0.0);
+    if (ZS == 1) {
+        build_chunk_tables(A.data(), B.data(), C.data(), m, P, LV, host.data());
+    } else {
+        // two chunks, couplings across the cut moved to the interface (PAPER.md:120-135 with the
+        // two CTAs of a cluster for its MPI tasks; the matrix is k-only, so everything the
+        // interface needs is precomputed here): with y = T_c^{-1} r on each chunk,
+        //   u_0 = y_0 - (C_cut F1) q_0,  u_1 = y_1 - (A_cut L0) p_1,   q_0 = T_0^{-1} e_last, p_1 = T_1^{-1} e_first,
+        //   L0 = u_0[last] = (y0L - k0 y1F) / (1 - k0 k1),  F1 = u_1[first] = (y1F - k1 y0L) / (1 - k0 k1),
+        //   k0 = C_cut q_0[last],  k1 = A_cut p_1[first].
+        const ld Ccut = C[nzc - 1], Acut = A[nzc];
+        std::vector<ld> A0(A.begin(), A.begin() + nzc), B0(B.begin(), B.begin() + nzc), C0(C.begin(), C.begin() + nzc);
+        std::vector<ld> A1(A.begin() + nzc, A.begin() + nzp), B1(B.begin() + nzc, B.begin() + nzp), C1(C.begin() + nzc, C.begin() + nzp);
+        C0[nzc - 1] = 0;
+        A1[0] = 0;
+        build_chunk_tables(A0.data(), B0.data(), C0.data(), m, P, LV, host.data());
+        build_chunk_tables(A1.data(), B1.data(), C1.data(), m, P, LV, host.data() + cstride);
+        std::vector<ld> q0, p1;
+        unit_response(A0.data(), B0.data(), C0.data(), nzc, nzc - 1, q0);
+        unit_response(A1.data(), B1.data(), C1.data(), nzc, 0, p1);
+        const ld k0 = Ccut * q0[nzc - 1], k1 = Acut * p1[0], g = (ld)1 / ((ld)1 - k0 * k1);
+        const size_t ocorr = 5 * (size_t)nzc + (size_t)LV * 4 * P + 2 * P;
+        for (int k = 0; k < nzc; ++k) {
+            host[ocorr + k] = (double)(Ccut * q0[k]);
+            host[cstride + ocorr + k] = (double)(Acut * p1[k]);
+        }
+        // X of a chunk = wOwn * (its own interface value of y) + wPeer * (the peer's)
+        host[ocorr + nzc] = (double)(-g * k1);            host[ocorr + nzc + 1] = (double)g;
+        host[cstride + ocorr + nzc] = (double)(-g * k0);  host[cstride + ocorr + nzc + 1] = (double)g;
+        if (cn_doubles > 0) build_chunk_tables(A.data(), B.data(), C.data(), m, pl->helm_cn_P, pl->helm_cn_levels, host.data() + pl->helm_cn_off);
     }
 
     // upload into a table set that no in-flight solve reads and no captured graph refers to (a

@@ -29,7 +29,7 @@ namespace pz {
 
 namespace {
 
-constexpr int kTX = 16;        // columns per tile
+constexpr int kTX = 16;        // columns per tile (32 in the wide variant: 256-byte rows)
 constexpr int kMaxFields = 4;  // fields per launch
 
 struct HelmArgs {
@@ -42,6 +42,8 @@ struct HelmArgs {
     double a, w0, w1;
 };
 
+__host__ __device__ constexpr int nzp_of(int P, int M) { return P * M; }
+
 template <int M> struct Limits {
     static constexpr int kMaxThreads = 512;                // 8 column pairs x P <= 64 sub-domains
     static constexpr int kMinBlocks = (M >= 16) ? 1 : 2;   // m = 16: 2 x 16 doubles of d per thread
@@ -52,17 +54,20 @@ __device__ __forceinline__ void st2(double *p, double2 v) { *reinterpret_cast<do
 __device__ __forceinline__ void st2g(double *p, double2 v) { __stcs(reinterpret_cast<double2 *>(p), v); }
 
 // Shared-memory carve-up in doubles; host and device agree through these helpers.
-template <int M> struct Smem {
+template <int M, int TX = kTX, int ZS = 1> struct Smem {
+    static constexpr int kTX = TX;
     static constexpr int TS = M + 2; // table stride per sub-domain: even (16-byte pairs)
-    __host__ __device__ static int box_rows(int P) { return P * M <= 256 ? P * M : 256; }
-    __host__ __device__ static int nbox(int P) { return (P * M + box_rows(P) - 1) / box_rows(P); }
+    // as few boxes of at most 256 rows as cover the P M rows, all of one size (a multiple of 8 rows)
+    __host__ __device__ static int nbox(int P) { return (P * M + 255) / 256; }
+    __host__ __device__ static int box_rows(int P) { return (((P * M + nbox(P) - 1) / nbox(P)) + 7) & ~7; }
     __host__ __device__ static size_t tile(int P) { return (size_t)box_rows(P) * nbox(P) * kTX; }
     __host__ __device__ static size_t xch(int P) { return (size_t)2 * 2 * P * kTX; }
-    __host__ __device__ static size_t tab(int P) { return (size_t)5 * P * TS; }
+    __host__ __device__ static size_t tab(int P) { return (size_t)(ZS > 1 ? 6 : 5) * P * TS; }   // 6th table: z-split correction
     __host__ __device__ static size_t pcr(int P, int levels) { return (size_t)levels * 4 * P + 2 * P; }
+    __host__ __device__ static size_t zx() { return ZS > 1 ? (size_t)2 * 2 * TX : 0; } // z-split: [parity][own/peer][TX]
     __host__ __device__ static size_t bytes(int P, int levels, bool cn = false)
     {
-        return ((cn ? 2 : 1) * tile(P) + xch(P) + tab(P) + pcr(P, levels)) * sizeof(double) + 16;
+        return ((cn ? 2 : 1) * tile(P) + xch(P) + tab(P) + pcr(P, levels) + zx()) * sizeof(double) + 16;
     }
 };
 
@@ -70,24 +75,35 @@ template <int M> struct Smem {
 // CN: the whole of Eq. (11), PAPER.md:76 -- a second tile holds u^k and the right-hand side
 // u** - a L_z u^k is formed in registers while the rows are copied out (the separate pass of
 // helmholtz_z_rhs and its 16 B/point round trip disappear); one CTA per SM.
-template <int M, bool FULL, int CN>
+// ZS = 2: the column is cut into two chunks of P sub-domains each, owned by the two CTAs of a
+// cluster (PAPER.md:120-135 with CTAs for MPI tasks): each solves its chunk with the couplings
+// across the cut removed (tables of that chunk), the two interface values cross through
+// distributed shared memory, and the reconstruction adds the precomputed k-only correction.
+template <int M, bool FULL, int CN, int TX = 16, int ZS = 1>
 __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M>::kMinBlocks)
-    helmholtz_tma_kernel(const __grid_constant__ HelmArgs args, const double *__restrict__ tab, size_t plane, int nz,
+    helmholtz_tma_kernel(const __grid_constant__ HelmArgs args, const double *__restrict__ tab_all, size_t plane, int nz,
                          int P, int levels, int tiles_per_field, int total_tiles, int probe, int box_rows, int nbox, int csz)
 {
+    static_assert(ZS == 1 || CN == 0, "the fused step kernel takes whole columns");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    using L = Smem<M>;
+    using L = Smem<M, TX, ZS>;
     constexpr int TS = L::TS;
+    constexpr int kTX = TX; // shadows the file-level default
     const int nzp = P * M, n2 = 2 * P;
     double *tile = reinterpret_cast<double *>(smem_raw);   // rows x 16
     double *qtile = tile + L::tile(P);                     // CN only: rows x 16 of u^k
     double *xch = qtile + (CN == 1 ? L::tile(P) : 0);           // [buffer][first/last][s][16]
     double *stab = xch + L::xch(P);                        // [table][s][TS]
     double *spcr = stab + L::tab(P);                       // [level][s][4], then [s][2]
-    uint64_t *bar = reinterpret_cast<uint64_t *>(spcr + L::pcr(P, levels));
+    double *zx = spcr + L::pcr(P, levels);                 // ZS = 2: interface values [parity][own / peer][TX]
+    uint64_t *bar = reinterpret_cast<uint64_t *>(zx + L::zx());
 
-    const int tid = threadIdx.x, c2 = 2 * (tid & 7), s = tid >> 3;
-    const int k0 = s * M;
+    const int tid = threadIdx.x, c2 = 2 * (tid % (TX / 2)), s = tid / (TX / 2);
+    // z-split: chunk of this CTA (rank in the cluster), its first global row and its table block
+    const int crank = (ZS > 1) ? (int)(blockIdx.x % ZS) : 0;
+    const int kc0 = crank * nzp_of(P, M);
+    const double *tab = tab_all + (size_t)crank * (6 * (size_t)P * M + L::pcr(P, levels) + 2);
+    const int k0 = s * M;                                  // row inside the chunk
     const unsigned tile_bytes = (unsigned)((CN == 1 ? 2 : 1) * L::tile(P) * sizeof(double));
 
     if (tid == 0) {
@@ -99,6 +115,13 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
         stab[(size_t)t * P * TS + (k / M) * TS + (k % M)] = tab[q];
     }
     for (int q = tid; q < (int)L::pcr(P, levels); q += blockDim.x) spcr[q] = tab[5 * (size_t)nzp + q];
+    double w_own = 0.0, w_peer = 0.0;
+    if constexpr (ZS > 1) {
+        const double *corr = tab + 5 * (size_t)nzp + L::pcr(P, levels);
+        for (int k = tid; k < nzp; k += blockDim.x) stab[(size_t)5 * P * TS + (k / M) * TS + (k % M)] = corr[k];
+        w_own = corr[nzp];
+        w_peer = corr[nzp + 1];
+    }
     __syncthreads();
 
     const uint64_t pol = l2_policy_evict_first(); // every tile is read once
@@ -111,20 +134,24 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
             return;
         }
         for (int b = 0; b < nbox; ++b)
-            tma_load_2d_hint(tile + (size_t)b * box_rows * kTX, &args.map[f], col0, b * box_rows, bar, pol);
+            tma_load_2d_hint(tile + (size_t)b * box_rows * kTX, &args.map[f], col0, kc0 + b * box_rows, bar, pol);
         if constexpr (CN == 1)
             for (int b = 0; b < nbox; ++b)
                 tma_load_2d_hint(qtile + (size_t)b * box_rows * kTX, &args.qmap, col0, b * box_rows, bar, pol);
     };
 
-    int t = blockIdx.x;
+    // tiles walk by CTA (ZS = 1) or by cluster (ZS = 2: both CTAs own the same columns)
+    const int tstep = (int)gridDim.x / ZS;
+    int t = (int)blockIdx.x / ZS;
     if (tid == 0 && t < total_tiles) fetch(t);
 
     const double *fA = stab + s * TS, *bC = fA + P * TS, *rb = bC + P * TS, *ra = rb + P * TS, *rc = ra + P * TS;
     const int sm1 = max(s - 1, 0), sp1 = min(s + 1, P - 1);
     unsigned phase = 0;
 
-    for (; t < total_tiles; t += gridDim.x) {
+    const double *rx = stab + (size_t)5 * P * TS + s * TS; // ZS = 2: correction per row
+    int zpar = 0;
+    for (; t < total_tiles; t += tstep) {
         double da[M], db[M]; // the two columns
         mbar_wait(bar, phase);
         phase ^= 1;
@@ -173,19 +200,19 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
         // every thread holds its rows: the buffer is free again.  With a cluster (csz > 1) the
         // CTAs of the cluster, which own neighbouring tiles, also meet here, so that their next
         // fetches (and their stores) reach DRAM together as 128*csz contiguous bytes per row.
-        if (csz > 1) {
+        if (csz > 1 && ZS == 1) {
             asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
         } else {
             __syncthreads();
         }
-        if (tid == 0 && t + (int)gridDim.x < total_tiles) fetch(t + gridDim.x);
+        if (tid == 0 && t + tstep < total_tiles) fetch(t + tstep);
 
         if (kProbes && probe == 2) { // diagnostic: pipeline skeleton only (load, store)
             const int f = t / tiles_per_field;
-            double *up = args.u[f] + (size_t)(t - f * tiles_per_field) * kTX + c2 + (size_t)k0 * plane;
+            double *up = args.u[f] + (size_t)(t - f * tiles_per_field) * kTX + c2 + (size_t)(kc0 + k0) * plane;
 #pragma unroll
             for (int i = 0; i < M; ++i)
-                if (FULL || k0 + i < nz) st2g(up + (size_t)i * plane, make_double2(da[i], db[i]));
+                if (FULL || kc0 + k0 + i < nz) st2g(up + (size_t)i * plane, make_double2(da[i], db[i]));
             continue;
         }
         // Step 2: runtime reduction, d only (forward i = 2..M-1, backward i = M-3..0)
@@ -242,10 +269,29 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
             x1.x *= rbr.y; x1.y *= rbr.y;
         }
 
+        // z-split: x0 / x1 are the chunk-local solution y at the sub-domain ends.  The chunk's
+        // interface value (last row of chunk 0, first row of chunk 1) goes to both CTAs; the value
+        // of the neighbouring chunk's interface row follows from the precomputed 2 x 2 system.
+        double2 X = make_double2(0.0, 0.0);
+        if constexpr (ZS > 1) {
+            double *slot = zx + (size_t)zpar * 2 * TX;
+            if ((crank == 0 && s == P - 1) || (crank == 1 && s == 0)) {
+                const double2 mine = (crank == 0) ? x1 : x0;
+                st2(slot + c2, mine);
+                unsigned remote;
+                asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(slot + TX + c2)), "r"(crank ^ 1));
+                asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(remote), "d"(mine.x), "d"(mine.y) : "memory");
+            }
+            asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+            const double2 own = ld2(slot + c2), peer = ld2(slot + TX + c2);
+            X = make_double2(fma(w_own, own.x, w_peer * peer.x), fma(w_own, own.y, w_peer * peer.y));
+            zpar ^= 1;
+        }
+
         // Step 4: reconstruct and store
         if (kProbes && (probe == 1 || probe == 3) && x0.x != 1.2345e300) continue; // diagnostic: no stores
         const int f = t / tiles_per_field;
-        double *up = args.u[f] + (size_t)(t - f * tiles_per_field) * kTX + c2 + (size_t)k0 * plane;
+        double *up = args.u[f] + (size_t)(t - f * tiles_per_field) * kTX + c2 + (size_t)(kc0 + k0) * plane;
 #pragma unroll
         for (int i = 0; i < M; i += 2) {
             const double2 qb = ld2(rb + i), qa = ld2(ra + i), qc = ld2(rc + i);
@@ -262,38 +308,46 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
                 w.x = fma(-qc.y, x1.x, fma(-qa.y, x0.x, qb.y * da[i + 1]));
                 w.y = fma(-qc.y, x1.y, fma(-qa.y, x0.y, qb.y * db[i + 1]));
             }
-            if (FULL || k0 + i < nz) st2g(up + (size_t)i * plane, v);
-            if (FULL || k0 + i + 1 < nz) st2g(up + (size_t)(i + 1) * plane, w);
+            if constexpr (ZS > 1) {
+                const double2 cr = ld2(rx + i);
+                v.x = fma(-cr.x, X.x, v.x); v.y = fma(-cr.x, X.y, v.y);
+                w.x = fma(-cr.y, X.x, w.x); w.y = fma(-cr.y, X.y, w.y);
+            }
+            if (FULL || kc0 + k0 + i < nz) st2g(up + (size_t)i * plane, v);
+            if (FULL || kc0 + k0 + i + 1 < nz) st2g(up + (size_t)(i + 1) * plane, w);
         }
     }
+    // no CTA of the cluster leaves while its peer may still write into its shared memory
+    if constexpr (ZS > 1) asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
-template <int M, bool FULL>
+template <int M, bool FULL, int TX = kTX, int ZS = 1>
 int prepare_mf(pz_plan *pl)
 {
-    const size_t smem = Smem<M>::bytes(pl->helm_P, pl->helm_levels);
-    auto kern = helmholtz_tma_kernel<M, FULL, 0>;
+    const size_t smem = Smem<M, TX, ZS>::bytes(pl->helm_P, pl->helm_levels);
+    auto kern = helmholtz_tma_kernel<M, FULL, 0, TX, ZS>;
     if (smem > 227 * 1024) { set_error("helmholtz (TMA variant): tile of %zu bytes does not fit shared memory", smem); return PZ_EUNSUPPORTED; }
     {
         const int rc = smem_optin(pl, kern, 227 * 1024);
         if (rc != PZ_OK) return rc;
     }
     int bps = 0;
-    PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, (kTX / 2) * pl->helm_P, smem));
+    PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, (TX / 2) * pl->helm_P, smem));
     if (bps < 1) { set_error("helmholtz (TMA variant): kernel does not fit an SM"); return PZ_ECUDA; }
     pl->helm_bps = bps;
     pl->helm_nclusters[0] = pl->helm_nclusters[1] = pl->helm_nclusters[2] = 0;
     return PZ_OK;
 }
 
-template <int M, bool FULL>
+template <int M, bool FULL, int TX = kTX, int ZS = 1>
 int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStream_t st)
 {
+    constexpr int kTX = TX; // shadows the file-level default
     const int P = pl->helm_P;
     const size_t plane = (size_t)pl->nx * pl->ny;
-    const size_t smem = Smem<M>::bytes(P, pl->helm_levels);
-    const bool wide = (pl->opt.helm_probe == 3) && (P * M) % 512 == 0;
-    int box_rows = Smem<M>::box_rows(P), nbox = Smem<M>::nbox(P);
+    const size_t smem = Smem<M, TX, ZS>::bytes(P, pl->helm_levels);
+    const bool wide = (pl->opt.helm_probe == 3) && (P * M) % 512 == 0 && TX == 16;
+    int box_rows = Smem<M, TX>::box_rows(P), nbox = Smem<M, TX>::nbox(P);
     if (pl->opt.helm_box_rows > 0 && (P * M) % pl->opt.helm_box_rows == 0 && pl->opt.helm_box_rows <= 256) {
         box_rows = pl->opt.helm_box_rows;
         nbox = P * M / box_rows;
@@ -311,7 +365,7 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
     const int tiles_per_field = (int)(plane / kTX);
     const long long total = (long long)tiles_per_field * n;
     long long blocks = (long long)pl->num_sms * pl->helm_bps;
-    if (blocks > total) blocks = total;
+    if (blocks > total * ZS) blocks = total * ZS;
     // CTAs of a cluster own neighbouring tiles and meet once per tile, so their fetches and stores
     // reach DRAM together (256 contiguous bytes per row for a pair).  Measured (profiles/r01c):
     // +15-20 % with m = 16, a loss with the smaller sub-domains (two or more CTAs per SM).
@@ -319,6 +373,7 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
     if (csz == 0) csz = (M == 16) ? 2 : 1;
     if (csz != 2 && csz != 4 && csz != 8) csz = 1;
     while (csz > 1 && (tiles_per_field % csz != 0 || blocks < csz)) csz /= 2;
+    if (ZS > 1) csz = ZS; // the cluster is the pair of chunks of one tile
     const int probe = wide ? 3 : (pl->opt.helm_probe == 3 ? 1 : pl->opt.helm_probe);
     cudaLaunchConfig_t cfg = {};
     cfg.blockDim = dim3((kTX / 2) * P);
@@ -336,7 +391,7 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
         if (pl->helm_nclusters[csz == 2 ? 0 : csz == 4 ? 1 : 2] == 0) {
             cfg.gridDim = dim3((unsigned)((long long)pl->num_sms * pl->helm_bps / csz * csz));
             int nclusters = 0;
-            PZ_CUDA(cudaOccupancyMaxActiveClusters(&nclusters, helmholtz_tma_kernel<M, FULL, 0>, &cfg));
+            PZ_CUDA(cudaOccupancyMaxActiveClusters(&nclusters, helmholtz_tma_kernel<M, FULL, 0, TX, ZS>, &cfg));
             if (nclusters < 1) { set_error("helmholtz (TMA variant): no cluster of %d CTAs fits", csz); return PZ_ECUDA; }
             pl->helm_nclusters[csz == 2 ? 0 : csz == 4 ? 1 : 2] = nclusters;
         }
@@ -345,7 +400,7 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
     }
     blocks = blocks / csz * csz;
     cfg.gridDim = dim3((unsigned)blocks);
-    PZ_CUDA(cudaLaunchKernelEx(&cfg, helmholtz_tma_kernel<M, FULL, 0>, args, tab, plane, pl->nz, P, pl->helm_levels,
+    PZ_CUDA(cudaLaunchKernelEx(&cfg, helmholtz_tma_kernel<M, FULL, 0, TX, ZS>, args, tab, plane, pl->nz, P, pl->helm_levels,
                                tiles_per_field, (int)total, probe, box_rows, nbox, csz));
     count_launch();
     PZ_CUDA(cudaGetLastError());
@@ -357,9 +412,9 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
 template <int M, bool FULL, int CN>
 int launch_cn_mfc(pz_plan *pl, double *u2, const double *uk, const double *tab, cudaStream_t st)
 {
-    const int P = pl->helm_P;
+    const int P = pl->helm_cn_P;
     const size_t plane = (size_t)pl->nx * pl->ny;
-    const size_t smem = Smem<M>::bytes(P, pl->helm_levels, CN == 1);
+    const size_t smem = Smem<M>::bytes(P, pl->helm_cn_levels, CN == 1);
     auto kern = helmholtz_tma_kernel<M, FULL, CN>;
     int rc = smem_optin(pl, kern, 227 * 1024);
     if (rc != PZ_OK) return rc;
@@ -375,7 +430,7 @@ int launch_cn_mfc(pz_plan *pl, double *u2, const double *uk, const double *tab, 
     args.A = pl->d_A; args.C = pl->d_C; args.a = pl->helm_a; args.w0 = pl->wall_w0; args.w1 = pl->wall_w1;
     const int tiles = (int)(plane / kTX);
     int blocks = pl->num_sms < tiles ? pl->num_sms : tiles;
-    kern<<<blocks, (kTX / 2) * P, smem, st>>>(args, tab, plane, pl->nz, P, pl->helm_levels, tiles, tiles, 0, box_rows, nbox, 1);
+    kern<<<blocks, (kTX / 2) * P, smem, st>>>(args, tab + pl->helm_cn_off, plane, pl->nz, P, pl->helm_cn_levels, tiles, tiles, 0, box_rows, nbox, 1);
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
@@ -386,9 +441,9 @@ int launch_cn_mfc(pz_plan *pl, double *u2, const double *uk, const double *tab, 
 template <int M, bool FULL>
 int launch_cn_mf(pz_plan *pl, double *u2, const double *uk, const double *tab, cudaStream_t st)
 {
-    if (Smem<M>::bytes(pl->helm_P, pl->helm_levels, true) <= 227 * 1024 && pl->opt.step_fused != 2)
+    if (Smem<M>::bytes(pl->helm_cn_P, pl->helm_cn_levels, true) <= 227 * 1024 && pl->opt.step_fused != 2)
         return launch_cn_mfc<M, FULL, 1>(pl, u2, uk, tab, st);
-    if (Smem<M>::bytes(pl->helm_P, pl->helm_levels, false) > 227 * 1024) return PZ_EUNSUPPORTED;
+    if (Smem<M>::bytes(pl->helm_cn_P, pl->helm_cn_levels, false) > 227 * 1024) return PZ_EUNSUPPORTED;
     return launch_cn_mfc<M, FULL, 2>(pl, u2, uk, tab, st);
 }
 
@@ -396,7 +451,8 @@ int launch_cn_mf(pz_plan *pl, double *u2, const double *uk, const double *tab, c
 
 int launch_helmholtz_tma_cn(pz_plan *pl, double *u2, const double *uk, const double *tab, cudaStream_t st)
 {
-    const bool full = (pl->helm_P * pl->helm_m == pl->nz);
+    if (pl->helm_cn_P <= 0) return PZ_EUNSUPPORTED; // no whole-column tables (nz > 1024): the caller runs the right-hand side as its own pass
+    const bool full = (pl->helm_cn_P * pl->helm_m == pl->nz);
 #define PZ_HC(MM) (full ? launch_cn_mf<MM, true>(pl, u2, uk, tab, st) : launch_cn_mf<MM, false>(pl, u2, uk, tab, st))
     switch (pl->helm_m) {
     case 4: return PZ_HC(4);
@@ -410,12 +466,16 @@ int launch_helmholtz_tma_cn(pz_plan *pl, double *u2, const double *uk, const dou
 // Called when the launch geometry (m, P) changes: shared-memory opt-in and resident CTAs per SM.
 int helmholtz_tma_prepare(pz_plan *pl)
 {
-    const bool full = (pl->helm_P * pl->helm_m == pl->nz);
+    const bool full = (pl->helm_zs * pl->helm_P * pl->helm_m == pl->nz);
 #define PZ_HP(MM) (full ? prepare_mf<MM, true>(pl) : prepare_mf<MM, false>(pl))
     switch (pl->helm_m) {
     case 4: return PZ_HP(4);
     case 8: return PZ_HP(8);
-    case 16: return PZ_HP(16);
+    case 16:
+        if (pl->helm_zs == 2 && pl->helm_tx == 32) return full ? prepare_mf<16, true, 32, 2>(pl) : prepare_mf<16, false, 32, 2>(pl);
+        if (pl->helm_zs == 2) return full ? prepare_mf<16, true, 16, 2>(pl) : prepare_mf<16, false, 16, 2>(pl);
+        if (pl->helm_tx == 32) return full ? prepare_mf<16, true, 32>(pl) : prepare_mf<16, false, 32>(pl);
+        return PZ_HP(16);
     default: set_error("helmholtz: bad sub-domain size %d", pl->helm_m); return PZ_EINVAL;
     }
 #undef PZ_HP
@@ -428,12 +488,16 @@ int launch_helmholtz_tma(pz_plan *pl, double *const *u, int n, const double *tab
     if (n < 1 || n > kMaxFields) { set_error("helmholtz (TMA variant): 1..4 fields per launch"); return PZ_EINVAL; }
     for (int f = 0; f < n; ++f)
         if (((uintptr_t)u[f] & 15) != 0) { set_error("helmholtz_z_solve: u must be 16-byte aligned"); return PZ_EINVAL; }
-    const bool full = (pl->helm_P * pl->helm_m == pl->nz);
+    const bool full = (pl->helm_zs * pl->helm_P * pl->helm_m == pl->nz);
 #define PZ_HT(MM) (full ? launch_mf<MM, true>(pl, u, n, tab, st) : launch_mf<MM, false>(pl, u, n, tab, st))
     switch (pl->helm_m) {
     case 4: return PZ_HT(4);
     case 8: return PZ_HT(8);
-    case 16: return PZ_HT(16);
+    case 16:
+        if (pl->helm_zs == 2 && pl->helm_tx == 32) return full ? launch_mf<16, true, 32, 2>(pl, u, n, tab, st) : launch_mf<16, false, 32, 2>(pl, u, n, tab, st);
+        if (pl->helm_zs == 2) return full ? launch_mf<16, true, 16, 2>(pl, u, n, tab, st) : launch_mf<16, false, 16, 2>(pl, u, n, tab, st);
+        if (pl->helm_tx == 32) return full ? launch_mf<16, true, 32>(pl, u, n, tab, st) : launch_mf<16, false, 32>(pl, u, n, tab, st);
+        return PZ_HT(16);
     default: set_error("helmholtz: bad sub-domain size %d", pl->helm_m); return PZ_EINVAL;
     }
 #undef PZ_HT

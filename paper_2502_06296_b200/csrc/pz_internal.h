@@ -47,6 +47,7 @@ struct Options {
     int helm_probe = 0;       // diagnostic (variant 1): 1 = no stores, 2 = no arithmetic (results are wrong)
     int helm_tx = 0;          // 0 = auto: columns per CTA in the Helmholtz kernel (variant 0)
     int helm_m = 0;           // 0 = auto: rows per sub-domain in the Helmholtz kernel
+    int helm_zsplit = 0;      // 0 = auto: 1 = whole columns per CTA, 2 = column cut over the two CTAs of a cluster
     int fft_y_p0 = 1;         // 1 = pair-0 conversion inside the y-FFT kernel, 0 = separate small kernel
     int step_fused = 1;       // helmholtz_z_step: 1 = right-hand side of Eq. (11) formed inside the solve kernel
     int div_fused = 1;        // pz_pressure_correction: 1 = divergence formed inside the forward x transform
@@ -92,7 +93,10 @@ struct pz_plan {
     double helm_a = -1.0;
     int helm_m = 0, helm_P = 0, helm_tx = 0, helm_levels = 0;
     int helm_variant = 0;            // variant the current tables were built for
+    int helm_zs = 1;                 // variant 1: chunks the column is cut into (CTAs of a cluster), helm_P = sub-domains per chunk
     int helm_bps = 0;                // variant 1: resident CTAs per SM
+    int helm_cn_P = 0, helm_cn_levels = 0; // whole-column tables for the one-kernel step of Eq. (11) (0 = none)
+    size_t helm_cn_off = 0;          // their offset (doubles) in a table set
     int helm_nclusters[3] = {0, 0, 0}; // variant 1: resident clusters of 2 / 4 / 8 CTAs (0 = not yet queried)
     std::vector<pz::HelmTables> helm; // table sets: the current one, one being uploaded, and any a captured graph reads
     int helm_cur = -1;

@@ -294,6 +294,15 @@ HELM_CASES = [
     (8, 8, 64, 0.0, 0.0, []),            # a = 0: identity
     (8, 8, 64, 1.8, 10.0, []),           # strongly implicit
     (256, 128, 300, 1.8, 5e-5, []),      # 2048 tiles of 16 columns: several per resident CTA; 2 TMA boxes
+    (64, 32, 513, 1.8, 5e-5, []),        # column cut over the two CTAs of a cluster; padding rows in the second chunk
+    (64, 32, 700, 2.0, 5e-5, []),
+    (64, 32, 1024, 1.8, 2.5e-5, []),     # cut column, 32-column tiles, no padding
+    (64, 32, 1024, 1.8, 2.5e-5, [("helm_zsplit", 1)]),   # whole columns per CTA
+    (8, 8, 1024, 1.8, 10.0, []),         # strongly implicit across the cut
+    (12, 12, 600, 1.8, 5e-5, []),        # cut column, 16-column tiles (144 columns)
+    (64, 32, 1594, 1.8, 2.5e-5, []),     # the paper's nz on the pipeline: 50 sub-domains per chunk
+    (16, 8, 1920, 1.8, 2.5e-5, []),      # largest nz of the pipeline
+    (16, 8, 2048, 1.8, 2.5e-5, []),      # beyond: register-tile kernel
     (128, 64, 48, 1.8, 5e-5, []),
 ]
 
@@ -311,7 +320,8 @@ def test_helmholtz_matches_oracle(torch, pz, wl, oracle, nx, ny, nz, beta, a, op
     for k, v in options:
         pz.pz_set_option(plan, k, v)
     pz.helmholtz_z_setup(plan, a)
-    assert pz.pz_get_option(plan, "helm_variant_actual") == (variant if nz <= 1024 else 0)
+    whole = ("helm_zsplit", 1) in options
+    assert pz.pz_get_option(plan, "helm_variant_actual") == (variant if nz <= (1024 if whole else 1920) else 0)
     u = torch.from_numpy(r).cuda()
     pz.helmholtz_z_solve(plan, u)
     torch.cuda.synchronize()
