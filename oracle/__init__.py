@@ -27,6 +27,8 @@ from .cpu import (  # noqa: F401
     poisson_solve,
     helmholtz_z_solve,
     helmholtz_z_solve_columns,
+    helmholtz_w_matrix,
+    helmholtz_w_solve,
     apply_helmholtz3d_operator,
     helmholtz3d_solve,
 )

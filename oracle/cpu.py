@@ -178,6 +178,28 @@ def helmholtz_z_solve(zc, zf, a: float, r: np.ndarray) -> np.ndarray:
     return u
 
 
+def helmholtz_w_matrix(zc, zf, a: float):
+    """(lo, di, up) of I - a L_z^w for the face-centred wall-normal velocity (reading R16)."""
+    zc, zf = _c(zc), _c(zf)
+    nz = zc.size
+    lo, di, up = np.empty(nz), np.empty(nz), np.empty(nz)
+    lib().orc_helmholtz_w_matrix(ctypes.c_int(nz), _p(zc), _p(zf), ctypes.c_double(a), _p(lo), _p(di), _p(up))
+    return lo, di, up
+
+
+def helmholtz_w_solve(zc, zf, a: float, r: np.ndarray) -> np.ndarray:
+    """r[nz][ny][nx] -> w on the z faces zf[1..nz] (w[nz-1] = the top wall face, unchanged)."""
+    r = _c(r)
+    nz, ny, nx = r.shape
+    zc, zf = _c(zc), _c(zf)
+    w = np.empty_like(r)
+    rc = lib().orc_helmholtz_w_solve(ctypes.c_int(nx), ctypes.c_int(ny), ctypes.c_int(nz),
+                                     _p(zc), _p(zf), ctypes.c_double(a), _p(r), _p(w))
+    if rc != 0:
+        raise MemoryError("orc_helmholtz_w_solve: allocation failed")
+    return w
+
+
 def helmholtz_z_solve_columns(zc, zf, a: float, rcols: np.ndarray) -> np.ndarray:
     """rcols[ncols][nz] -> ucols; the same column solve on sampled columns only."""
     rcols = _c(rcols)

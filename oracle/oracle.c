@@ -401,6 +401,52 @@ int orc_helmholtz_z_solve_columns(int nz, const double *zc, const double *zf, do
     return 0;
 }
 
+/* --------------------------- wall-normal diffusion of the FACE-centred component w */
+
+/* Matrix of (I - a L_z^w) for the wall-normal velocity, which lives on the z FACES of the
+ * staggered grid ("staggered ... grid"; reading R16): w_k on the face
+ * zf[k+1], k = 0..nz-1; the bottom wall face zf[0] carries w = 0 and is not stored, the top
+ * wall face is k = nz-1 and keeps its value (identity row).  For k = 0..nz-2
+ *   (L_z^w w)_k = [ (w_{k+1} - w_k)/dzf_{k+1} - (w_k - w_{k-1})/dzf_k ] / dzc_k,
+ * the second difference of the face values across the two neighbouring cells, with
+ * w_{-1} = 0 and w_{nz-1} = 0 (the walls):
+ *   lo_k = -a Aw_k,  up_k = -a Cw_k,  di_k = 1 + a (1/(dzc_k dzf_k) + 1/(dzc_k dzf_{k+1})),
+ *   Aw_k = 1/(dzc_k dzf_k) (k >= 1, else 0),  Cw_k = 1/(dzc_k dzf_{k+1}) (k <= nz-3, else 0). */
+void orc_helmholtz_w_matrix(int nz, const double *zc, const double *zf, double a,
+                            double *lo, double *di, double *up)
+{
+    for (int k = 0; k < nz; ++k) {
+        if (k == nz - 1) { lo[k] = 0.0; up[k] = 0.0; di[k] = 1.0; continue; }
+        const double dzc = zc[k + 1] - zc[k];
+        const double dzm = zf[k + 1] - zf[k], dzp = zf[k + 2] - zf[k + 1];
+        const double Aw = 1.0 / (dzc * dzm), Cw = 1.0 / (dzc * dzp);
+        lo[k] = (k >= 1) ? -a * Aw : 0.0;
+        up[k] = (k <= nz - 3) ? -a * Cw : 0.0;
+        di[k] = 1.0 + a * (Aw + Cw);
+    }
+}
+
+/* r[N] -> w[N]: one plain Thomas solve per (i,j) column (Eq. 11 for the third component). */
+int orc_helmholtz_w_solve(int nx, int ny, int nz, const double *zc, const double *zf,
+                          double a, const double *r, double *w)
+{
+    const size_t plane = (size_t)nx * ny;
+    double *m = (double *)malloc(sizeof(double) * 3 * (size_t)nz);
+    if (!m) return 1;
+    double *lo = m, *di = m + nz, *up = m + 2 * nz;
+    orc_helmholtz_w_matrix(nz, zc, zf, a, lo, di, up);
+#pragma omp parallel
+    {
+        double *work = (double *)malloc(sizeof(double) * 2 * (size_t)nz);
+#pragma omp for schedule(static)
+        for (long long c = 0; c < (long long)plane; ++c)
+            orc_thomas(nz, lo, di, up, r + c, w + c, plane, work);
+        free(work);
+    }
+    free(m);
+    return 0;
+}
+
 /* ------------------------------------------- fully implicit diffusion, Eq. (8) */
 
 /* u -> (I - a L_h) u with periodic x, y and Dirichlet walls in z (definition O-H3):
