@@ -137,6 +137,19 @@ PZ_API int helmholtz_z_solve(pz_plan *plan, double *u, void *stream);
 PZ_API int helmholtz_z_solve_n(pz_plan *plan, double *const *u, int n, void *stream);
 
 /*
+ * The same solve for the wall-normal velocity component w, which lives on the z FACES of the
+ * staggered grid: w[k] on the face zf[k+1], k = 0..nz-1; the bottom wall face zf[0]
+ * carries w = 0 and is not stored, the top wall face is row nz-1 and keeps its value.  For
+ * k = 0..nz-2 (w_{-1} = w_{nz-1} = 0 in the operator):
+ *   w_k - a [ (w_{k+1} - w_k)/dzf_{k+1} - (w_k - w_{k-1})/dzf_k ] / dzc_k = r_k.
+ * Its coefficient tables are independent of those of helmholtz_z_setup: a time step sets up both
+ * and solves u, v with helmholtz_z_solve_n and w with helmholtz_w_solve.  Same kernels, same
+ * CUDA-graph rules.  Errors as helmholtz_z_setup / helmholtz_z_solve.
+ */
+PZ_API int helmholtz_w_setup(pz_plan *plan, double a);
+PZ_API int helmholtz_w_solve(pz_plan *plan, double *w, void *stream);
+
+/*
  * The whole of Eq. (11):  u* - a L_z u* = u** - a L_z u^k  with the a of the last
  * helmholtz_z_setup.  helmholtz_z_rhs overwrites ustar2 (on entry u**) with the right-hand side
  * u** - a L_z u^k, L_z the operator above; helmholtz_z_step does that and then helmholtz_z_solve:

@@ -33,6 +33,8 @@ SIGNATURES = {
     "poisson_solve_reduce": (_i, [_vp, _vp, _vp, _vp]),
     "poisson_solve_finish": (_i, [_vp, _vp, _vp, _vp]),
     "helmholtz_z_setup": (_i, [_vp, _d]),
+    "helmholtz_w_setup": (_i, [_vp, _d]),
+    "helmholtz_w_solve": (_i, [_vp, _vp, _vp]),
     "helmholtz_z_solve": (_i, [_vp, _vp, _vp]),
     "helmholtz_z_solve_n": (_i, [_vp, ctypes.POINTER(_vp), _i, _vp]),
     "poisson_solve_host": (_i, [_vp, _vp, _vp]),
@@ -197,6 +199,14 @@ def helmholtz_z_solve(plan: Plan, u, stream=None) -> None:
 def helmholtz_z_solve_n(plan: Plan, fields, stream=None) -> None:
     ptrs = (_vp * len(fields))(*[_dev_ptr(u, plan.n) for u in fields])
     _check(lib().helmholtz_z_solve_n(plan.handle, ptrs, len(fields), _stream_ptr(stream)))
+
+
+def helmholtz_w_setup(plan: Plan, a: float) -> None:
+    _check(lib().helmholtz_w_setup(plan.handle, float(a)))
+
+
+def helmholtz_w_solve(plan: Plan, w, stream=None) -> None:
+    _check(lib().helmholtz_w_solve(plan.handle, _dev_ptr(w, plan.n), _stream_ptr(stream)))
 
 
 def poisson_solve_host(plan: Plan, p_host, stream=None) -> None:

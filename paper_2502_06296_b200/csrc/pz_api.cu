@@ -515,6 +515,22 @@ int helmholtz_z_setup(pz_plan *pl, double a)
     return helmholtz_build_tables(pl, a);
 }
 
+int helmholtz_w_setup(pz_plan *pl, double a)
+{
+    if (!pl) { set_error("helmholtz_w_setup: plan is NULL"); return PZ_EINVAL; }
+    if (!(a >= 0.0) || !std::isfinite(a)) { set_error("helmholtz_w_setup: a must be finite and >= 0"); return PZ_EINVAL; }
+    if (pl->slab_G > 0) { set_error("helmholtz_w_setup: not available on a z-slab plan (columns are cut; shard Helmholtz solves in y)"); return PZ_EUNSUPPORTED; }
+    return helmholtz_build_tables(pl, a, 1);
+}
+
+int helmholtz_w_solve(pz_plan *pl, double *w, void *stream)
+{
+    if (!pl || !w) { set_error("helmholtz_w_solve: NULL argument"); return PZ_EINVAL; }
+    if (pl->helm_w_cur < 0) { set_error("helmholtz_w_solve: call helmholtz_w_setup first"); return PZ_ENOTSETUP; }
+    double *one[1] = {w};
+    return launch_helmholtz_n(pl, one, 1, (cudaStream_t)stream, 1);
+}
+
 int helmholtz_z_solve(pz_plan *pl, double *u, void *stream)
 {
     if (!pl || !u) { set_error("helmholtz_z_solve: NULL argument"); return PZ_EINVAL; }
@@ -681,8 +697,13 @@ int pz_set_option(pz_plan *pl, const char *key, int value)
         return PZ_EUNSUPPORTED;
     }
     *slot = value;
-    if ((slot == &pl->opt.helm_tx || slot == &pl->opt.helm_m || slot == &pl->opt.helm_variant || slot == &pl->opt.helm_zsplit) && pl->helm_cur >= 0)
-        return helmholtz_build_tables(pl, pl->helm_a); // geometry changed: rebuild the tables
+    if (slot == &pl->opt.helm_tx || slot == &pl->opt.helm_m || slot == &pl->opt.helm_variant || slot == &pl->opt.helm_zsplit) {
+        // geometry changed: rebuild the tables
+        int rc = PZ_OK;
+        if (pl->helm_cur >= 0) rc = helmholtz_build_tables(pl, pl->helm_a, 0);
+        if (rc == PZ_OK && pl->helm_w_cur >= 0) rc = helmholtz_build_tables(pl, pl->helm_w_a, 1);
+        return rc;
+    }
     return PZ_OK;
 }
 

@@ -246,7 +246,7 @@ void unit_response(const ld *A, const ld *B, const ld *C, int n, int j, std::vec
 static size_t chunk_doubles(int nzc, int P, int LV) { return 6 * (size_t)nzc + (size_t)LV * 4 * P + 2 * P + 2; }
 
 // Algorithm 2 Step 1 on the host, plus the precomputed PCR of the boundary system.
-int helmholtz_build_tables(pz_plan *pl, double a)
+int helmholtz_build_tables(pz_plan *pl, double a, int kind)
 {
     helm_geometry(pl);
     const int nz = pl->nz, m = pl->helm_m, P = pl->helm_P, ZS = pl->helm_zs, nzc = P * m, LV = pl->helm_levels;
@@ -278,13 +278,22 @@ int helmholtz_build_tables(pz_plan *pl, double a)
     // matrix of I - a L_z with Dirichlet walls, padded with identity rows
     const int nzw = (cn_doubles > 0 && pl->helm_cn_P * m > nzp) ? pl->helm_cn_P * m : nzp;
     std::vector<ld> A(nzw, 0), B(nzw, 1), C(nzw, 0);
-    for (int k = 0; k < nz; ++k) {
+    for (int k = 0; k < nz && kind == 0; ++k) {
         ld W = 0;
         if (k == 0) W += (ld)2 / ((ld)pl->dzf[0] * ((ld)2 * ((ld)pl->zc[0] - (ld)pl->zf[0])));
         if (k == nz - 1) W += (ld)2 / ((ld)pl->dzf[nz - 1] * ((ld)2 * ((ld)pl->zf[nz] - (ld)pl->zc[nz - 1])));
         A[k] = -(ld)a * (ld)pl->A[k];
         C[k] = -(ld)a * (ld)pl->C[k];
         B[k] = (ld)1 + (ld)a * ((ld)pl->A[k] + (ld)pl->C[k] + W);
+    }
+    // kind 1: the face-centred component w (w_k on the face zf[k+1]; both wall faces 0, the top one
+    // is row nz-1 and keeps its value): second difference of the face values,
+    //   (L w)_k = [ (w_{k+1} - w_k)/dzf_{k+1} - (w_k - w_{k-1})/dzf_k ] / dzc_k   (reading R16)
+    for (int k = 0; k + 1 < nz && kind == 1; ++k) {
+        const ld Aw = (ld)1 / ((ld)pl->dzc[k] * (ld)pl->dzf[k]), Cw = (ld)1 / ((ld)pl->dzc[k] * (ld)pl->dzf[k + 1]);
+        A[k] = (k >= 1) ? -(ld)a * Aw : (ld)0;
+        C[k] = (k <= nz - 3) ? -(ld)a * Cw : (ld)0;
+        B[k] = (ld)1 + (ld)a * (Aw + Cw);
     }
     std::vector<double> host(ndbl, 0.0);
     if (ZS == 1) {
@@ -324,7 +333,7 @@ int helmholtz_build_tables(pz_plan *pl, double a)
     // keep solving with the coefficient of capture time -- across any number of later set-ups)
     int nb = -1;
     for (int i = 0; i < (int)pl->helm.size(); ++i)
-        if (i != pl->helm_cur && !pl->helm[i].captured) { nb = i; break; }
+        if (i != pl->helm_cur && i != pl->helm_w_cur && !pl->helm[i].captured) { nb = i; break; }
     if (nb < 0) {
         HelmTables fresh;
         PZ_CUDA(cudaEventCreateWithFlags(&fresh.uploaded, cudaEventDisableTiming));
@@ -355,8 +364,8 @@ int helmholtz_build_tables(pz_plan *pl, double a)
     PZ_CUDA(cudaEventRecord(t.uploaded, pl->upload_stream));
     t.upload_seen = false;
     t.used = true;
-    pl->helm_cur = nb;
-    pl->helm_a = a;
+    if (kind == 1) { pl->helm_w_cur = nb; pl->helm_w_a = a; }
+    else { pl->helm_cur = nb; pl->helm_a = a; }
     return PZ_OK;
 }
 
@@ -412,10 +421,10 @@ int launch_helmholtz_step(pz_plan *pl, double *u2, const double *uk, cudaStream_
     return rc;
 }
 
-int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st)
+int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st, int kind)
 {
     if (n == 0) return PZ_OK;
-    HelmTables &t = pl->helm[pl->helm_cur];
+    HelmTables &t = pl->helm[kind == 1 ? pl->helm_w_cur : pl->helm_cur];
     bool capturing = false;
     {
         const int rc0 = order_after_upload(t, st, &capturing);

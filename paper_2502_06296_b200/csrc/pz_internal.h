@@ -99,7 +99,9 @@ struct pz_plan {
     size_t helm_cn_off = 0;          // their offset (doubles) in a table set
     int helm_nclusters[3] = {0, 0, 0}; // variant 1: resident clusters of 2 / 4 / 8 CTAs (0 = not yet queried)
     std::vector<pz::HelmTables> helm; // table sets: the current one, one being uploaded, and any a captured graph reads
-    int helm_cur = -1;
+    int helm_cur = -1;               // current set of the cell-centred operator (u, v)
+    int helm_w_cur = -1;             // current set of the face-centred operator (w), helmholtz_w_setup
+    double helm_w_a = -1.0;
     cudaStream_t upload_stream = nullptr;
 
     // z-slab of a distributed Poisson solve (poisson_slab_plan_create): nz above is the slab's own
@@ -187,12 +189,12 @@ int launch_fft_xy_inv(pz_plan *pl, double *p, cudaStream_t st);
 int launch_slab_coefficients(pz_plan *pl, cudaStream_t st);
 int launch_slab_reduce(pz_plan *pl, const double *p, double *bout, cudaStream_t st);
 int launch_slab_finish(pz_plan *pl, double *p, const double *ball, cudaStream_t st);
-int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st);
+int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st, int kind = 0); // kind 1: face-centred w
 int launch_helmholtz_tma(pz_plan *pl, double *const *u, int n, const double *tab, cudaStream_t st);
 int helmholtz_tma_prepare(pz_plan *pl);
 int launch_helmholtz_tma_cn(pz_plan *pl, double *u2, const double *uk, const double *tab, cudaStream_t st);
 int launch_helmholtz_step(pz_plan *pl, double *u2, const double *uk, cudaStream_t st);
-int helmholtz_build_tables(pz_plan *pl, double a);
+int helmholtz_build_tables(pz_plan *pl, double a, int kind = 0);
 // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (plan, kernel)
 int ensure_smem_optin(pz_plan *pl, const void *kernel, int bytes);
 template <class K> int smem_optin(const pz_plan *pl, K kernel, size_t bytes)

@@ -330,6 +330,40 @@ def test_helmholtz_matches_oracle(torch, pz, wl, oracle, nx, ny, nz, beta, a, op
         assert np.array_equal(u.cpu().numpy(), r)
 
 
+@pytest.mark.parametrize("nx,ny,nz,beta,a", [(8, 8, 4, 0.0, 0.1), (32, 16, 100, 1.8, 5e-5), (16, 16, 256, 2.0, 1e-3),
+                                             (64, 32, 512, 1.8, 5e-5), (64, 32, 700, 1.8, 5e-5), (16, 8, 1024, 1.8, 10.0),
+                                             (16, 8, 1594, 1.8, 2.5e-5), (8, 8, 2048, 1.8, 2.5e-5)])
+def test_helmholtz_w_face_centred_matches_oracle(torch, pz, wl, oracle, nx, ny, nz, beta, a):
+    """The wall-normal component on the z faces (reading R16) through every kernel variant the size
+    selects, beside a cell-centred set-up with another coefficient on the same plan."""
+    zf = wl.z_faces(nz, 2.0, beta)
+    zc = wl.z_centres(zf)
+    rng = np.random.default_rng(nz + 3 * nx)
+    r = rng.standard_normal((nz, ny, nx))
+    plan = pz.poisson_plan_create(nx, ny, nz, 1.0, 1.0, zc, zf)
+    w = torch.from_numpy(r).cuda()
+    with pytest.raises(pz.PzError) as ei:
+        pz.helmholtz_w_solve(plan, w)
+    assert ei.value.status == pz.PZ_ENOTSETUP
+    pz.helmholtz_z_setup(plan, 3 * a)
+    pz.helmholtz_w_setup(plan, a)
+    u = torch.from_numpy(r).cuda()
+    pz.helmholtz_w_solve(plan, w)
+    pz.helmholtz_z_solve(plan, u)
+    torch.cuda.synchronize()
+    assert rel_err(w.cpu().numpy(), oracle.helmholtz_w_solve(zc, zf, a, r)) <= TOL
+    assert rel_err(u.cpu().numpy(), oracle.helmholtz_z_solve(zc, zf, 3 * a, r)) <= TOL
+    assert torch.equal(w[-1], torch.from_numpy(r[-1]).cuda())       # the top wall face keeps its value
+    pz.helmholtz_w_setup(plan, 2 * a)                                 # re-set-up, cell-centred tables untouched
+    w2, u2 = torch.from_numpy(r).cuda(), torch.from_numpy(r).cuda()
+    pz.helmholtz_w_solve(plan, w2)
+    pz.helmholtz_z_solve(plan, u2)
+    torch.cuda.synchronize()
+    assert rel_err(w2.cpu().numpy(), oracle.helmholtz_w_solve(zc, zf, 2 * a, r)) <= TOL
+    assert torch.equal(u2, u)
+    pz.poisson_plan_destroy(plan)
+
+
 def test_helmholtz_not_setup_and_resetup(torch, pz, wl, oracle):
     nx, ny, nz = 16, 16, 96
     zf = wl.z_faces(nz, 2.0, 1.8)
