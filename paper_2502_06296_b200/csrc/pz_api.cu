@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -190,6 +191,8 @@ const char *pz_last_error(void) { return g_err; }
 long long pz_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 int pz_version(void) { return 100; }
 
+static int slab_state_create(pz_plan *pl, int n_slabs, const int *kbounds, bool internal);
+
 // kb0 / nk: the planes [kb0, kb0 + nk) this plan transforms and owns (the whole grid for an ordinary plan)
 static int plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double ly, const double *zc, const double *zf,
                        int bc, int kb0, int nk)
@@ -277,6 +280,28 @@ static int plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double 
     if (ce != cudaSuccess) { cudaGetLastError(); set_error("plan counters: %s", cudaGetErrorString(ce)); return fail(PZ_ENOMEM); }
     // measured at 512 x 512 x nz: variant 2 wins from nz = 256 up to 1024, variant 1 below
     pl->opt.zsolve_variant = (nz <= 128) ? 1 : (nz <= 1024) ? 2 : 0;
+    const char *cut_env = getenv("PZ_ZCUT_ABOVE");   // tuning aid: internal cut for nz above this (default 1024)
+    const int cut_above = cut_env ? atoi(cut_env) : 1024;
+    if (nk == nz && nz > cut_above && nz <= 16 * 512) {
+        // whole columns longer than the pipeline's tile: the plan's own cut in z (pz_zslab.cu), slabs of
+        // at most 512 planes (16 rows per lane: three pipeline stages fit shared memory)
+        // full slabs of 512 planes (no padding rows in their tiles) and one remainder of at least 3
+        int G = (nz + 511) / 512;
+        std::vector<int> kb(G + 1, 0);
+        for (int g = 0; g < G; ++g) kb[g + 1] = (g + 1 < G) ? 512 * (g + 1) : nz;
+        if (nz - kb[G - 1] < 3) kb[G - 1] -= 3;
+        if (slab_state_create(pl, G, kb.data(), true) == PZ_OK) {
+            pl->opt.zsolve_variant = 3;
+        } else {
+            // not enough memory for the coefficient planes: the thread-per-column sweep needs one field of workspace
+            cudaGetLastError();
+            if (pl->d_slab_kb) { cudaFree(pl->d_slab_kb); pl->d_slab_kb = nullptr; }
+            if (pl->slab_coef) { cudaFree(pl->slab_coef); pl->slab_coef = nullptr; }
+            if (pl->slab_phi) { cudaFree(pl->slab_phi); pl->slab_phi = nullptr; }
+            if (pl->islab_ball) { cudaFree(pl->islab_ball); pl->islab_ball = nullptr; }
+            pl->slab_G = 0; pl->slab_internal = false;
+        }
+    }
     if (nk == nz && pl->opt.zsolve_variant == 0 && (rc = ensure_zwork(pl)) != PZ_OK) return fail(rc);
     *out = pl;
     return PZ_OK;
@@ -288,6 +313,35 @@ int poisson_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double
     return plan_create(out, nx, ny, nz, lx, ly, zc, zf, bc, 0, nz);
 }
 
+// Device state of a cut in z (coefficient planes of every slab, this slab's phi_prev / phi_next):
+// shared by the distributed plans and by the internal cut of a single-GPU plan with nz > 1024.
+static int slab_state_create(pz_plan *pl, int n_slabs, const int *kbounds, bool internal)
+{
+    const size_t plane = (size_t)pl->nx * pl->ny;
+    int nkmax = 0;
+    for (int j = 0; j < n_slabs; ++j)
+        if (kbounds[j + 1] - kbounds[j] > nkmax) nkmax = kbounds[j + 1] - kbounds[j];
+    pl->slab_G = n_slabs;
+    pl->slab_kb.assign(kbounds, kbounds + n_slabs + 1);
+    pl->slab_bstride = 2 * plane + (size_t)((nkmax + 1) & ~1);
+    pl->slab_internal = internal;
+    cudaError_t ce;
+    if ((ce = cudaMalloc(&pl->d_slab_kb, (n_slabs + 1) * sizeof(int))) != cudaSuccess ||
+        (ce = cudaMalloc(&pl->slab_coef, (size_t)n_slabs * 6 * plane * sizeof(double))) != cudaSuccess ||
+        (ce = cudaMalloc(&pl->slab_phi, 2 * plane * sizeof(double))) != cudaSuccess ||
+        (internal && (ce = cudaMalloc(&pl->islab_ball, (size_t)n_slabs * pl->slab_bstride * sizeof(double))) != cudaSuccess)) {
+        cudaGetLastError();
+        set_error("z-slab state: %s", cudaGetErrorString(ce));
+        return PZ_ENOMEM;
+    }
+    if ((ce = cudaMemcpy(pl->d_slab_kb, kbounds, (n_slabs + 1) * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(ce, "cudaMemcpy(kbounds)");
+    // every rank computes the interface coefficients of ALL slabs itself (PAPER.md:199): no collective
+    int rc;
+    if ((rc = launch_slab_coefficients(pl, nullptr)) != PZ_OK) return rc;
+    if ((ce = cudaDeviceSynchronize()) != cudaSuccess) return cuda_fail(ce, "slab coefficients");
+    return PZ_OK;
+}
+
 int poisson_slab_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double ly, const double *zc,
                              const double *zf, int bc, int n_slabs, int slab, const int *kbounds)
 {
@@ -297,6 +351,7 @@ int poisson_slab_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, d
         return PZ_EINVAL;
     }
     if (kbounds[0] != 0 || kbounds[n_slabs] != nz) { set_error("poisson_slab_plan_create: kbounds must run from 0 to nz"); return PZ_EINVAL; }
+    if (nz > 16384) { set_error("poisson_slab_plan_create: at most 16384 planes in all (got %d)", nz); return PZ_EUNSUPPORTED; }
     int nkmax = 0;
     for (int j = 0; j < n_slabs; ++j) {
         const int nk = kbounds[j + 1] - kbounds[j];
@@ -308,35 +363,21 @@ int poisson_slab_plan_create(pz_plan **out, int nx, int ny, int nz, double lx, d
     int rc = plan_create(&pl, nx, ny, nz, lx, ly, zc, zf, bc, kbounds[slab], kbounds[slab + 1] - kbounds[slab]);
     if (rc != PZ_OK) return rc;
     auto fail = [&](int code) { poisson_plan_destroy(pl); return code; };
-    pl->slab_G = n_slabs; pl->slab_g = slab;
-    pl->slab_kb.assign(kbounds, kbounds + n_slabs + 1);
-    const size_t plane = (size_t)nx * ny;
-    pl->slab_bstride = 2 * plane + (size_t)((nkmax + 1) & ~1);
-    cudaError_t ce;
-    if ((ce = cudaMalloc(&pl->d_slab_kb, (n_slabs + 1) * sizeof(int))) != cudaSuccess ||
-        (ce = cudaMalloc(&pl->slab_coef, (size_t)n_slabs * 6 * plane * sizeof(double))) != cudaSuccess ||
-        (ce = cudaMalloc(&pl->slab_phi, 2 * plane * sizeof(double))) != cudaSuccess) {
-        cudaGetLastError();
-        set_error("poisson_slab_plan_create: %s", cudaGetErrorString(ce));
-        return fail(PZ_ENOMEM);
-    }
-    if ((ce = cudaMemcpy(pl->d_slab_kb, kbounds, (n_slabs + 1) * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(cuda_fail(ce, "cudaMemcpy(kbounds)"));
-    // every rank computes the interface coefficients of ALL slabs itself (PAPER.md:199): no collective
-    if ((rc = launch_slab_coefficients(pl, nullptr)) != PZ_OK) return fail(rc);
-    if ((ce = cudaDeviceSynchronize()) != cudaSuccess) return fail(cuda_fail(ce, "slab coefficients"));
+    pl->slab_g = slab;
+    if ((rc = slab_state_create(pl, n_slabs, kbounds, false)) != PZ_OK) return fail(rc);
     *out = pl;
     return PZ_OK;
 }
 
 long long poisson_slab_boundary_doubles(const pz_plan *pl)
 {
-    return (pl && pl->slab_G > 0) ? (long long)pl->slab_bstride : 0;
+    return (pl && pl->slab_G > 0 && !pl->slab_internal) ? (long long)pl->slab_bstride : 0;
 }
 
 int poisson_solve_reduce(pz_plan *pl, double *p, double *boundary_out, void *stream)
 {
     if (!pl || !p || !boundary_out) { set_error("poisson_solve_reduce: NULL argument"); return PZ_EINVAL; }
-    if (pl->slab_G < 1) { set_error("poisson_solve_reduce: the plan is not a slab plan"); return PZ_EINVAL; }
+    if (pl->slab_G < 1 || pl->slab_internal) { set_error("poisson_solve_reduce: the plan is not a slab plan"); return PZ_EINVAL; }
     if ((((uintptr_t)p | (uintptr_t)boundary_out) & 15) != 0) { set_error("poisson_solve_reduce: buffers must be 16-byte aligned"); return PZ_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
@@ -348,7 +389,7 @@ int poisson_solve_reduce(pz_plan *pl, double *p, double *boundary_out, void *str
 int poisson_solve_finish(pz_plan *pl, double *p, const double *boundary_all, void *stream)
 {
     if (!pl || !p || !boundary_all) { set_error("poisson_solve_finish: NULL argument"); return PZ_EINVAL; }
-    if (pl->slab_G < 1) { set_error("poisson_solve_finish: the plan is not a slab plan"); return PZ_EINVAL; }
+    if (pl->slab_G < 1 || pl->slab_internal) { set_error("poisson_solve_finish: the plan is not a slab plan"); return PZ_EINVAL; }
     if ((((uintptr_t)p | (uintptr_t)boundary_all) & 15) != 0) { set_error("poisson_solve_finish: buffers must be 16-byte aligned"); return PZ_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
@@ -368,6 +409,7 @@ int poisson_plan_destroy(pz_plan *pl)
     if (pl->d_slab_kb) cudaFree(pl->d_slab_kb);
     if (pl->slab_coef) cudaFree(pl->slab_coef);
     if (pl->slab_phi) cudaFree(pl->slab_phi);
+    if (pl->islab_ball) cudaFree(pl->islab_ball);
     for (int b = 0; b < 3; ++b)
         if (pl->d_batch_stage[b]) cudaFree(pl->d_batch_stage[b]);
     if (pl->h2d_stream) cudaStreamDestroy(pl->h2d_stream);
@@ -414,7 +456,7 @@ int pz_poisson_stage(pz_plan *pl, double *p, int stage, void *stream)
 int poisson_solve(pz_plan *pl, double *p, void *stream)
 {
     if (!pl || !p) { set_error("poisson_solve: NULL argument"); return PZ_EINVAL; }
-    if (pl->slab_G > 0) { set_error("poisson_solve: a slab plan solves through poisson_solve_reduce / poisson_solve_finish"); return PZ_EINVAL; }
+    if (pl->slab_G > 0 && !pl->slab_internal) { set_error("poisson_solve: a slab plan solves through poisson_solve_reduce / poisson_solve_finish"); return PZ_EINVAL; }
     if (((uintptr_t)p & 15) != 0) { set_error("poisson_solve: p must be 16-byte aligned"); return PZ_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
@@ -498,7 +540,7 @@ int helmholtz3d_solve(pz_plan *pl, double *u, void *stream)
     if (!pl || !u) { set_error("helmholtz3d_solve: NULL argument"); return PZ_EINVAL; }
     if (((uintptr_t)u & 15) != 0) { set_error("helmholtz3d_solve: u must be 16-byte aligned"); return PZ_EINVAL; }
     if (pl->h3_a < 0.0) { set_error("helmholtz3d_solve: call helmholtz3d_setup first"); return PZ_ENOTSETUP; }
-    if (pl->slab_G > 0) { set_error("helmholtz3d_solve: not available on a z-slab plan"); return PZ_EUNSUPPORTED; }
+    if (pl->slab_G > 0 && !pl->slab_internal) { set_error("helmholtz3d_solve: not available on a z-slab plan"); return PZ_EUNSUPPORTED; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
     if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 64) * sizeof(int), st));
@@ -511,7 +553,7 @@ int helmholtz_z_setup(pz_plan *pl, double a)
 {
     if (!pl) { set_error("helmholtz_z_setup: plan is NULL"); return PZ_EINVAL; }
     if (!(a >= 0.0) || !std::isfinite(a)) { set_error("helmholtz_z_setup: a must be finite and >= 0"); return PZ_EINVAL; }
-    if (pl->slab_G > 0) { set_error("helmholtz_z_setup: not available on a z-slab plan (columns are cut; shard Helmholtz solves in y)"); return PZ_EUNSUPPORTED; }
+    if (pl->slab_G > 0 && !pl->slab_internal) { set_error("helmholtz_z_setup: not available on a z-slab plan (columns are cut; shard Helmholtz solves in y)"); return PZ_EUNSUPPORTED; }
     return helmholtz_build_tables(pl, a);
 }
 
@@ -519,7 +561,7 @@ int helmholtz_w_setup(pz_plan *pl, double a)
 {
     if (!pl) { set_error("helmholtz_w_setup: plan is NULL"); return PZ_EINVAL; }
     if (!(a >= 0.0) || !std::isfinite(a)) { set_error("helmholtz_w_setup: a must be finite and >= 0"); return PZ_EINVAL; }
-    if (pl->slab_G > 0) { set_error("helmholtz_w_setup: not available on a z-slab plan (columns are cut; shard Helmholtz solves in y)"); return PZ_EUNSUPPORTED; }
+    if (pl->slab_G > 0 && !pl->slab_internal) { set_error("helmholtz_w_setup: not available on a z-slab plan (columns are cut; shard Helmholtz solves in y)"); return PZ_EUNSUPPORTED; }
     return helmholtz_build_tables(pl, a, 1);
 }
 
@@ -689,8 +731,9 @@ int pz_set_option(pz_plan *pl, const char *key, int value)
     int *slot = option_slot(pl, key);
     if (!slot) { set_error("pz_set_option: unknown key '%s'", key); return PZ_EUNSUPPORTED; }
     if (slot == &pl->opt.zsolve_variant) {
-        if (value < 0 || value > 2) { set_error("zsolve_variant must be 0, 1 or 2"); return PZ_EUNSUPPORTED; }
-        if (value >= 1 && pl->nz > 1024) { set_error("zsolve_variant %d supports nz <= 1024", value); return PZ_EUNSUPPORTED; }
+        if (value < 0 || value > 3) { set_error("zsolve_variant must be 0, 1, 2 or 3"); return PZ_EUNSUPPORTED; }
+        if ((value == 1 || value == 2) && pl->nz > 1024) { set_error("zsolve_variant %d supports nz <= 1024", value); return PZ_EUNSUPPORTED; }
+        if (value == 3 && !pl->slab_internal) { set_error("zsolve_variant 3 is the plan's own z cut (nz > 1024)"); return PZ_EUNSUPPORTED; }
         if (value == 0) { const int rc = ensure_zwork(pl); if (rc != PZ_OK) return rc; }
     } else if (value < 0) {
         set_error("pz_set_option: '%s' must be >= 0", key);

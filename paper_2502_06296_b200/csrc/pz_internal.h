@@ -27,7 +27,8 @@ struct HelmTables {
 };
 
 struct Options {
-    int zsolve_variant = 0;   // 0 = thread-per-column Thomas through global memory (2 sweeps)
+    int zsolve_variant = 0;   // 3 = nz > 1024: the plan's own z-slabs through variant 2 (pz_zslab.cu)
+                              // 0 = thread-per-column Thomas through global memory (2 sweeps)
                               // 1 = chunked cyclic reduction in shared memory
                               // 2 = the same solve inside a TMA load / solve / TMA store pipeline
     int zsolve_probe = 0;     // diagnostic (variant 2): 2 = no arithmetic (results are wrong)
@@ -112,10 +113,12 @@ struct pz_plan {
     double *slab_coef = nullptr;     // [G][6][nx ny] interface coefficients of every slab
     double *slab_phi = nullptr;      // [2][nx ny] phi_prev, phi_next of this rank's slab
     size_t slab_bstride = 0;         // doubles per rank in the gathered boundary buffer
+    bool slab_internal = false;      // the cut is the plan's own (one GPU, nz > 1024): poisson_solve runs all slabs
+    double *islab_ball = nullptr;    // internal cut: the boundary buffers of all slabs
 
     // z-solve variant 2: launch geometry per (sub-domain rows M, HELM), queried once per plan (= per device)
     struct ZtGeo { int blocks = 0, stages = 0; };
-    ZtGeo zt[4][2];
+    ZtGeo zt[4][4];   // [M][whole columns, HELM, slab reduce, slab finish]
 
     // tensor maps of the column-tile kernels, keyed by (field pointer, geometry): a solve that sees the
     // same field again encodes nothing
@@ -186,8 +189,11 @@ int launch_fft_x_generic(const pz_plan *pl, double *p, long long nlines, bool in
 int launch_fft_y_generic(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_t st);
 int launch_fft_xy_fwd(pz_plan *pl, double *p, cudaStream_t st);
 int launch_fft_xy_inv(pz_plan *pl, double *p, cudaStream_t st);
+int launch_zslab_tma(pz_plan *pl, double *p, int kb, int nk, double *bout, const double *phi_prev, const double *phi_next,
+                     cudaStream_t st);
 int launch_slab_coefficients(pz_plan *pl, cudaStream_t st);
-int launch_slab_reduce(pz_plan *pl, const double *p, double *bout, cudaStream_t st);
+int launch_slab_reduce(pz_plan *pl, double *p, double *bout, cudaStream_t st);
+int launch_zsolve_islab(pz_plan *pl, double *p, cudaStream_t st);
 int launch_slab_finish(pz_plan *pl, double *p, const double *ball, cudaStream_t st);
 int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st, int kind = 0); // kind 1: face-centred w
 int launch_helmholtz_tma(pz_plan *pl, double *const *u, int n, const double *tab, cudaStream_t st);

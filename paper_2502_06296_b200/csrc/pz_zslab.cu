@@ -45,119 +45,6 @@ struct RowAcc {
     __device__ __forceinline__ double2 &operator()(int i) const { return d[i * (kTX / 2)]; }
 };
 
-// Slab-local reduction of one column pair (or of its coefficient right-hand sides), one
-// sub-domain of M rows per lane: sweeps A / B of solve_pair with NC right-hand-side components,
-// the lane-boundary system by warp-shuffle PCR, then the first (F) and last (L) value of the
-// slab's solution.  rhs(i, out): the NC components of row i of this lane (0 on padding rows).
-template <int M, int NC, class Rhs>
-__device__ __forceinline__ void reduce_pair(const double *al, const double *ga, const double *ex, double sigma, int k0,
-                                            int nk, Rhs rhs, double (&F)[NC], double (&L)[NC])
-{
-    auto eps_of = [&](int i) { return (k0 + i < nk) ? ex[i] + sigma : 1.0; };
-    const int lane = threadIdx.x & 31;
-    double rp2[NC], rp[NC], t[NC], rcap[NC];
-    double chat = ga[M - 2], eps2 = eps_of(M - 2);
-    rhs(M - 2, rp2);
-    double rb2 = fast_rcp(al[M - 2] + chat + eps2);
-    double ahat = al[1], eps = eps_of(1);
-    rhs(1, rp);
-    double rbp = fast_rcp(ahat + ga[1] + eps);
-    double acap = 0.0;
-#pragma unroll
-    for (int c = 0; c < NC; ++c) rcap[c] = 0.0;
-    auto capture = [&](int i) {
-        if (k0 + i == nk - 1) {
-            acap = ahat * rbp;
-#pragma unroll
-            for (int c = 0; c < NC; ++c) rcap[c] = rp[c] * rbp;
-        }
-    };
-    capture(1);
-#pragma unroll
-    for (int s = 0; s < M - 2; ++s) {
-        {   // A: row i = M-3-s
-            const int i = M - 3 - s;
-            if (i >= 1) {
-                const double nn = ga[i] * rb2;
-                rhs(i, t);
-                chat = nn * chat;
-                eps2 = fma(nn, eps2, eps_of(i));
-#pragma unroll
-                for (int c = 0; c < NC; ++c) rp2[c] = fma(nn, rp2[c], t[c]);
-                rb2 = fast_rcp(al[i] + chat + eps2);
-            }
-        }
-        {   // B: row i = 2+s
-            const int i = 2 + s;
-            const double mm = al[i] * rbp;
-            rhs(i, t);
-            ahat = mm * ahat;
-            eps = fma(mm, eps, eps_of(i));
-#pragma unroll
-            for (int c = 0; c < NC; ++c) rp[c] = fma(mm, rp[c], t[c]);
-            rbp = fast_rcp(ahat + ga[i] + eps);
-            capture(i);
-        }
-    }
-    // normalised row 0:  -a0 X_{s-1} + x_0 - c0 X_s = r0, excess e0
-    double a0, c0, e0, r0[NC];
-    {
-        const double nn = ga[0] * rb2;
-        rhs(0, t);
-        a0 = al[0];
-        c0 = nn * chat;
-        e0 = fma(nn, eps2, eps_of(0));
-        const double rbn = fast_rcp(a0 + c0 + e0);
-#pragma unroll
-        for (int c = 0; c < NC; ++c) r0[c] = fma(nn, rp2[c], t[c]) * rbn;
-        a0 *= rbn; c0 *= rbn; e0 *= rbn;
-    }
-    // normalised last row:  -a x_0 + X_s - c (next lane's x_0) = r, excess e
-    double a = ahat * rbp, c = ga[M - 1] * rbp, e = eps * rbp, r[NC];
-#pragma unroll
-    for (int q = 0; q < NC; ++q) r[q] = rp[q] * rbp;
-    // eliminate the x_0 unknowns (local row 0 and the next lane's)
-    {
-        const double c0n = shfl_down(c0, 1), e0n = shfl_down(e0, 1);
-        const double k1 = a, k2 = c;
-#pragma unroll
-        for (int q = 0; q < NC; ++q) r[q] = fma(k1, r0[q], fma(k2, shfl_down(r0[q], 1), r[q]));
-        a = k1 * a0;
-        c = k2 * c0n;
-        e = fma(k1, e0, fma(k2, e0n, e));
-        const double rbn = fast_rcp(a + c + e);
-        a *= rbn; c *= rbn; e *= rbn;
-#pragma unroll
-        for (int q = 0; q < NC; ++q) r[q] *= rbn;
-    }
-#pragma unroll
-    for (int h = 1; h < kLanes; h *= 2) {
-        const double am = shfl_up(a, h), em = shfl_up(e, h);
-        const double cp = shfl_down(c, h), ep = shfl_down(e, h);
-        const double k1 = a, k2 = c;
-#pragma unroll
-        for (int q = 0; q < NC; ++q) r[q] = fma(k1, shfl_up(r[q], h), fma(k2, shfl_down(r[q], h), r[q]));
-        a = k1 * am;
-        c = k2 * cp;
-        e = fma(k1, em, fma(k2, ep, e));
-        const double rbn = fast_rcp(a + c + e);
-        a *= rbn; c *= rbn; e *= rbn;
-#pragma unroll
-        for (int q = 0; q < NC; ++q) r[q] *= rbn;
-    }
-    // r = X_s (last row of lane s); x_0 = r0 + a0 X_{s-1} + c0 X_s (lane 0: a0 = 0)
-    const int sL = (nk - 1) / M, iL = (nk - 1) - sL * M;
-#pragma unroll
-    for (int q = 0; q < NC; ++q) {
-        const double x0 = fma(a0, shfl_up(r[q], 1), fma(c0, r[q], r0[q]));
-        // last real row: x_0 of its lane if it is the lane's row 0, else (sweep B, row iL) rcap + acap x_0
-        const double lv = (iL == 0) ? x0 : fma(acap, x0, rcap[q]);
-        F[q] = __shfl_sync(0xffffffffu, x0, 0);
-        L[q] = __shfl_sync(0xffffffffu, lv, sL);
-    }
-    (void)lane;
-}
-
 // Shared-memory coefficient tables of one slab [kb, kb + nk) of the global grid, one sub-domain
 // of M rows per lane (stride CS): al / ga = sub- / super-diagonal magnitudes with the couplings
 // across the slab boundaries removed, ex = the diagonal excess those leave behind.
@@ -379,25 +266,76 @@ __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 
 
 // The (0,0) column, whole, from the gathered right-hand side (closed form of the singular Neumann
 // system: S_k = sum_{l<=k} dzf_l d_l, phi_{k+1} = phi_k + dzc_k S_k, then zero volume mean); this
-// rank's rows are written into its slab.  One warp: two serial passes over nz values.
-__global__ void slab_zero_mode_kernel(double *__restrict__ p, const double *__restrict__ ball, size_t bstride, size_t plane,
-                                      const int *__restrict__ kb, int G, int g, const double *__restrict__ dzf,
-                                      const double *__restrict__ zc, double inv_lz)
+// rank's rows are written into its slab (g >= 0) or, for the plan's own cut, all rows (g < 0, p =
+// the whole field).  One CTA of 1024 threads: two block-wide prefix sums per chunk of 1024 rows
+// with running carries (fixed summation tree: deterministic, the same on every rank).
+__device__ __forceinline__ double block_scan_incl(double v, double *wsum, double *total)
 {
-    if (threadIdx.x != 0) return;
-    const int nz = kb[G];
-    double mean = 0.0;
-    for (int pass = 0; pass < 2; ++pass) {
-        double S = 0.0, phi = 0.0, acc = 0.0;
-        int j = 0;
-        for (int k = 0; k < nz; ++k) {
-            while (k >= kb[j + 1]) ++j;
-            if (pass == 0) acc = fma(dzf[k], phi, acc);
-            else if (j == g) p[(size_t)(k - kb[g]) * plane] = phi - mean;
-            S = fma(dzf[k], ball[(size_t)j * bstride + 2 * plane + (k - kb[j])], S);
-            if (k + 1 < nz) phi = fma(zc[k + 1] - zc[k], S, phi);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o *= 2) {
+        const double t = __shfl_up_sync(0xffffffffu, v, o);
+        if (lane >= o) v += t;
+    }
+    __syncthreads(); // wsum free again
+    if (lane == 31) wsum[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        double w = wsum[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o *= 2) {
+            const double t = __shfl_up_sync(0xffffffffu, w, o);
+            if (lane >= o) w += t;
         }
-        if (pass == 0) mean = acc * inv_lz;
+        wsum[lane] = w;
+    }
+    __syncthreads();
+    *total = wsum[31];
+    return v + (warp > 0 ? wsum[warp - 1] : 0.0);
+}
+
+constexpr int kZmChunks = 16; // rows per column <= 16 * 1024
+
+__global__ void __launch_bounds__(1024)
+    slab_zero_mode_kernel(double *__restrict__ p, const double *__restrict__ ball, size_t bstride, size_t plane,
+                          const int *__restrict__ kb, int G, int g, const double *__restrict__ dzf,
+                          const double *__restrict__ zc, double inv_lz)
+{
+    __shared__ double wsum[32];
+    const int nz = kb[G];
+    double phi[kZmChunks];
+    double carryS = 0.0, carryP = 0.0, acc = 0.0;
+#pragma unroll
+    for (int c = 0; c < kZmChunks; ++c) {
+        phi[c] = 0.0;
+        if (c * 1024 < nz) {
+            const int k = c * 1024 + (int)threadIdx.x;
+            double t = 0.0;
+            if (k < nz) {
+                int j = 0;
+                while (k >= kb[j + 1]) ++j;
+                t = dzf[k] * ball[(size_t)j * bstride + 2 * plane + (k - kb[j])];
+            }
+            double totS, totP;
+            const double S = carryS + block_scan_incl(t, wsum, &totS);
+            const double u = (k + 1 < nz) ? (zc[k + 1] - zc[k]) * S : 0.0;
+            const double incl = block_scan_incl(u, wsum, &totP);
+            phi[c] = carryP + (incl - u); // exclusive: phi_k = sum_{l<k} dzc_l S_l
+            if (k < nz) acc = fma(dzf[k], phi[c], acc);
+            carryS += totS;
+            carryP += totP;
+        }
+    }
+    double tot;
+    block_scan_incl(acc, wsum, &tot);
+    const double mean = tot * inv_lz;
+#pragma unroll
+    for (int c = 0; c < kZmChunks; ++c) {
+        const int k = c * 1024 + (int)threadIdx.x;
+        if (k < nz) {
+            if (g < 0) p[(size_t)k * plane] = phi[c] - mean;
+            else if (k >= kb[g] && k < kb[g + 1]) p[(size_t)(k - kb[g]) * plane] = phi[c] - mean;
+        }
     }
 }
 
@@ -430,15 +368,18 @@ int launch_slab_coefficients(pz_plan *pl, cudaStream_t st)
     return PZ_OK;
 }
 
-int launch_slab_reduce(pz_plan *pl, const double *p, double *bout, cudaStream_t st)
+// Slab g of the plan's cut: p_slab points at its first plane.  Slabs of more than 128 planes take the
+// TMA pipeline of pz_zsolve_tma.cu (slab modes), thinner ones the kernels above.
+static int slab_reduce_g(pz_plan *pl, double *p_slab, int g, double *bout, cudaStream_t st)
 {
     const size_t plane = (size_t)pl->nx * pl->ny;
     const unsigned blocks = (unsigned)(plane / kTX);
-    const int kb = pl->slab_kb[pl->slab_g], nk = pl->nz;
+    const int kb = pl->slab_kb[g], nk = pl->slab_kb[g + 1] - kb;
+    if (nk > 128 && pl->opt.zsolve_variant != 1) return launch_zslab_tma(pl, p_slab, kb, nk, bout, nullptr, nullptr, st);
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
     PZ_SLAB_DISPATCH(nk, {
         { const int rc = smem_optin(pl, slab_reduce_kernel<MM>, slab_smem<MM>()); if (rc != PZ_OK) return rc; }
-        slab_reduce_kernel<MM><<<blocks, kPairs * kLanes, slab_smem<MM>(), st>>>(p, bout, pl->d_A, pl->d_C, pl->d_lamx, pl->d_lamy_nat,
+        slab_reduce_kernel<MM><<<blocks, kPairs * kLanes, slab_smem<MM>(), st>>>(p_slab, bout, pl->d_A, pl->d_C, pl->d_lamx, pl->d_lamy_nat,
                                                                                  pl->d_lamy_pk, pl->nx, plane, kb, nk);
     });
     count_launch();
@@ -446,24 +387,61 @@ int launch_slab_reduce(pz_plan *pl, const double *p, double *bout, cudaStream_t 
     return PZ_OK;
 }
 
-int launch_slab_finish(pz_plan *pl, double *p, const double *ball, cudaStream_t st)
+static int slab_finish_g(pz_plan *pl, double *p_slab, int g, const double *ball, cudaStream_t st)
 {
     const size_t plane = (size_t)pl->nx * pl->ny;
     const unsigned blocks = (unsigned)(plane / kTX);
-    const int g = pl->slab_g, G = pl->slab_G, kb = pl->slab_kb[g], nk = pl->nz;
+    const int G = pl->slab_G, kb = pl->slab_kb[g], nk = pl->slab_kb[g + 1] - kb;
+    {
+        ProfScope prof(pl, PZ_K_Z_SOLVE, st);
+        slab_interface_kernel<<<(unsigned)((plane + 255) / 256), 256, 0, st>>>(ball, pl->slab_bstride, pl->slab_coef, plane, G, g,
+                                                                             pl->slab_phi, pl->slab_phi + plane);
+        count_launch();
+        PZ_CUDA(cudaGetLastError());
+    }
+    if (nk > 128 && pl->opt.zsolve_variant != 1) {
+        const int rc = launch_zslab_tma(pl, p_slab, kb, nk, nullptr, pl->slab_phi, pl->slab_phi + plane, st);
+        if (rc != PZ_OK) return rc;
+    } else {
+        ProfScope prof(pl, PZ_K_Z_SOLVE, st);
+        PZ_SLAB_DISPATCH(nk, {
+            { const int rc = smem_optin(pl, slab_finish_kernel<MM>, slab_smem<MM>()); if (rc != PZ_OK) return rc; }
+            slab_finish_kernel<MM><<<blocks, kPairs * kLanes, slab_smem<MM>(), st>>>(p_slab, pl->slab_phi, pl->slab_phi + plane, pl->d_A, pl->d_C,
+                                                                                     pl->d_lamx, pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, plane, kb, nk);
+        });
+        count_launch();
+        PZ_CUDA(cudaGetLastError());
+    }
+    if (pl->slab_internal) return PZ_OK; // the plan's own cut writes the whole (0,0) column once (launch_zsolve_islab)
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
-    slab_interface_kernel<<<(unsigned)((plane + 255) / 256), 256, 0, st>>>(ball, pl->slab_bstride, pl->slab_coef, plane, G, g,
-                                                                         pl->slab_phi, pl->slab_phi + plane);
+    slab_zero_mode_kernel<<<1, 1024, 0, st>>>(p_slab, ball, pl->slab_bstride, plane, pl->d_slab_kb, G, g, pl->d_dzf, pl->d_zc, pl->inv_lz);
     count_launch();
     PZ_CUDA(cudaGetLastError());
-    PZ_SLAB_DISPATCH(nk, {
-        { const int rc = smem_optin(pl, slab_finish_kernel<MM>, slab_smem<MM>()); if (rc != PZ_OK) return rc; }
-        slab_finish_kernel<MM><<<blocks, kPairs * kLanes, slab_smem<MM>(), st>>>(p, pl->slab_phi, pl->slab_phi + plane, pl->d_A, pl->d_C,
-                                                                                 pl->d_lamx, pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, plane, kb, nk);
-    });
-    count_launch();
-    PZ_CUDA(cudaGetLastError());
-    slab_zero_mode_kernel<<<1, 32, 0, st>>>(p, ball, pl->slab_bstride, plane, pl->d_slab_kb, G, g, pl->d_dzf, pl->d_zc, pl->inv_lz);
+    return PZ_OK;
+}
+
+int launch_slab_reduce(pz_plan *pl, double *p, double *bout, cudaStream_t st) { return slab_reduce_g(pl, p, pl->slab_g, bout, st); }
+int launch_slab_finish(pz_plan *pl, double *p, const double *ball, cudaStream_t st) { return slab_finish_g(pl, p, pl->slab_g, ball, st); }
+
+// A whole column of more than 1024 rows on ONE GPU (the paper's wall-normal size is 1594,
+// PAPER.md:268): the plan cuts z into slabs of at most 1024 planes itself and runs the distributed
+// algorithm locally -- every slab's reduction, the interface systems, every slab's finish; the
+// "exchange" is the plan's own boundary buffer.  24 instead of 16 bytes per point cross HBM, against
+// 32 and an N-double workspace for the thread-per-column sweep of pz_zsolve.cu.
+int launch_zsolve_islab(pz_plan *pl, double *p, cudaStream_t st)
+{
+    const size_t plane = (size_t)pl->nx * pl->ny;
+    for (int g = 0; g < pl->slab_G; ++g) {
+        const int rc = slab_reduce_g(pl, p + (size_t)pl->slab_kb[g] * plane, g, pl->islab_ball + (size_t)g * pl->slab_bstride, st);
+        if (rc != PZ_OK) return rc;
+    }
+    for (int g = 0; g < pl->slab_G; ++g) {
+        const int rc = slab_finish_g(pl, p + (size_t)pl->slab_kb[g] * plane, g, pl->islab_ball, st);
+        if (rc != PZ_OK) return rc;
+    }
+    ProfScope prof(pl, PZ_K_Z_SOLVE, st);
+    slab_zero_mode_kernel<<<1, 1024, 0, st>>>(p, pl->islab_ball, pl->slab_bstride, plane, pl->d_slab_kb, pl->slab_G, -1, pl->d_dzf, pl->d_zc,
+                                              pl->inv_lz);
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;

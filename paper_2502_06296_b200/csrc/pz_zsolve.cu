@@ -77,6 +77,7 @@ __global__ void __launch_bounds__(128)
 
 int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
 {
+    if (pl->opt.zsolve_variant == 3 && helm_a < 0.0) return launch_zsolve_islab(pl, p, st);
     if (pl->opt.zsolve_variant == 1) return launch_zsolve_cr(pl, p, st, helm_a);
     if (pl->opt.zsolve_variant == 2) return launch_zsolve_tma(pl, p, st, helm_a);
     if (helm_a >= 0.0) {

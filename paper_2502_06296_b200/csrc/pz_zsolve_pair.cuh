@@ -218,4 +218,117 @@ __device__ __forceinline__ void solve_pair(const Acc d, const double *al, const 
     }
 }
 
+// Slab-local reduction of one column pair (or of its coefficient right-hand sides), one
+// sub-domain of M rows per lane: sweeps A / B of solve_pair with NC right-hand-side components,
+// the lane-boundary system by warp-shuffle PCR, then the first (F) and last (L) value of the
+// slab's solution.  rhs(i, out): the NC components of row i of this lane (0 on padding rows).
+template <int M, int NC, class Rhs>
+__device__ __forceinline__ void reduce_pair(const double *al, const double *ga, const double *ex, double sigma, int k0,
+                                            int nk, Rhs rhs, double (&F)[NC], double (&L)[NC])
+{
+    auto eps_of = [&](int i) { return (k0 + i < nk) ? ex[i] + sigma : 1.0; };
+    const int lane = threadIdx.x & 31;
+    double rp2[NC], rp[NC], t[NC], rcap[NC];
+    double chat = ga[M - 2], eps2 = eps_of(M - 2);
+    rhs(M - 2, rp2);
+    double rb2 = fast_rcp(al[M - 2] + chat + eps2);
+    double ahat = al[1], eps = eps_of(1);
+    rhs(1, rp);
+    double rbp = fast_rcp(ahat + ga[1] + eps);
+    double acap = 0.0;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) rcap[c] = 0.0;
+    auto capture = [&](int i) {
+        if (k0 + i == nk - 1) {
+            acap = ahat * rbp;
+#pragma unroll
+            for (int c = 0; c < NC; ++c) rcap[c] = rp[c] * rbp;
+        }
+    };
+    capture(1);
+#pragma unroll
+    for (int s = 0; s < M - 2; ++s) {
+        {   // A: row i = M-3-s
+            const int i = M - 3 - s;
+            if (i >= 1) {
+                const double nn = ga[i] * rb2;
+                rhs(i, t);
+                chat = nn * chat;
+                eps2 = fma(nn, eps2, eps_of(i));
+#pragma unroll
+                for (int c = 0; c < NC; ++c) rp2[c] = fma(nn, rp2[c], t[c]);
+                rb2 = fast_rcp(al[i] + chat + eps2);
+            }
+        }
+        {   // B: row i = 2+s
+            const int i = 2 + s;
+            const double mm = al[i] * rbp;
+            rhs(i, t);
+            ahat = mm * ahat;
+            eps = fma(mm, eps, eps_of(i));
+#pragma unroll
+            for (int c = 0; c < NC; ++c) rp[c] = fma(mm, rp[c], t[c]);
+            rbp = fast_rcp(ahat + ga[i] + eps);
+            capture(i);
+        }
+    }
+    // normalised row 0:  -a0 X_{s-1} + x_0 - c0 X_s = r0, excess e0
+    double a0, c0, e0, r0[NC];
+    {
+        const double nn = ga[0] * rb2;
+        rhs(0, t);
+        a0 = al[0];
+        c0 = nn * chat;
+        e0 = fma(nn, eps2, eps_of(0));
+        const double rbn = fast_rcp(a0 + c0 + e0);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) r0[c] = fma(nn, rp2[c], t[c]) * rbn;
+        a0 *= rbn; c0 *= rbn; e0 *= rbn;
+    }
+    // normalised last row:  -a x_0 + X_s - c (next lane's x_0) = r, excess e
+    double a = ahat * rbp, c = ga[M - 1] * rbp, e = eps * rbp, r[NC];
+#pragma unroll
+    for (int q = 0; q < NC; ++q) r[q] = rp[q] * rbp;
+    // eliminate the x_0 unknowns (local row 0 and the next lane's)
+    {
+        const double c0n = shfl_down(c0, 1), e0n = shfl_down(e0, 1);
+        const double k1 = a, k2 = c;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) r[q] = fma(k1, r0[q], fma(k2, shfl_down(r0[q], 1), r[q]));
+        a = k1 * a0;
+        c = k2 * c0n;
+        e = fma(k1, e0, fma(k2, e0n, e));
+        const double rbn = fast_rcp(a + c + e);
+        a *= rbn; c *= rbn; e *= rbn;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) r[q] *= rbn;
+    }
+#pragma unroll
+    for (int h = 1; h < kLanes; h *= 2) {
+        const double am = shfl_up(a, h), em = shfl_up(e, h);
+        const double cp = shfl_down(c, h), ep = shfl_down(e, h);
+        const double k1 = a, k2 = c;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) r[q] = fma(k1, shfl_up(r[q], h), fma(k2, shfl_down(r[q], h), r[q]));
+        a = k1 * am;
+        c = k2 * cp;
+        e = fma(k1, em, fma(k2, ep, e));
+        const double rbn = fast_rcp(a + c + e);
+        a *= rbn; c *= rbn; e *= rbn;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) r[q] *= rbn;
+    }
+    // r = X_s (last row of lane s); x_0 = r0 + a0 X_{s-1} + c0 X_s (lane 0: a0 = 0)
+    const int sL = (nk - 1) / M, iL = (nk - 1) - sL * M;
+#pragma unroll
+    for (int q = 0; q < NC; ++q) {
+        const double x0 = fma(a0, shfl_up(r[q], 1), fma(c0, r[q], r0[q]));
+        // last real row: x_0 of its lane if it is the lane's row 0, else (sweep B, row iL) rcap + acap x_0
+        const double lv = (iL == 0) ? x0 : fma(acap, x0, rcap[q]);
+        F[q] = __shfl_sync(0xffffffffu, x0, 0);
+        L[q] = __shfl_sync(0xffffffffu, lv, sL);
+    }
+    (void)lane;
+}
+
 } // namespace pz

@@ -53,16 +53,29 @@ template <int M> struct Geo {
     __host__ __device__ static size_t bytes(int stages) { return 1024 + stages * STAGE + COEF + 64; }
 };
 
+// z-slab of a cut column (pz_zslab.cu): what the slab modes need beside the tile
+struct SlabArgs {
+    int kb = 0;                       // first global row of the slab (the tile holds rows kb .. kb + nz - 1)
+    double *bout = nullptr;           // reduce: [RF (plane) | RL (plane) | (0,0) column (nz)]
+    const double *phi_prev = nullptr; // finish: value of the row below the slab, per real column
+    const double *phi_next = nullptr; //         and of the row above
+    size_t plane = 0;
+};
+
 // HELM = false: the Poisson systems (diagonal excess sigma = -(lambda_x + lambda_y), rhs -d, (0,0)
 // pinned).  HELM = true: the fully implicit Helmholtz systems of Eq. (8) with a = ha and the
 // Dirichlet wall terms hw0, hw1 (solve_pair, HELM).
-template <int M, bool HELM>
+// MODE 0: whole columns.  MODE 1 / 2: one z-slab of cut columns -- 1 = slab-local reduction (the
+// slab's boundary values of T^{-1}(-d) go to sa.bout, nothing is stored back), 2 = the slab solved
+// with its neighbours' boundary values on the right-hand side (solve_pair, OPEN), in place.
+template <int M, bool HELM, int MODE = 0>
 __global__ void __launch_bounds__(kThreads, 1)
     zsolve_tma_kernel(const __grid_constant__ CUtensorMap map, const double *__restrict__ A,
                       const double *__restrict__ C, const double *__restrict__ dzf, const double *__restrict__ lamx,
                       const double *__restrict__ lamy_nat, const double *__restrict__ lamy_pk, int nx, int ny, int nz,
-                      double inv_lz, int ntiles, int stages, double ha, double hw0, double hw1, int probe)
+                      double inv_lz, int ntiles, int stages, double ha, double hw0, double hw1, int probe, const SlabArgs sa)
 {
+    static_assert(!(HELM && MODE != 0), "slabs of cut columns are Poisson systems");
     using G = Geo<M>;
     extern __shared__ unsigned char smem_zt[];
     // 1024-byte aligned stage area (the swizzle pattern is a function of the address)
@@ -83,9 +96,17 @@ __global__ void __launch_bounds__(kThreads, 1)
     }
     for (int k = threadIdx.x; k < kLanes * M; k += blockDim.x) {
         const double sc = HELM ? ha : 1.0;
-        s_al[(k / M) * G::CS + (k % M)] = (k < nz) ? sc * A[k] : 0.0;
-        s_ga[(k / M) * G::CS + (k % M)] = (k < nz) ? sc * C[k] : 0.0;
-        s_e0[(k / M) * G::CS + (k % M)] = 1.0 + ha * ((k == 0 ? hw0 : 0.0) + (k == nz - 1 ? hw1 : 0.0));
+        double al = (k < nz) ? sc * A[sa.kb + k] : 0.0, ga = (k < nz) ? sc * C[sa.kb + k] : 0.0;
+        double ex = 1.0 + ha * ((k == 0 ? hw0 : 0.0) + (k == nz - 1 ? hw1 : 0.0));
+        if constexpr (MODE != 0) {
+            // couplings across the slab's ends leave the matrix; their magnitude stays on the diagonal
+            ex = 0.0;
+            if (k == 0) { ex += al; al = 0.0; }
+            if (k == nz - 1) { ex += ga; ga = 0.0; }
+        }
+        s_al[(k / M) * G::CS + (k % M)] = al;
+        s_ga[(k / M) * G::CS + (k % M)] = ga;
+        s_e0[(k / M) * G::CS + (k % M)] = ex;
     }
     __syncthreads();
 
@@ -105,11 +126,13 @@ __global__ void __launch_bounds__(kThreads, 1)
             for (int it = 0; it < my_tiles; ++it) {
                 const int b = it % stages, col0 = ((int)blockIdx.x + it * (int)gridDim.x) * kTX;
                 mbar_wait(&done[b], (it / stages) & 1);
-                for (int l = 0; l < kLanes; ++l)
-                    if (l * M < nz) tma_store_2d(&map, base + b * G::STAGE + (size_t)l * G::SLOT * 128, col0, l * M);
-                tma_store_commit();
+                if constexpr (MODE != 1) {
+                    for (int l = 0; l < kLanes; ++l)
+                        if (l * M < nz) tma_store_2d(&map, base + b * G::STAGE + (size_t)l * G::SLOT * 128, col0, l * M);
+                    tma_store_commit();
+                }
                 if (it + stages < my_tiles) {
-                    tma_store_wait_read<0>();
+                    if constexpr (MODE != 1) tma_store_wait_read<0>();
                     load(it + stages);
                 }
             }
@@ -135,7 +158,48 @@ __global__ void __launch_bounds__(kThreads, 1)
         const double sig0 = -(lamx[i] + ly), sig1 = -(lamx[i + 1] + ly);
         d.slot = base + b * G::STAGE + (size_t)R0 * 128;
         mbar_wait(&full[b], (it / stages) & 1);
-        if (kProbes && probe == 2) {
+        if constexpr (MODE == 1) {
+            const double *ex = s_e0 + lane * G::CS;
+            double2 rf, rl;
+            if (sig0 == sig1) {
+                double F[2], L[2];
+                reduce_pair<M, 2>(al, ga, ex, sig0, k0, nz,
+                                  [&](int r, double(&o)[2]) {
+                                      const bool live = k0 + r < nz;
+                                      const double2 v = d(r);
+                                      o[0] = live ? -v.x : 0.0;
+                                      o[1] = live ? -v.y : 0.0;
+                                  },
+                                  F, L);
+                rf = make_double2(F[0], F[1]);
+                rl = make_double2(L[0], L[1]);
+            } else {
+                double F[1], L[1];
+                reduce_pair<M, 1>(al, ga, ex, sig0, k0, nz, [&](int r, double(&o)[1]) { o[0] = (k0 + r < nz) ? -d(r).x : 0.0; }, F, L);
+                rf.x = F[0]; rl.x = L[0];
+                reduce_pair<M, 1>(al, ga, ex, sig1, k0, nz, [&](int r, double(&o)[1]) { o[0] = (k0 + r < nz) ? -d(r).y : 0.0; }, F, L);
+                rf.y = F[0]; rl.y = L[0];
+            }
+            if (lane == 0) {
+                *reinterpret_cast<double2 *>(sa.bout + col) = rf;
+                *reinterpret_cast<double2 *>(sa.bout + sa.plane + col) = rl;
+            }
+            if (col == 0) // the slab's rows of the singular (0,0) column travel whole
+#pragma unroll
+                for (int r = 0; r < M; ++r)
+                    if (k0 + r < nz) sa.bout[2 * sa.plane + k0 + r] = d(r).x;
+        } else if constexpr (MODE == 2) {
+            const double *ex = s_e0 + lane * G::CS;
+            const double aopen = A[sa.kb], copen = C[sa.kb + nz - 1];
+            const double2 pp = *reinterpret_cast<const double2 *>(sa.phi_prev + col), pn = *reinterpret_cast<const double2 *>(sa.phi_next + col);
+            const double2 bp = make_double2(aopen * pp.x, aopen * pp.y), bn = make_double2(copen * pn.x, copen * pn.y);
+            if (sig0 == sig1) {
+                solve_pair<M, 3, false, false, false, true>(d, al, ga, sig0, k0, nz, nullptr, 0.0, ex, bp, bn);
+            } else {
+                solve_pair<M, 1, false, false, false, true>(d, al, ga, sig0, k0, nz, nullptr, 0.0, ex, bp, bn);
+                solve_pair<M, 2, false, false, false, true>(d, al, ga, sig1, k0, nz, nullptr, 0.0, ex, bp, bn);
+            }
+        } else if (kProbes && probe == 2) {
             // diagnostic: pipeline skeleton only (TMA load, TMA store), no arithmetic
         } else if constexpr (HELM) {
             const double *e0 = s_e0 + lane * G::CS;
@@ -162,24 +226,25 @@ __global__ void __launch_bounds__(kThreads, 1)
     }
 }
 
-template <int M, bool HELM>
-int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha)
+// nk: rows of the tile (the plan's nz for whole columns, the slab's for MODE 1 / 2)
+template <int M, bool HELM, int MODE = 0>
+int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha, int nk, const SlabArgs &sa)
 {
     using G = Geo<M>;
     int stages = (int)((227 * 1024 - 1024 - G::COEF - 64) / G::STAGE);
     if (stages > 3) stages = 3;
     if (pl->opt.zsolve_stages > 0 && pl->opt.zsolve_stages < stages) stages = pl->opt.zsolve_stages;
-    if (stages < 1) { set_error("z-solve variant 2: nz = %d does not fit shared memory", pl->nz); return PZ_EUNSUPPORTED; }
+    if (stages < 1) { set_error("z-solve variant 2: nz = %d does not fit shared memory", nk); return PZ_EUNSUPPORTED; }
     const size_t smem = G::bytes(stages);
     const size_t plane = (size_t)pl->nx * pl->ny;
     const int ntiles = (int)(plane / kTX);
     // per plan (= per device): shared-memory opt-in and resident CTAs, queried once
     constexpr int mi = (M == 4) ? 0 : (M == 8) ? 1 : (M == 16) ? 2 : 3;
-    pz_plan::ZtGeo &g = pl->zt[mi][HELM ? 1 : 0];
+    pz_plan::ZtGeo &g = pl->zt[mi][HELM ? 1 : (MODE == 0 ? 0 : MODE + 1)];
     if (g.blocks == 0 || g.stages != stages) {
-        { const int rc = smem_optin(pl, zsolve_tma_kernel<M, HELM>, 227 * 1024); if (rc != PZ_OK) return rc; }
+        { const int rc = smem_optin(pl, zsolve_tma_kernel<M, HELM, MODE>, 227 * 1024); if (rc != PZ_OK) return rc; }
         int occ = 1;
-        if (smem * 2 <= 227 * 1024) PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, zsolve_tma_kernel<M, HELM>, kThreads, smem));
+        if (smem * 2 <= 227 * 1024) PZ_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, zsolve_tma_kernel<M, HELM, MODE>, kThreads, smem));
         if (occ < 1) occ = 1;
         g.blocks = pl->num_sms * occ;
         g.stages = stages;
@@ -187,14 +252,14 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha)
     int blocks = g.blocks;
     if (blocks > ntiles) blocks = ntiles;
     const CUtensorMap *mapp = nullptr;
-    const int rc = cached_column_map(pl, &mapp, p, plane, pl->nz, kTX, M, 1, /*swizzle128=*/true);
+    const int rc = cached_column_map(pl, &mapp, p, plane, nk, kTX, M, 1, /*swizzle128=*/true);
     if (rc != PZ_OK) return rc;
     const CUtensorMap &map = *mapp;
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
-    zsolve_tma_kernel<M, HELM><<<blocks, kThreads, smem, st>>>(map, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
-                                                                pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, pl->nz,
-                                                                pl->inv_lz, ntiles, stages, ha, pl->wall_w0, pl->wall_w1,
-                                                                pl->opt.zsolve_probe);
+    zsolve_tma_kernel<M, HELM, MODE><<<blocks, kThreads, smem, st>>>(map, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
+                                                                      pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, nk,
+                                                                      pl->inv_lz, ntiles, stages, ha, pl->wall_w0, pl->wall_w1,
+                                                                      pl->opt.zsolve_probe, sa);
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
@@ -206,13 +271,31 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha)
 int launch_zsolve_tma(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
 {
     const int nz = pl->nz;
-#define PZ_ZT(MM) (helm_a >= 0.0 ? launch_m<MM, true>(pl, p, st, helm_a) : launch_m<MM, false>(pl, p, st, 0.0))
+    const SlabArgs none;
+#define PZ_ZT(MM) (helm_a >= 0.0 ? launch_m<MM, true>(pl, p, st, helm_a, nz, none) : launch_m<MM, false>(pl, p, st, 0.0, nz, none))
     if (nz <= 32 * 4) return PZ_ZT(4);
     if (nz <= 32 * 8) return PZ_ZT(8);
     if (nz <= 32 * 16) return PZ_ZT(16);
     if (nz <= 32 * 32) return PZ_ZT(32);
 #undef PZ_ZT
     set_error("z-solve variant 2 supports nz <= 1024 (got %d); use zsolve_variant = 0", nz);
+    return PZ_EUNSUPPORTED;
+}
+
+// One z-slab [kb, kb + nk) of cut columns through the same pipeline (pz_zslab.cu): p points at the
+// slab's first plane.  reduce: boundary values into bout; finish: in place with phi_prev / phi_next.
+int launch_zslab_tma(pz_plan *pl, double *p, int kb, int nk, double *bout, const double *phi_prev, const double *phi_next,
+                     cudaStream_t st)
+{
+    SlabArgs sa;
+    sa.kb = kb; sa.bout = bout; sa.phi_prev = phi_prev; sa.phi_next = phi_next; sa.plane = (size_t)pl->nx * pl->ny;
+#define PZ_ZS(MM) (bout ? launch_m<MM, false, 1>(pl, p, st, 0.0, nk, sa) : launch_m<MM, false, 2>(pl, p, st, 0.0, nk, sa))
+    if (nk <= 32 * 4) return PZ_ZS(4);
+    if (nk <= 32 * 8) return PZ_ZS(8);
+    if (nk <= 32 * 16) return PZ_ZS(16);
+    if (nk <= 32 * 32) return PZ_ZS(32);
+#undef PZ_ZS
+    set_error("z-slab: %d planes per slab (at most 1024)", nk);
     return PZ_EUNSUPPORTED;
 }
 

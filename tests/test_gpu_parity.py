@@ -88,6 +88,27 @@ def test_poisson_matches_oracle(torch, pz, wl, oracle, base, nx, ny, nz, variant
     assert abs(wm) <= 1e-13 * np.abs(got).max()
 
 
+@pytest.mark.parametrize("base,nx,ny,nz", [("c1", 16, 16, 1100), ("c3", 32, 16, 1594), ("c1", 16, 8, 2048), ("c1", 8, 8, 2500)])
+@pytest.mark.parametrize("variant", [3, 0])   # 3: the plan's own z cut through the pipeline (default); 0: thread-per-column sweep
+def test_poisson_beyond_1024_planes_matches_oracle(torch, pz, wl, oracle, base, nx, ny, nz, variant):
+    """Whole columns longer than the pipeline's tile (the paper's wall-normal size is 1594)."""
+    w = wl.scaled(wl.CONFIGS[base], nx, ny, nz)
+    zc, zf = wl.grid(w)
+    f = wl.poisson_rhs(w)
+    ref = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)
+    plan = pz.poisson_plan_create(nx, ny, nz, w.lx, w.ly, zc, zf)
+    assert pz.pz_get_option(plan, "zsolve_variant") == 3
+    pz.pz_set_option(plan, "zsolve_variant", variant)
+    p = torch.from_numpy(f).cuda()
+    pz.poisson_solve(plan, p)
+    torch.cuda.synchronize()
+    got = p.cpu().numpy()
+    pz.poisson_plan_destroy(plan)
+    assert rel_err(got, ref) <= TOL
+    dzf = np.diff(zf)
+    assert abs(np.einsum("k,kji->", dzf, got)) / (dzf.sum() * nx * ny) <= 1e-13 * np.abs(got).max()
+
+
 @pytest.mark.parametrize("slab", [1, 3, 1000])
 def test_poisson_slab_size_does_not_change_the_result(torch, pz, wl, slab):
     w = wl.scaled(wl.CONFIGS["c1"], 64, 32, 40)
@@ -643,7 +664,7 @@ def test_helmholtz_z_rhs_and_step_match_oracle(torch, pz, wl, oracle, nx, ny, nz
 def test_error_paths_of_the_widened_entry_points(torch, pz, wl):
     zf = wl.z_faces(1100, 2.0, 1.8)
     plan = pz.poisson_plan_create(16, 16, 1100, 1.0, 1.0, wl.z_centres(zf), zf)
-    assert pz.pz_get_option(plan, "zsolve_variant") == 0          # thread-per-column fallback above nz = 1024
+    assert pz.pz_get_option(plan, "zsolve_variant") == 3          # the plan's own z cut above nz = 1024
     with pytest.raises(pz.PzError) as ei:
         pz.helmholtz3d_setup(plan, -1e-3)
     assert ei.value.status == pz.PZ_EINVAL
