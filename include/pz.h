@@ -50,8 +50,19 @@ enum pz_status {
     PZ_ENOTSETUP = 5     /* helmholtz_z_solve before helmholtz_z_setup */
 };
 
-/* The only boundary-condition set on the hot path: x, y periodic; Poisson: zero wall-normal
- * gradient at both walls (Neumann); Helmholtz: u = 0 at both wall faces (Dirichlet). */
+/* Boundary conditions of the Poisson solve ("Fourier / cosine / sine" expansions,
+ * "multiple combinations of boundary conditions"), one code per direction, combined with PZ_BC:
+ *   x, y:  PZ_PERIODIC, PZ_NEUMANN (zero gradient at both ends: cosine transform) or PZ_DIRICHLET
+ *          (zero value at both end FACES: sine transform);
+ *   z:     PZ_Z_NN (zero wall-normal gradient at both walls), PZ_Z_DD (zero value at both wall
+ *          faces), PZ_Z_ND (gradient at the bottom, value at the top), PZ_Z_DN.
+ * bc = 0 is the hot path of BASELINE.json: periodic x, y, Neumann walls.  Wherever no direction has
+ * a constant eigenvector (any Dirichlet end) the problem is non-singular and nothing is pinned.
+ * The Helmholtz solves keep u = 0 on the wall faces whatever bc; helmholtz3d_*, the z-slab plans
+ * and the pressure-correction calls need bc = 0. */
+enum pz_bc_dir { PZ_PERIODIC = 0, PZ_NEUMANN = 1, PZ_DIRICHLET = 2 };
+enum pz_bc_z { PZ_Z_NN = 0, PZ_Z_DD = 1, PZ_Z_ND = 2, PZ_Z_DN = 3 };
+#define PZ_BC(bcx, bcy, bcz) ((bcx) + 4 * (bcy) + 16 * (bcz))
 enum pz_bc { PZ_BC_PERIODIC_XY_NEUMANN_P_DIRICHLET_U = 0 };
 
 /*

@@ -61,6 +61,14 @@ SIGNATURES = {
 _lib = None
 
 
+def pz_bc(bcx: str = "P", bcy: str = "P", bcz: str = "NN") -> int:
+    """PZ_BC(...) of include/pz.h from letters: x, y in 'P' (periodic), 'N' (zero gradient), 'D' (zero
+    value at the end faces); z in 'NN', 'DD', 'ND', 'DN' (bottom, top)."""
+    d = {"P": 0, "N": 1, "D": 2}
+    z = {"NN": 0, "DD": 1, "ND": 2, "DN": 3}
+    return d[bcx] + 4 * d[bcy] + 16 * z[bcz]
+
+
 class PzError(RuntimeError):
     def __init__(self, status: int, message: str):
         super().__init__(f"pz status {status}: {message}")

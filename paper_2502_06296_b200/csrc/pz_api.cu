@@ -70,6 +70,15 @@ typedef long double ld;
 const ld kPi = 3.141592653589793238462643383279502884L;
 
 // lambda_q = -4 sin^2(pi q / n) / delta^2, folded to q <= n/2 (R1, R6)
+// eigenvalue q of the second difference with zero-gradient (half = 0) or zero-value (half = 1) ends,
+// -4 sin^2(pi (q + half) / (2 n)) / delta^2 (reading R17)
+double lambda_r2r(int q, int n, double length, int dirichlet)
+{
+    const ld delta = (ld)length / (ld)n;
+    const ld s = sinl(kPi * (ld)(q + (dirichlet ? 1 : 0)) / (ld)(2 * (long long)n));
+    return (double)(-(ld)4 * s * s / (delta * delta));
+}
+
 double lambda(int q, int n, double length)
 {
     if (q > n - q) q = n - q;
@@ -138,7 +147,7 @@ bool fused_sizes(const pz_plan *pl)
 
 bool use_fused(const pz_plan *pl)
 {
-    if (pl->opt.slab_planes > 0 || pl->opt.fft_fused == 0 || !fused_sizes(pl)) return false;
+    if (pl->opt.slab_planes > 0 || pl->opt.fft_fused == 0 || !fused_sizes(pl) || pl->bcx || pl->bcy) return false;
     if (pl->opt.fft_fused == 1) return true;
     // auto: the fused kernel hands a plane from the x to the y transform through L2 (16 instead of
     // 32 DRAM bytes per point, ncu r02); that needs a few planes in flight to stay L2-resident, which
@@ -203,8 +212,11 @@ static int plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double 
     if (!zc || !zf) { set_error("poisson_plan_create: zc/zf is NULL"); return PZ_EINVAL; }
     if (nx <= 0 || ny <= 0 || nz <= 0) { set_error("poisson_plan_create: non-positive size %d x %d x %d", nx, ny, nz); return PZ_EINVAL; }
     if (!(lx > 0.0) || !(ly > 0.0) || !std::isfinite(lx) || !std::isfinite(ly)) { set_error("poisson_plan_create: lx, ly must be positive and finite"); return PZ_EINVAL; }
-    if (bc != PZ_BC_PERIODIC_XY_NEUMANN_P_DIRICHLET_U) { set_error("poisson_plan_create: unsupported bc %d", bc); return PZ_EUNSUPPORTED; }
-    if (!(fast_fft_len(nx) || generic_fft_x_ok(nx)) || !(fast_fft_len(ny) || generic_fft_y_ok(ny)) || ((long long)nx * ny) % 16 != 0) {
+    const int bcx = bc & 3, bcy = (bc >> 2) & 3, bcz = (bc >> 4) & 3;
+    if (bc < 0 || bc >= 64 || bcx == 3 || bcy == 3) { set_error("poisson_plan_create: unsupported bc %d", bc); return PZ_EUNSUPPORTED; }
+    if (bc != 0 && nk != nz) { set_error("poisson_slab_plan_create: z-slab plans need bc = 0 (got %d)", bc); return PZ_EUNSUPPORTED; }
+    if (!((bcx == PZ_PERIODIC && fast_fft_len(nx)) || generic_fft_x_ok(nx)) || !((bcy == PZ_PERIODIC && bcx == PZ_PERIODIC && fast_fft_len(ny)) || generic_fft_y_ok(ny)) ||
+        ((long long)nx * ny) % 16 != 0) {
         set_error("poisson_plan_create: nx, ny must be even with nx / 2 and ny products of 2, 3, 5, 7 (nx <= 16384, ny <= 8192) and "
                   "nx ny a multiple of 16 (got %d, %d)", nx, ny);
         return PZ_EUNSUPPORTED;
@@ -247,23 +259,34 @@ static int plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double 
     pl->inv_lz = 1.0 / lz;
     pl->wall_w0 = 2.0 / (pl->dzf[0] * (2.0 * (zc[0] - zf[0])));
     pl->wall_w1 = 2.0 / (pl->dzf[nz - 1] * (2.0 * (zf[nz] - zc[nz - 1])));
+    pl->bcx = bcx; pl->bcy = bcy; pl->bcz = bcz;
+    pl->pw0 = (bcz == PZ_Z_DD || bcz == PZ_Z_DN) ? pl->wall_w0 : 0.0;
+    pl->pw1 = (bcz == PZ_Z_DD || bcz == PZ_Z_ND) ? pl->wall_w1 : 0.0;
+    pl->singular00 = (bcx != PZ_DIRICHLET && bcy != PZ_DIRICHLET && bcz == PZ_Z_NN);
 
     // one device allocation for all tables
-    const size_t ndbl = 4 * (size_t)nz + (size_t)nx + 2 * (size_t)ny + 2 * (size_t)nx + 2 * (size_t)ny + 10;
+    const size_t ndbl = 4 * (size_t)nz + (size_t)nx + 2 * (size_t)ny + 4 * (size_t)nx + 4 * (size_t)ny + 14;
     std::vector<double> host(ndbl, 0.0);
     size_t off = 0;
     auto take = [&](size_t cnt) { size_t o = off; off += (cnt + 1) & ~(size_t)1; return o; }; // keep 16-B alignment
     const size_t oA = take(nz), oC = take(nz), oD = take(nz), oZc = take(nz), oLx = take(nx), oLyn = take(ny), oLyp = take(ny);
-    const size_t oTx = take(2 * (size_t)nx), oTy = take(2 * (size_t)ny);
+    const size_t oTx = take(2 * (size_t)nx), oTy = take(2 * (size_t)ny), oQx = take(2 * (size_t)nx), oQy = take(2 * (size_t)ny);
     for (int k = 0; k < nz; ++k) { host[oA + k] = pl->A[k]; host[oC + k] = pl->C[k]; host[oD + k] = pl->dzf[k]; host[oZc + k] = zc[k]; }
     // modified wavenumbers re-ordered for the packed layout
-    for (int i = 0; i < nx; ++i) host[oLx + i] = lambda(i == 0 ? 0 : (i == 1 ? nx / 2 : i / 2), nx, lx);
+    // (cosine / sine expansions: one real coefficient per index, natural order)
+    for (int i = 0; i < nx; ++i)
+        host[oLx + i] = (bcx == PZ_PERIODIC) ? lambda(i == 0 ? 0 : (i == 1 ? nx / 2 : i / 2), nx, lx) : lambda_r2r(i, nx, lx, bcx == PZ_DIRICHLET);
     for (int j = 0; j < ny; ++j) {
-        host[oLyn + j] = lambda(j, ny, ly);
-        host[oLyp + j] = lambda(j == 0 ? 0 : (j == 1 ? ny / 2 : j / 2), ny, ly);
+        host[oLyn + j] = (bcy == PZ_PERIODIC) ? lambda(j, ny, ly) : lambda_r2r(j, ny, ly, bcy == PZ_DIRICHLET);
+        host[oLyp + j] = (bcy == PZ_PERIODIC) ? lambda(j == 0 ? 0 : (j == 1 ? ny / 2 : j / 2), ny, ly) : host[oLyn + j];
+        // x in cosines / sines, y periodic: EVERY column is a real sequence whose spectrum along y is packed
+        if (bcx != PZ_PERIODIC && bcy == PZ_PERIODIC) host[oLyn + j] = host[oLyp + j];
     }
     for (int k = 0; k < nx; ++k) twiddle(k, nx, &host[oTx + 2 * k], &host[oTx + 2 * k + 1]);
     for (int k = 0; k < ny; ++k) twiddle(k, ny, &host[oTy + 2 * k], &host[oTy + 2 * k + 1]);
+    // exp(-i pi k / (2 n)) = the 4n-th roots of unity, for the cosine / sine expansions
+    for (int k = 0; k < nx; ++k) { host[oQx + 2 * k] = (double)cosl(kPi * (ld)k / (ld)(2 * nx)); host[oQx + 2 * k + 1] = (double)-sinl(kPi * (ld)k / (ld)(2 * nx)); }
+    for (int k = 0; k < ny; ++k) { host[oQy + 2 * k] = (double)cosl(kPi * (ld)k / (ld)(2 * ny)); host[oQy + 2 * k + 1] = (double)-sinl(kPi * (ld)k / (ld)(2 * ny)); }
 
     ce = cudaMalloc(&pl->tables, off * sizeof(double));
     if (ce != cudaSuccess) { cudaGetLastError(); set_error("plan tables: %s", cudaGetErrorString(ce)); return fail(PZ_ENOMEM); }
@@ -273,6 +296,8 @@ static int plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double 
     pl->d_lamx = pl->tables + oLx; pl->d_lamy_nat = pl->tables + oLyn; pl->d_lamy_pk = pl->tables + oLyp;
     pl->d_twx = reinterpret_cast<double2 *>(pl->tables + oTx);
     pl->d_twy = reinterpret_cast<double2 *>(pl->tables + oTy);
+    pl->d_tw4x = reinterpret_cast<double2 *>(pl->tables + oQx);
+    pl->d_tw4y = reinterpret_cast<double2 *>(pl->tables + oQy);
 
     ce = cudaStreamCreateWithFlags(&pl->upload_stream, cudaStreamNonBlocking);
     if (ce != cudaSuccess) return fail(cuda_fail(ce, "cudaStreamCreate"));
@@ -282,7 +307,7 @@ static int plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double 
     pl->opt.zsolve_variant = (nz <= 128) ? 1 : (nz <= 1024) ? 2 : 0;
     const char *cut_env = getenv("PZ_ZCUT_ABOVE");   // tuning aid: internal cut for nz above this (default 1024)
     const int cut_above = cut_env ? atoi(cut_env) : 1024;
-    if (nk == nz && nz > cut_above && nz <= 16 * 512) {
+    if (nk == nz && nz > cut_above && nz <= 16 * 512 && bc == 0) {
         // whole columns longer than the pipeline's tile: the plan's own cut in z (pz_zslab.cu), slabs of
         // at most 512 planes (16 rows per lane: three pipeline stages fit shared memory)
         // full slabs of 512 planes (no padding rows in their tiles) and one remainder of at least 3
@@ -473,6 +498,7 @@ int pz_divergence_rhs(pz_plan *pl, const double *u, const double *v, const doubl
     if (!pl || !u || !v || !w || !rhs) { set_error("pz_divergence_rhs: NULL argument"); return PZ_EINVAL; }
     if (misaligned(u) || misaligned(v) || misaligned(w) || misaligned(rhs)) { set_error("pz_divergence_rhs: fields must be 16-byte aligned"); return PZ_EINVAL; }
     if (!std::isfinite(inv_gdt)) { set_error("pz_divergence_rhs: 1/(gamma dt) must be finite"); return PZ_EINVAL; }
+    if (pl->bcx || pl->bcy || pl->bcz) { set_error("pz_divergence_rhs: needs a plan with bc = 0"); return PZ_EUNSUPPORTED; }
     return launch_divergence_rhs(pl, u, v, w, rhs, inv_gdt, (cudaStream_t)stream);
 }
 
@@ -481,6 +507,7 @@ int pz_project(pz_plan *pl, double *u, double *v, double *w, double *p, const do
     if (!pl || !u || !v || !w || !p || !phi) { set_error("pz_project: NULL argument"); return PZ_EINVAL; }
     if (misaligned(u) || misaligned(v) || misaligned(w) || misaligned(p) || misaligned(phi)) { set_error("pz_project: fields must be 16-byte aligned"); return PZ_EINVAL; }
     if (!std::isfinite(gdt)) { set_error("pz_project: gamma dt must be finite"); return PZ_EINVAL; }
+    if (pl->bcx || pl->bcy || pl->bcz) { set_error("pz_project: needs a plan with bc = 0"); return PZ_EUNSUPPORTED; }
     return launch_project(pl, u, v, w, p, phi, gdt, (cudaStream_t)stream);
 }
 
@@ -488,7 +515,7 @@ int pz_pressure_correction(pz_plan *pl, double *u, double *v, double *w, double 
 {
     if (!(gdt > 0.0) || !std::isfinite(gdt)) { set_error("pz_pressure_correction: gamma dt must be positive and finite"); return PZ_EINVAL; }
     int rc;
-    if (pl && u && v && w && work && pl->opt.div_fused != 0 && pl->opt.slab_planes == 0 && fast_fft_len(pl->nx) &&
+    if (pl && u && v && w && work && pl->opt.div_fused != 0 && pl->opt.slab_planes == 0 && fast_fft_len(pl->nx) && !pl->bcx && !pl->bcy && !pl->bcz &&
         !misaligned(u) && !misaligned(v) && !misaligned(w) && !misaligned(work)) {
         // Eq. (4)'s right-hand side is formed inside the forward x transform: it never touches HBM
         cudaStream_t st = (cudaStream_t)stream;
@@ -540,6 +567,7 @@ int helmholtz3d_solve(pz_plan *pl, double *u, void *stream)
     if (!pl || !u) { set_error("helmholtz3d_solve: NULL argument"); return PZ_EINVAL; }
     if (((uintptr_t)u & 15) != 0) { set_error("helmholtz3d_solve: u must be 16-byte aligned"); return PZ_EINVAL; }
     if (pl->h3_a < 0.0) { set_error("helmholtz3d_solve: call helmholtz3d_setup first"); return PZ_ENOTSETUP; }
+    if (pl->bcx || pl->bcy || pl->bcz) { set_error("helmholtz3d_solve: needs a plan with bc = 0"); return PZ_EUNSUPPORTED; }
     if (pl->slab_G > 0 && !pl->slab_internal) { set_error("helmholtz3d_solve: not available on a z-slab plan"); return PZ_EUNSUPPORTED; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;

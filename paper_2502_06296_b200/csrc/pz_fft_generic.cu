@@ -217,6 +217,214 @@ __global__ void __launch_bounds__(kT, 1) gen_fft_y_kernel(double *__restrict__ p
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Cosine / sine expansions ("Fourier / cosine / sine"; reading R17) for
+// directions with zero-gradient (N) or zero-value (D) ends, through the same passes:
+//   C_k = sum_i x_i cos(pi k (i + 1/2) / L)  =  (1/2) [w_k V_k + conj(w_k) V_{L-k}],  w_k = exp(-i pi k / (2L)),
+//   V = FFT_L(v),  v_m = x_{2m},  v_{L-1-m} = x_{2m+1}                     (reordering of Makhoul)
+// a complex-linear identity, so a complex column (two real sequences) transforms in one go;
+//   S_k = sum_i x_i sin(pi (k+1) (i + 1/2) / L) = C_{L-1-k} of (-1)^i x_i.
+// Inverse: V_0 = C_0, V_k = conj(w_k) (C_k - i C_{L-k}), v = IFFT_L(V) (unnormalised: L v).
+// tw4[k] = exp(-i pi k / (2L)).
+__device__ __forceinline__ double2 mul_i(double2 a) { return make_double2(-a.y, a.x); }
+
+template <bool INV>
+__global__ void __launch_bounds__(kT, 1) gen_r2r_y_kernel(double *__restrict__ p, const double2 *__restrict__ twy, const double2 *__restrict__ tw4,
+                                                        int nx, int L, int tc, Radices rl, int dirichlet)
+{
+    extern __shared__ double2 smem_ry[];
+    double *base = p + (size_t)blockIdx.y * nx * L + 2 * (size_t)blockIdx.x * tc;
+    auto at = [&](int row, int c) { return reinterpret_cast<double2 *>(base + (size_t)row * nx + 2 * c); };
+    if constexpr (!INV) {
+        for (int q = threadIdx.x; q < L * tc; q += kT) {
+            const int row = q / tc, c = q - row * tc;
+            double2 t = *at(row, c);
+            if (dirichlet && (row & 1)) t = make_double2(-t.x, -t.y);
+            const int pos = (row & 1) ? L - 1 - (row >> 1) : (row >> 1);
+            smem_ry[pos * tc + c] = t;
+        }
+        __syncthreads();
+        all_passes(smem_ry, L, tc, 1, tc, twy, 1, rl);
+        for (int q = threadIdx.x; q < (L / 2 + 1) * tc; q += kT) {
+            const int k = q / tc, c = q - k * tc;
+            const double2 vk = smem_ry[k * tc + c];
+            if (k == 0) {
+                *at(dirichlet ? L - 1 : 0, c) = vk;
+            } else {
+                const double2 vm = smem_ry[(L - k) * tc + c], w = __ldg(&tw4[k]);
+                const double2 a = cmul(vk, w), b = cmul_conj(vm, w);
+                const double2 ck = make_double2(0.5 * (a.x + b.x), 0.5 * (a.y + b.y));
+                const double2 cm = mul_i(make_double2(0.5 * (a.x - b.x), 0.5 * (a.y - b.y)));
+                *at(dirichlet ? L - 1 - k : k, c) = ck;
+                if (k != L - k) *at(dirichlet ? k - 1 : L - k, c) = cm;
+            }
+        }
+    } else {
+        for (int q = threadIdx.x; q < L * tc; q += kT) {
+            const int k = q / tc, c = q - k * tc;
+            smem_ry[q] = *at(dirichlet ? L - 1 - k : k, c);
+        }
+        __syncthreads();
+        double2 va[(kE + 1) / 2 + 1], vb[(kE + 1) / 2 + 1];
+#pragma unroll
+        for (int e = 0; e < (kE + 1) / 2 + 1; ++e) {
+            const int q = threadIdx.x + e * kT;
+            if (q < (L / 2 + 1) * tc) {
+                const int k = q / tc, c = q - k * tc;
+                const double2 xk = smem_ry[k * tc + c];
+                if (k == 0) {
+                    va[e] = xk;
+                } else {
+                    const double2 xm = smem_ry[(L - k) * tc + c], w = __ldg(&tw4[k]);
+                    // V_k = conj(w_k) (C_k - i C_{L-k}),  V_{L-k} = w_k (C_k + i C_{L-k})
+                    va[e] = cmul_conj(make_double2(xk.x + xm.y, xk.y - xm.x), w);
+                    vb[e] = cmul(make_double2(xk.x - xm.y, xk.y + xm.x), w);
+                }
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < (kE + 1) / 2 + 1; ++e) {
+            const int q = threadIdx.x + e * kT;
+            if (q < (L / 2 + 1) * tc) {
+                const int k = q / tc, c = q - k * tc;
+                smem_ry[k * tc + c] = cconj(va[e]);
+                if (k != 0 && k != L - k) smem_ry[(L - k) * tc + c] = cconj(vb[e]);
+            }
+        }
+        __syncthreads();
+        all_passes(smem_ry, L, tc, 1, tc, twy, 1, rl);
+        for (int q = threadIdx.x; q < L * tc; q += kT) {
+            const int row = q / tc, c = q - row * tc;
+            const int pos = (row & 1) ? L - 1 - (row >> 1) : (row >> 1);
+            double2 t = cconj(smem_ry[pos * tc + c]);
+            if (dirichlet && (row & 1)) t = make_double2(-t.x, -t.y);
+            *at(row, c) = t;
+        }
+    }
+}
+
+// The same expansions along x: lines of n = 2M REAL points.  The reordered line v is transformed
+// as one complex transform of length M plus the real-to-complex split (as gen_fft_x_kernel), then
+//   C_k = Re(w_k V_k),  C_{n-k} = -Im(w_k V_k)   (0 < k < M),  C_0 = V_0,  C_M = Re(w_M V_M);
+// inverse: V_k = conj(w_k) (C_k - i C_{n-k}), complex-to-real merge, passes, un-reordering.
+// Output / input: n real coefficients per line in natural order (sine: reversed, see above).
+template <bool INV>
+__global__ void __launch_bounds__(kT, 1) gen_r2r_x_kernel(double *__restrict__ p, const double2 *__restrict__ twx, const double2 *__restrict__ tw4,
+                                                        int M, long long nlines, int lpb, Radices rl, double scale, int dirichlet)
+{
+    extern __shared__ double2 smem_rx[];
+    double *sd = reinterpret_cast<double *>(smem_rx);
+    const int n = 2 * M;
+    const long long l0 = (long long)blockIdx.x * lpb;
+    const int nl = (int)((nlines - l0 < lpb) ? nlines - l0 : lpb);
+    double *g = p + (size_t)l0 * n;
+    if constexpr (!INV) {
+        for (int q = threadIdx.x; q < nl * n; q += kT) {
+            const int ln = q / n, i = q - ln * n;
+            double v = g[q];
+            if (dirichlet && (i & 1)) v = -v;
+            sd[ln * n + ((i & 1) ? n - 1 - (i >> 1) : (i >> 1))] = v;
+        }
+        __syncthreads();
+        all_passes(smem_rx, M, nl, M, 1, twx, 2, rl);
+        for (int q = threadIdx.x; q < nl * (M + 1); q += kT) {
+            const int ln = q / (M + 1), k = q - ln * (M + 1);
+            const double2 *z = smem_rx + (size_t)ln * M;
+            double *o = g + (size_t)ln * n;
+            auto put = [&](int coef, double val) { o[dirichlet ? n - 1 - coef : coef] = val; };
+            if (k == 0) {
+                put(0, z[0].x + z[0].y);
+            } else if (k == M) {
+                put(M, (z[0].x - z[0].y) * __ldg(&tw4[M]).x);
+            } else {
+                const double2 zk = z[k], zm = cconj(z[M - k]);
+                const double2 ev = make_double2(0.5 * (zk.x + zm.x), 0.5 * (zk.y + zm.y));
+                const double2 d = csub(zk, zm);
+                const double2 vk = cadd(ev, cmul(make_double2(0.5 * d.y, -0.5 * d.x), __ldg(&twx[k])));
+                const double2 t = cmul(vk, __ldg(&tw4[k]));
+                put(k, t.x);
+                put(n - k, -t.y);
+            }
+        }
+    } else {
+        for (int q = threadIdx.x; q < nl * n; q += kT) {
+            const int ln = q / n, k = q - ln * n;
+            sd[q] = g[(size_t)ln * n + (dirichlet ? n - 1 - k : k)];
+        }
+        __syncthreads();
+        // half spectrum V_k (k = 0..M) of the real reordered line, merged into the complex line of length M
+        double2 zr[kE];
+#pragma unroll
+        for (int e = 0; e < kE; ++e) {
+            const int q = threadIdx.x + e * kT;
+            if (q < nl * M) {
+                const int ln = q / M, k = q - ln * M;
+                const double *c = sd + (size_t)ln * n;
+                auto V = [&](int kk) {   // kk in 1..M
+                    const double2 w = __ldg(&tw4[kk]);
+                    return cmul_conj(make_double2(c[kk], -c[n - kk]), w);
+                };
+                if (k == 0) {
+                    const double v0 = c[0], vm = V(M).x;   // V_M is real
+                    zr[e] = make_double2(v0 + vm, -(v0 - vm));
+                } else {
+                    const double2 xk = V(k), xm = cconj(V(M - k));
+                    const double2 sm = cadd(xk, xm), cc = cmul_conj(csub(xk, xm), __ldg(&twx[k]));
+                    zr[e] = make_double2(sm.x - cc.y, -(sm.y + cc.x));
+                }
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < kE; ++e) {
+            const int q = threadIdx.x + e * kT;
+            if (q < nl * M) smem_rx[q] = zr[e];
+        }
+        __syncthreads();
+        all_passes(smem_rx, M, nl, M, 1, twx, 2, rl);
+        for (int q = threadIdx.x; q < nl * n; q += kT) {
+            const int ln = q / n, i = q - ln * n;
+            const int pos = (i & 1) ? n - 1 - (i >> 1) : (i >> 1);
+            double v = sd[ln * n + pos];
+            if (pos & 1) v = -v;                       // imaginary parts come out conjugated
+            if (dirichlet && (i & 1)) v = -v;
+            g[q] = v * scale;
+        }
+    }
+}
+
+// Separation of the two real sequences held by EVERY packed pair after a complex transform along y
+// (x expanded in cosines / sines: neighbouring columns are different real modes), as pair0_kernel
+// of pz_fft_y.cu does for pair 0: rows (2r, 2r+1) hold (Re A_r, Re B_r), (Im A_r, Im B_r); rows
+// 0, 1 hold r = 0, L/2.  One CTA per (pair, plane).
+template <bool INV>
+__global__ void __launch_bounds__(256) gen_allpairs_kernel(double *__restrict__ p, int nx, int L)
+{
+    extern __shared__ double2 smem_ap[];
+    double *base = p + (size_t)blockIdx.y * nx * L + 2 * (size_t)blockIdx.x;
+    auto at = [&](int row) { return reinterpret_cast<double2 *>(base + (size_t)row * nx); };
+    for (int r = threadIdx.x; r < L; r += blockDim.x) smem_ap[r] = *at(r);
+    __syncthreads();
+    const int h = L / 2;
+    for (int r = threadIdx.x; r <= h; r += blockDim.x) {
+        if constexpr (!INV) {
+            if (r == 0 || r == h) { *at(r == 0 ? 0 : 1) = smem_ap[r]; continue; }
+            const double2 w = smem_ap[r], wm = cconj(smem_ap[L - r]);
+            const double2 a = make_double2(0.5 * (w.x + wm.x), 0.5 * (w.y + wm.y));
+            const double2 d = csub(w, wm);
+            const double2 b = make_double2(0.5 * d.y, -0.5 * d.x);
+            *at(2 * r) = make_double2(a.x, b.x);
+            *at(2 * r + 1) = make_double2(a.y, b.y);
+        } else {
+            if (r == 0 || r == h) { *at(r) = smem_ap[r == 0 ? 0 : 1]; continue; }
+            const double2 lo = smem_ap[2 * r], hi = smem_ap[2 * r + 1];
+            *at(r) = make_double2(lo.x - hi.y, hi.x + lo.y);        // A_r + i B_r
+            *at(L - r) = make_double2(lo.x + hi.y, lo.y - hi.x);    // conj(A_r) + i conj(B_r)
+        }
+    }
+}
+
 bool factor(int n, Radices *out)
 {
     out->n = 0;
@@ -283,6 +491,72 @@ int launch_fft_y_generic(const pz_plan *pl, double *p, int nk, bool inverse, cud
     ProfScope prof(pl, inverse ? PZ_K_FFT_Y_INV : PZ_K_FFT_Y_FWD, st);
     if (inverse) gen_fft_y_kernel<true><<<grid, kT, smem, st>>>(p, pl->d_twy, pl->nx, L, tc, rl);
     else gen_fft_y_kernel<false><<<grid, kT, smem, st>>>(p, pl->d_twy, pl->nx, L, tc, rl);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+} // namespace pz
+
+namespace pz {
+
+// ---- cosine / sine expansions (bcx / bcy = PZ_NEUMANN, PZ_DIRICHLET)
+int launch_r2r_x(const pz_plan *pl, double *p, long long nlines, bool inverse, cudaStream_t st)
+{
+    const int M = pl->nx / 2;
+    Radices rl;
+    if (!factor(M, &rl)) { set_error("r2r_x: nx / 2 = %d has a prime factor above 7", M); return PZ_EUNSUPPORTED; }
+    int lpb = kPts / M;
+    if (lpb > 64) lpb = 64;
+    while (lpb > 1 && (nlines + lpb - 1) / lpb < 4LL * pl->num_sms) lpb /= 2;
+    const size_t smem = (size_t)lpb * M * sizeof(double2);
+    const long long blocks = (nlines + lpb - 1) / lpb;
+    const double scale = 1.0 / ((double)pl->nx * (double)pl->ny);
+    const int dir = (pl->bcx == PZ_DIRICHLET) ? 1 : 0;
+    int rc;
+    if ((rc = smem_optin(pl, gen_r2r_x_kernel<false>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
+    if ((rc = smem_optin(pl, gen_r2r_x_kernel<true>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
+    ProfScope prof(pl, inverse ? PZ_K_FFT_X_INV : PZ_K_FFT_X_FWD, st);
+    if (inverse) gen_r2r_x_kernel<true><<<(unsigned)blocks, kT, smem, st>>>(p, pl->d_twx, pl->d_tw4x, M, nlines, lpb, rl, scale, dir);
+    else gen_r2r_x_kernel<false><<<(unsigned)blocks, kT, smem, st>>>(p, pl->d_twx, pl->d_tw4x, M, nlines, lpb, rl, scale, dir);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+int launch_r2r_y(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_t st)
+{
+    const int L = pl->ny, npairs = pl->nx / 2;
+    Radices rl;
+    if (!factor(L, &rl)) { set_error("r2r_y: ny = %d has a prime factor above 7", L); return PZ_EUNSUPPORTED; }
+    int tc = 8;
+    while (tc > 1 && (npairs % tc != 0 || tc * L > kPts)) tc /= 2;
+    if (tc * L > kPts) { set_error("r2r_y: ny = %d exceeds the %d-point buffer", L, kPts); return PZ_EUNSUPPORTED; }
+    const size_t smem = (size_t)tc * L * sizeof(double2);
+    const int dir = (pl->bcy == PZ_DIRICHLET) ? 1 : 0;
+    int rc;
+    if ((rc = smem_optin(pl, gen_r2r_y_kernel<false>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
+    if ((rc = smem_optin(pl, gen_r2r_y_kernel<true>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
+    dim3 grid((unsigned)(npairs / tc), (unsigned)nk);
+    ProfScope prof(pl, inverse ? PZ_K_FFT_Y_INV : PZ_K_FFT_Y_FWD, st);
+    if (inverse) gen_r2r_y_kernel<true><<<grid, kT, smem, st>>>(p, pl->d_twy, pl->d_tw4y, pl->nx, L, tc, rl, dir);
+    else gen_r2r_y_kernel<false><<<grid, kT, smem, st>>>(p, pl->d_twy, pl->d_tw4y, pl->nx, L, tc, rl, dir);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+// x in cosines / sines, y periodic: every pair of columns holds two real sequences
+int launch_allpairs(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_t st)
+{
+    const size_t smem = (size_t)pl->ny * sizeof(double2);
+    int rc;
+    if ((rc = smem_optin(pl, gen_allpairs_kernel<false>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
+    if ((rc = smem_optin(pl, gen_allpairs_kernel<true>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
+    dim3 grid((unsigned)(pl->nx / 2), (unsigned)nk);
+    ProfScope prof(pl, inverse ? PZ_K_PAIR0_INV : PZ_K_PAIR0_FWD, st);
+    if (inverse) gen_allpairs_kernel<true><<<grid, 256, smem, st>>>(p, pl->nx, pl->ny);
+    else gen_allpairs_kernel<false><<<grid, 256, smem, st>>>(p, pl->nx, pl->ny);
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;

@@ -196,6 +196,10 @@ int launch_fft_x(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cud
     double *base = p + (size_t)k0 * pl->nx * pl->ny;
     const long long nlines = (long long)nk * pl->ny;
     if (div && (inverse || k0 != 0 || nk != pl->nz)) { set_error("fft_x: the fused divergence needs the whole field, forward"); return PZ_EINVAL; }
+    if (pl->bcx != PZ_PERIODIC) {
+        if (div) { set_error("fft_x: the fused divergence needs periodic x"); return PZ_EUNSUPPORTED; }
+        return launch_r2r_x(pl, base, nlines, inverse, st);
+    }
     if (!fast_fft_len(pl->nx)) {
         if (div) { set_error("fft_x: the fused divergence needs a power-of-two nx"); return PZ_EUNSUPPORTED; }
         return launch_fft_x_generic(pl, base, nlines, inverse, st);

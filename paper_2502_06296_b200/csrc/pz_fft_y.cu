@@ -227,12 +227,16 @@ int dispatch(const pz_plan *pl, double *p, int nk, cudaStream_t st)
 int launch_fft_y(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st)
 {
     double *base = p + (size_t)k0 * pl->nx * pl->ny;
-    if (!fast_fft_len(pl->ny) || (pl->nx / 2) % 2 != 0) return launch_fft_y_generic(pl, base, nk, inverse, st);
+    if (pl->bcy != PZ_PERIODIC) return launch_r2r_y(pl, base, nk, inverse, st);
+    // x in cosines / sines: no pair is special, the separate conversion pass handles all of them
+    if (!fast_fft_len(pl->ny) || (pl->nx / 2) % 2 != 0 || pl->bcx != PZ_PERIODIC) return launch_fft_y_generic(pl, base, nk, inverse, st);
     return inverse ? dispatch<true>(pl, base, nk, st) : dispatch<false>(pl, base, nk, st);
 }
 
 int launch_pair0(const pz_plan *pl, double *p, int k0, int nk, bool inverse, cudaStream_t st)
 {
+    if (pl->bcy != PZ_PERIODIC) return PZ_OK; // cosine / sine coefficients of real sequences are real: nothing is packed
+    if (pl->bcx != PZ_PERIODIC) return launch_allpairs(pl, p + (size_t)k0 * pl->nx * pl->ny, nk, inverse, st);
     if (pl->opt.fft_y_p0 != 0 && fast_fft_len(pl->ny) && (pl->nx / 2) % 2 == 0) return PZ_OK; // done inside fft_y_kernel
     double *base = p + (size_t)k0 * pl->nx * pl->ny;
     const size_t smem = (size_t)pl->ny * sizeof(double2);

@@ -76,9 +76,15 @@ struct pz_plan {
     double *d_lamy_pk = nullptr;     // ny: lambda_y, packed order (columns i = 0, 1)
     double2 *d_twx = nullptr;        // nx: exp(-2 pi i k / nx)
     double2 *d_twy = nullptr;        // ny: exp(-2 pi i k / ny)
+    double2 *d_tw4x = nullptr;       // nx: exp(-i pi k / (2 nx)), cosine / sine expansions
+    double2 *d_tw4y = nullptr;       // ny: exp(-i pi k / (2 ny))
     double inv_lz = 0;               // 1 / sum dzf
     double wall_w0 = 0, wall_w1 = 0; // Dirichlet wall terms W_0, W_{nz-1} of the Helmholtz operators
     double h3_a = -1.0;              // helmholtz3d_setup: a of the fully implicit Helmholtz solve
+    int bcx = 0, bcy = 0, bcz = 0;   // pz_bc_dir, pz_bc_dir, pz_bc_z of the Poisson solve
+    double pw0 = 0, pw1 = 0;         // Poisson: Dirichlet wall terms of the first / last z row (0 = Neumann)
+    bool singular00 = true;          // the (0,0) column is singular (no Dirichlet end anywhere) and is pinned
+    int zflags() const { return ((pw0 != 0.0 || pw1 != 0.0) ? 1 : 0) | (singular00 ? 2 : 0); }
 
     // optional workspaces (allocated on first use)
     double *d_zwork = nullptr;       // variant-0 z solve: N doubles
@@ -187,6 +193,9 @@ bool generic_fft_y_ok(int ny);
 inline bool fast_fft_len(int n) { return n >= 8 && n <= 4096 && (n & (n - 1)) == 0; }
 int launch_fft_x_generic(const pz_plan *pl, double *p, long long nlines, bool inverse, cudaStream_t st);
 int launch_fft_y_generic(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_t st);
+int launch_r2r_x(const pz_plan *pl, double *p, long long nlines, bool inverse, cudaStream_t st);
+int launch_r2r_y(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_t st);
+int launch_allpairs(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_t st);
 int launch_fft_xy_fwd(pz_plan *pl, double *p, cudaStream_t st);
 int launch_fft_xy_inv(pz_plan *pl, double *p, cudaStream_t st);
 int launch_zslab_tma(pz_plan *pl, double *p, int kb, int nk, double *bout, const double *phi_prev, const double *phi_next,

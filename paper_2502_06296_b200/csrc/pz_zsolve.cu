@@ -27,17 +27,18 @@ __global__ void __launch_bounds__(128)
     zsolve_thomas_kernel(double *__restrict__ p, double *__restrict__ work, const double *__restrict__ A,
                          const double *__restrict__ C, const double *__restrict__ dzf,
                          const double *__restrict__ lamx, const double *__restrict__ lamy_nat,
-                         const double *__restrict__ lamy_pk, int nx, int ny, int nz, double inv_lz)
+                         const double *__restrict__ lamy_pk, int nx, int ny, int nz, double inv_lz, double pw0,
+                         double pw1, int zflags)
 {
     const size_t plane = (size_t)nx * ny;
     const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= plane) return;
     const int i = (int)(col % nx), j = (int)(col / nx);
     const double sigma = -(lamx[i] + (i < 2 ? lamy_pk[j] : lamy_nat[j]));
-    const bool singular = (i == 0 && j == 0);
+    const bool singular = (i == 0 && j == 0) && (zflags & 2);
 
     // forward: p_k = C_k + e_k, e_k = sigma + A_k e_{k-1}/p_{k-1}; g_k = (-d_k + A_k g_{k-1})/p_k
-    double e = sigma;
+    double e = sigma + pw0;   // Dirichlet wall: extra diagonal term of the first row
     double pk = C[0] + e;
     double rp = 1.0 / pk;
     double g = -p[col] * rp;
@@ -46,7 +47,7 @@ __global__ void __launch_bounds__(128)
     for (int k = 1; k < nz; ++k) {
         const double a = A[k], c = C[k];
         const double d = p[(size_t)k * plane + col];
-        e = fma(a * e, rp, sigma);
+        e = fma(a * e, rp, sigma) + (k == nz - 1 ? pw1 : 0.0);
         pk = c + e;
         if (singular && k == nz - 1) {
             // gauge: the last equation of the singular (0,0) system is replaced by phi = 0
@@ -95,7 +96,8 @@ int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
     const unsigned blocks = (unsigned)((plane + 127) / 128);
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
     zsolve_thomas_kernel<<<blocks, 128, 0, st>>>(p, pl->d_zwork, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
-                                                  pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, pl->nz, pl->inv_lz);
+                                                  pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, pl->nz, pl->inv_lz, pl->pw0, pl->pw1,
+                                                  pl->zflags());
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;

@@ -34,7 +34,7 @@ __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 
     zsolve_cr_kernel(double *__restrict__ p, const double *__restrict__ A, const double *__restrict__ C,
                      const double *__restrict__ dzf, const double *__restrict__ lamx,
                      const double *__restrict__ lamy_nat, const double *__restrict__ lamy_pk, int nx, int ny,
-                     int nz, double inv_lz, double ha, double hw0, double hw1)
+                     int nz, double inv_lz, double ha, double hw0, double hw1, int zflags)
 {
     constexpr int CH = M * kTX + 2;  // doubles per sub-domain in the tile (+2: bank spread, 16-B aligned)
     constexpr int CS = M + 1;        // coefficient stride per lane (bank spread)
@@ -58,7 +58,8 @@ __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 
             const double sc = HELM ? ha : 1.0;
             s_al[(k / M) * CS + (k % M)] = (k < nz) ? sc * A[k] : 0.0;
             s_ga[(k / M) * CS + (k % M)] = (k < nz) ? sc * C[k] : 0.0;
-            s_e0[(k / M) * CS + (k % M)] = 1.0 + ha * ((k == 0 ? hw0 : 0.0) + (k == nz - 1 ? hw1 : 0.0));
+            const double wk = (k == 0 ? hw0 : 0.0) + (k == nz - 1 ? hw1 : 0.0);
+            s_e0[(k / M) * CS + (k % M)] = HELM ? 1.0 + ha * wk : wk;
         }
     }
     __syncthreads();
@@ -80,11 +81,21 @@ __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 
                 solve_pair<M, 1, false, false, true>(d, al, ga, ha * sig0, k0, nz, dzf, inv_lz, e0);
                 solve_pair<M, 2, false, false, true>(d, al, ga, ha * sig1, k0, nz, dzf, inv_lz, e0);
             }
+        } else if (zflags & 1) {
+            // Dirichlet wall(s): the wall rows carry the excess W (s_e0); no column is singular
+            const double *ex = s_e0 + lane * CS;
+            const double2 z2 = make_double2(0.0, 0.0);
+            if (sig0 == sig1) {
+                solve_pair<M, 3, false, false, false, true>(d, al, ga, sig0, k0, nz, nullptr, 0.0, ex, z2, z2);
+            } else {
+                solve_pair<M, 1, false, false, false, true>(d, al, ga, sig0, k0, nz, nullptr, 0.0, ex, z2, z2);
+                solve_pair<M, 2, false, false, false, true>(d, al, ga, sig1, k0, nz, nullptr, 0.0, ex, z2, z2);
+            }
         } else if (sig0 == sig1) {
             solve_pair<M, 3, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
         } else {
             // pair 0 of a row: x-modes 0 and nx/2 have different eigenvalues; (0,0) is singular
-            if (i == 0 && j == 0)
+            if (i == 0 && j == 0 && (zflags & 2))
                 solve_pair<M, 1, true>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
             else
                 solve_pair<M, 1, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
@@ -115,7 +126,8 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha)
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
     zsolve_cr_kernel<M, HELM><<<blocks, kPairs * kLanes, smem, st>>>(p, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
                                                                       pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny,
-                                                                      pl->nz, pl->inv_lz, ha, pl->wall_w0, pl->wall_w1);
+                                                                      pl->nz, pl->inv_lz, ha, HELM ? pl->wall_w0 : pl->pw0,
+                                                                      HELM ? pl->wall_w1 : pl->pw1, pl->zflags());
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;

@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(kThreads, 1)
     zsolve_tma_kernel(const __grid_constant__ CUtensorMap map, const double *__restrict__ A,
                       const double *__restrict__ C, const double *__restrict__ dzf, const double *__restrict__ lamx,
                       const double *__restrict__ lamy_nat, const double *__restrict__ lamy_pk, int nx, int ny, int nz,
-                      double inv_lz, int ntiles, int stages, double ha, double hw0, double hw1, int probe, const SlabArgs sa)
+                      double inv_lz, int ntiles, int stages, double ha, double hw0, double hw1, int probe, const SlabArgs sa, int zflags)
 {
     static_assert(!(HELM && MODE != 0), "slabs of cut columns are Poisson systems");
     using G = Geo<M>;
@@ -97,7 +97,9 @@ __global__ void __launch_bounds__(kThreads, 1)
     for (int k = threadIdx.x; k < kLanes * M; k += blockDim.x) {
         const double sc = HELM ? ha : 1.0;
         double al = (k < nz) ? sc * A[sa.kb + k] : 0.0, ga = (k < nz) ? sc * C[sa.kb + k] : 0.0;
-        double ex = 1.0 + ha * ((k == 0 ? hw0 : 0.0) + (k == nz - 1 ? hw1 : 0.0));
+        // HELM: 1 + a W_k; Poisson with Dirichlet walls (zflags bit 0): W_k, the wall rows' extra diagonal
+        const double wk = (k == 0 ? hw0 : 0.0) + (k == nz - 1 ? hw1 : 0.0);
+        double ex = HELM ? 1.0 + ha * wk : wk;
         if constexpr (MODE != 0) {
             // couplings across the slab's ends leave the matrix; their magnitude stays on the diagonal
             ex = 0.0;
@@ -209,12 +211,22 @@ __global__ void __launch_bounds__(kThreads, 1)
                 solve_pair<M, 1, false, false, true>(d, al, ga, ha * sig0, k0, nz, dzf, inv_lz, e0);
                 solve_pair<M, 2, false, false, true>(d, al, ga, ha * sig1, k0, nz, dzf, inv_lz, e0);
             }
+        } else if (zflags & 1) {
+            // Dirichlet wall(s): the wall rows carry the excess W (s_e0); no column is singular
+            const double *ex = s_e0 + lane * G::CS;
+            const double2 z2 = make_double2(0.0, 0.0);
+            if (sig0 == sig1) {
+                solve_pair<M, 3, false, false, false, true>(d, al, ga, sig0, k0, nz, nullptr, 0.0, ex, z2, z2);
+            } else {
+                solve_pair<M, 1, false, false, false, true>(d, al, ga, sig0, k0, nz, nullptr, 0.0, ex, z2, z2);
+                solve_pair<M, 2, false, false, false, true>(d, al, ga, sig1, k0, nz, nullptr, 0.0, ex, z2, z2);
+            }
         } else if (sig0 == sig1) {
             if (no_pad) solve_pair<M, 3, false, true>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
             else solve_pair<M, 3, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
         } else {
             // pair 0 of a row: x-modes 0 and nx/2 have different eigenvalues; (0,0) is singular
-            if (i == 0 && j == 0)
+            if (i == 0 && j == 0 && (zflags & 2))
                 solve_pair<M, 1, true>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
             else
                 solve_pair<M, 1, false>(d, al, ga, sig0, k0, nz, dzf, inv_lz);
@@ -258,8 +270,8 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha, int nk, const S
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
     zsolve_tma_kernel<M, HELM, MODE><<<blocks, kThreads, smem, st>>>(map, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
                                                                       pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, nk,
-                                                                      pl->inv_lz, ntiles, stages, ha, pl->wall_w0, pl->wall_w1,
-                                                                      pl->opt.zsolve_probe, sa);
+                                                                      pl->inv_lz, ntiles, stages, ha, HELM ? pl->wall_w0 : pl->pw0,
+                                                                      HELM ? pl->wall_w1 : pl->pw1, pl->opt.zsolve_probe, sa, pl->zflags());
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
