@@ -19,9 +19,10 @@ namespace pz {
 
 namespace {
 
-constexpr int kT = 512;   // threads per CTA
 constexpr int kE = 16;    // complex points per thread, at most
-constexpr int kPts = kT * kE;
+constexpr int kPts = 512 * kE;   // largest buffer: 512 threads
+// Threads per CTA: 512 (8192-point buffer, one CTA per SM) where a line or a useful tile needs it,
+// else 256 (4096 points, two CTAs per SM: the loads of one overlap the passes of the other).
 
 struct Radices { int n; int r[20]; };
 
@@ -53,6 +54,15 @@ template <> __device__ __forceinline__ void dft<8>(double2 (&v)[8])
     for (int i = 0; i < 8; ++i) t[i] = v[i];
 #pragma unroll
     for (int i = 0; i < 8; ++i) v[i] = t[bitrev(i, 3)];
+}
+template <> __device__ __forceinline__ void dft<16>(double2 (&v)[16])
+{
+    dif<16, 1>(v);
+    double2 t[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) t[i] = v[i];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = t[bitrev(i, 4)];
 }
 template <> __device__ __forceinline__ void dft<3>(double2 (&v)[3])
 {
@@ -97,63 +107,66 @@ template <> __device__ __forceinline__ void dft<7>(double2 (&v)[7])
 
 // One in-place pass over `nlines` lines of complex length L in shared memory; element pos of line
 // ln sits at s[ln * sl + pos * sp].  tw[k * tws] = exp(-2 pi i k / L).
-template <int R>
+template <int R, int kT>
 __device__ __forceinline__ void pass(double2 *s, int L, int Ns, int nlines, int sl, int sp, const double2 *__restrict__ tw, int tws)
 {
     constexpr int Q = (kE + R - 1) / R;
     const int nb = L / R, W = nlines * nb, step = (L / (Ns * R)) * tws;
+    const int instr = nb * sp, outstr = Ns * sp;
     double2 v[Q][R];
+    int obase[Q];
 #pragma unroll
     for (int q = 0; q < Q; ++q) {
-        const int w = threadIdx.x + q * kT;
-        if (w < W) {
-            // lines fastest when they are interleaved in memory (sl == 1), butterflies fastest otherwise
-            const int ln = (sl == 1) ? w % nlines : w / nb, j = (sl == 1) ? w / nlines : w % nb;
-            const double2 *x = s + (size_t)ln * sl + (size_t)j * sp;
-            const int jm = j % Ns;
+        // work items past the end recompute item 0 and store nothing (no divergent definitions)
+        const int w0 = (int)threadIdx.x + q * kT, w = (w0 < W) ? w0 : 0;
+        // lines fastest when they are interleaved in memory (sl == 1), butterflies fastest otherwise
+        const int ln = (sl == 1) ? w % nlines : w / nb, j = (sl == 1) ? w / nlines : w % nb;
+        const int jm = j % Ns;
+        const double2 *x = s + (ln * sl + j * sp);
+        obase[q] = (w0 < W) ? ln * sl + ((j - jm) * R + jm) * sp : -1;
+        const int tstep = jm * step;
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                double2 t = x[(size_t)r * nb * sp];
-                if (r > 0 && Ns > 1) t = cmul(t, __ldg(&tw[(size_t)r * jm * step]));
-                v[q][r] = t;
-            }
-            dft<R>(v[q]);
+        for (int r = 0; r < R; ++r) {
+            double2 t = x[r * instr];
+            if (r > 0) t = cmul(t, __ldg(&tw[r * tstep]));
+            v[q][r] = t;
         }
+        dft<R>(v[q]);
     }
     __syncthreads();
 #pragma unroll
     for (int q = 0; q < Q; ++q) {
-        const int w = threadIdx.x + q * kT;
-        if (w < W) {
-            const int ln = (sl == 1) ? w % nlines : w / nb, j = (sl == 1) ? w / nlines : w % nb;
-            double2 *y = s + (size_t)ln * sl + (size_t)((j / Ns) * Ns * R + (j % Ns)) * sp;
+        if (obase[q] >= 0) {
+            double2 *y = s + obase[q];
 #pragma unroll
-            for (int r = 0; r < R; ++r) y[(size_t)r * Ns * sp] = v[q][r];
+            for (int r = 0; r < R; ++r) y[r * outstr] = v[q][r];
         }
     }
     __syncthreads();
 }
 
+template <int kT>
 __device__ __forceinline__ void all_passes(double2 *s, int L, int nlines, int sl, int sp, const double2 *__restrict__ tw, int tws,
                                            const Radices &rl)
 {
     int Ns = 1;
     for (int i = 0; i < rl.n; ++i) {
         switch (rl.r[i]) {
-        case 2: pass<2>(s, L, Ns, nlines, sl, sp, tw, tws); break;
-        case 3: pass<3>(s, L, Ns, nlines, sl, sp, tw, tws); break;
-        case 4: pass<4>(s, L, Ns, nlines, sl, sp, tw, tws); break;
-        case 5: pass<5>(s, L, Ns, nlines, sl, sp, tw, tws); break;
-        case 7: pass<7>(s, L, Ns, nlines, sl, sp, tw, tws); break;
-        default: pass<8>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        case 2: pass<2, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        case 3: pass<3, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        case 4: pass<4, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        case 5: pass<5, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        case 7: pass<7, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        case 16: pass<16, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+        default: pass<8, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
         }
         Ns *= rl.r[i];
     }
 }
 
 // x lines: lpb lines of n = 2M reals per CTA.  twx[k] = exp(-2 pi i k / n).
-template <bool INV>
-__global__ void __launch_bounds__(kT, 1) gen_fft_x_kernel(double *__restrict__ p, const double2 *__restrict__ twx, int M, long long nlines,
+template <bool INV, int kT>
+__global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_fft_x_kernel(double *__restrict__ p, const double2 *__restrict__ twx, int M, long long nlines,
                                                         int lpb, Radices rl, double scale)
 {
     extern __shared__ double2 smem_gx[];
@@ -176,7 +189,7 @@ __global__ void __launch_bounds__(kT, 1) gen_fft_x_kernel(double *__restrict__ p
         smem_gx[q] = z;
     }
     __syncthreads();
-    all_passes(smem_gx, M, nl, M, 1, twx, 2, rl);
+    all_passes<kT>(smem_gx, M, nl, M, 1, twx, 2, rl);
     for (int q = threadIdx.x; q < nl * M; q += kT) {
         const int ln = q / M, k = q - ln * M;
         const double2 z = smem_gx[q];
@@ -197,8 +210,8 @@ __global__ void __launch_bounds__(kT, 1) gen_fft_x_kernel(double *__restrict__ p
 }
 
 // y columns: TC neighbouring packed pairs x all ny rows of one plane per CTA.  twy[k] = exp(-2 pi i k / ny).
-template <bool INV>
-__global__ void __launch_bounds__(kT, 1) gen_fft_y_kernel(double *__restrict__ p, const double2 *__restrict__ twy, int nx, int ny, int tc,
+template <bool INV, int kT>
+__global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_fft_y_kernel(double *__restrict__ p, const double2 *__restrict__ twy, int nx, int ny, int tc,
                                                         Radices rl)
 {
     extern __shared__ double2 smem_gy[];
@@ -209,7 +222,7 @@ __global__ void __launch_bounds__(kT, 1) gen_fft_y_kernel(double *__restrict__ p
         smem_gy[q] = INV ? cconj(t) : t;
     }
     __syncthreads();
-    all_passes(smem_gy, ny, tc, 1, tc, twy, 1, rl);
+    all_passes<kT>(smem_gy, ny, tc, 1, tc, twy, 1, rl);
     for (int q = threadIdx.x; q < ny * tc; q += kT) {
         const int row = q / tc, c = q - row * tc;
         const double2 t = smem_gy[q];
@@ -228,8 +241,8 @@ __global__ void __launch_bounds__(kT, 1) gen_fft_y_kernel(double *__restrict__ p
 // tw4[k] = exp(-i pi k / (2L)).
 __device__ __forceinline__ double2 mul_i(double2 a) { return make_double2(-a.y, a.x); }
 
-template <bool INV>
-__global__ void __launch_bounds__(kT, 1) gen_r2r_y_kernel(double *__restrict__ p, const double2 *__restrict__ twy, const double2 *__restrict__ tw4,
+template <bool INV, int kT>
+__global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_r2r_y_kernel(double *__restrict__ p, const double2 *__restrict__ twy, const double2 *__restrict__ tw4,
                                                         int nx, int L, int tc, Radices rl, int dirichlet)
 {
     extern __shared__ double2 smem_ry[];
@@ -244,7 +257,7 @@ __global__ void __launch_bounds__(kT, 1) gen_r2r_y_kernel(double *__restrict__ p
             smem_ry[pos * tc + c] = t;
         }
         __syncthreads();
-        all_passes(smem_ry, L, tc, 1, tc, twy, 1, rl);
+        all_passes<kT>(smem_ry, L, tc, 1, tc, twy, 1, rl);
         for (int q = threadIdx.x; q < (L / 2 + 1) * tc; q += kT) {
             const int k = q / tc, c = q - k * tc;
             const double2 vk = smem_ry[k * tc + c];
@@ -293,7 +306,7 @@ __global__ void __launch_bounds__(kT, 1) gen_r2r_y_kernel(double *__restrict__ p
             }
         }
         __syncthreads();
-        all_passes(smem_ry, L, tc, 1, tc, twy, 1, rl);
+        all_passes<kT>(smem_ry, L, tc, 1, tc, twy, 1, rl);
         for (int q = threadIdx.x; q < L * tc; q += kT) {
             const int row = q / tc, c = q - row * tc;
             const int pos = (row & 1) ? L - 1 - (row >> 1) : (row >> 1);
@@ -309,8 +322,8 @@ __global__ void __launch_bounds__(kT, 1) gen_r2r_y_kernel(double *__restrict__ p
 //   C_k = Re(w_k V_k),  C_{n-k} = -Im(w_k V_k)   (0 < k < M),  C_0 = V_0,  C_M = Re(w_M V_M);
 // inverse: V_k = conj(w_k) (C_k - i C_{n-k}), complex-to-real merge, passes, un-reordering.
 // Output / input: n real coefficients per line in natural order (sine: reversed, see above).
-template <bool INV>
-__global__ void __launch_bounds__(kT, 1) gen_r2r_x_kernel(double *__restrict__ p, const double2 *__restrict__ twx, const double2 *__restrict__ tw4,
+template <bool INV, int kT>
+__global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_r2r_x_kernel(double *__restrict__ p, const double2 *__restrict__ twx, const double2 *__restrict__ tw4,
                                                         int M, long long nlines, int lpb, Radices rl, double scale, int dirichlet)
 {
     extern __shared__ double2 smem_rx[];
@@ -327,7 +340,7 @@ __global__ void __launch_bounds__(kT, 1) gen_r2r_x_kernel(double *__restrict__ p
             sd[ln * n + ((i & 1) ? n - 1 - (i >> 1) : (i >> 1))] = v;
         }
         __syncthreads();
-        all_passes(smem_rx, M, nl, M, 1, twx, 2, rl);
+        all_passes<kT>(smem_rx, M, nl, M, 1, twx, 2, rl);
         for (int q = threadIdx.x; q < nl * (M + 1); q += kT) {
             const int ln = q / (M + 1), k = q - ln * (M + 1);
             const double2 *z = smem_rx + (size_t)ln * M;
@@ -382,7 +395,7 @@ __global__ void __launch_bounds__(kT, 1) gen_r2r_x_kernel(double *__restrict__ p
             if (q < nl * M) smem_rx[q] = zr[e];
         }
         __syncthreads();
-        all_passes(smem_rx, M, nl, M, 1, twx, 2, rl);
+        all_passes<kT>(smem_rx, M, nl, M, 1, twx, 2, rl);
         for (int q = threadIdx.x; q < nl * n; q += kT) {
             const int ln = q / n, i = q - ln * n;
             const int pos = (i & 1) ? n - 1 - (i >> 1) : (i >> 1);
@@ -431,6 +444,7 @@ bool factor(int n, Radices *out)
     // odd radices first: their strided writes of the first pass are free of bank conflicts
     for (int f : {7, 5, 3})
         while (n % f == 0) { out->r[out->n++] = f; n /= f; }
+    while (n % 16 == 0) { out->r[out->n++] = 16; n /= 16; }
     while (n % 8 == 0) { out->r[out->n++] = 8; n /= 8; }
     if (n % 4 == 0) { out->r[out->n++] = 4; n /= 4; }
     if (n % 2 == 0) { out->r[out->n++] = 2; n /= 2; }
@@ -452,53 +466,76 @@ bool generic_fft_y_ok(int ny)
     return ny >= 8 && !(ny & 1) && ny <= kPts && factor(ny, &r);
 }
 
+// launch geometry of the x kernels: lines per CTA and threads per CTA
+static void x_geometry(const pz_plan *pl, int M, long long nlines, int *lpb, int *kt)
+{
+    *kt = (M <= 256 * kE) ? 256 : 512;
+    int l = (*kt * kE) / M;
+    if (l > 64) l = 64;
+    // keep the grid a few waves deep on small fields
+    while (l > 1 && (nlines + l - 1) / l < 4LL * pl->num_sms) l /= 2;
+    *lpb = l;
+}
+
+// pairs per CTA and threads per CTA of the y kernels: rows as wide as the buffer allows (<= 128 bytes)
+static int y_geometry(const pz_plan *pl, int L, int *tc, int *kt)
+{
+    const int npairs = pl->nx / 2;
+    int t = 8;
+    while (t > 1 && (npairs % t != 0 || t * L > kPts)) t /= 2;
+    if (t * L > kPts) { set_error("fft_y: ny = %d exceeds the %d-point buffer", L, kPts); return PZ_EUNSUPPORTED; }
+    *tc = t;
+    *kt = (t * L <= 256 * kE) ? 256 : 512;
+    return PZ_OK;
+}
+
+#define PZ_GEN_LAUNCH(KERNEL, GRID, SMEM, ...)                                                                    \
+    do {                                                                                                           \
+        int rc_;                                                                                                   \
+        if (kt == 256) {                                                                                           \
+            if ((rc_ = smem_optin(pl, KERNEL<false, 256>, (size_t)256 * kE * sizeof(double2))) != PZ_OK) return rc_; \
+            if ((rc_ = smem_optin(pl, KERNEL<true, 256>, (size_t)256 * kE * sizeof(double2))) != PZ_OK) return rc_;  \
+            if (inverse) KERNEL<true, 256><<<GRID, 256, SMEM, st>>>(__VA_ARGS__);                                  \
+            else KERNEL<false, 256><<<GRID, 256, SMEM, st>>>(__VA_ARGS__);                                         \
+        } else {                                                                                                   \
+            if ((rc_ = smem_optin(pl, KERNEL<false, 512>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc_;   \
+            if ((rc_ = smem_optin(pl, KERNEL<true, 512>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc_;    \
+            if (inverse) KERNEL<true, 512><<<GRID, 512, SMEM, st>>>(__VA_ARGS__);                                  \
+            else KERNEL<false, 512><<<GRID, 512, SMEM, st>>>(__VA_ARGS__);                                         \
+        }                                                                                                          \
+        count_launch();                                                                                            \
+        PZ_CUDA(cudaGetLastError());                                                                               \
+    } while (0)
+
 int launch_fft_x_generic(const pz_plan *pl, double *p, long long nlines, bool inverse, cudaStream_t st)
 {
     const int M = pl->nx / 2;
     Radices rl;
     if (!factor(M, &rl)) { set_error("fft_x: nx / 2 = %d has a prime factor above 7", M); return PZ_EUNSUPPORTED; }
-    int lpb = kPts / M;
-    if (lpb > 64) lpb = 64;
-    // keep the grid a few waves deep on small fields
-    while (lpb > 1 && (nlines + lpb - 1) / lpb < 4LL * pl->num_sms) lpb /= 2;
+    int lpb, kt;
+    x_geometry(pl, M, nlines, &lpb, &kt);
     const size_t smem = (size_t)lpb * M * sizeof(double2);
-    const long long blocks = (nlines + lpb - 1) / lpb;
+    const unsigned blocks = (unsigned)((nlines + lpb - 1) / lpb);
     const double scale = 1.0 / ((double)pl->nx * (double)pl->ny);
-    int rc;
-    if ((rc = smem_optin(pl, gen_fft_x_kernel<false>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
-    if ((rc = smem_optin(pl, gen_fft_x_kernel<true>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
     ProfScope prof(pl, inverse ? PZ_K_FFT_X_INV : PZ_K_FFT_X_FWD, st);
-    if (inverse) gen_fft_x_kernel<true><<<(unsigned)blocks, kT, smem, st>>>(p, pl->d_twx, M, nlines, lpb, rl, scale);
-    else gen_fft_x_kernel<false><<<(unsigned)blocks, kT, smem, st>>>(p, pl->d_twx, M, nlines, lpb, rl, scale);
-    count_launch();
-    PZ_CUDA(cudaGetLastError());
+    PZ_GEN_LAUNCH(gen_fft_x_kernel, blocks, smem, p, pl->d_twx, M, nlines, lpb, rl, scale);
     return PZ_OK;
 }
 
 int launch_fft_y_generic(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_t st)
 {
-    const int L = pl->ny, npairs = pl->nx / 2;
+    const int L = pl->ny;
     Radices rl;
     if (!factor(L, &rl)) { set_error("fft_y: ny = %d has a prime factor above 7", L); return PZ_EUNSUPPORTED; }
-    int tc = 8;
-    while (tc > 1 && (npairs % tc != 0 || tc * L > kPts)) tc /= 2;
-    if (tc * L > kPts) { set_error("fft_y: ny = %d exceeds the %d-point buffer", L, kPts); return PZ_EUNSUPPORTED; }
+    int tc, kt;
+    const int rc = y_geometry(pl, L, &tc, &kt);
+    if (rc != PZ_OK) return rc;
     const size_t smem = (size_t)tc * L * sizeof(double2);
-    int rc;
-    if ((rc = smem_optin(pl, gen_fft_y_kernel<false>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
-    if ((rc = smem_optin(pl, gen_fft_y_kernel<true>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
-    dim3 grid((unsigned)(npairs / tc), (unsigned)nk);
+    dim3 grid((unsigned)(pl->nx / 2 / tc), (unsigned)nk);
     ProfScope prof(pl, inverse ? PZ_K_FFT_Y_INV : PZ_K_FFT_Y_FWD, st);
-    if (inverse) gen_fft_y_kernel<true><<<grid, kT, smem, st>>>(p, pl->d_twy, pl->nx, L, tc, rl);
-    else gen_fft_y_kernel<false><<<grid, kT, smem, st>>>(p, pl->d_twy, pl->nx, L, tc, rl);
-    count_launch();
-    PZ_CUDA(cudaGetLastError());
+    PZ_GEN_LAUNCH(gen_fft_y_kernel, grid, smem, p, pl->d_twy, pl->nx, L, tc, rl);
     return PZ_OK;
 }
-
-} // namespace pz
-
-namespace pz {
 
 // ---- cosine / sine expansions (bcx / bcy = PZ_NEUMANN, PZ_DIRICHLET)
 int launch_r2r_x(const pz_plan *pl, double *p, long long nlines, bool inverse, cudaStream_t st)
@@ -506,43 +543,30 @@ int launch_r2r_x(const pz_plan *pl, double *p, long long nlines, bool inverse, c
     const int M = pl->nx / 2;
     Radices rl;
     if (!factor(M, &rl)) { set_error("r2r_x: nx / 2 = %d has a prime factor above 7", M); return PZ_EUNSUPPORTED; }
-    int lpb = kPts / M;
-    if (lpb > 64) lpb = 64;
-    while (lpb > 1 && (nlines + lpb - 1) / lpb < 4LL * pl->num_sms) lpb /= 2;
+    int lpb, kt;
+    x_geometry(pl, M, nlines, &lpb, &kt);
     const size_t smem = (size_t)lpb * M * sizeof(double2);
-    const long long blocks = (nlines + lpb - 1) / lpb;
+    const unsigned blocks = (unsigned)((nlines + lpb - 1) / lpb);
     const double scale = 1.0 / ((double)pl->nx * (double)pl->ny);
     const int dir = (pl->bcx == PZ_DIRICHLET) ? 1 : 0;
-    int rc;
-    if ((rc = smem_optin(pl, gen_r2r_x_kernel<false>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
-    if ((rc = smem_optin(pl, gen_r2r_x_kernel<true>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
     ProfScope prof(pl, inverse ? PZ_K_FFT_X_INV : PZ_K_FFT_X_FWD, st);
-    if (inverse) gen_r2r_x_kernel<true><<<(unsigned)blocks, kT, smem, st>>>(p, pl->d_twx, pl->d_tw4x, M, nlines, lpb, rl, scale, dir);
-    else gen_r2r_x_kernel<false><<<(unsigned)blocks, kT, smem, st>>>(p, pl->d_twx, pl->d_tw4x, M, nlines, lpb, rl, scale, dir);
-    count_launch();
-    PZ_CUDA(cudaGetLastError());
+    PZ_GEN_LAUNCH(gen_r2r_x_kernel, blocks, smem, p, pl->d_twx, pl->d_tw4x, M, nlines, lpb, rl, scale, dir);
     return PZ_OK;
 }
 
 int launch_r2r_y(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_t st)
 {
-    const int L = pl->ny, npairs = pl->nx / 2;
+    const int L = pl->ny;
     Radices rl;
     if (!factor(L, &rl)) { set_error("r2r_y: ny = %d has a prime factor above 7", L); return PZ_EUNSUPPORTED; }
-    int tc = 8;
-    while (tc > 1 && (npairs % tc != 0 || tc * L > kPts)) tc /= 2;
-    if (tc * L > kPts) { set_error("r2r_y: ny = %d exceeds the %d-point buffer", L, kPts); return PZ_EUNSUPPORTED; }
+    int tc, kt;
+    const int rc = y_geometry(pl, L, &tc, &kt);
+    if (rc != PZ_OK) return rc;
     const size_t smem = (size_t)tc * L * sizeof(double2);
     const int dir = (pl->bcy == PZ_DIRICHLET) ? 1 : 0;
-    int rc;
-    if ((rc = smem_optin(pl, gen_r2r_y_kernel<false>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
-    if ((rc = smem_optin(pl, gen_r2r_y_kernel<true>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc;
-    dim3 grid((unsigned)(npairs / tc), (unsigned)nk);
+    dim3 grid((unsigned)(pl->nx / 2 / tc), (unsigned)nk);
     ProfScope prof(pl, inverse ? PZ_K_FFT_Y_INV : PZ_K_FFT_Y_FWD, st);
-    if (inverse) gen_r2r_y_kernel<true><<<grid, kT, smem, st>>>(p, pl->d_twy, pl->d_tw4y, pl->nx, L, tc, rl, dir);
-    else gen_r2r_y_kernel<false><<<grid, kT, smem, st>>>(p, pl->d_twy, pl->d_tw4y, pl->nx, L, tc, rl, dir);
-    count_launch();
-    PZ_CUDA(cudaGetLastError());
+    PZ_GEN_LAUNCH(gen_r2r_y_kernel, grid, smem, p, pl->d_twy, pl->d_tw4y, pl->nx, L, tc, rl, dir);
     return PZ_OK;
 }
 

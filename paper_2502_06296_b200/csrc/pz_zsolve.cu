@@ -74,12 +74,69 @@ __global__ void __launch_bounds__(128)
     }
 }
 
+// Variant 4 (nz <= 32, e.g. the 30 planes per GPU of the paper's weak-scaling grid):
+// one thread per column, the whole column in registers -- one coalesced read and one write per
+// point, the same pivot recurrence as above.  Rows past nz are identity rows.
+constexpr int kSmallNz = 32;
+
+__global__ void __launch_bounds__(128)
+    zsolve_small_kernel(double *__restrict__ p, const double *__restrict__ A, const double *__restrict__ C,
+                        const double *__restrict__ dzf, const double *__restrict__ lamx, const double *__restrict__ lamy_nat,
+                        const double *__restrict__ lamy_pk, int nx, int ny, int nz, double inv_lz, double pw0, double pw1,
+                        int zflags)
+{
+    const size_t plane = (size_t)nx * ny;
+    const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= plane) return;
+    const int i = (int)(col % nx), j = (int)(col / nx);
+    const double sigma = -(lamx[i] + (i < 2 ? lamy_pk[j] : lamy_nat[j]));
+    const bool singular = (i == 0 && j == 0) && (zflags & 2);
+    double g[kSmallNz], cw[kSmallNz];
+#pragma unroll
+    for (int k = 0; k < kSmallNz; ++k) g[k] = (k < nz) ? p[(size_t)k * plane + col] : 0.0;
+    double e = 0.0, rp = 0.0, gp = 0.0;
+#pragma unroll
+    for (int k = 0; k < kSmallNz; ++k) {
+        const bool live = k < nz;
+        const double a = (live && k > 0) ? A[k] : 0.0, c = live ? C[k] : 0.0;
+        e = fma(a * e, rp, sigma) + (k == 0 ? pw0 : 0.0) + (k == nz - 1 ? pw1 : 0.0);
+        const bool gauge = singular && k == nz - 1;   // last equation of the singular column replaced by phi = 0
+        const double pk = (live && !gauge) ? c + e : 1.0;
+        rp = 1.0 / pk;
+        gp = (live && !gauge) ? fma(a, gp, -g[k]) * rp : 0.0;
+        if (!live || gauge) rp = 0.0;
+        g[k] = gp;
+        cw[k] = c * rp;
+    }
+    double x = 0.0, s = 0.0;
+#pragma unroll
+    for (int k = kSmallNz - 1; k >= 0; --k) {
+        x = fma(cw[k], x, g[k]);
+        g[k] = x;
+        if (k < nz) s = fma(dzf[k], x, s);
+    }
+    const double shift = singular ? s * inv_lz : 0.0;
+#pragma unroll
+    for (int k = 0; k < kSmallNz; ++k)
+        if (k < nz) p[(size_t)k * plane + col] = g[k] - shift;
+}
+
 } // namespace
 
 int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
 {
+    if (pl->opt.zsolve_variant == 4 && helm_a < 0.0) {
+        const size_t plane = (size_t)pl->nx * pl->ny;
+        ProfScope prof(pl, PZ_K_Z_SOLVE, st);
+        zsolve_small_kernel<<<(unsigned)((plane + 127) / 128), 128, 0, st>>>(p, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx, pl->d_lamy_nat,
+                                                                             pl->d_lamy_pk, pl->nx, pl->ny, pl->nz, pl->inv_lz, pl->pw0,
+                                                                             pl->pw1, pl->zflags());
+        count_launch();
+        PZ_CUDA(cudaGetLastError());
+        return PZ_OK;
+    }
     if (pl->opt.zsolve_variant == 3 && helm_a < 0.0) return launch_zsolve_islab(pl, p, st);
-    if (pl->opt.zsolve_variant == 1) return launch_zsolve_cr(pl, p, st, helm_a);
+    if (pl->opt.zsolve_variant == 1 || pl->opt.zsolve_variant == 4) return launch_zsolve_cr(pl, p, st, helm_a);
     if (pl->opt.zsolve_variant == 2) return launch_zsolve_tma(pl, p, st, helm_a);
     if (helm_a >= 0.0) {
         set_error("helmholtz3d_solve needs z-solve variant 1 or 2 (nz <= 1024)");
