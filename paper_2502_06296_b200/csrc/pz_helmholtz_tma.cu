@@ -100,7 +100,9 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
 
     const int tid = threadIdx.x, c2 = 2 * (tid % (TX / 2)), s = tid / (TX / 2);
     // z-split: chunk of this CTA (rank in the cluster), its first global row and its table block
-    const int crank = (ZS > 1) ? (int)(blockIdx.x % ZS) : 0;
+    // cluster of csz = ZS * TP CTAs: rank = tp * ZS + chunk; TP neighbouring tiles walk in step
+    const int cl_rank = (ZS > 1) ? (int)(blockIdx.x % csz) : 0;
+    const int crank = cl_rank % ZS, ctile = cl_rank / ZS, TP = (ZS > 1) ? csz / ZS : 1;
     const int kc0 = crank * nzp_of(P, M);
     const double *tab = tab_all + (size_t)crank * (6 * (size_t)P * M + L::pcr(P, levels) + 2);
     const int k0 = s * M;                                  // row inside the chunk
@@ -141,8 +143,8 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
     };
 
     // tiles walk by CTA (ZS = 1) or by cluster (ZS = 2: both CTAs own the same columns)
-    const int tstep = (int)gridDim.x / ZS;
-    int t = (int)blockIdx.x / ZS;
+    const int tstep = (ZS > 1) ? ((int)gridDim.x / csz) * TP : (int)gridDim.x;
+    int t = (ZS > 1) ? ((int)blockIdx.x / csz) * TP + ctile : (int)blockIdx.x;
     if (tid == 0 && t < total_tiles) fetch(t);
 
     const double *fA = stab + s * TS, *bC = fA + P * TS, *rb = bC + P * TS, *ra = rb + P * TS, *rc = ra + P * TS;
@@ -279,7 +281,7 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
                 const double2 mine = (crank == 0) ? x1 : x0;
                 st2(slot + c2, mine);
                 unsigned remote;
-                asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(slot + TX + c2)), "r"(crank ^ 1));
+                asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(slot + TX + c2)), "r"(cl_rank ^ 1));
                 asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(remote), "d"(mine.x), "d"(mine.y) : "memory");
             }
             // (an st.async + mbarrier hand-over without this barrier was measured SLOWER, 1.17 against
@@ -375,7 +377,12 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
     if (csz == 0) csz = (M == 16) ? 2 : 1;
     if (csz != 2 && csz != 4 && csz != 8) csz = 1;
     while (csz > 1 && (tiles_per_field % csz != 0 || blocks < csz)) csz /= 2;
-    if (ZS > 1) csz = ZS; // the cluster is the pair of chunks of one tile
+    if (ZS > 1) {
+        // the cluster is the pair of chunks of one tile; helm_cluster = 4 adds a neighbouring tile in
+        // step (measured slower: 1.18 against 1.10 ms at 512^3 x 3, 10.0 against 9.0 ms at 1024^3 x 3)
+        const int tp = (pl->opt.helm_cluster == 4 && total % 2 == 0) ? 2 : 1;
+        csz = ZS * tp;
+    }
     const int probe = wide ? 3 : (pl->opt.helm_probe == 3 ? 1 : pl->opt.helm_probe);
     cudaLaunchConfig_t cfg = {};
     cfg.blockDim = dim3((kTX / 2) * P);
