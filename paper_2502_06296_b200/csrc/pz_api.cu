@@ -198,7 +198,7 @@ extern "C" {
 
 const char *pz_last_error(void) { return g_err; }
 long long pz_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
-int pz_version(void) { return 100; }
+int pz_version(void) { return 200; }
 
 static int slab_state_create(pz_plan *pl, int n_slabs, const int *kbounds, bool internal);
 
