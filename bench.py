@@ -365,7 +365,18 @@ def bench_strong(args, w, torch, pz, ranks, wl, rank, world, local, dist):
     jp = jh = p = None
     us = []
     if w.poisson:
-        jp = sharded.SlabPoisson(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf, rank, world)
+        exchange = args.exchange
+        try:
+            jp = sharded.SlabPoisson(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf, rank, world, exchange=exchange,
+                                     group=(dist.group.WORLD if (dist is not None and exchange == "p2p") else None))
+            if exchange == "p2p" and dist is None:
+                sharded.SlabPoisson.connect([jp])
+        except Exception as exc:  # symmetric memory not available on this node: the collective always is
+            if exchange != "p2p":
+                raise
+            sys.stderr.write(f"bench.py: p2p exchange unavailable ({exc}); falling back to all-gather\n")
+            exchange = "allgather"
+            jp = sharded.SlabPoisson(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf, rank, world)
         for kv in args.option:
             k, v = kv.split("=")
             pz.pz_set_option(jp.plan, k, int(v))
@@ -471,7 +482,7 @@ def bench_strong(args, w, torch, pz, ranks, wl, rank, world, local, dist):
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "fields_per_step": fields,
                    "step": f"{1 if w.poisson else 0} Poisson solve + {w.n_helmholtz} Helmholtz solves of ONE problem, in place",
-                   "parallelism": (f"z-slabs x{world} (P-TDMA, one all-gather of {jp.bytes_exchanged_per_solve if jp else 0} B per rank and solve)"
+                   "parallelism": (f"z-slabs x{world} (P-TDMA, exchange = {jp.exchange if jp else None}: {jp.bytes_exchanged_per_solve if jp else 0} B per rank and solve)"
                                    if w.poisson else "") + (f" y-slabs x{world} (no collective)" if w.n_helmholtz else ""),
                    "l2": "every rank's slab is larger than the 126 MB L2 up to 8 ranks at c3 / c4; no flush",
                    "options": args.option},
@@ -505,6 +516,9 @@ def main():
     ap.add_argument("--scaling", default=None, choices=["weak", "strong"],
                     help="N > 1: weak = replicas (default c1, c2), strong = one problem by z-/y-slabs (default c3, c4)")
     ap.add_argument("--no-extras", action="store_true", help="skip the sub-records measured outside the timed region")
+    ap.add_argument("--exchange", default="allgather", choices=["allgather", "p2p"],
+                    help="--scaling strong: boundary exchange of the z-slab Poisson solve (NCCL all-gather, or stores of the "
+                         "reduction kernel into peer memory)")
     args = ap.parse_args()
 
     from paper_2502_06296_b200 import workloads as wl

@@ -122,6 +122,27 @@ PZ_API int poisson_solve_reduce(pz_plan *plan, double *p, double *boundary_out, 
 PZ_API int poisson_solve_finish(pz_plan *plan, double *p, const double *boundary_all, void *stream);
 
 /*
+ * The same solve with the exchange done by the kernels themselves over peer memory (NVLink /
+ * NVSwitch) instead of a collective: every rank owns a gathered buffer boundary_all (n_slabs *
+ * poisson_slab_boundary_doubles doubles) and a flag array (n_slabs 64-bit integers, zero-initialised)
+ * that ALL ranks of the node can address (peer-mapped / symmetric memory; the caller obtains the
+ * pointers, e.g. torch.distributed._symmetric_memory).
+ *   poisson_solve_reduce_push   forward transforms and reduction; the reduction kernel stores this
+ *                               rank's block straight into its slot of EVERY rank's boundary_all
+ *                               (boundary_all_of_rank[r], host array of n_slabs device pointers),
+ *                               then releases flags_of_rank[r][slab] = epoch at system scope.
+ *   poisson_solve_finish_wait   waits on the device until all n_slabs entries of this rank's own
+ *                               flag array have reached epoch, then poisson_solve_finish.
+ * epoch must grow by one per solve.  Every rank must enqueue its push before its wait (the wait
+ * spins on the device); the buffers of solve e must not be rewritten before every rank has
+ * finished solve e (two buffer sets alternate in sharded.SlabPoisson).
+ */
+PZ_API int poisson_solve_reduce_push(pz_plan *plan, double *p, double *const *boundary_all_of_rank,
+                                     long long *const *flags_of_rank, long long epoch, void *stream);
+PZ_API int poisson_solve_finish_wait(pz_plan *plan, double *p, const double *boundary_all, const long long *flags,
+                                     long long epoch, void *stream);
+
+/*
  * Wall-normal implicit diffusion, Eq. (11), with the paper's split of the
  * cyclic-reduction solver into pre-processing and runtime (Algorithm 2).
  *

@@ -31,6 +31,8 @@ SIGNATURES = {
     "poisson_slab_plan_create": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _d, _d, _dp, _dp, _i, _i, _i, ctypes.POINTER(_i)]),
     "poisson_slab_boundary_doubles": (ctypes.c_longlong, [_vp]),
     "poisson_solve_reduce": (_i, [_vp, _vp, _vp, _vp]),
+    "poisson_solve_reduce_push": (_i, [_vp, _vp, ctypes.POINTER(_vp), ctypes.POINTER(_vp), ctypes.c_longlong, _vp]),
+    "poisson_solve_finish_wait": (_i, [_vp, _vp, _vp, _vp, ctypes.c_longlong, _vp]),
     "poisson_solve_finish": (_i, [_vp, _vp, _vp, _vp]),
     "helmholtz_z_setup": (_i, [_vp, _d]),
     "helmholtz_w_setup": (_i, [_vp, _d]),
@@ -180,6 +182,19 @@ def poisson_slab_boundary_doubles(plan: Plan) -> int:
 def poisson_solve_reduce(plan: Plan, p, boundary_out, stream=None) -> None:
     _check(lib().poisson_solve_reduce(plan.handle, _dev_ptr(p, plan.n), _dev_ptr(boundary_out, poisson_slab_boundary_doubles(plan)),
                                       _stream_ptr(stream)))
+
+
+def poisson_solve_reduce_push(plan: Plan, p, ball_ptrs, flag_ptrs, epoch: int, stream=None) -> None:
+    """ball_ptrs / flag_ptrs: device addresses (ints) of every rank's gathered buffer / flag array."""
+    n = len(ball_ptrs)
+    a = (_vp * n)(*[int(x) for x in ball_ptrs])
+    f = (_vp * n)(*[int(x) for x in flag_ptrs])
+    _check(lib().poisson_solve_reduce_push(plan.handle, _dev_ptr(p, plan.n), a, f, int(epoch), _stream_ptr(stream)))
+
+
+def poisson_solve_finish_wait(plan: Plan, p, boundary_all, flags, epoch: int, stream=None) -> None:
+    _check(lib().poisson_solve_finish_wait(plan.handle, _dev_ptr(p, plan.n), _dev_ptr(boundary_all, None), int(flags.data_ptr()),
+                                           int(epoch), _stream_ptr(stream)))
 
 
 def poisson_solve_finish(plan: Plan, p, boundary_all, stream=None) -> None:

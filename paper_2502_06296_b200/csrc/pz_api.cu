@@ -408,7 +408,43 @@ int poisson_solve_reduce(pz_plan *pl, double *p, double *boundary_out, void *str
     int rc;
     if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 64) * sizeof(int), st));
     if ((rc = forward_xy(pl, p, st)) != PZ_OK) return rc;
-    return launch_slab_reduce(pl, p, boundary_out, st);
+    BoutSet one;
+    one.n = 1;
+    one.p[0] = boundary_out;
+    return launch_slab_reduce(pl, p, one, st);
+}
+
+int poisson_solve_reduce_push(pz_plan *pl, double *p, double *const *boundary_all_of_rank, long long *const *flags_of_rank,
+                              long long epoch, void *stream)
+{
+    if (!pl || !p || !boundary_all_of_rank || !flags_of_rank) { set_error("poisson_solve_reduce_push: NULL argument"); return PZ_EINVAL; }
+    if (pl->slab_G < 1 || pl->slab_internal) { set_error("poisson_solve_reduce_push: the plan is not a slab plan"); return PZ_EINVAL; }
+    BoutSet all;
+    all.n = pl->slab_G;
+    for (int r = 0; r < pl->slab_G; ++r) {
+        if (!boundary_all_of_rank[r] || !flags_of_rank[r] || ((uintptr_t)boundary_all_of_rank[r] & 15) != 0) {
+            set_error("poisson_solve_reduce_push: buffer of rank %d is NULL or not 16-byte aligned", r);
+            return PZ_EINVAL;
+        }
+        all.p[r] = boundary_all_of_rank[r] + (size_t)pl->slab_g * pl->slab_bstride; // this rank's slot in rank r's gathered buffer
+    }
+    if (((uintptr_t)p & 15) != 0) { set_error("poisson_solve_reduce_push: p must be 16-byte aligned"); return PZ_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if (use_fused(pl)) PZ_CUDA(cudaMemsetAsync(pl->d_xyctr, 0, 2 * (size_t)(pl->nz + 64) * sizeof(int), st));
+    if ((rc = forward_xy(pl, p, st)) != PZ_OK) return rc;
+    if ((rc = launch_slab_reduce(pl, p, all, st)) != PZ_OK) return rc;
+    return launch_slab_signal(pl, flags_of_rank, pl->slab_G, pl->slab_g, epoch, st);
+}
+
+int poisson_solve_finish_wait(pz_plan *pl, double *p, const double *boundary_all, const long long *flags, long long epoch,
+                              void *stream)
+{
+    if (!pl || !flags) { set_error("poisson_solve_finish_wait: NULL argument"); return PZ_EINVAL; }
+    if (pl->slab_G < 1 || pl->slab_internal) { set_error("poisson_solve_finish_wait: the plan is not a slab plan"); return PZ_EINVAL; }
+    const int rc = launch_slab_wait(pl, flags, pl->slab_G, epoch, (cudaStream_t)stream);
+    if (rc != PZ_OK) return rc;
+    return poisson_solve_finish(pl, p, boundary_all, stream);
 }
 
 int poisson_solve_finish(pz_plan *pl, double *p, const double *boundary_all, void *stream)

@@ -198,10 +198,16 @@ int launch_r2r_y(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_
 int launch_allpairs(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_t st);
 int launch_fft_xy_fwd(pz_plan *pl, double *p, cudaStream_t st);
 int launch_fft_xy_inv(pz_plan *pl, double *p, cudaStream_t st);
-int launch_zslab_tma(pz_plan *pl, double *p, int kb, int nk, double *bout, const double *phi_prev, const double *phi_next,
+// where a slab's boundary block goes: one buffer (all-gather by the caller) or the slot of this
+// rank in the gathered buffer of EVERY rank (peer memory over NVLink: the reduction kernel's own
+// stores are the exchange)
+struct BoutSet { double *p[16]; int n = 0; };
+int launch_zslab_tma(pz_plan *pl, double *p, int kb, int nk, const BoutSet *bout, const double *phi_prev, const double *phi_next,
                      cudaStream_t st);
 int launch_slab_coefficients(pz_plan *pl, cudaStream_t st);
-int launch_slab_reduce(pz_plan *pl, double *p, double *bout, cudaStream_t st);
+int launch_slab_reduce(pz_plan *pl, double *p, const BoutSet &bout, cudaStream_t st);
+int launch_slab_signal(pz_plan *pl, long long *const *flags, int n, int slot, long long epoch, cudaStream_t st);
+int launch_slab_wait(pz_plan *pl, const long long *flags, int n, long long epoch, cudaStream_t st);
 int launch_zsolve_islab(pz_plan *pl, double *p, cudaStream_t st);
 int launch_slab_finish(pz_plan *pl, double *p, const double *ball, cudaStream_t st);
 int launch_helmholtz_n(pz_plan *pl, double *const *u, int n, cudaStream_t st, int kind = 0); // kind 1: face-centred w

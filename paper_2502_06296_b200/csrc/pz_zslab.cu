@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(kPairs *kLanes)
 // the slab's rows of the (0,0) column.  bout = [RF (plane) | RL (plane) | d00 (nk)].
 template <int M>
 __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 1))
-    slab_reduce_kernel(const double *__restrict__ p, double *__restrict__ bout, const double *__restrict__ A,
+    slab_reduce_kernel(const double *__restrict__ p, const BoutSet bouts, const double *__restrict__ A,
                        const double *__restrict__ C, const double *__restrict__ lamx,
                        const double *__restrict__ lamy_nat, const double *__restrict__ lamy_pk, int nx, size_t plane,
                        int kb, int nk)
@@ -163,12 +163,15 @@ __global__ void __launch_bounds__(kPairs *kLanes, (M <= 8) ? 3 : (M == 16 ? 2 : 
         reduce_pair<M, 1>(al, ga, ex, sig1, k0, nk, [&](int i, double(&o)[1]) { o[0] = (k0 + i < nk) ? -d(i).y : 0.0; }, F, L);
         rf.y = F[0]; rl.y = L[0];
     }
-    if (lane == 0) {
-        *reinterpret_cast<double2 *>(bout + col) = rf;
-        *reinterpret_cast<double2 *>(bout + plane + col) = rl;
+    for (int dst = 0; dst < bouts.n; ++dst) {
+        double *bout = bouts.p[dst];
+        if (lane == 0) {
+            *reinterpret_cast<double2 *>(bout + col) = rf;
+            *reinterpret_cast<double2 *>(bout + plane + col) = rl;
+        }
+        if (blockIdx.x == 0)
+            for (int k = threadIdx.x; k < nk; k += blockDim.x) bout[2 * plane + k] = tile[(k / M) * CH + (k % M) * kTX];
     }
-    if (blockIdx.x == 0)
-        for (int k = threadIdx.x; k < nk; k += blockDim.x) bout[2 * plane + k] = tile[(k / M) * CH + (k % M) * kTX];
 }
 
 // The reduced systems of size 2G, one per real column (PAPER.md:128 step 5), every rank for itself.
@@ -370,12 +373,12 @@ int launch_slab_coefficients(pz_plan *pl, cudaStream_t st)
 
 // Slab g of the plan's cut: p_slab points at its first plane.  Slabs of more than 128 planes take the
 // TMA pipeline of pz_zsolve_tma.cu (slab modes), thinner ones the kernels above.
-static int slab_reduce_g(pz_plan *pl, double *p_slab, int g, double *bout, cudaStream_t st)
+static int slab_reduce_g(pz_plan *pl, double *p_slab, int g, const BoutSet &bout, cudaStream_t st)
 {
     const size_t plane = (size_t)pl->nx * pl->ny;
     const unsigned blocks = (unsigned)(plane / kTX);
     const int kb = pl->slab_kb[g], nk = pl->slab_kb[g + 1] - kb;
-    if (nk > 128 && pl->opt.zsolve_variant != 1) return launch_zslab_tma(pl, p_slab, kb, nk, bout, nullptr, nullptr, st);
+    if (nk > 128 && pl->opt.zsolve_variant != 1) return launch_zslab_tma(pl, p_slab, kb, nk, &bout, nullptr, nullptr, st);
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
     PZ_SLAB_DISPATCH(nk, {
         { const int rc = smem_optin(pl, slab_reduce_kernel<MM>, slab_smem<MM>()); if (rc != PZ_OK) return rc; }
@@ -420,7 +423,52 @@ static int slab_finish_g(pz_plan *pl, double *p_slab, int g, const double *ball,
     return PZ_OK;
 }
 
-int launch_slab_reduce(pz_plan *pl, double *p, double *bout, cudaStream_t st) { return slab_reduce_g(pl, p, pl->slab_g, bout, st); }
+// Peer-memory exchange: after the reduction kernel has stored this rank's block into every rank's
+// gathered buffer, one thread makes those stores visible system-wide and raises this rank's flag in
+// every rank's flag array; a finish first waits until all ranks' flags of its own array carry the epoch.
+struct FlagSet { long long *p[16]; int n; };
+__global__ void slab_signal_kernel(const FlagSet fl, int slot, long long epoch)
+{
+    __threadfence_system();
+    for (int r = threadIdx.x; r < fl.n; r += blockDim.x) {
+        long long *f = fl.p[r] + slot;
+        asm volatile("st.release.sys.global.s64 [%0], %1;" ::"l"(f), "l"(epoch) : "memory");
+    }
+}
+__global__ void slab_wait_kernel(const long long *__restrict__ flags, int n, long long epoch)
+{
+    for (int r = threadIdx.x; r < n; r += blockDim.x) {
+        long long v;
+        do {
+            asm volatile("ld.acquire.sys.global.s64 %0, [%1];" : "=l"(v) : "l"(flags + r) : "memory");
+            if (v < epoch) __nanosleep(200);
+        } while (v < epoch);
+    }
+    __threadfence_system();
+}
+
+int launch_slab_signal(pz_plan *pl, long long *const *flags, int n, int slot, long long epoch, cudaStream_t st)
+{
+    (void)pl;
+    FlagSet fl;
+    fl.n = n;
+    for (int r = 0; r < n; ++r) fl.p[r] = flags[r];
+    slab_signal_kernel<<<1, 32, 0, st>>>(fl, slot, epoch);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+int launch_slab_wait(pz_plan *pl, const long long *flags, int n, long long epoch, cudaStream_t st)
+{
+    (void)pl;
+    slab_wait_kernel<<<1, 32, 0, st>>>(flags, n, epoch);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
+
+int launch_slab_reduce(pz_plan *pl, double *p, const BoutSet &bout, cudaStream_t st) { return slab_reduce_g(pl, p, pl->slab_g, bout, st); }
 int launch_slab_finish(pz_plan *pl, double *p, const double *ball, cudaStream_t st) { return slab_finish_g(pl, p, pl->slab_g, ball, st); }
 
 // A whole column of more than 1024 rows on ONE GPU (the paper's wall-normal size is 1594,
@@ -432,7 +480,10 @@ int launch_zsolve_islab(pz_plan *pl, double *p, cudaStream_t st)
 {
     const size_t plane = (size_t)pl->nx * pl->ny;
     for (int g = 0; g < pl->slab_G; ++g) {
-        const int rc = slab_reduce_g(pl, p + (size_t)pl->slab_kb[g] * plane, g, pl->islab_ball + (size_t)g * pl->slab_bstride, st);
+        BoutSet one;
+        one.n = 1;
+        one.p[0] = pl->islab_ball + (size_t)g * pl->slab_bstride;
+        const int rc = slab_reduce_g(pl, p + (size_t)pl->slab_kb[g] * plane, g, one, st);
         if (rc != PZ_OK) return rc;
     }
     for (int g = 0; g < pl->slab_G; ++g) {

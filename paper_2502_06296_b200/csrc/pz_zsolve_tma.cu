@@ -56,7 +56,7 @@ template <int M> struct Geo {
 // z-slab of a cut column (pz_zslab.cu): what the slab modes need beside the tile
 struct SlabArgs {
     int kb = 0;                       // first global row of the slab (the tile holds rows kb .. kb + nz - 1)
-    double *bout = nullptr;           // reduce: [RF (plane) | RL (plane) | (0,0) column (nz)]
+    BoutSet bout;                     // reduce: destinations of [RF (plane) | RL (plane) | (0,0) column (nz)]
     const double *phi_prev = nullptr; // finish: value of the row below the slab, per real column
     const double *phi_next = nullptr; //         and of the row above
     size_t plane = 0;
@@ -182,14 +182,17 @@ __global__ void __launch_bounds__(kThreads, 1)
                 reduce_pair<M, 1>(al, ga, ex, sig1, k0, nz, [&](int r, double(&o)[1]) { o[0] = (k0 + r < nz) ? -d(r).y : 0.0; }, F, L);
                 rf.y = F[0]; rl.y = L[0];
             }
-            if (lane == 0) {
-                *reinterpret_cast<double2 *>(sa.bout + col) = rf;
-                *reinterpret_cast<double2 *>(sa.bout + sa.plane + col) = rl;
-            }
-            if (col == 0) // the slab's rows of the singular (0,0) column travel whole
+            for (int dst = 0; dst < sa.bout.n; ++dst) {
+                double *bo = sa.bout.p[dst];
+                if (lane == 0) {
+                    *reinterpret_cast<double2 *>(bo + col) = rf;
+                    *reinterpret_cast<double2 *>(bo + sa.plane + col) = rl;
+                }
+                if (col == 0) // the slab's rows of the singular (0,0) column travel whole
 #pragma unroll
-                for (int r = 0; r < M; ++r)
-                    if (k0 + r < nz) sa.bout[2 * sa.plane + k0 + r] = d(r).x;
+                    for (int r = 0; r < M; ++r)
+                        if (k0 + r < nz) bo[2 * sa.plane + k0 + r] = d(r).x;
+            }
         } else if constexpr (MODE == 2) {
             const double *ex = s_e0 + lane * G::CS;
             const double aopen = A[sa.kb], copen = C[sa.kb + nz - 1];
@@ -283,7 +286,7 @@ int launch_m(pz_plan *pl, double *p, cudaStream_t st, double ha, int nk, const S
 int launch_zsolve_tma(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
 {
     const int nz = pl->nz;
-    const SlabArgs none;
+    const SlabArgs none{};
 #define PZ_ZT(MM) (helm_a >= 0.0 ? launch_m<MM, true>(pl, p, st, helm_a, nz, none) : launch_m<MM, false>(pl, p, st, 0.0, nz, none))
     if (nz <= 32 * 4) return PZ_ZT(4);
     if (nz <= 32 * 8) return PZ_ZT(8);
@@ -296,11 +299,11 @@ int launch_zsolve_tma(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
 
 // One z-slab [kb, kb + nk) of cut columns through the same pipeline (pz_zslab.cu): p points at the
 // slab's first plane.  reduce: boundary values into bout; finish: in place with phi_prev / phi_next.
-int launch_zslab_tma(pz_plan *pl, double *p, int kb, int nk, double *bout, const double *phi_prev, const double *phi_next,
+int launch_zslab_tma(pz_plan *pl, double *p, int kb, int nk, const BoutSet *bout, const double *phi_prev, const double *phi_next,
                      cudaStream_t st)
 {
     SlabArgs sa;
-    sa.kb = kb; sa.bout = bout; sa.phi_prev = phi_prev; sa.phi_next = phi_next; sa.plane = (size_t)pl->nx * pl->ny;
+    sa.kb = kb; if (bout) sa.bout = *bout; sa.phi_prev = phi_prev; sa.phi_next = phi_next; sa.plane = (size_t)pl->nx * pl->ny;
 #define PZ_ZS(MM) (bout ? launch_m<MM, false, 1>(pl, p, st, 0.0, nk, sa) : launch_m<MM, false, 2>(pl, p, st, 0.0, nk, sa))
     if (nk <= 32 * 4) return PZ_ZS(4);
     if (nk <= 32 * 8) return PZ_ZS(8);

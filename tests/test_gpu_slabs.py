@@ -102,6 +102,33 @@ def test_poisson_z_slabs_at_512_columns_even_split(env, world):
     assert rel_err(got, ref) <= TOL
 
 
+@pytest.mark.parametrize("base,nx,ny,nz,kb", [("c1", 32, 16, 48, [0, 24, 48]), ("c3", 64, 32, 100, [0, 3, 40, 45, 100]),
+                                            ("c3", 16, 32, 700, [0, 300, 700]), ("c2", 512, 512, 64, [0, 8, 16, 24, 32, 40, 48, 56, 64])])
+def test_poisson_z_slabs_with_the_exchange_done_by_the_kernels(env, base, nx, ny, nz, kb):
+    """exchange = "p2p": every rank's reduction kernel stores its boundary block into every rank's
+    gathered buffer and raises a flag; the finish waits on the flags on the device.  The ranks of the
+    job live in this process (their buffers are ordinary device memory of this GPU); all pushes are
+    enqueued before any wait, as on a node.  Three solves in a row alternate the two buffer sets."""
+    torch, pz, wl, oracle, ranks, sharded = env
+    w = wl.scaled(wl.CONFIGS[base], nx, ny, nz)
+    zc, zf = wl.grid(w)
+    G = len(kb) - 1
+    jobs = [sharded.SlabPoisson(nx, ny, nz, w.lx, w.ly, zc, zf, g, G, kb, exchange="p2p") for g in range(G)]
+    sharded.SlabPoisson.connect(jobs)
+    for it in range(3):
+        f = wl.remove_weighted_mean(np.random.default_rng(100 + it).standard_normal((nz, ny, nx)), zf)
+        parts = [torch.from_numpy(s).cuda() for s in sharded.split_z(f, kb)]
+        for j, p in zip(jobs, parts):
+            j.reduce(p)
+        for j, p in zip(jobs, parts):
+            j.finish(p)
+        torch.cuda.synchronize()
+        got = np.concatenate([p.cpu().numpy() for p in parts], axis=0)
+        assert rel_err(got, oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)) <= TOL
+    for j in jobs:
+        j.destroy()
+
+
 def test_slab_driver_single_rank_and_error_paths(env):
     torch, pz, wl, oracle, ranks, sharded = env
     w = wl.scaled(wl.CONFIGS["c1"], 32, 16, 40)
