@@ -201,9 +201,10 @@ PZ_API int helmholtz_z_step(pz_plan *plan, double *ustar2, const double *uk, voi
  * with diagonal 1 + a (A_k + C_k + W_k - lambda_x - lambda_y), inverse transforms.  The systems
  * are non-singular for every mode (no pinned column).  helmholtz3d_setup only records a (the
  * coefficient tables are scaled inside the kernel), so it may be called between any two solves.
- *   u  device, nx*ny*nz doubles, 16-byte aligned, in place.  nz <= 1024.
+ *   u  device, nx*ny*nz doubles, 16-byte aligned, in place.  Above 1024 planes the z stage runs as a
+ *      thread-per-column sweep (one field of workspace, allocated on first use).
  * Errors: PZ_ENOTSETUP before the first setup; PZ_EINVAL for a < 0 or null pointers;
- * PZ_EUNSUPPORTED for nz > 1024.
+ * PZ_EUNSUPPORTED on plans with bc != 0 or z-slab plans.
  */
 PZ_API int helmholtz3d_setup(pz_plan *plan, double a);
 PZ_API int helmholtz3d_solve(pz_plan *plan, double *u, void *stream);

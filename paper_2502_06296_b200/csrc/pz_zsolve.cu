@@ -28,25 +28,33 @@ __global__ void __launch_bounds__(128)
                          const double *__restrict__ C, const double *__restrict__ dzf,
                          const double *__restrict__ lamx, const double *__restrict__ lamy_nat,
                          const double *__restrict__ lamy_pk, int nx, int ny, int nz, double inv_lz, double pw0,
-                         double pw1, int zflags)
+                         double pw1, int zflags, double ha)
 {
+    // ha >= 0: the fully implicit Helmholtz systems of Eq. (8), the same recurrence on
+    //   -a A x_{k-1} + (a A + a C + (1 + a sigma) + a W_k) x_k - a C x_{k+1} = +d
+    // (pw0, pw1 are then the Dirichlet wall terms W of the velocity, no singular column)
+    const bool helm = ha >= 0.0;
+    const double sc = helm ? ha : 1.0, rs = helm ? -1.0 : 1.0;
+    pw0 *= sc;
+    pw1 *= sc;
     const size_t plane = (size_t)nx * ny;
     const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (col >= plane) return;
     const int i = (int)(col % nx), j = (int)(col / nx);
-    const double sigma = -(lamx[i] + (i < 2 ? lamy_pk[j] : lamy_nat[j]));
-    const bool singular = (i == 0 && j == 0) && (zflags & 2);
+    const double sig = -(lamx[i] + (i < 2 ? lamy_pk[j] : lamy_nat[j]));
+    const double sigma = helm ? 1.0 + ha * sig : sig;
+    const bool singular = (i == 0 && j == 0) && (zflags & 2) && !helm;
 
     // forward: p_k = C_k + e_k, e_k = sigma + A_k e_{k-1}/p_{k-1}; g_k = (-d_k + A_k g_{k-1})/p_k
     double e = sigma + pw0;   // Dirichlet wall: extra diagonal term of the first row
-    double pk = C[0] + e;
+    double pk = sc * C[0] + e;
     double rp = 1.0 / pk;
-    double g = -p[col] * rp;
+    double g = -rs * p[col] * rp;
     p[col] = g;
-    work[col] = C[0] * rp;
+    work[col] = sc * C[0] * rp;
     for (int k = 1; k < nz; ++k) {
-        const double a = A[k], c = C[k];
-        const double d = p[(size_t)k * plane + col];
+        const double a = sc * A[k], c = sc * C[k];
+        const double d = rs * p[(size_t)k * plane + col];
         e = fma(a * e, rp, sigma) + (k == nz - 1 ? pw1 : 0.0);
         pk = c + e;
         if (singular && k == nz - 1) {
@@ -138,10 +146,7 @@ int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
     if (pl->opt.zsolve_variant == 3 && helm_a < 0.0) return launch_zsolve_islab(pl, p, st);
     if (pl->opt.zsolve_variant == 1 || pl->opt.zsolve_variant == 4) return launch_zsolve_cr(pl, p, st, helm_a);
     if (pl->opt.zsolve_variant == 2) return launch_zsolve_tma(pl, p, st, helm_a);
-    if (helm_a >= 0.0) {
-        set_error("helmholtz3d_solve needs z-solve variant 1 or 2 (nz <= 1024)");
-        return PZ_EUNSUPPORTED;
-    }
+    // helm_a >= 0 above 1024 planes: the thread-per-column sweep takes the Helmholtz systems too
     if (!pl->d_zwork) {
         cudaError_t e = cudaMalloc(&pl->d_zwork, pl->n * sizeof(double));
         if (e != cudaSuccess) {
@@ -153,8 +158,9 @@ int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
     const unsigned blocks = (unsigned)((plane + 127) / 128);
     ProfScope prof(pl, PZ_K_Z_SOLVE, st);
     zsolve_thomas_kernel<<<blocks, 128, 0, st>>>(p, pl->d_zwork, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx,
-                                                  pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, pl->nz, pl->inv_lz, pl->pw0, pl->pw1,
-                                                  pl->zflags());
+                                                  pl->d_lamy_nat, pl->d_lamy_pk, pl->nx, pl->ny, pl->nz, pl->inv_lz,
+                                                  helm_a >= 0.0 ? pl->wall_w0 : pl->pw0, helm_a >= 0.0 ? pl->wall_w1 : pl->pw1,
+                                                  pl->zflags(), helm_a);
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;

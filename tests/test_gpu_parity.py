@@ -524,6 +524,23 @@ H3_CASES = [
 ]
 
 
+@pytest.mark.parametrize("base,nx,ny,nz,a", [("c1", 16, 16, 1100, 2.5e-5), ("c3", 32, 16, 1594, 1e-3), ("c1", 16, 8, 40, 5e-5)])
+def test_helmholtz3d_through_the_thread_per_column_sweep(torch, pz, wl, oracle, base, nx, ny, nz, a):
+    """Above 1024 planes (and with zsolve_variant 0) the Eq. (8) systems take the sweep of pz_zsolve.cu."""
+    w = wl.scaled(wl.CONFIGS[base], nx, ny, nz)
+    zc, zf = wl.grid(w)
+    r = np.random.default_rng(nx + nz).standard_normal((nz, ny, nx))
+    plan = pz.poisson_plan_create(nx, ny, nz, w.lx, w.ly, zc, zf)
+    if nz <= 1024:
+        pz.pz_set_option(plan, "zsolve_variant", 0)
+    pz.helmholtz3d_setup(plan, a)
+    u = torch.from_numpy(r).cuda()
+    pz.helmholtz3d_solve(plan, u)
+    torch.cuda.synchronize()
+    assert rel_err(u.cpu().numpy(), oracle.helmholtz3d_solve(w.lx, w.ly, zc, zf, a, r, 1)) <= TOL
+    pz.poisson_plan_destroy(plan)
+
+
 @pytest.mark.parametrize("base,nx,ny,nz,a", H3_CASES)
 @pytest.mark.parametrize("variant", [1, 2])
 def test_helmholtz3d_matches_oracle(torch, pz, wl, oracle, base, nx, ny, nz, a, variant):
@@ -674,9 +691,7 @@ def test_error_paths_of_the_widened_entry_points(torch, pz, wl):
     assert ei.value.status == pz.PZ_EINVAL
     pz.helmholtz3d_setup(plan, 1e-3)
     u = torch.zeros(1100, 16, 16, dtype=torch.float64, device="cuda")
-    with pytest.raises(pz.PzError) as ei:
-        pz.helmholtz3d_solve(plan, u)                              # needs a shared-memory z-solve variant
-    assert ei.value.status == pz.PZ_EUNSUPPORTED
+    pz.helmholtz3d_solve(plan, u)                                  # above 1024 planes: thread-per-column sweep
     with pytest.raises(pz.PzError) as ei:
         pz.pz_set_option(plan, "zsolve_variant", 2)
     assert ei.value.status == pz.PZ_EUNSUPPORTED
