@@ -8,7 +8,7 @@
 * ONE Poisson problem: z-slabs ``[k0:k1, :, :]`` and the paper's parallel tridiagonal solver
   (PAPER.md:120-135): one all-gather of 2 nx ny boundary values per rank and solve
   (:func:`gather_boundaries`).
-* Independent Poisson problems (replicas): dealt round-robin, no collective.
+* Independent problems (replicas, ``bench.py --scaling weak``): every rank its own, no collective.
 
 This module holds no arithmetic of the method and works with the ``gloo`` backend on CPU (tests)
 and ``nccl`` on GPUs.
@@ -70,11 +70,6 @@ def gather_boundaries(ball, bout, dist=None) -> None:
     if ball.numel() != bout.numel() * dist.get_world_size():
         raise ValueError("gather_boundaries: ball must hold world_size buffers of bout's size")
     dist.all_gather_into_tensor(ball, bout)
-
-
-def deal_fields(n_fields: int, rank: int, world: int) -> List[int]:
-    """Indices of the independent fields solved by ``rank`` (round-robin)."""
-    return list(range(rank, n_fields, world))
 
 
 def rank_seed(seed: int, rank: int) -> int:

@@ -28,9 +28,7 @@ def test_y_slab_partitions_cover_exactly():
         ranks.y_slab(8, 2, 2)
 
 
-def test_deal_fields_and_rates():
-    assert ranks.deal_fields(3, 0, 2) == [0, 2] and ranks.deal_fields(3, 1, 2) == [1]
-    assert sorted(sum((ranks.deal_fields(7, r, 4) for r in range(4)), [])) == list(range(7))
+def test_seeds_and_rates():
     assert ranks.rank_seed(5, 0) == 5 and ranks.rank_seed(5, 3) == 3005
     assert ranks.whole_job_rate(1e6, 4, 2.0) == pytest.approx(2e9)
     assert ranks.max_over_ranks(1.5) == 1.5
