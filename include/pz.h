@@ -162,7 +162,8 @@ PZ_API int poisson_solve_finish_wait(pz_plan *plan, double *p, const double *bou
  * (u = 0 on the wall faces), touching only the right-hand side (Algorithm 2 Steps 2-4).
  *   u  device, nx*ny*nz doubles, in place: on entry r, on return u.
  * helmholtz_z_solve_n applies the same operator to n fields (the three velocity components).
- * Errors: PZ_ENOTSETUP before the first setup; PZ_EINVAL for a < 0 or null pointers.
+ * Errors: PZ_ENOTSETUP before the first setup; PZ_EINVAL for a < 0 or null pointers;
+ * PZ_EUNSUPPORTED from the set-up for nz > 3584 (a column chunk no longer fits shared memory).
  */
 PZ_API int helmholtz_z_setup(pz_plan *plan, double a);
 PZ_API int helmholtz_z_solve(pz_plan *plan, double *u, void *stream);

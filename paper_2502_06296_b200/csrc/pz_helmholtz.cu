@@ -114,9 +114,13 @@ int ilog2_ceil(int n)
 static void helm_geometry(pz_plan *pl)
 {
     int variant = pl->opt.helm_variant;
-    // variant 1 up to nz = 1920: beyond, the tile of a chunk plus the tables exceed shared memory
-    if (variant != 0 && variant != 1) variant = (pl->nz <= 1920) ? 1 : 0;
-    if (variant == 1 && (pl->nz > 1920 || (pl->nz > 1024 && pl->opt.helm_zsplit == 1))) variant = 0;
+    // variant 1 up to nz = 1920 with two chunks per column and up to 3584 with four: beyond, the tile
+    // of a chunk plus the tables exceed shared memory
+    const int zopt = pl->opt.helm_zsplit;
+    const int vmax = (zopt == 1) ? 1024 : (zopt == 2) ? 1920 : 3584;
+    if (variant != 0 && variant != 1) variant = (pl->nz <= vmax) ? 1 : 0;
+    if (variant == 1 && pl->nz > vmax) variant = 0;
+    if (variant == 0 && pl->nz > 2048 && pl->nz <= vmax) variant = 1;   // the register tile stops at 2048 planes
     pl->helm_variant = variant;
     int m = pl->opt.helm_m;
     pl->helm_zs = 1;
@@ -133,14 +137,18 @@ static void helm_geometry(pz_plan *pl)
         // nz = 512 and for nz up to 1920 at all.  Measured, 3 fields: 512^3 5.96 TB/s against 5.73
         // (whole columns, 32-column tiles) and 5.45 (16-column tiles); 1024^3 5.80 against 5.13 TB/s.
         int zs = pl->opt.helm_zsplit;
-        if (zs != 1 && zs != 2) zs = (m == 16) ? 2 : 1;
-        if (zs == 2 && (m != 16 || pl->nz < 4 * m)) zs = 1;
-        if (zs == 2) P = (P + 1) / 2;            // sub-domains per chunk
+        // (four chunks were measured slower than two wherever two fit: 1.17 against 1.09 ms at 512^3 x 3,
+        // 9.8 against 9.0 ms at 1024^3 x 3; they serve 1920 < nz <= 3584)
+        if (zs != 1 && zs != 2 && zs != 4) zs = (m != 16) ? 1 : (pl->nz > 1920 ? 4 : 2);
+        if (zs >= 2 && (m != 16 || pl->nz < 4 * m)) zs = 1;
+        if (zs == 4 && pl->nz < 8 * m) zs = 2;   // at least two sub-domains per chunk
+        if (zs >= 2) P = (P + zs - 1) / zs;      // sub-domains per chunk
         pl->helm_zs = zs;
         pl->helm_P = P;
         // wide tiles (32 columns, 256-byte rows) where one of them fits shared memory and 512 threads
         // (measured: 5.76 against 5.45 TB/s at 512^3 x 3 fields, 5.81 against 5.17 TB/s at 1024 x 1024 x 512 x 3)
         pl->helm_tx = (pl->opt.helm_tx != 16 && m == 16 && P <= 32 && even64) ? 32 : 16;
+        if (zs == 4 && pl->opt.helm_tx == 64 && P <= 16 && ((size_t)pl->nx * pl->ny) % 128 == 0) pl->helm_tx = 64;
         pl->helm_levels = ilog2_ceil(2 * P);
         return;
     }
@@ -243,7 +251,11 @@ void unit_response(const ld *A, const ld *B, const ld *C, int n, int j, std::vec
 } // namespace
 
 // Doubles of one chunk's table block: [5 nzc | PCR | corr (nzc) | wOwn, wPeer]
-static size_t chunk_doubles(int nzc, int P, int LV) { return 6 * (size_t)nzc + (size_t)LV * 4 * P + 2 * P + 2; }
+// (four chunks: [5 nzc | PCR | corrP (nzc) | corrN (nzc) | wP (8) | wN (8)])
+static size_t chunk_doubles(int nzc, int P, int LV, int ZS = 1)
+{
+    return (ZS > 2 ? 7 : 6) * (size_t)nzc + (size_t)LV * 4 * P + 2 * P + (ZS > 2 ? 4 * ZS : 2);
+}
 
 // Algorithm 2 Step 1 on the host, plus the precomputed PCR of the boundary system.
 int helmholtz_build_tables(pz_plan *pl, double a, int kind)
@@ -258,7 +270,8 @@ int helmholtz_build_tables(pz_plan *pl, double a, int kind)
         set_error("helmholtz: nz = %d is too large for the register-tile kernel (P = %d sub-domains)", nz, P);
         return PZ_EUNSUPPORTED;
     }
-    const size_t cstride = chunk_doubles(nzc, P, LV);
+    const size_t cstride = chunk_doubles(nzc, P, LV, ZS);
+    pl->helm_cstride = cstride;
     // the one-kernel step of Eq. (11) (helmholtz_z_step) takes whole columns: its own table block
     // behind the chunks' where the columns are cut and a whole one still fits the kernel (nz <= 1024)
     pl->helm_cn_P = 0; pl->helm_cn_levels = 0; pl->helm_cn_off = 0;
@@ -298,6 +311,70 @@ int helmholtz_build_tables(pz_plan *pl, double a, int kind)
     std::vector<double> host(ndbl, 0.0);
     if (ZS == 1) {
         build_chunk_tables(A.data(), B.data(), C.data(), m, P, LV, host.data());
+    } else if (ZS > 2) {
+        // ZS chunks (ZS CTAs of a cluster).  With y = T_c^{-1} r on every chunk,
+        //   u_c = y_c - corrP_c L_{c-1} - corrN_c F_{c+1},  corrP_c = A_cut,c T_c^{-1} e_first,  corrN_c = C_cut,c T_c^{-1} e_last,
+        // L_c / F_c the last / first value of u on chunk c; evaluated at the chunks' ends that is a
+        // linear system for the 2 (ZS - 1) interface values, inverted here once: every chunk gets the
+        // weights that turn the 2 ZS end values of y (F_0.., L_0..) into its L_{c-1} and F_{c+1}.
+        const int nu = 2 * (ZS - 1);
+        std::vector<std::vector<ld>> cP(ZS), cN(ZS);
+        for (int c = 0; c < ZS; ++c) {
+            std::vector<ld> Ac(A.begin() + c * nzc, A.begin() + (c + 1) * nzc), Bc(B.begin() + c * nzc, B.begin() + (c + 1) * nzc),
+                Cc(C.begin() + c * nzc, C.begin() + (c + 1) * nzc);
+            const ld Acut = Ac[0], Ccut = Cc[nzc - 1];
+            Ac[0] = 0;
+            Cc[nzc - 1] = 0;
+            build_chunk_tables(Ac.data(), Bc.data(), Cc.data(), m, P, LV, host.data() + c * cstride);
+            std::vector<ld> pr, qr;
+            unit_response(Ac.data(), Bc.data(), Cc.data(), nzc, 0, pr);
+            unit_response(Ac.data(), Bc.data(), Cc.data(), nzc, nzc - 1, qr);
+            cP[c].resize(nzc);
+            cN[c].resize(nzc);
+            for (int k = 0; k < nzc; ++k) { cP[c][k] = (c > 0 ? Acut : (ld)0) * pr[k]; cN[c][k] = (c + 1 < ZS ? Ccut : (ld)0) * qr[k]; }
+        }
+        // unknown index: F_c (c = 1..ZS-1) -> c - 1;  L_c (c = 0..ZS-2) -> ZS - 1 + c
+        auto iF = [&](int c) { return c - 1; };
+        auto iL = [&](int c) { return ZS - 1 + c; };
+        std::vector<std::vector<ld>> Mx(nu, std::vector<ld>(nu + 2 * ZS, 0)); // [matrix | selection of the y values]
+        for (int c = 1; c < ZS; ++c) {            // F_c + kPF L_{c-1} + kNF F_{c+1} = yF_c
+            auto &row = Mx[iF(c)];
+            row[iF(c)] += 1;
+            row[iL(c - 1)] += cP[c][0];
+            if (c + 1 < ZS) row[iF(c + 1)] += cN[c][0];
+            row[nu + c] = 1;                      // yF_c
+        }
+        for (int c = 0; c + 1 < ZS; ++c) {        // L_c + kPL L_{c-1} + kNL F_{c+1} = yL_c
+            auto &row = Mx[iL(c)];
+            row[iL(c)] += 1;
+            if (c > 0) row[iL(c - 1)] += cP[c][nzc - 1];
+            row[iF(c + 1)] += cN[c][nzc - 1];
+            row[nu + ZS + c] = 1;                 // yL_c
+        }
+        for (int col = 0; col < nu; ++col) {      // Gauss-Jordan with partial pivoting (diagonally dominant: benign)
+            int piv = col;
+            for (int r = col + 1; r < nu; ++r)
+                if (fabsl(Mx[r][col]) > fabsl(Mx[piv][col])) piv = r;
+            std::swap(Mx[col], Mx[piv]);
+            const ld inv = (ld)1 / Mx[col][col];
+            for (auto &v : Mx[col]) v *= inv;
+            for (int r = 0; r < nu; ++r) {
+                if (r == col) continue;
+                const ld f = Mx[r][col];
+                if (f == 0) continue;
+                for (int q = 0; q < nu + 2 * ZS; ++q) Mx[r][q] -= f * Mx[col][q];
+            }
+        }
+        const size_t ocorr = 5 * (size_t)nzc + (size_t)LV * 4 * P + 2 * P;
+        for (int c = 0; c < ZS; ++c) {
+            double *blk = host.data() + c * cstride + ocorr;
+            for (int k = 0; k < nzc; ++k) { blk[k] = (double)cP[c][k]; blk[nzc + k] = (double)cN[c][k]; }
+            for (int q = 0; q < 2 * ZS; ++q) {
+                blk[2 * nzc + q] = (c > 0) ? (double)Mx[iL(c - 1)][nu + q] : 0.0;               // L_{c-1}
+                blk[2 * nzc + 2 * ZS + q] = (c + 1 < ZS) ? (double)Mx[iF(c + 1)][nu + q] : 0.0; // F_{c+1}
+            }
+        }
+        if (cn_doubles > 0) build_chunk_tables(A.data(), B.data(), C.data(), m, pl->helm_cn_P, pl->helm_cn_levels, host.data() + pl->helm_cn_off);
     } else {
         // two chunks, couplings across the cut moved to the interface (PAPER.md:120-135 with the
         // two CTAs of a cluster for its MPI tasks; the matrix is k-only, so everything the

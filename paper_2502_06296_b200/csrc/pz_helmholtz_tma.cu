@@ -62,9 +62,10 @@ template <int M, int TX = kTX, int ZS = 1> struct Smem {
     __host__ __device__ static int box_rows(int P) { return (((P * M + nbox(P) - 1) / nbox(P)) + 7) & ~7; }
     __host__ __device__ static size_t tile(int P) { return (size_t)box_rows(P) * nbox(P) * kTX; }
     __host__ __device__ static size_t xch(int P) { return (size_t)2 * 2 * P * kTX; }
-    __host__ __device__ static size_t tab(int P) { return (size_t)(ZS > 1 ? 6 : 5) * P * TS; }   // 6th table: z-split correction
+    __host__ __device__ static size_t tab(int P) { return (size_t)(ZS > 2 ? 7 : ZS > 1 ? 6 : 5) * P * TS; }   // 6th / 7th table: z-split corrections
     __host__ __device__ static size_t pcr(int P, int levels) { return (size_t)levels * 4 * P + 2 * P; }
-    __host__ __device__ static size_t zx() { return ZS > 1 ? (size_t)2 * 2 * TX : 0; } // z-split: [parity][own/peer][TX]
+    // z-split interface values: ZS = 2 [parity][own / peer][TX]; ZS = 4 [parity][chunk][first / last][TX]
+    __host__ __device__ static size_t zx() { return ZS > 2 ? (size_t)2 * ZS * 2 * TX : ZS > 1 ? (size_t)2 * 2 * TX : 0; }
     __host__ __device__ static size_t bytes(int P, int levels, bool cn = false)
     {
         return ((cn ? 2 : 1) * tile(P) + xch(P) + tab(P) + pcr(P, levels) + zx()) * sizeof(double) + 16;
@@ -82,7 +83,8 @@ template <int M, int TX = kTX, int ZS = 1> struct Smem {
 template <int M, bool FULL, int CN, int TX = 16, int ZS = 1>
 __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M>::kMinBlocks)
     helmholtz_tma_kernel(const __grid_constant__ HelmArgs args, const double *__restrict__ tab_all, size_t plane, int nz,
-                         int P, int levels, int tiles_per_field, int total_tiles, int probe, int box_rows, int nbox, int csz)
+                         int P, int levels, int tiles_per_field, int total_tiles, int probe, int box_rows, int nbox, int csz,
+                         size_t cstride)
 {
     static_assert(ZS == 1 || CN == 0, "the fused step kernel takes whole columns");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -104,7 +106,7 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
     const int cl_rank = (ZS > 1) ? (int)(blockIdx.x % csz) : 0;
     const int crank = cl_rank % ZS, ctile = cl_rank / ZS, TP = (ZS > 1) ? csz / ZS : 1;
     const int kc0 = crank * nzp_of(P, M);
-    const double *tab = tab_all + (size_t)crank * (6 * (size_t)P * M + L::pcr(P, levels) + 2);
+    const double *tab = tab_all + (size_t)crank * cstride;
     const int k0 = s * M;                                  // row inside the chunk
     const unsigned tile_bytes = (unsigned)((CN == 1 ? 2 : 1) * L::tile(P) * sizeof(double));
 
@@ -118,11 +120,20 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
     }
     for (int q = tid; q < (int)L::pcr(P, levels); q += blockDim.x) spcr[q] = tab[5 * (size_t)nzp + q];
     double w_own = 0.0, w_peer = 0.0;
-    if constexpr (ZS > 1) {
+    double wP[ZS > 2 ? 2 * ZS : 1], wN[ZS > 2 ? 2 * ZS : 1]; // ZS = 4: weights of the 2 ZS end values of y
+    if constexpr (ZS == 2) {
         const double *corr = tab + 5 * (size_t)nzp + L::pcr(P, levels);
         for (int k = tid; k < nzp; k += blockDim.x) stab[(size_t)5 * P * TS + (k / M) * TS + (k % M)] = corr[k];
         w_own = corr[nzp];
         w_peer = corr[nzp + 1];
+    } else if constexpr (ZS > 2) {
+        const double *corr = tab + 5 * (size_t)nzp + L::pcr(P, levels);
+        for (int k = tid; k < 2 * nzp; k += blockDim.x) {
+            const int t6 = k / nzp, kk = k - t6 * nzp;
+            stab[(size_t)(5 + t6) * P * TS + (kk / M) * TS + (kk % M)] = corr[k];
+        }
+#pragma unroll
+        for (int q = 0; q < 2 * ZS; ++q) { wP[q] = corr[2 * nzp + q]; wN[q] = corr[2 * nzp + 2 * ZS + q]; }
     }
     __syncthreads();
 
@@ -274,8 +285,38 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
         // z-split: x0 / x1 are the chunk-local solution y at the sub-domain ends.  The chunk's
         // interface value (last row of chunk 0, first row of chunk 1) goes to both CTAs; the value
         // of the neighbouring chunk's interface row follows from the precomputed 2 x 2 system.
-        double2 X = make_double2(0.0, 0.0);
-        if constexpr (ZS > 1) {
+        double2 X = make_double2(0.0, 0.0), Xn = make_double2(0.0, 0.0);
+        if constexpr (ZS > 2) {
+            // every chunk's first and last value of y go to all CTAs of the cluster; the values of the
+            // neighbouring chunks' interface rows are precomputed linear combinations of them
+            double *slot = zx + (size_t)zpar * (ZS * 2 * TX);
+            const int cbase = (cl_rank / ZS) * ZS;
+            if (s == 0 || s == P - 1) {
+#pragma unroll
+                for (int r = 0; r < ZS; ++r) {
+                    if (s == 0) {
+                        unsigned ra;
+                        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(smem_u32(slot + (crank * 2 + 0) * TX + c2)), "r"(cbase + r));
+                        asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(ra), "d"(x0.x), "d"(x0.y) : "memory");
+                    }
+                    if (s == P - 1) {
+                        unsigned ra;
+                        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(smem_u32(slot + (crank * 2 + 1) * TX + c2)), "r"(cbase + r));
+                        asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(ra), "d"(x1.x), "d"(x1.y) : "memory");
+                    }
+                }
+            }
+            asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+#pragma unroll
+            for (int r = 0; r < ZS; ++r) {
+                const double2 yf = ld2(slot + (r * 2 + 0) * TX + c2), yl = ld2(slot + (r * 2 + 1) * TX + c2);
+                X.x = fma(wP[r], yf.x, fma(wP[ZS + r], yl.x, X.x));
+                X.y = fma(wP[r], yf.y, fma(wP[ZS + r], yl.y, X.y));
+                Xn.x = fma(wN[r], yf.x, fma(wN[ZS + r], yl.x, Xn.x));
+                Xn.y = fma(wN[r], yf.y, fma(wN[ZS + r], yl.y, Xn.y));
+            }
+            zpar ^= 1;
+        } else if constexpr (ZS > 1) {
             double *slot = zx + (size_t)zpar * 2 * TX;
             if ((crank == 0 && s == P - 1) || (crank == 1 && s == 0)) {
                 const double2 mine = (crank == 0) ? x1 : x0;
@@ -316,6 +357,11 @@ __global__ void __launch_bounds__(Limits<M>::kMaxThreads, CN != 0 ? 1 : Limits<M
                 const double2 cr = ld2(rx + i);
                 v.x = fma(-cr.x, X.x, v.x); v.y = fma(-cr.x, X.y, v.y);
                 w.x = fma(-cr.y, X.x, w.x); w.y = fma(-cr.y, X.y, w.y);
+            }
+            if constexpr (ZS > 2) {
+                const double2 cn = ld2(rx + (size_t)P * TS + i);
+                v.x = fma(-cn.x, Xn.x, v.x); v.y = fma(-cn.x, Xn.y, v.y);
+                w.x = fma(-cn.y, Xn.x, w.x); w.y = fma(-cn.y, Xn.y, w.y);
             }
             if (FULL || kc0 + k0 + i < nz) st2g(up + (size_t)i * plane, v);
             if (FULL || kc0 + k0 + i + 1 < nz) st2g(up + (size_t)(i + 1) * plane, w);
@@ -410,7 +456,7 @@ int launch_mf(pz_plan *pl, double *const *u, int n, const double *tab, cudaStrea
     blocks = blocks / csz * csz;
     cfg.gridDim = dim3((unsigned)blocks);
     PZ_CUDA(cudaLaunchKernelEx(&cfg, helmholtz_tma_kernel<M, FULL, 0, TX, ZS>, args, tab, plane, pl->nz, P, pl->helm_levels,
-                               tiles_per_field, (int)total, probe, box_rows, nbox, csz));
+                               tiles_per_field, (int)total, probe, box_rows, nbox, csz, pl->helm_cstride));
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
@@ -439,7 +485,8 @@ int launch_cn_mfc(pz_plan *pl, double *u2, const double *uk, const double *tab, 
     args.A = pl->d_A; args.C = pl->d_C; args.a = pl->helm_a; args.w0 = pl->wall_w0; args.w1 = pl->wall_w1;
     const int tiles = (int)(plane / kTX);
     int blocks = pl->num_sms < tiles ? pl->num_sms : tiles;
-    kern<<<blocks, (kTX / 2) * P, smem, st>>>(args, tab + pl->helm_cn_off, plane, pl->nz, P, pl->helm_cn_levels, tiles, tiles, 0, box_rows, nbox, 1);
+    kern<<<blocks, (kTX / 2) * P, smem, st>>>(args, tab + pl->helm_cn_off, plane, pl->nz, P, pl->helm_cn_levels, tiles, tiles, 0, box_rows, nbox, 1,
+                                              (size_t)0);
     count_launch();
     PZ_CUDA(cudaGetLastError());
     return PZ_OK;
@@ -481,6 +528,9 @@ int helmholtz_tma_prepare(pz_plan *pl)
     case 4: return PZ_HP(4);
     case 8: return PZ_HP(8);
     case 16:
+        if (pl->helm_zs == 4 && pl->helm_tx == 64) return full ? prepare_mf<16, true, 64, 4>(pl) : prepare_mf<16, false, 64, 4>(pl);
+        if (pl->helm_zs == 4 && pl->helm_tx == 32) return full ? prepare_mf<16, true, 32, 4>(pl) : prepare_mf<16, false, 32, 4>(pl);
+        if (pl->helm_zs == 4) return full ? prepare_mf<16, true, 16, 4>(pl) : prepare_mf<16, false, 16, 4>(pl);
         if (pl->helm_zs == 2 && pl->helm_tx == 32) return full ? prepare_mf<16, true, 32, 2>(pl) : prepare_mf<16, false, 32, 2>(pl);
         if (pl->helm_zs == 2) return full ? prepare_mf<16, true, 16, 2>(pl) : prepare_mf<16, false, 16, 2>(pl);
         if (pl->helm_tx == 32) return full ? prepare_mf<16, true, 32>(pl) : prepare_mf<16, false, 32>(pl);
@@ -503,6 +553,9 @@ int launch_helmholtz_tma(pz_plan *pl, double *const *u, int n, const double *tab
     case 4: return PZ_HT(4);
     case 8: return PZ_HT(8);
     case 16:
+        if (pl->helm_zs == 4 && pl->helm_tx == 64) return full ? launch_mf<16, true, 64, 4>(pl, u, n, tab, st) : launch_mf<16, false, 64, 4>(pl, u, n, tab, st);
+        if (pl->helm_zs == 4 && pl->helm_tx == 32) return full ? launch_mf<16, true, 32, 4>(pl, u, n, tab, st) : launch_mf<16, false, 32, 4>(pl, u, n, tab, st);
+        if (pl->helm_zs == 4) return full ? launch_mf<16, true, 16, 4>(pl, u, n, tab, st) : launch_mf<16, false, 16, 4>(pl, u, n, tab, st);
         if (pl->helm_zs == 2 && pl->helm_tx == 32) return full ? launch_mf<16, true, 32, 2>(pl, u, n, tab, st) : launch_mf<16, false, 32, 2>(pl, u, n, tab, st);
         if (pl->helm_zs == 2) return full ? launch_mf<16, true, 16, 2>(pl, u, n, tab, st) : launch_mf<16, false, 16, 2>(pl, u, n, tab, st);
         if (pl->helm_tx == 32) return full ? launch_mf<16, true, 32>(pl, u, n, tab, st) : launch_mf<16, false, 32>(pl, u, n, tab, st);

@@ -104,6 +104,7 @@ struct pz_plan {
     int helm_bps = 0;                // variant 1: resident CTAs per SM
     int helm_cn_P = 0, helm_cn_levels = 0; // whole-column tables for the one-kernel step of Eq. (11) (0 = none)
     size_t helm_cn_off = 0;          // their offset (doubles) in a table set
+    size_t helm_cstride = 0;         // doubles of one chunk's table block
     int helm_nclusters[3] = {0, 0, 0}; // variant 1: resident clusters of 2 / 4 / 8 CTAs (0 = not yet queried)
     std::vector<pz::HelmTables> helm; // table sets: the current one, one being uploaded, and any a captured graph reads
     int helm_cur = -1;               // current set of the cell-centred operator (u, v)

@@ -324,10 +324,18 @@ HELM_CASES = [
     (64, 32, 1024, 1.8, 2.5e-5, []),     # cut column, 32-column tiles, no padding
     (64, 32, 1024, 1.8, 2.5e-5, [("helm_zsplit", 1)]),   # whole columns per CTA
     (8, 8, 1024, 1.8, 10.0, []),         # strongly implicit across the cut
+    (64, 32, 1024, 1.8, 2.5e-5, [("helm_zsplit", 4)]),                   # four chunks per column
+    (64, 32, 512, 1.8, 10.0, [("helm_zsplit", 4)]),                      # strongly implicit across three cuts
+    (64, 32, 512, 1.8, 5e-5, [("helm_zsplit", 4), ("helm_tx", 64)]),     # 64-column tiles
+    (64, 32, 700, 2.0, 5e-5, [("helm_zsplit", 4)]),                      # padding rows in the last chunk
+    (12, 12, 300, 1.8, 5e-5, [("helm_zsplit", 4)]),                      # 16-column tiles
+    (64, 32, 1594, 1.8, 2.5e-5, [("helm_zsplit", 4)]),
     (12, 12, 600, 1.8, 5e-5, []),        # cut column, 16-column tiles (144 columns)
     (64, 32, 1594, 1.8, 2.5e-5, []),     # the paper's nz on the pipeline: 50 sub-domains per chunk
     (16, 8, 1920, 1.8, 2.5e-5, []),      # largest nz of the pipeline
-    (16, 8, 2048, 1.8, 2.5e-5, []),      # beyond: register-tile kernel
+    (16, 8, 2048, 1.8, 2.5e-5, []),      # beyond: four chunks per column
+    (16, 8, 3000, 1.8, 2.5e-5, []),
+    (16, 8, 3584, 1.8, 2.5e-5, []),      # largest nz of the pipeline
     (128, 64, 48, 1.8, 5e-5, []),
 ]
 
@@ -346,7 +354,10 @@ def test_helmholtz_matches_oracle(torch, pz, wl, oracle, nx, ny, nz, beta, a, op
         pz.pz_set_option(plan, k, v)
     pz.helmholtz_z_setup(plan, a)
     whole = ("helm_zsplit", 1) in options
-    assert pz.pz_get_option(plan, "helm_variant_actual") == (variant if nz <= (1024 if whole else 1920) else 0)
+    expect = variant if nz <= (1024 if whole else 3584) else 0
+    if nz > 2048:
+        expect = 1                                   # the register-tile kernel stops at 2048 planes
+    assert pz.pz_get_option(plan, "helm_variant_actual") == expect
     u = torch.from_numpy(r).cuda()
     pz.helmholtz_z_solve(plan, u)
     torch.cuda.synchronize()
@@ -357,7 +368,7 @@ def test_helmholtz_matches_oracle(torch, pz, wl, oracle, nx, ny, nz, beta, a, op
 
 @pytest.mark.parametrize("nx,ny,nz,beta,a", [(8, 8, 4, 0.0, 0.1), (32, 16, 100, 1.8, 5e-5), (16, 16, 256, 2.0, 1e-3),
                                              (64, 32, 512, 1.8, 5e-5), (64, 32, 700, 1.8, 5e-5), (16, 8, 1024, 1.8, 10.0),
-                                             (16, 8, 1594, 1.8, 2.5e-5), (8, 8, 2048, 1.8, 2.5e-5)])
+                                             (16, 8, 1594, 1.8, 2.5e-5), (8, 8, 2048, 1.8, 2.5e-5), (8, 8, 3200, 1.8, 2.5e-5)])
 def test_helmholtz_w_face_centred_matches_oracle(torch, pz, wl, oracle, nx, ny, nz, beta, a):
     """The wall-normal component on the z faces (reading R16) through every kernel variant the size
     selects, beside a cell-centred set-up with another coefficient on the same plan."""
@@ -386,6 +397,15 @@ def test_helmholtz_w_face_centred_matches_oracle(torch, pz, wl, oracle, nx, ny, 
     torch.cuda.synchronize()
     assert rel_err(w2.cpu().numpy(), oracle.helmholtz_w_solve(zc, zf, 2 * a, r)) <= TOL
     assert torch.equal(u2, u)
+    pz.poisson_plan_destroy(plan)
+
+
+def test_helmholtz_beyond_3584_planes_is_refused(torch, pz, wl):
+    zf = wl.z_faces(4000, 2.0, 1.8)
+    plan = pz.poisson_plan_create(8, 8, 4000, 1.0, 1.0, wl.z_centres(zf), zf)
+    with pytest.raises(pz.PzError) as ei:
+        pz.helmholtz_z_setup(plan, 1e-4)
+    assert ei.value.status == pz.PZ_EUNSUPPORTED
     pz.poisson_plan_destroy(plan)
 
 
