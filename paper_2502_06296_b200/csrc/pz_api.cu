@@ -6,7 +6,6 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -305,9 +304,9 @@ static int plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double 
     if (ce != cudaSuccess) { cudaGetLastError(); set_error("plan counters: %s", cudaGetErrorString(ce)); return fail(PZ_ENOMEM); }
     // measured at 512 x 512 x nz: variant 2 wins from nz = 256 up to 1024, variant 1 below
     pl->opt.zsolve_variant = (nz <= 32) ? 4 : (nz <= 128) ? 1 : (nz <= 1024) ? 2 : 0;
-    const char *cut_env = getenv("PZ_ZCUT_ABOVE");   // tuning aid: internal cut for nz above this (default 1024)
-    const int cut_above = cut_env ? atoi(cut_env) : 1024;
-    if (nk == nz && nz > cut_above && nz <= 16 * 512 && bc == 0) {
+    // (cutting columns of 1024 planes or fewer was measured slower than the whole-column pipeline:
+    // 2.06 against 1.74 ms at 512 x 512 x 1024)
+    if (nk == nz && nz > 1024 && nz <= 16 * 512 && bc == 0) {
         // whole columns longer than the pipeline's tile: the plan's own cut in z (pz_zslab.cu), slabs of
         // at most 512 planes (16 rows per lane: three pipeline stages fit shared memory)
         // full slabs of 512 planes (no padding rows in their tiles) and one remainder of at least 3
