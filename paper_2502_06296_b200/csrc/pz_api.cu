@@ -303,7 +303,7 @@ static int plan_create(pz_plan **out, int nx, int ny, int nz, double lx, double 
     ce = cudaMalloc(&pl->d_xyctr, 2 * (size_t)(nk + 64) * sizeof(int));
     if (ce != cudaSuccess) { cudaGetLastError(); set_error("plan counters: %s", cudaGetErrorString(ce)); return fail(PZ_ENOMEM); }
     // measured at 512 x 512 x nz: variant 2 wins from nz = 256 up to 1024, variant 1 below
-    pl->opt.zsolve_variant = (nz <= 32) ? 4 : (nz <= 128) ? 1 : (nz <= 1024) ? 2 : 0;
+    pl->opt.zsolve_variant = (nz <= 64) ? 4 : (nz <= 128) ? 1 : (nz <= 1024) ? 2 : 0;
     // (cutting columns of 1024 planes or fewer was measured slower than the whole-column pipeline:
     // 2.06 against 1.74 ms at 512 x 512 x 1024)
     if (nk == nz && nz > 1024 && nz <= 16 * 512 && bc == 0) {
@@ -795,7 +795,7 @@ int pz_set_option(pz_plan *pl, const char *key, int value)
     if (!slot) { set_error("pz_set_option: unknown key '%s'", key); return PZ_EUNSUPPORTED; }
     if (slot == &pl->opt.zsolve_variant) {
         if (value < 0 || value > 4) { set_error("zsolve_variant must be 0 ... 4"); return PZ_EUNSUPPORTED; }
-        if (value == 4 && pl->nz > 32) { set_error("zsolve_variant 4 supports nz <= 32"); return PZ_EUNSUPPORTED; }
+        if (value == 4 && pl->nz > 64) { set_error("zsolve_variant 4 supports nz <= 64"); return PZ_EUNSUPPORTED; }
         if ((value == 1 || value == 2) && pl->nz > 1024) { set_error("zsolve_variant %d supports nz <= 1024", value); return PZ_EUNSUPPORTED; }
         if (value == 3 && !pl->slab_internal) { set_error("zsolve_variant 3 is the plan's own z cut (nz > 1024)"); return PZ_EUNSUPPORTED; }
         if (value == 0) { const int rc = ensure_zwork(pl); if (rc != PZ_OK) return rc; }

@@ -20,7 +20,8 @@ namespace pz {
 namespace {
 
 constexpr int kE = 16;    // complex points per thread, at most
-constexpr int kPts = 512 * kE;   // largest buffer: 512 threads
+constexpr int kMaxT = 512;        // threads per CTA, at most (128 registers each)
+constexpr int kPts = kMaxT * kE;  // largest buffer
 // Threads per CTA: 512 (8192-point buffer, one CTA per SM) where a line or a useful tile needs it,
 // else 256 (4096 points, two CTAs per SM: the loads of one overlap the passes of the other).
 
@@ -105,79 +106,172 @@ template <> __device__ __forceinline__ void dft<7>(double2 (&v)[7])
     v[3] = cadd(e3, d3); v[4] = csub(e3, d3);
 }
 
-// One in-place pass over `nlines` lines of complex length L in shared memory; element pos of line
-// ln sits at s[ln * sl + pos * sp].  tw[k * tws] = exp(-2 pi i k / L).
-template <int R, int kT>
-__device__ __forceinline__ void pass(double2 *s, int L, int Ns, int nlines, int sl, int sp, const double2 *__restrict__ tw, int tws)
+// Composite radices.  Coprime factors (6, 10, 12, 14, 15): the prime-factor map, input
+// n = (R2 n1 + R1 n2) mod R, output k with k = k1 (mod R1), k = k2 (mod R2), needs no twiddles
+// between the two stages.  9 = 3 x 3: Cooley-Tukey with the constants w_9, w_9^2, w_9^4.
+__host__ __device__ constexpr int crt_index(int R1, int R2, int k1, int k2)
 {
-    constexpr int Q = (kE + R - 1) / R;
-    const int nb = L / R, W = nlines * nb, step = (L / (Ns * R)) * tws;
-    const int instr = nb * sp, outstr = Ns * sp;
+    for (int k = 0; k < R1 * R2; ++k)
+        if (k % R1 == k1 && k % R2 == k2) return k;
+    return 0;
+}
+template <int R1, int R2> __device__ __forceinline__ void dft_pfa(double2 (&v)[R1 * R2])
+{
+    constexpr int R = R1 * R2;
+    double2 a[R2][R1];
+#pragma unroll
+    for (int n2 = 0; n2 < R2; ++n2)
+#pragma unroll
+        for (int n1 = 0; n1 < R1; ++n1) a[n2][n1] = v[(R2 * n1 + R1 * n2) % R];
+#pragma unroll
+    for (int n2 = 0; n2 < R2; ++n2) dft<R1>(a[n2]);
+#pragma unroll
+    for (int k1 = 0; k1 < R1; ++k1) {
+        double2 b[R2];
+#pragma unroll
+        for (int n2 = 0; n2 < R2; ++n2) b[n2] = a[n2][k1];
+        dft<R2>(b);
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) v[crt_index(R1, R2, k1, k2)] = b[k2];
+    }
+}
+template <> __device__ __forceinline__ void dft<6>(double2 (&v)[6]) { dft_pfa<3, 2>(v); }
+template <> __device__ __forceinline__ void dft<10>(double2 (&v)[10]) { dft_pfa<5, 2>(v); }
+template <> __device__ __forceinline__ void dft<12>(double2 (&v)[12]) { dft_pfa<3, 4>(v); }
+template <> __device__ __forceinline__ void dft<14>(double2 (&v)[14]) { dft_pfa<7, 2>(v); }
+template <> __device__ __forceinline__ void dft<15>(double2 (&v)[15]) { dft_pfa<3, 5>(v); }
+template <> __device__ __forceinline__ void dft<9>(double2 (&v)[9])
+{
+    // X[k1 + 3 k2] = sum_n2 w_9^{n2 k1} w_3^{n2 k2} sum_n1 x[3 n1 + n2] w_3^{n1 k1}
+    constexpr double c1 = 0.766044443118978, s1 = 0.6427876096865393;    // cos, sin of 2 pi / 9
+    constexpr double c2 = 0.17364817766693041, s2 = 0.984807753012208;   // of 4 pi / 9
+    constexpr double c4 = -0.9396926207859084, s4 = 0.3420201433256687;  // of 8 pi / 9
+    double2 a[3][3];
+#pragma unroll
+    for (int n2 = 0; n2 < 3; ++n2) {
+#pragma unroll
+        for (int n1 = 0; n1 < 3; ++n1) a[n2][n1] = v[3 * n1 + n2];
+        dft<3>(a[n2]);
+    }
+    a[1][1] = cmul(a[1][1], make_double2(c1, -s1));
+    a[1][2] = cmul(a[1][2], make_double2(c2, -s2));
+    a[2][1] = cmul(a[2][1], make_double2(c2, -s2));
+    a[2][2] = cmul(a[2][2], make_double2(c4, -s4));
+#pragma unroll
+    for (int k1 = 0; k1 < 3; ++k1) {
+        double2 b[3] = {a[0][k1], a[1][k1], a[2][k1]};
+        dft<3>(b);
+#pragma unroll
+        for (int k2 = 0; k2 < 3; ++k2) v[k1 + 3 * k2] = b[k2];
+    }
+}
+
+// butterflies per thread and pass: kE points or a little more (at most 21) up to radix 9, ONE
+// butterfly of 10 ... 16 points above; the launch geometry sizes the CTA so that every pass fits
+__host__ __device__ constexpr int bfly_per_thread(int R) { return R <= 9 ? (kE + R - 1) / R : 1; }
+
+// Where a pass reads and writes: element pos of line ln sits at base[ln * sl + pos * sp].  A pass
+// may read from global memory (the first one) or write to it (the last one): the lines then make
+// no extra round trip through shared memory on their way in and out.  The imaginary part is
+// negated on the way in where im < 0, the result multiplied by (re, im) on the way out (conjugation
+// and scaling of the inverse transforms).
+struct Side {
+    double2 *base;
+    int sl, sp;
+    double re, im;
+};
+
+// One pass over `nlines` lines of complex length L.  tw[k * tws] = exp(-2 pi i k / L).
+// lines_fastest: consecutive threads take the same butterfly of neighbouring lines (y columns).
+template <int R>
+__device__ __forceinline__ void pass(const Side in, const Side out, bool in_place, bool out_shared, int L, int Ns, int nlines,
+                                     bool lines_fastest, const double2 *__restrict__ tw, int tws)
+{
+    constexpr int Q = bfly_per_thread(R);
+    const int nb = L / R, W = nlines * nb, step = (L / (Ns * R)) * tws, kT = (int)blockDim.x;
+    const int instr = nb * in.sp, outstr = Ns * out.sp;
+    const bool conj_in = in.im < 0.0, scaled = out.re != 1.0 || out.im != 1.0;
     double2 v[Q][R];
     int obase[Q];
 #pragma unroll
     for (int q = 0; q < Q; ++q) {
         // work items past the end recompute item 0 and store nothing (no divergent definitions)
         const int w0 = (int)threadIdx.x + q * kT, w = (w0 < W) ? w0 : 0;
-        // lines fastest when they are interleaved in memory (sl == 1), butterflies fastest otherwise
-        const int ln = (sl == 1) ? w % nlines : w / nb, j = (sl == 1) ? w / nlines : w % nb;
+        const int ln = lines_fastest ? w % nlines : w / nb, j = lines_fastest ? w / nlines : w % nb;
         const int jm = j % Ns;
-        const double2 *x = s + (ln * sl + j * sp);
-        obase[q] = (w0 < W) ? ln * sl + ((j - jm) * R + jm) * sp : -1;
-        const int tstep = jm * step;
+        const double2 *x = in.base + (ln * in.sl + j * in.sp);
+        obase[q] = (w0 < W) ? ln * out.sl + ((j - jm) * R + jm) * out.sp : -1;
+        // ONE twiddle look-up per butterfly, w = w_{Ns R}^{jm}; the powers w^r are products of at most
+        // log2 R factors (ncu r02: with R - 1 scattered 16-byte look-ups per butterfly the kernels were
+        // bound by the L1 / shared-memory data pipe at 17 % of the DRAM rate)
+        double2 wp[R];
+        wp[0] = make_double2(1.0, 0.0);
+        if constexpr (R > 1) wp[1] = __ldg(&tw[jm * step]);
+#pragma unroll
+        for (int r = 2; r < R; ++r) {
+            int hb = 1;
+            while (hb * 2 <= r) hb *= 2;
+            wp[r] = (r == hb) ? cmul(wp[hb / 2], wp[hb / 2]) : cmul(wp[hb], wp[r - hb]);
+        }
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             double2 t = x[r * instr];
-            if (r > 0) t = cmul(t, __ldg(&tw[r * tstep]));
+            if (conj_in) t.y = -t.y;
+            if (r > 0) t = cmul(t, wp[r]);
             v[q][r] = t;
         }
         dft<R>(v[q]);
     }
-    __syncthreads();
+    if (in_place) __syncthreads();
 #pragma unroll
     for (int q = 0; q < Q; ++q) {
         if (obase[q] >= 0) {
-            double2 *y = s + obase[q];
+            double2 *y = out.base + obase[q];
 #pragma unroll
-            for (int r = 0; r < R; ++r) y[r * outstr] = v[q][r];
+            for (int r = 0; r < R; ++r) y[r * outstr] = scaled ? make_double2(v[q][r].x * out.re, v[q][r].y * out.im) : v[q][r];
         }
     }
-    __syncthreads();
+    if (out_shared) __syncthreads();
 }
 
-template <int kT>
-__device__ __forceinline__ void all_passes(double2 *s, int L, int nlines, int sl, int sp, const double2 *__restrict__ tw, int tws,
-                                           const Radices &rl)
+// All passes of the lines of a CTA: the first reads `src`, the last writes `dst`, the ones between
+// work in place in the shared-memory buffer `mid`.  src / dst may be `mid` itself.
+__device__ __forceinline__ void all_passes(const Side src, const Side mid, const Side dst, int L, int nlines, bool lines_fastest,
+                                           const double2 *__restrict__ tw, int tws, const Radices &rl)
 {
     int Ns = 1;
     for (int i = 0; i < rl.n; ++i) {
+        const Side in = (i == 0) ? src : mid, out = (i == rl.n - 1) ? dst : mid;
+        const bool in_place = in.base == out.base, out_shared = out.base == mid.base;
         switch (rl.r[i]) {
-        case 2: pass<2, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
-        case 3: pass<3, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
-        case 4: pass<4, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
-        case 5: pass<5, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
-        case 7: pass<7, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
-        case 16: pass<16, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
-        default: pass<8, kT>(s, L, Ns, nlines, sl, sp, tw, tws); break;
+#define PZ_PASS(R_) case R_: pass<R_>(in, out, in_place, out_shared, L, Ns, nlines, lines_fastest, tw, tws); break;
+        PZ_PASS(2) PZ_PASS(3) PZ_PASS(4) PZ_PASS(5) PZ_PASS(6) PZ_PASS(7) PZ_PASS(8) PZ_PASS(9) PZ_PASS(10) PZ_PASS(12)
+        PZ_PASS(14) PZ_PASS(15)
+#undef PZ_PASS
+        default: pass<16>(in, out, in_place, out_shared, L, Ns, nlines, lines_fastest, tw, tws); break;
         }
         Ns *= rl.r[i];
     }
 }
 
 // x lines: lpb lines of n = 2M reals per CTA.  twx[k] = exp(-2 pi i k / n).
-template <bool INV, int kT>
-__global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_fft_x_kernel(double *__restrict__ p, const double2 *__restrict__ twx, int M, long long nlines,
-                                                        int lpb, Radices rl, double scale)
+template <bool INV>
+__global__ void __launch_bounds__(kMaxT) gen_fft_x_kernel(double *__restrict__ p, const double2 *__restrict__ twx, int M, long long nlines, int lpb,
+                                                          Radices rl, double scale)
 {
     extern __shared__ double2 smem_gx[];
+    const int kT = (int)blockDim.x;
     const long long l0 = (long long)blockIdx.x * lpb;
     const int nl = (int)((nlines - l0 < lpb) ? nlines - l0 : lpb);
     double2 *g = reinterpret_cast<double2 *>(p) + (size_t)l0 * M;
-    for (int q = threadIdx.x; q < nl * M; q += kT) {
-        const int ln = q / M, k = q - ln * M;
-        double2 z = g[q];
-        if constexpr (INV) {
-            // merge of the complex-to-real transform, conjugated (inverse through the forward passes)
+    const Side glob{g, M, 1, 1.0, 1.0}, mid{smem_gx, M, 1, 1.0, 1.0};
+    if constexpr (INV) {
+        // merge of the complex-to-real transform, conjugated (inverse through the forward passes),
+        // staged through shared memory (formed on the way into the first pass it was slower: 3.7
+        // against 2.8 ms on 3456 x 3072 x 30)
+        for (int q = threadIdx.x; q < nl * M; q += kT) {
+            const int ln = q / M, k = q - ln * M;
+            double2 z = g[q];
             if (k == 0) {
                 z = make_double2(z.x + z.y, -(z.x - z.y));
             } else {
@@ -185,49 +279,41 @@ __global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_fft_x_kernel(double
                 const double2 sm = cadd(z, xm), c = cmul_conj(csub(z, xm), __ldg(&twx[k]));
                 z = make_double2(sm.x - c.y, -(sm.y + c.x));
             }
+            smem_gx[q] = z;
         }
-        smem_gx[q] = z;
-    }
-    __syncthreads();
-    all_passes<kT>(smem_gx, M, nl, M, 1, twx, 2, rl);
-    for (int q = threadIdx.x; q < nl * M; q += kT) {
-        const int ln = q / M, k = q - ln * M;
-        const double2 z = smem_gx[q];
-        double2 o;
-        if constexpr (INV) {
-            o = make_double2(z.x * scale, -z.y * scale);
-        } else if (k == 0) {
-            o = make_double2(z.x + z.y, z.x - z.y); // Re X_0, Re X_{n/2}
-        } else {
-            // split: X_k = (Z_k + conj Z_{M-k}) / 2 - (i/2) w_n^k (Z_k - conj Z_{M-k})
-            const double2 zm = cconj(smem_gx[ln * M + (M - k)]);
-            const double2 ev = make_double2(0.5 * (z.x + zm.x), 0.5 * (z.y + zm.y));
-            const double2 d = csub(z, zm);
-            o = cadd(ev, cmul(make_double2(0.5 * d.y, -0.5 * d.x), __ldg(&twx[k])));
+        __syncthreads();
+        // every global read of the lines precedes this barrier: the last pass stores in place
+        const Side dst{g, M, 1, scale, -scale};
+        all_passes(mid, mid, dst, M, nl, false, twx, 2, rl);
+    } else {
+        all_passes(glob, mid, mid, M, nl, false, twx, 2, rl);
+        for (int q = threadIdx.x; q < nl * M; q += kT) {
+            const int ln = q / M, k = q - ln * M;
+            const double2 z = smem_gx[q];
+            double2 o;
+            if (k == 0) {
+                o = make_double2(z.x + z.y, z.x - z.y); // Re X_0, Re X_{n/2}
+            } else {
+                // split: X_k = (Z_k + conj Z_{M-k}) / 2 - (i/2) w_n^k (Z_k - conj Z_{M-k})
+                const double2 zm = cconj(smem_gx[ln * M + (M - k)]);
+                const double2 ev = make_double2(0.5 * (z.x + zm.x), 0.5 * (z.y + zm.y));
+                const double2 d = csub(z, zm);
+                o = cadd(ev, cmul(make_double2(0.5 * d.y, -0.5 * d.x), __ldg(&twx[k])));
+            }
+            g[q] = o;
         }
-        g[q] = o;
     }
 }
 
 // y columns: TC neighbouring packed pairs x all ny rows of one plane per CTA.  twy[k] = exp(-2 pi i k / ny).
-template <bool INV, int kT>
-__global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_fft_y_kernel(double *__restrict__ p, const double2 *__restrict__ twy, int nx, int ny, int tc,
-                                                        Radices rl)
+// The first pass reads the rows from global memory, the last one stores them.
+template <bool INV>
+__global__ void __launch_bounds__(kMaxT) gen_fft_y_kernel(double *__restrict__ p, const double2 *__restrict__ twy, int nx, int ny, int tc, Radices rl)
 {
     extern __shared__ double2 smem_gy[];
-    double *base = p + (size_t)blockIdx.y * nx * ny + 2 * (size_t)blockIdx.x * tc;
-    for (int q = threadIdx.x; q < ny * tc; q += kT) {
-        const int row = q / tc, c = q - row * tc;
-        const double2 t = *reinterpret_cast<const double2 *>(base + (size_t)row * nx + 2 * c);
-        smem_gy[q] = INV ? cconj(t) : t;
-    }
-    __syncthreads();
-    all_passes<kT>(smem_gy, ny, tc, 1, tc, twy, 1, rl);
-    for (int q = threadIdx.x; q < ny * tc; q += kT) {
-        const int row = q / tc, c = q - row * tc;
-        const double2 t = smem_gy[q];
-        *reinterpret_cast<double2 *>(base + (size_t)row * nx + 2 * c) = INV ? cconj(t) : t;
-    }
+    double2 *gb = reinterpret_cast<double2 *>(p + (size_t)blockIdx.y * nx * ny) + (size_t)blockIdx.x * tc;
+    const Side src{gb, 1, nx / 2, 1.0, INV ? -1.0 : 1.0}, dst{gb, 1, nx / 2, 1.0, INV ? -1.0 : 1.0}, mid{smem_gy, 1, tc, 1.0, 1.0};
+    all_passes(src, mid, dst, ny, tc, true, twy, 1, rl);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -241,11 +327,13 @@ __global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_fft_y_kernel(double
 // tw4[k] = exp(-i pi k / (2L)).
 __device__ __forceinline__ double2 mul_i(double2 a) { return make_double2(-a.y, a.x); }
 
-template <bool INV, int kT>
-__global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_r2r_y_kernel(double *__restrict__ p, const double2 *__restrict__ twy, const double2 *__restrict__ tw4,
-                                                        int nx, int L, int tc, Radices rl, int dirichlet)
+template <bool INV>
+__global__ void __launch_bounds__(kMaxT) gen_r2r_y_kernel(double *__restrict__ p, const double2 *__restrict__ twy, const double2 *__restrict__ tw4, int nx, int L,
+                                                          int tc, Radices rl, int dirichlet)
 {
     extern __shared__ double2 smem_ry[];
+    const int kT = (int)blockDim.x;
+    const Side mid{smem_ry, 1, tc, 1.0, 1.0};
     double *base = p + (size_t)blockIdx.y * nx * L + 2 * (size_t)blockIdx.x * tc;
     auto at = [&](int row, int c) { return reinterpret_cast<double2 *>(base + (size_t)row * nx + 2 * c); };
     if constexpr (!INV) {
@@ -257,7 +345,7 @@ __global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_r2r_y_kernel(double
             smem_ry[pos * tc + c] = t;
         }
         __syncthreads();
-        all_passes<kT>(smem_ry, L, tc, 1, tc, twy, 1, rl);
+        all_passes(mid, mid, mid, L, tc, true, twy, 1, rl);
         for (int q = threadIdx.x; q < (L / 2 + 1) * tc; q += kT) {
             const int k = q / tc, c = q - k * tc;
             const double2 vk = smem_ry[k * tc + c];
@@ -306,7 +394,7 @@ __global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_r2r_y_kernel(double
             }
         }
         __syncthreads();
-        all_passes<kT>(smem_ry, L, tc, 1, tc, twy, 1, rl);
+        all_passes(mid, mid, mid, L, tc, true, twy, 1, rl);
         for (int q = threadIdx.x; q < L * tc; q += kT) {
             const int row = q / tc, c = q - row * tc;
             const int pos = (row & 1) ? L - 1 - (row >> 1) : (row >> 1);
@@ -322,11 +410,13 @@ __global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_r2r_y_kernel(double
 //   C_k = Re(w_k V_k),  C_{n-k} = -Im(w_k V_k)   (0 < k < M),  C_0 = V_0,  C_M = Re(w_M V_M);
 // inverse: V_k = conj(w_k) (C_k - i C_{n-k}), complex-to-real merge, passes, un-reordering.
 // Output / input: n real coefficients per line in natural order (sine: reversed, see above).
-template <bool INV, int kT>
-__global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_r2r_x_kernel(double *__restrict__ p, const double2 *__restrict__ twx, const double2 *__restrict__ tw4,
-                                                        int M, long long nlines, int lpb, Radices rl, double scale, int dirichlet)
+template <bool INV>
+__global__ void __launch_bounds__(kMaxT) gen_r2r_x_kernel(double *__restrict__ p, const double2 *__restrict__ twx, const double2 *__restrict__ tw4, int M,
+                                                          long long nlines, int lpb, Radices rl, double scale, int dirichlet)
 {
     extern __shared__ double2 smem_rx[];
+    const int kT = (int)blockDim.x;
+    const Side mid{smem_rx, M, 1, 1.0, 1.0};
     double *sd = reinterpret_cast<double *>(smem_rx);
     const int n = 2 * M;
     const long long l0 = (long long)blockIdx.x * lpb;
@@ -340,7 +430,7 @@ __global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_r2r_x_kernel(double
             sd[ln * n + ((i & 1) ? n - 1 - (i >> 1) : (i >> 1))] = v;
         }
         __syncthreads();
-        all_passes<kT>(smem_rx, M, nl, M, 1, twx, 2, rl);
+        all_passes(mid, mid, mid, M, nl, false, twx, 2, rl);
         for (int q = threadIdx.x; q < nl * (M + 1); q += kT) {
             const int ln = q / (M + 1), k = q - ln * (M + 1);
             const double2 *z = smem_rx + (size_t)ln * M;
@@ -395,7 +485,7 @@ __global__ void __launch_bounds__(kT, kT == 256 ? 2 : 1) gen_r2r_x_kernel(double
             if (q < nl * M) smem_rx[q] = zr[e];
         }
         __syncthreads();
-        all_passes<kT>(smem_rx, M, nl, M, 1, twx, 2, rl);
+        all_passes(mid, mid, mid, M, nl, false, twx, 2, rl);
         for (int q = threadIdx.x; q < nl * n; q += kT) {
             const int ln = q / n, i = q - ln * n;
             const int pos = (i & 1) ? n - 1 - (i >> 1) : (i >> 1);
@@ -438,17 +528,87 @@ __global__ void __launch_bounds__(256) gen_allpairs_kernel(double *__restrict__ 
     }
 }
 
-bool factor(int n, Radices *out)
+// Factorisation by a small cost model (shared-memory wavefronts per 32 points): 10 per pass (4 + 4
+// for the reads and writes, 2 for the barriers) plus 4 per extra way of bank conflict of the FIRST
+// pass, which writes with a stride of R elements (free of conflicts for odd R; later passes write
+// runs of Ns consecutive elements).  Ties go to the most points per thread.  need_cap: a line (or
+// tile) too long for 512 threads rules out the radices that keep fewer points per thread.
+constexpr int kRadix[] = {16, 15, 14, 12, 10, 9, 8, 7, 6, 5, 4, 3, 2};
+int points_per_thread(int R) { const int c = bfly_per_thread(R) * R; return c < kE ? c : kE; }
+
+// bank-conflict ways of the first pass: 8 lanes of a quarter warp store 16-byte elements at
+// (j R) sp + c, c < sp the line, j the butterfly
+int first_pass_ways(int R, int sp)
+{
+    const int per = sp < 8 ? sp : 8;
+    int hits[8] = {0}, ways = 1;
+    for (int l = 0; l < 8; ++l) {
+        const int c = l % per, j = l / per, unit = (j * R * sp + c) & 7;
+        if (++hits[unit] > ways) ways = hits[unit];
+    }
+    return ways;
+}
+
+struct Search { int n, r[20], cost, cap, need_cap, sp; };
+void search(int n, int start, int depth, int *cur, Search *best)
+{
+    if (n == 1) {
+        int cap = kE, ways = 8;
+        for (int i = 0; i < depth; ++i) {
+            if (points_per_thread(cur[i]) < cap) cap = points_per_thread(cur[i]);
+            if (first_pass_ways(cur[i], best->sp) < ways) ways = first_pass_ways(cur[i], best->sp);
+        }
+        const int cost = 10 * depth + 2 * (ways - 1);
+        if (cost < best->cost || (cost == best->cost && cap > best->cap)) {
+            best->n = depth;
+            best->cost = cost;
+            best->cap = cap;
+            for (int i = 0; i < depth; ++i) best->r[i] = cur[i];
+        }
+        return;
+    }
+    if (10 * (depth + 1) > best->cost || depth >= 19) return;
+    for (int i = start; i < (int)(sizeof(kRadix) / sizeof(kRadix[0])); ++i)
+        if (n % kRadix[i] == 0 && points_per_thread(kRadix[i]) >= best->need_cap) {
+            cur[depth] = kRadix[i];
+            search(n / kRadix[i], i, depth + 1, cur, best);
+        }
+}
+
+bool factor(int n, Radices *out, int need_cap = 1, int sp = 1)
 {
     out->n = 0;
-    // odd radices first: their strided writes of the first pass are free of bank conflicts
-    for (int f : {7, 5, 3})
-        while (n % f == 0) { out->r[out->n++] = f; n /= f; }
-    while (n % 16 == 0) { out->r[out->n++] = 16; n /= 16; }
-    while (n % 8 == 0) { out->r[out->n++] = 8; n /= 8; }
-    if (n % 4 == 0) { out->r[out->n++] = 4; n /= 4; }
-    if (n % 2 == 0) { out->r[out->n++] = 2; n /= 2; }
-    return n == 1 && out->n <= 20;
+    if (n < 2 || need_cap > kE) return false;
+    Search best;
+    best.n = 0;
+    best.cost = 1 << 30;
+    best.cap = 0;
+    best.need_cap = need_cap;
+    best.sp = sp;
+    int cur[20];
+    search(n, 0, 0, cur, &best);
+    if (best.n == 0) return false;
+    // radices come out in descending order; the one with the fewest conflicts goes first
+    int first = 0;
+    for (int i = 1; i < best.n; ++i)
+        if (first_pass_ways(best.r[i], sp) < first_pass_ways(best.r[first], sp)) first = i;
+    const int f = best.r[first];
+    for (int i = first; i > 0; --i) best.r[i] = best.r[i - 1];
+    best.r[0] = f;
+    out->n = best.n;
+    for (int i = 0; i < best.n; ++i) out->r[i] = best.r[i];
+    return true;
+}
+
+// threads a CTA needs for `pts` points: every pass must fit (one or a few butterflies per thread)
+int threads_for(const Radices &rl, int pts)
+{
+    int t = (pts + kE - 1) / kE;
+    for (int i = 0; i < rl.n; ++i) {
+        const int R = rl.r[i], need = (pts / R + bfly_per_thread(R) - 1) / bfly_per_thread(R);
+        if (need > t) t = need;
+    }
+    return (t + 31) / 32 * 32;
 }
 
 } // namespace
@@ -458,62 +618,110 @@ bool factor(int n, Radices *out)
 bool generic_fft_x_ok(int nx)
 {
     Radices r;
-    return nx >= 8 && !(nx & 1) && nx / 2 <= kPts && factor(nx / 2, &r);
+    const int M = nx / 2;
+    return nx >= 8 && !(nx & 1) && M <= kPts && factor(M, &r, (M + kMaxT - 1) / kMaxT, 1) && threads_for(r, M) <= kMaxT;
 }
 bool generic_fft_y_ok(int ny)
 {
     Radices r;
-    return ny >= 8 && !(ny & 1) && ny <= kPts && factor(ny, &r);
+    return ny >= 8 && !(ny & 1) && ny <= kPts && factor(ny, &r, (ny + kMaxT - 1) / kMaxT, 1) && threads_for(r, ny) <= kMaxT;
 }
 
-// launch geometry of the x kernels: lines per CTA and threads per CTA
-static void x_geometry(const pz_plan *pl, int M, long long nlines, int *lpb, int *kt)
+// launch geometry of the x kernels: lines per CTA and threads per CTA, chosen for the most points
+// in flight per SM (128 registers per thread: 512 threads per SM)
+static int x_geometry(const pz_plan *pl, const Radices &rl, int M, long long nlines, int *lpb, int *kt)
 {
-    *kt = (M <= 256 * kE) ? 256 : 512;
-    int l = (*kt * kE) / M;
-    if (l > 64) l = 64;
+    int best = 0, bl = 0;
+    for (int l = 1; l <= 64 && l * M <= kPts; ++l) {
+        const int pts = l * M, t = threads_for(rl, pts);
+        if (t > kMaxT) continue;
+        int ctas = kMaxT / t;
+        const int by_smem = (227 * 1024) / (pts * (int)sizeof(double2) + 1024);
+        if (by_smem < ctas) ctas = by_smem;
+        if (ctas > 16) ctas = 16;
+        // a lone CTA per SM cannot overlap its loads with another's passes
+        const int value = ctas >= 2 ? ctas * pts : (ctas * pts * 5) / 8;
+        if (value > best) { best = value; bl = l; }
+    }
+    if (!bl) { set_error("fft_x: nx = %d does not fit the %d-point buffer", 2 * M, kPts); return PZ_EUNSUPPORTED; }
     // keep the grid a few waves deep on small fields
-    while (l > 1 && (nlines + l - 1) / l < 4LL * pl->num_sms) l /= 2;
-    *lpb = l;
-}
-
-// pairs per CTA and threads per CTA of the y kernels: rows as wide as the buffer allows (<= 128 bytes)
-static int y_geometry(const pz_plan *pl, int L, int *tc, int *kt)
-{
-    const int npairs = pl->nx / 2;
-    int t = 8;
-    while (t > 1 && (npairs % t != 0 || t * L > kPts)) t /= 2;
-    if (t * L > kPts) { set_error("fft_y: ny = %d exceeds the %d-point buffer", L, kPts); return PZ_EUNSUPPORTED; }
-    *tc = t;
-    *kt = (t * L <= 256 * kE) ? 256 : 512;
+    while (bl > 1 && (nlines + bl - 1) / bl < 4LL * pl->num_sms) bl /= 2;
+    *lpb = bl;
+    *kt = threads_for(rl, bl * M);
     return PZ_OK;
 }
 
-#define PZ_GEN_LAUNCH(KERNEL, GRID, SMEM, ...)                                                                    \
-    do {                                                                                                           \
-        int rc_;                                                                                                   \
-        if (kt == 256) {                                                                                           \
-            if ((rc_ = smem_optin(pl, KERNEL<false, 256>, (size_t)256 * kE * sizeof(double2))) != PZ_OK) return rc_; \
-            if ((rc_ = smem_optin(pl, KERNEL<true, 256>, (size_t)256 * kE * sizeof(double2))) != PZ_OK) return rc_;  \
-            if (inverse) KERNEL<true, 256><<<GRID, 256, SMEM, st>>>(__VA_ARGS__);                                  \
-            else KERNEL<false, 256><<<GRID, 256, SMEM, st>>>(__VA_ARGS__);                                         \
-        } else {                                                                                                   \
-            if ((rc_ = smem_optin(pl, KERNEL<false, 512>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc_;   \
-            if ((rc_ = smem_optin(pl, KERNEL<true, 512>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc_;    \
-            if (inverse) KERNEL<true, 512><<<GRID, 512, SMEM, st>>>(__VA_ARGS__);                                  \
-            else KERNEL<false, 512><<<GRID, 512, SMEM, st>>>(__VA_ARGS__);                                         \
-        }                                                                                                          \
-        count_launch();                                                                                            \
-        PZ_CUDA(cudaGetLastError());                                                                               \
+#define PZ_GEN_LAUNCH(KERNEL, GRID, SMEM, ...)                                                                 \
+    do {                                                                                                        \
+        int rc_;                                                                                                \
+        if ((rc_ = smem_optin(pl, KERNEL<false>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc_;         \
+        if ((rc_ = smem_optin(pl, KERNEL<true>, (size_t)kPts * sizeof(double2))) != PZ_OK) return rc_;          \
+        if (inverse) KERNEL<true><<<GRID, kt, SMEM, st>>>(__VA_ARGS__);                                         \
+        else KERNEL<false><<<GRID, kt, SMEM, st>>>(__VA_ARGS__);                                                \
+        count_launch();                                                                                         \
+        PZ_CUDA(cudaGetLastError());                                                                            \
     } while (0)
+
+// radices + geometry of the x kernels (slot 0: Fourier, 2: cosine / sine), cached in the plan
+static int x_setup(const pz_plan *pl, int slot, long long nlines, Radices *rl, int *lpb, int *kt)
+{
+    pz_plan::GenGeo &g = const_cast<pz_plan *>(pl)->gen_geo[slot];
+    if (g.key != nlines) {
+        const int M = pl->nx / 2;
+        Radices r;
+        if (!factor(M, &r, (M + kMaxT - 1) / kMaxT, 1)) {
+            set_error("fft_x: nx / 2 = %d is not a product of 2, 3, 5, 7 that fits one CTA", M);
+            return PZ_EUNSUPPORTED;
+        }
+        int l, t;
+        const int rc = x_geometry(pl, r, M, nlines, &l, &t);
+        if (rc != PZ_OK) return rc;
+        g.n = r.n;
+        for (int i = 0; i < r.n; ++i) g.r[i] = r.r[i];
+        g.per_cta = l;
+        g.threads = t;
+        g.key = nlines;
+    }
+    rl->n = g.n;
+    for (int i = 0; i < g.n; ++i) rl->r[i] = g.r[i];
+    *lpb = g.per_cta;
+    *kt = g.threads;
+    return PZ_OK;
+}
+
+// radices + geometry of the y kernels (slot 1: Fourier, 3: cosine / sine): the widest rows (pairs
+// per CTA) for which a factorisation fits 512 threads
+static int y_setup(const pz_plan *pl, int slot, Radices *rl, int *tc, int *kt)
+{
+    pz_plan::GenGeo &g = const_cast<pz_plan *>(pl)->gen_geo[slot];
+    if (g.key != 0) {
+        const int L = pl->ny, npairs = pl->nx / 2;
+        Radices r;
+        int t = 8;
+        for (;; t /= 2) {
+            if (t == 0) { set_error("fft_y: ny = %d is not a product of 2, 3, 5, 7 that fits one CTA", L); return PZ_EUNSUPPORTED; }
+            if (npairs % t != 0 || t * L > kPts) continue;
+            if (factor(L, &r, (t * L + kMaxT - 1) / kMaxT, t) && threads_for(r, t * L) <= kMaxT) break;
+        }
+        g.n = r.n;
+        for (int i = 0; i < r.n; ++i) g.r[i] = r.r[i];
+        g.per_cta = t;
+        g.threads = threads_for(r, t * L);
+        g.key = 0;
+    }
+    rl->n = g.n;
+    for (int i = 0; i < g.n; ++i) rl->r[i] = g.r[i];
+    *tc = g.per_cta;
+    *kt = g.threads;
+    return PZ_OK;
+}
 
 int launch_fft_x_generic(const pz_plan *pl, double *p, long long nlines, bool inverse, cudaStream_t st)
 {
     const int M = pl->nx / 2;
     Radices rl;
-    if (!factor(M, &rl)) { set_error("fft_x: nx / 2 = %d has a prime factor above 7", M); return PZ_EUNSUPPORTED; }
-    int lpb, kt;
-    x_geometry(pl, M, nlines, &lpb, &kt);
+    int lpb, kt, rc;
+    if ((rc = x_setup(pl, 0, nlines, &rl, &lpb, &kt)) != PZ_OK) return rc;
     const size_t smem = (size_t)lpb * M * sizeof(double2);
     const unsigned blocks = (unsigned)((nlines + lpb - 1) / lpb);
     const double scale = 1.0 / ((double)pl->nx * (double)pl->ny);
@@ -526,10 +734,8 @@ int launch_fft_y_generic(const pz_plan *pl, double *p, int nk, bool inverse, cud
 {
     const int L = pl->ny;
     Radices rl;
-    if (!factor(L, &rl)) { set_error("fft_y: ny = %d has a prime factor above 7", L); return PZ_EUNSUPPORTED; }
-    int tc, kt;
-    const int rc = y_geometry(pl, L, &tc, &kt);
-    if (rc != PZ_OK) return rc;
+    int tc, kt, rc;
+    if ((rc = y_setup(pl, 1, &rl, &tc, &kt)) != PZ_OK) return rc;
     const size_t smem = (size_t)tc * L * sizeof(double2);
     dim3 grid((unsigned)(pl->nx / 2 / tc), (unsigned)nk);
     ProfScope prof(pl, inverse ? PZ_K_FFT_Y_INV : PZ_K_FFT_Y_FWD, st);
@@ -542,9 +748,8 @@ int launch_r2r_x(const pz_plan *pl, double *p, long long nlines, bool inverse, c
 {
     const int M = pl->nx / 2;
     Radices rl;
-    if (!factor(M, &rl)) { set_error("r2r_x: nx / 2 = %d has a prime factor above 7", M); return PZ_EUNSUPPORTED; }
-    int lpb, kt;
-    x_geometry(pl, M, nlines, &lpb, &kt);
+    int lpb, kt, rc;
+    if ((rc = x_setup(pl, 2, nlines, &rl, &lpb, &kt)) != PZ_OK) return rc;
     const size_t smem = (size_t)lpb * M * sizeof(double2);
     const unsigned blocks = (unsigned)((nlines + lpb - 1) / lpb);
     const double scale = 1.0 / ((double)pl->nx * (double)pl->ny);
@@ -558,10 +763,8 @@ int launch_r2r_y(const pz_plan *pl, double *p, int nk, bool inverse, cudaStream_
 {
     const int L = pl->ny;
     Radices rl;
-    if (!factor(L, &rl)) { set_error("r2r_y: ny = %d has a prime factor above 7", L); return PZ_EUNSUPPORTED; }
-    int tc, kt;
-    const int rc = y_geometry(pl, L, &tc, &kt);
-    if (rc != PZ_OK) return rc;
+    int tc, kt, rc;
+    if ((rc = y_setup(pl, 3, &rl, &tc, &kt)) != PZ_OK) return rc;
     const size_t smem = (size_t)tc * L * sizeof(double2);
     const int dir = (pl->bcy == PZ_DIRICHLET) ? 1 : 0;
     dim3 grid((unsigned)(pl->nx / 2 / tc), (unsigned)nk);

@@ -123,6 +123,11 @@ struct pz_plan {
     bool slab_internal = false;      // the cut is the plan's own (one GPU, nz > 1024): poisson_solve runs all slabs
     double *islab_ball = nullptr;    // internal cut: the boundary buffers of all slabs
 
+    // mixed-radix transforms (pz_fft_generic.cu): radices and launch geometry, worked out once per
+    // (kernel family, number of lines); [x, y, cosine / sine x, cosine / sine y]
+    struct GenGeo { long long key = -1; int n = 0, r[20] = {0}, per_cta = 0, threads = 0; };
+    GenGeo gen_geo[4];
+
     // z-solve variant 2: launch geometry per (sub-domain rows M, HELM), queried once per plan (= per device)
     struct ZtGeo { int blocks = 0, stages = 0; };
     ZtGeo zt[4][4];   // [M][whole columns, HELM, slab reduce, slab finish]

@@ -15,6 +15,7 @@
 // operations along the third domain direction"), forward result and C_k/p_k staged in HBM.
 // Variant 1 (pz_zsolve_cr.cu): chunked cyclic reduction in shared memory (Algorithm 1).
 #include "pz_internal.h"
+#include "pz_zsolve_pair.cuh"
 
 namespace pz {
 
@@ -82,51 +83,73 @@ __global__ void __launch_bounds__(128)
     }
 }
 
-// Variant 4 (nz <= 32, e.g. the 30 planes per GPU of the paper's weak-scaling grid):
+// Variant 4 (nz <= 64, e.g. the 30 planes per GPU of the paper's weak-scaling grid):
 // one thread per column, the whole column in registers -- one coalesced read and one write per
 // point, the same pivot recurrence as above.  Rows past nz are identity rows.
-constexpr int kSmallNz = 32;
 
-__global__ void __launch_bounds__(128)
+template <int kCap>   // rows held per thread: nz rounded up to 8, 16, 24, 32, 48 or 64
+__global__ void __launch_bounds__(128, (kCap > 32) ? 3 : (kCap > 16) ? 4 : 6)
     zsolve_small_kernel(double *__restrict__ p, const double *__restrict__ A, const double *__restrict__ C,
                         const double *__restrict__ dzf, const double *__restrict__ lamx, const double *__restrict__ lamy_nat,
                         const double *__restrict__ lamy_pk, int nx, int ny, int nz, double inv_lz, double pw0, double pw1,
                         int zflags)
 {
+    // The column goes through shared memory ([row][thread]: conflict-free) by asynchronous copies:
+    // all its loads are in flight at once and hold no registers (ncu r02: with plain loads ptxas
+    // scheduled one load per step of the recurrence and every step waited a DRAM latency), several
+    // CTAs per SM are in different phases, so loads, recurrence and stores overlap.
+    extern __shared__ double smem_small[];
+    double (*sg)[128] = reinterpret_cast<double (*)[128]>(smem_small);
+    double *sA = smem_small + kCap * 128, *sC = sA + kCap, *sD = sC + kCap;
     const size_t plane = (size_t)nx * ny;
-    const size_t col = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (col >= plane) return;
+    const size_t col0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = col0 < plane;
+    const size_t col = active ? col0 : 0;
+#pragma unroll
+    for (int k = 0; k < kCap; ++k) {
+        if (k < nz) {
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(&sg[k][threadIdx.x]);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(p + (size_t)k * plane + col) : "memory");
+        }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    if (threadIdx.x < kCap) {
+        const int k = threadIdx.x;
+        sA[k] = (k < nz && k > 0) ? A[k] : 0.0;
+        sC[k] = (k < nz) ? C[k] : 0.0;
+        sD[k] = (k < nz) ? dzf[k] : 0.0;
+    }
     const int i = (int)(col % nx), j = (int)(col / nx);
     const double sigma = -(lamx[i] + (i < 2 ? lamy_pk[j] : lamy_nat[j]));
     const bool singular = (i == 0 && j == 0) && (zflags & 2);
-    double g[kSmallNz], cw[kSmallNz];
-#pragma unroll
-    for (int k = 0; k < kSmallNz; ++k) g[k] = (k < nz) ? p[(size_t)k * plane + col] : 0.0;
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();   // sA, sC, sD
+    double cw[kCap];
     double e = 0.0, rp = 0.0, gp = 0.0;
 #pragma unroll
-    for (int k = 0; k < kSmallNz; ++k) {
+    for (int k = 0; k < kCap; ++k) {
         const bool live = k < nz;
-        const double a = (live && k > 0) ? A[k] : 0.0, c = live ? C[k] : 0.0;
+        const double a = sA[k], c = sC[k];
         e = fma(a * e, rp, sigma) + (k == 0 ? pw0 : 0.0) + (k == nz - 1 ? pw1 : 0.0);
         const bool gauge = singular && k == nz - 1;   // last equation of the singular column replaced by phi = 0
         const double pk = (live && !gauge) ? c + e : 1.0;
-        rp = 1.0 / pk;
-        gp = (live && !gauge) ? fma(a, gp, -g[k]) * rp : 0.0;
+        rp = fast_rcp(pk);
+        gp = (live && !gauge) ? fma(a, gp, -sg[k][threadIdx.x]) * rp : 0.0;
         if (!live || gauge) rp = 0.0;
-        g[k] = gp;
+        sg[k][threadIdx.x] = gp;
         cw[k] = c * rp;
     }
     double x = 0.0, s = 0.0;
 #pragma unroll
-    for (int k = kSmallNz - 1; k >= 0; --k) {
-        x = fma(cw[k], x, g[k]);
-        g[k] = x;
-        if (k < nz) s = fma(dzf[k], x, s);
+    for (int k = kCap - 1; k >= 0; --k) {
+        x = fma(cw[k], x, sg[k][threadIdx.x]);
+        sg[k][threadIdx.x] = x;
+        s = fma(sD[k], x, s);
     }
     const double shift = singular ? s * inv_lz : 0.0;
 #pragma unroll
-    for (int k = 0; k < kSmallNz; ++k)
-        if (k < nz) p[(size_t)k * plane + col] = g[k] - shift;
+    for (int k = 0; k < kCap; ++k)
+        if (k < nz && active) p[(size_t)k * plane + col] = sg[k][threadIdx.x] - shift;
 }
 
 } // namespace
@@ -136,9 +159,23 @@ int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
     if (pl->opt.zsolve_variant == 4 && helm_a < 0.0) {
         const size_t plane = (size_t)pl->nx * pl->ny;
         ProfScope prof(pl, PZ_K_Z_SOLVE, st);
-        zsolve_small_kernel<<<(unsigned)((plane + 127) / 128), 128, 0, st>>>(p, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx, pl->d_lamy_nat,
-                                                                             pl->d_lamy_pk, pl->nx, pl->ny, pl->nz, pl->inv_lz, pl->pw0,
-                                                                             pl->pw1, pl->zflags());
+        const unsigned blocks = (unsigned)((plane + 127) / 128);
+#define PZ_SMALL(CAP)                                                                                                       \
+    do {                                                                                                                    \
+        const size_t smem = (size_t)(CAP) * (128 + 3) * sizeof(double);                                                     \
+        const int rc = smem_optin(pl, zsolve_small_kernel<CAP>, smem);                                                      \
+        if (rc != PZ_OK) return rc;                                                                                         \
+        zsolve_small_kernel<CAP><<<blocks, 128, smem, st>>>(p, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx, pl->d_lamy_nat,      \
+                                                            pl->d_lamy_pk, pl->nx, pl->ny, pl->nz, pl->inv_lz, pl->pw0,     \
+                                                            pl->pw1, pl->zflags());                                         \
+    } while (0)
+        if (pl->nz <= 8) PZ_SMALL(8);
+        else if (pl->nz <= 16) PZ_SMALL(16);
+        else if (pl->nz <= 24) PZ_SMALL(24);
+        else if (pl->nz <= 32) PZ_SMALL(32);
+        else if (pl->nz <= 48) PZ_SMALL(48);
+        else PZ_SMALL(64);
+#undef PZ_SMALL
         count_launch();
         PZ_CUDA(cudaGetLastError());
         return PZ_OK;

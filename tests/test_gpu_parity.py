@@ -69,6 +69,7 @@ POISSON_SHAPES = [
     ("c1", 64, 128, 129),     # one row past a sub-domain multiple
     ("c3", 256, 64, 96),      # beta = 2.0, long x
     ("c3", 32, 256, 33),
+    ("c3", 160, 24, 57),      # thread-per-column range (nz <= 64), ragged last CTA
     ("c2", 64, 64, 128),      # few-mode right-hand side
     ("c1", 16, 16, 1024),     # one shared-memory stage (m = 32)
     ("c3", 32, 16, 700),      # ragged, m = 32
@@ -79,8 +80,8 @@ POISSON_SHAPES = [
 @pytest.mark.parametrize("base,nx,ny,nz", POISSON_SHAPES)
 @pytest.mark.parametrize("variant", [0, 1, 2, 4])
 def test_poisson_matches_oracle(torch, pz, wl, oracle, base, nx, ny, nz, variant):
-    if variant == 4 and nz > 32:
-        pytest.skip("variant 4 keeps the column in registers: nz <= 32")
+    if variant == 4 and nz > 64:
+        pytest.skip("variant 4 keeps the column on chip per thread: nz <= 64")
     w = wl.scaled(wl.CONFIGS[base], nx, ny, nz)
     zc, zf = wl.grid(w)
     f = wl.poisson_rhs(w)
