@@ -265,21 +265,25 @@ __global__ void __launch_bounds__(kMaxT) gen_fft_x_kernel(double *__restrict__ p
     const int nl = (int)((nlines - l0 < lpb) ? nlines - l0 : lpb);
     double2 *g = reinterpret_cast<double2 *>(p) + (size_t)l0 * M;
     const Side glob{g, M, 1, 1.0, 1.0}, mid{smem_gx, M, 1, 1.0, 1.0};
+    const int H = M / 2 + 1;   // spectral indices k and M - k are handled together, k = 0 .. M/2
     if constexpr (INV) {
-        // merge of the complex-to-real transform, conjugated (inverse through the forward passes),
-        // staged through shared memory (formed on the way into the first pass it was slower: 3.7
-        // against 2.8 ms on 3456 x 3072 x 30)
-        for (int q = threadIdx.x; q < nl * M; q += kT) {
-            const int ln = q / M, k = q - ln * M;
-            double2 z = g[q];
+        // merge of the complex-to-real transform, conjugated (inverse through the forward passes):
+        //   conj Z'_k = conj(s + i c),  s = X_k + conj X_{M-k},  c = conj(w_n^k) (X_k - conj X_{M-k}),
+        // and, with w_n^{M-k} = -conj(w_n^k), Z'_{M-k} = conj(s) + i conj(c): both from one pair of
+        // loads and one twiddle.  Staged through shared memory (formed on the way into the first
+        // pass it was slower: 3.7 against 2.8 ms on 3456 x 3072 x 30).
+#pragma unroll 4
+        for (int q = threadIdx.x; q < nl * H; q += kT) {
+            const int ln = q / H, k = q - ln * H;
+            const double2 xk = g[(size_t)ln * M + k];
             if (k == 0) {
-                z = make_double2(z.x + z.y, -(z.x - z.y));
+                smem_gx[ln * M] = make_double2(xk.x + xk.y, -(xk.x - xk.y));
             } else {
                 const double2 xm = cconj(g[(size_t)ln * M + (M - k)]);
-                const double2 sm = cadd(z, xm), c = cmul_conj(csub(z, xm), __ldg(&twx[k]));
-                z = make_double2(sm.x - c.y, -(sm.y + c.x));
+                const double2 sm = cadd(xk, xm), c = cmul_conj(csub(xk, xm), __ldg(&twx[k]));
+                smem_gx[ln * M + k] = make_double2(sm.x - c.y, -(sm.y + c.x));
+                if (2 * k != M) smem_gx[ln * M + (M - k)] = make_double2(sm.x + c.y, sm.y - c.x);
             }
-            smem_gx[q] = z;
         }
         __syncthreads();
         // every global read of the lines precedes this barrier: the last pass stores in place
@@ -287,20 +291,21 @@ __global__ void __launch_bounds__(kMaxT) gen_fft_x_kernel(double *__restrict__ p
         all_passes(mid, mid, dst, M, nl, false, twx, 2, rl);
     } else {
         all_passes(glob, mid, mid, M, nl, false, twx, 2, rl);
-        for (int q = threadIdx.x; q < nl * M; q += kT) {
-            const int ln = q / M, k = q - ln * M;
-            const double2 z = smem_gx[q];
-            double2 o;
+        // split: X_k = e + t, X_{M-k} = conj(e - t),  e = (Z_k + conj Z_{M-k}) / 2,
+        //        t = -(i/2) w_n^k (Z_k - conj Z_{M-k})
+        for (int q = threadIdx.x; q < nl * H; q += kT) {
+            const int ln = q / H, k = q - ln * H;
+            const double2 z = smem_gx[ln * M + k];
             if (k == 0) {
-                o = make_double2(z.x + z.y, z.x - z.y); // Re X_0, Re X_{n/2}
+                g[(size_t)ln * M] = make_double2(z.x + z.y, z.x - z.y); // Re X_0, Re X_{n/2}
             } else {
-                // split: X_k = (Z_k + conj Z_{M-k}) / 2 - (i/2) w_n^k (Z_k - conj Z_{M-k})
                 const double2 zm = cconj(smem_gx[ln * M + (M - k)]);
                 const double2 ev = make_double2(0.5 * (z.x + zm.x), 0.5 * (z.y + zm.y));
                 const double2 d = csub(z, zm);
-                o = cadd(ev, cmul(make_double2(0.5 * d.y, -0.5 * d.x), __ldg(&twx[k])));
+                const double2 t = cmul(make_double2(0.5 * d.y, -0.5 * d.x), __ldg(&twx[k]));
+                g[(size_t)ln * M + k] = cadd(ev, t);
+                if (2 * k != M) g[(size_t)ln * M + (M - k)] = make_double2(ev.x - t.x, -(ev.y - t.y));
             }
-            g[q] = o;
         }
     }
 }
