@@ -507,7 +507,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c2", help="c1, c2 (default), c3 or c4 of BASELINE.json")
+    ap.add_argument("--workload", default="c2",
+                    help="c1, c2 (default), c3 or c4 of BASELINE.json; 'paper' = only the 3456x3072x30 sub-record (for profiling)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -523,6 +524,14 @@ def main():
 
     from paper_2502_06296_b200 import workloads as wl
 
+    if args.workload == "paper":   # the mixed-radix sub-record on its own: one JSON object, not the bench line
+        import torch
+
+        from paper_2502_06296_b200 import binding as pz
+
+        pz.lib()
+        print(json.dumps(sub_paper_shape(torch, pz, wl, measured_peak()[0], 0)))
+        return
     w = wl.CONFIGS[args.workload]
     if args.impl == "reference":
         return bench_reference(args, w)

@@ -272,17 +272,32 @@ __global__ void __launch_bounds__(kMaxT) gen_fft_x_kernel(double *__restrict__ p
         // and, with w_n^{M-k} = -conj(w_n^k), Z'_{M-k} = conj(s) + i conj(c): both from one pair of
         // loads and one twiddle.  Staged through shared memory (formed on the way into the first
         // pass it was slower: 3.7 against 2.8 ms on 3456 x 3072 x 30).
-#pragma unroll 4
-        for (int q = threadIdx.x; q < nl * H; q += kT) {
-            const int ln = q / H, k = q - ln * H;
-            const double2 xk = g[(size_t)ln * M + k];
-            if (k == 0) {
-                smem_gx[ln * M] = make_double2(xk.x + xk.y, -(xk.x - xk.y));
-            } else {
-                const double2 xm = cconj(g[(size_t)ln * M + (M - k)]);
-                const double2 sm = cadd(xk, xm), c = cmul_conj(csub(xk, xm), __ldg(&twx[k]));
-                smem_gx[ln * M + k] = make_double2(sm.x - c.y, -(sm.y + c.x));
-                if (2 * k != M) smem_gx[ln * M + (M - k)] = make_double2(sm.x + c.y, sm.y - c.x);
+        // four items per trip, their loads issued together (one item per trip left every trip
+        // waiting on its own loads: ncu stall long_scoreboard 3.9 per issue)
+        for (int q0 = threadIdx.x; q0 < nl * H; q0 += 4 * kT) {
+            double2 xk[4], xp[4], w[4];
+            int pos[4], kk[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int q = q0 + u * kT, qq = (q < nl * H) ? q : 0;
+                const int ln = qq / H, k = qq - ln * H;
+                pos[u] = ln * M;
+                kk[u] = (q < nl * H) ? k : -1;
+                xk[u] = g[(size_t)ln * M + k];
+                xp[u] = g[(size_t)ln * M + (k ? M - k : 0)];
+                w[u] = __ldg(&twx[k]);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int k = kk[u];
+                if (k == 0) {
+                    smem_gx[pos[u]] = make_double2(xk[u].x + xk[u].y, -(xk[u].x - xk[u].y));
+                } else if (k > 0) {
+                    const double2 xm = cconj(xp[u]);
+                    const double2 sm = cadd(xk[u], xm), c = cmul_conj(csub(xk[u], xm), w[u]);
+                    smem_gx[pos[u] + k] = make_double2(sm.x - c.y, -(sm.y + c.x));
+                    if (2 * k != M) smem_gx[pos[u] + (M - k)] = make_double2(sm.x + c.y, sm.y - c.x);
+                }
             }
         }
         __syncthreads();
