@@ -296,6 +296,14 @@ enum pz_kernel_class {
 PZ_API int pz_profile_enable(pz_plan *plan, int on);
 PZ_API int pz_profile_read(pz_plan *plan, int kernel_class, double *total_ms, long long *launches);
 
+/* Host logic of the mixed-radix transforms (paper: "in-house mixed-radix FFT"; DESIGN.md
+ * section 14): the radices, first pass first, that the kernels use for a complex transform of length
+ * n whose lines are stored `stride` elements apart in shared memory (1: x lines, the pairs per CTA: y
+ * columns) when every thread must keep at least `min_points` points (1 = no constraint).  Writes at
+ * most `cap` entries to radices (host pointer) and returns their number, 0 if n has a prime factor
+ * above 7 or no factorisation meets min_points.  Needs no GPU. */
+PZ_API int pz_fft_radices(int n, int min_points, int stride, int *radices, int cap);
+
 /* Number of kernels this library has launched since it was loaded (host-side counter). */
 PZ_API long long pz_launch_count(void);
 

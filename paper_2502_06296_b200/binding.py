@@ -58,6 +58,7 @@ SIGNATURES = {
     "pz_profile_read": (_i, [_vp, _i, ctypes.POINTER(_d), ctypes.POINTER(ctypes.c_longlong)]),
     "pz_launch_count": (ctypes.c_longlong, []),
     "pz_version": (_i, []),
+    "pz_fft_radices": (_i, [_i, _i, _i, ctypes.POINTER(ctypes.c_int), _i]),
 }
 
 _lib = None
@@ -317,6 +318,13 @@ def pz_launch_count() -> int:
 
 def pz_version() -> int:
     return int(lib().pz_version())
+
+
+def pz_fft_radices(n: int, min_points: int = 1, stride: int = 1):
+    """Radices (first pass first) of the mixed-radix kernels for a complex length n; [] if unsupported."""
+    buf = (ctypes.c_int * 20)()
+    cnt = int(lib().pz_fft_radices(n, min_points, stride, buf, 20))
+    return [int(buf[i]) for i in range(cnt)]
 
 
 def pz_last_error() -> str:

@@ -198,6 +198,11 @@ extern "C" {
 const char *pz_last_error(void) { return g_err; }
 long long pz_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 int pz_version(void) { return 200; }
+int pz_fft_radices(int n, int min_points, int stride, int *radices, int cap)
+{
+    if (!radices || cap < 0) return 0;
+    return pz::fft_radices(n, min_points, stride, radices, cap);
+}
 
 static int slab_state_create(pz_plan *pl, int n_slabs, const int *kbounds, bool internal);
 

@@ -633,6 +633,14 @@ int threads_for(const Radices &rl, int pts)
 
 } // namespace
 
+int fft_radices(int n, int min_points, int stride, int *radices, int cap)
+{
+    Radices r;
+    if (!factor(n, &r, min_points < 1 ? 1 : min_points, stride < 1 ? 1 : stride)) return 0;
+    for (int i = 0; i < r.n && i < cap; ++i) radices[i] = r.r[i];
+    return r.n;
+}
+
 // lengths the mixed-radix kernels take: even, 7-smooth (nx / 2 resp. ny), a line within the
 // 8192-point shared-memory buffer
 bool generic_fft_x_ok(int nx)

@@ -194,6 +194,7 @@ int launch_divergence_rhs(pz_plan *pl, const double *u, const double *v, const d
 int launch_helmholtz_z_rhs(pz_plan *pl, double *u2, const double *uk, double a, cudaStream_t st);
 int launch_project(pz_plan *pl, double *u, double *v, double *w, double *p, const double *phi, double gdt, cudaStream_t st);
 // mixed-radix (2, 3, 5, 7) transforms for lengths the power-of-two kernels do not take (pz_fft_generic.cu)
+int fft_radices(int n, int min_points, int stride, int *radices, int cap);
 bool generic_fft_x_ok(int nx);
 bool generic_fft_y_ok(int ny);
 inline bool fast_fft_len(int n) { return n >= 8 && n <= 4096 && (n & (n - 1)) == 0; }
