@@ -8,7 +8,8 @@ options, fields resident in HBM, in-place solves).
 * c3 (2048x1024x512): Poisson; element by element against the oracle on the c3 recipe at
   2048x1024x128 (the transform kernels of c3: nx = 2048, ny = 1024) and at 64x64x512 with beta = 2.0
   (c3's z-solve template: 16 rows per sub-domain, no padding rows), and on the full grid when the
-  box has the host memory for the oracle's work arrays; beside them, at the full size, the
+  box has the host memory for the oracle's work arrays; at the full size on any box, element by
+  element on a few-mode right-hand side (one oracle tridiagonal solve per mode); beside them the
   oracle's operator applied to the GPU solution on the host (normwise backward error plus the
   zero weighted mean, readings R3, R11) and linearity, a property that holds at any size.
 * the paper's per-GPU weak-scaling grid 3456x3072x30 (bench sub-record): element by element at the
@@ -210,43 +211,60 @@ def test_c3_full_element_by_element_when_host_memory_allows(env):
     assert float(np.abs(got).max()) / scale <= TOL
 
 
-def test_paper_weak_scaling_grid_full_size_few_modes(env):
-    """The paper's per-GPU weak-scaling grid 3456 x 3072 x 30 (PAPER.md:280; bench sub-record
-    `paper_weak_shape`: mixed-radix transforms, thread-per-column z-solve) at FULL size, element by
-    element.  The right-hand side is a sum of a few horizontal eigenfunctions
-    cos(2 pi p i / nx + a) cos(2 pi q j / ny + b) times seeded z profiles, so the exact discrete
-    solution is the same sum with each profile replaced by ONE tridiagonal solve of the oracle
-    (orc_thomas_poisson with lambda_x(p) + lambda_y(q); the closed-form (0,0) column): the oracle
-    works column by column and the comparison covers every grid point."""
+def few_mode_check(env, w, modes, seed):
+    """Full-size element-by-element parity on a right-hand side that is a sum of a few horizontal
+    eigenfunctions cos(2 pi p i / nx + a) cos(2 pi q j / ny + b) times seeded z profiles: the exact
+    discrete solution is the same sum with each profile replaced by ONE tridiagonal solve of the
+    oracle (orc_thomas_poisson with lambda_x(p) + lambda_y(q); the closed-form (0,0) column), so the
+    oracle works column by column, the reference is assembled on the host plane by plane, and the
+    comparison covers every grid point."""
     torch, pz, wl, oracle = env
-    w = wl.scaled(wl.CONFIGS["c3"], 3456, 3072, 30, name="paper_weak_3456x3072x30")
     zc, zf = wl.grid(w)
     dzf, dzc, A, C = oracle.z_tables(zc, zf)
     lamx, lamy = oracle.modified_wavenumbers(w.nx, w.lx), oracle.modified_wavenumbers(w.ny, w.ly)
-    rng = np.random.default_rng(2502)
-    modes = [(0, 0), (1, 0), (0, 1), (3, 2), (w.nx // 2, 0), (0, w.ny // 2), (w.nx // 2, w.ny // 2), (577, 1001),
-             (1727, 1535), (864, 3), (5, 768), (1152, 1024)]
+    rng = np.random.default_rng(seed)
     i, j = np.arange(w.nx), np.arange(w.ny)
     cx = np.stack([np.cos(2 * np.pi * ((p * i) % w.nx) / w.nx + rng.uniform(0, 2 * np.pi) * (p % (w.nx // 2) != 0)) for p, _ in modes])
     cy = np.stack([np.cos(2 * np.pi * ((q * j) % w.ny) / w.ny + rng.uniform(0, 2 * np.pi) * (q % (w.ny // 2) != 0)) for _, q in modes])
     g = rng.standard_normal((len(modes), w.nz))
-    g[0] -= np.dot(dzf, g[0]) / dzf.sum()                  # solvability of the (0,0) mode (reading R3)
     cols = np.empty_like(g)
     for m, (p, q) in enumerate(modes):
         sigma = -(lamx[p] + lamy[q])
-        g[m] *= max(sigma, 1.0)                            # every mode contributes O(1) to the solution
-        cols[m] = oracle.zero_mode_column(dzf, dzc, g[m]) if (p, q) == (0, 0) else oracle.thomas_poisson(A, C, sigma, g[m])
+        if (p, q) == (0, 0):
+            g[m] -= np.dot(dzf, g[m]) / dzf.sum()          # solvability of the (0,0) mode (reading R3)
+            cols[m] = oracle.zero_mode_column(dzf, dzc, g[m])
+        else:
+            g[m] *= max(sigma, 1.0)                        # every mode contributes O(1) to the solution
+            cols[m] = oracle.thomas_poisson(A, C, sigma, g[m])
     f = torch.einsum("mk,mj,mi->kji", torch.from_numpy(g).cuda(), torch.from_numpy(cy).cuda(), torch.from_numpy(cx).cuda()).contiguous()
     plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
     pz.poisson_solve(plan, f)
     torch.cuda.synchronize()
-    got = f.cpu().numpy()
-    del f
-    ref = np.einsum("mk,mj,mi->kji", cols, cy, cx, optimize=True)
-    scale = np.abs(ref).max()
-    assert scale > 0.5
-    err = 0.0
+    err, scale = 0.0, 0.0
     for k in range(w.nz):
-        err = max(err, float(np.abs(got[k] - ref[k]).max()))
-    assert err <= TOL * scale
+        ref = np.einsum("m,mj,mi->ji", cols[:, k], cy, cx, optimize=True)
+        err = max(err, float(np.abs(f[k].cpu().numpy() - ref).max()))
+        scale = max(scale, float(np.abs(ref).max()))
     pz.poisson_plan_destroy(plan)
+    assert scale > 0.5
+    assert err <= TOL * scale
+
+
+def test_c3_full_size_few_modes(env):
+    """c3 (2048 x 1024 x 512) at FULL size, element by element, in the launch configuration bench.py
+    times; needs no field-sized oracle arrays, so it runs on any box."""
+    wl = env[2]
+    w = wl.CONFIGS["c3"]
+    modes = [(0, 0), (1, 0), (0, 1), (2, 3), (w.nx // 2, 0), (0, w.ny // 2), (w.nx // 2, w.ny // 2), (333, 77), (1023, 511),
+             (512, 1), (7, 256), (1500, 900)]
+    few_mode_check(env, w, modes, 2048)
+
+
+def test_paper_weak_scaling_grid_full_size_few_modes(env):
+    """The paper's per-GPU weak-scaling grid 3456 x 3072 x 30 (PAPER.md:280; bench sub-record
+    `paper_weak_shape`: mixed-radix transforms, thread-per-column z-solve) at FULL size."""
+    wl = env[2]
+    w = wl.scaled(wl.CONFIGS["c3"], 3456, 3072, 30, name="paper_weak_3456x3072x30")
+    modes = [(0, 0), (1, 0), (0, 1), (3, 2), (w.nx // 2, 0), (0, w.ny // 2), (w.nx // 2, w.ny // 2), (577, 1001),
+             (1727, 1535), (864, 3), (5, 768), (1152, 1024)]
+    few_mode_check(env, w, modes, 2502)
