@@ -93,16 +93,24 @@ def test_poisson_matches_oracle(torch, pz, wl, oracle, base, nx, ny, nz, variant
     assert abs(wm) <= 1e-13 * np.abs(got).max()
 
 
-@pytest.mark.parametrize("base,nx,ny,nz", [("c1", 16, 16, 1100), ("c3", 32, 16, 1594), ("c1", 16, 8, 2048), ("c1", 8, 8, 2500)])
-@pytest.mark.parametrize("variant", [3, 0])   # 3: the plan's own z cut through the pipeline (default); 0: thread-per-column sweep
-def test_poisson_beyond_1024_planes_matches_oracle(torch, pz, wl, oracle, base, nx, ny, nz, variant):
-    """Whole columns longer than the pipeline's tile (the paper's wall-normal size is 1594)."""
+LONG_COLUMNS = [("c1", 16, 16, 1100), ("c3", 32, 16, 1594), ("c1", 16, 8, 2048), ("c1", 8, 8, 2500), ("c3", 64, 32, 900), ("c1", 32, 16, 513),
+                ("c3", 16, 16, 1024), ("c1", 48, 32, 3000), ("c1", 16, 16, 4096), ("c1", 8, 8, 4500)]
+
+
+@pytest.mark.parametrize("base,nx,ny,nz", LONG_COLUMNS)
+# 3: the plan's own z cut through the pipeline (default above 1024 planes); 2: whole columns, one stage (default up to 1024);
+# 0: thread-per-column sweep
+@pytest.mark.parametrize("variant", [3, 2, 0])
+def test_poisson_beyond_512_planes_matches_oracle(torch, pz, wl, oracle, base, nx, ny, nz, variant):
+    """Columns longer than the pipeline's three-stage tile (the paper's wall-normal sizes are 900 and 1594)."""
+    if (variant == 2) != (nz <= 1024) and variant != 0:
+        pytest.skip("variant not defined for this nz")
     w = wl.scaled(wl.CONFIGS[base], nx, ny, nz)
     zc, zf = wl.grid(w)
     f = wl.poisson_rhs(w)
     ref = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)
     plan = pz.poisson_plan_create(nx, ny, nz, w.lx, w.ly, zc, zf)
-    assert pz.pz_get_option(plan, "zsolve_variant") == 3
+    assert pz.pz_get_option(plan, "zsolve_variant") == (2 if nz <= 1024 else 3)
     pz.pz_set_option(plan, "zsolve_variant", variant)
     p = torch.from_numpy(f).cuda()
     pz.poisson_solve(plan, p)
