@@ -250,6 +250,29 @@ PZ_API int helmholtz_z_solve_host(pz_plan *plan, double *u_host, void *stream);
  */
 PZ_API int pz_solve_host_batch(pz_plan *plan, double *p_host, double *const *u_host, int n_u, void *stream);
 
+/* Step a3 alone (the z tridiagonal solves of Eq. 12; steps 4-6 of PAPER.md:127-129)
+ * for callers that may not allocate: code under CUDA-graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc.  The thread-per-column sweep (z-solve variant 0) stages its
+ * multipliers C_k / p_k in a workspace of N doubles, which the ordinary path allocates on first use;
+ * here that workspace is a file-scope device array of the library of
+ *     PZ_NOALLOC_MAX_POINTS = 2^21 doubles (16 MiB),
+ * which every GPU that loads libpz_b200.so holds until the process exits.
+ *   plan    an ordinary plan (poisson_plan_create; not a z-slab plan), any boundary-condition code
+ *   p       device, N = nx ny nz doubles, the field AFTER the forward transforms (packed spectral
+ *           layout, as PZ_STAGE_Z_SOLVE of pz_poisson_stage takes it); solved in place
+ *   stream  cudaStream_t or NULL
+ * The call itself calls no cudaMalloc / cudaFree and no allocating library routine (the first call on
+ * a device looks the array's address up with cudaGetSymbolAddress).  The plan's device must be
+ * current.  PZ_EUNSUPPORTED if N > PZ_NOALLOC_MAX_POINTS (nothing is launched), PZ_EINVAL for NULL /
+ * misaligned pointers, a z-slab plan or another current device, PZ_ECUDA for CUDA errors.
+ * ALL calls, from every plan and stream of the process, share the one array: calls that overlap on
+ * the GPU race and give wrong results -- keep them on one stream or order them with events.  Nothing
+ * in the array needs to start at zero (every entry is written by the forward sweep before the
+ * backward sweep reads it), so the contents a previous call leaves behind are harmless.
+ * Result: bitwise the one of pz_poisson_stage(plan, p, PZ_STAGE_Z_SOLVE) with zsolve_variant = 0. */
+#define PZ_NOALLOC_MAX_POINTS (1LL << 21)
+PZ_API int poisson_zsolve_noalloc(pz_plan *plan, double *p, void *stream);
+
 /* Frees every device and host resource of the plan.  NULL is accepted. */
 PZ_API int poisson_plan_destroy(pz_plan *plan);
 

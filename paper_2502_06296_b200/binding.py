@@ -49,6 +49,7 @@ SIGNATURES = {
     "pz_project": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_double, _vp]),
     "pz_pressure_correction": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_double, _vp]),
     "pz_solve_host_batch": (_i, [_vp, _vp, ctypes.POINTER(_vp), ctypes.c_int, _vp]),
+    "poisson_zsolve_noalloc": (_i, [_vp, _vp, _vp]),
     "poisson_plan_destroy": (_i, [_vp]),
     "pz_last_error": (ctypes.c_char_p, []),
     "pz_poisson_stage": (_i, [_vp, _vp, _i, _vp]),
@@ -285,6 +286,14 @@ def helmholtz_z_solve_host(plan: Plan, u_host, stream=None) -> None:
 
 def pz_poisson_stage(plan: Plan, p, stage: int, stream=None) -> None:
     _check(lib().pz_poisson_stage(plan.handle, _dev_ptr(p, plan.n), int(stage), _stream_ptr(stream)))
+
+
+PZ_NOALLOC_MAX_POINTS = 1 << 21
+
+
+def poisson_zsolve_noalloc(plan: Plan, p, stream=None) -> None:
+    """Step a3 on the spectral field p, in place, with the library's static workspace (no allocation)."""
+    _check(lib().poisson_zsolve_noalloc(plan.handle, _dev_ptr(p, plan.n), _stream_ptr(stream)))
 
 
 def pz_set_option(plan: Plan, key: str, value: int) -> None:

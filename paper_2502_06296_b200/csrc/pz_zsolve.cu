@@ -204,3 +204,62 @@ int launch_zsolve(pz_plan *pl, double *p, cudaStream_t st, double helm_a)
 }
 
 } // namespace pz
+
+// -------------------------------------------------------------------------------------------------
+// poisson_zsolve_noalloc (include/pz.h): the sweep above with its workspace in a file-scope device
+// array instead of pl->d_zwork, for callers that may not allocate.  In host code `g_noalloc_work` is
+// only a stand-in for the device symbol -- a kernel given it would fault (or, where the GPU can
+// reach host memory, quietly use the wrong memory) --, so its device address is looked up once per
+// device, with that device current, and that pointer goes to the kernel.
+namespace pz {
+namespace {
+
+static __device__ __align__(256) double g_noalloc_work[PZ_NOALLOC_MAX_POINTS];
+
+constexpr int kMaxDevices = 64;
+double *g_noalloc_ptr[kMaxDevices];   // device address of g_noalloc_work on each device (nullptr: not yet looked up)
+
+int noalloc_workspace(int device, double **out)
+{
+    if (device < 0 || device >= kMaxDevices) { set_error("poisson_zsolve_noalloc: device %d out of range", device); return PZ_EUNSUPPORTED; }
+    double *ptr = __atomic_load_n(&g_noalloc_ptr[device], __ATOMIC_ACQUIRE);
+    if (!ptr) {
+        // the same address whoever gets here first: a race between two threads is benign
+        const cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void **>(&ptr), g_noalloc_work);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(g_noalloc_work)");
+        if (!ptr) { set_error("poisson_zsolve_noalloc: the workspace symbol has no device address"); return PZ_ECUDA; }
+        __atomic_store_n(&g_noalloc_ptr[device], ptr, __ATOMIC_RELEASE);
+    }
+    *out = ptr;
+    return PZ_OK;
+}
+
+} // namespace
+} // namespace pz
+
+extern "C" int poisson_zsolve_noalloc(pz_plan *pl, double *p, void *stream)
+{
+    using namespace pz;
+    if (!pl || !p) { set_error("poisson_zsolve_noalloc: NULL argument"); return PZ_EINVAL; }
+    if (((uintptr_t)p & 7) != 0) { set_error("poisson_zsolve_noalloc: p must be 8-byte aligned"); return PZ_EINVAL; }
+    if (pl->slab_G > 0 && !pl->slab_internal) { set_error("poisson_zsolve_noalloc: a z-slab plan holds part of every column"); return PZ_EINVAL; }
+    if (pl->n > (size_t)PZ_NOALLOC_MAX_POINTS) {
+        set_error("poisson_zsolve_noalloc: %zu points exceed the static workspace of %lld (PZ_NOALLOC_MAX_POINTS); use poisson_solve", pl->n,
+                  (long long)PZ_NOALLOC_MAX_POINTS);
+        return PZ_EUNSUPPORTED;
+    }
+    int dev = -1;
+    PZ_CUDA(cudaGetDevice(&dev));
+    if (dev != pl->device) { set_error("poisson_zsolve_noalloc: the plan lives on device %d, device %d is current", pl->device, dev); return PZ_EINVAL; }
+    double *work = nullptr;
+    const int rc = noalloc_workspace(dev, &work);
+    if (rc != PZ_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t plane = (size_t)pl->nx * pl->ny;
+    const unsigned blocks = (unsigned)((plane + 127) / 128);
+    zsolve_thomas_kernel<<<blocks, 128, 0, st>>>(p, work, pl->d_A, pl->d_C, pl->d_dzf, pl->d_lamx, pl->d_lamy_nat, pl->d_lamy_pk, pl->nx,
+                                                  pl->ny, pl->nz, pl->inv_lz, pl->pw0, pl->pw1, pl->zflags(), -1.0);
+    count_launch();
+    PZ_CUDA(cudaGetLastError());
+    return PZ_OK;
+}
