@@ -106,7 +106,9 @@ __host__ __device__ constexpr int bitrev(int p, int bits)
 // TWMODE 0: every twiddle w^{r jm} is looked up (cheap when all lanes of a warp share jm: the y
 // kernels).  TWMODE 1: only w^{jm}, w^{2jm}, w^{4jm}, w^{8jm} are looked up and the other powers are
 // products of two of them (one rounding more; the x kernels, whose lanes hit 16-32 different
-// table lines per lookup and would otherwise be bound by L1 wavefronts).
+// table lines per lookup and would otherwise be bound by L1 wavefronts).  TWMODE 2: ONE look-up,
+// w^{jm}; w^2, w^4, w^8 by squaring (at most three roundings more; the x kernels and the y kernels
+// from 1024 points: 3.69 -> 3.27 ms for the x transform at nx = 2048, 19.1 -> 18.2 ms per c3 solve).
 template <int L, int E, int R, int NS, int TWSTRIDE, int TWMODE>
 __device__ __forceinline__ void pass_butterflies(double2 (&v)[E], int tid, const double2 *__restrict__ tw)
 {
@@ -125,8 +127,15 @@ __device__ __forceinline__ void pass_butterflies(double2 (&v)[E], int tid, const
                 }
             } else {
                 double2 w[R];
+                if constexpr (TWMODE == 2) {
+                    // ONE look-up; w^2, w^4, w^8 by squaring (two roundings more on the highest power)
+                    w[1] = __ldg(&tw[jm * STEP]);
 #pragma unroll
-                for (int r = 1; r < R; r *= 2) w[r] = __ldg(&tw[r * jm * STEP]);
+                    for (int r = 2; r < R; r *= 2) w[r] = cmul(w[r / 2], w[r / 2]);
+                } else {
+#pragma unroll
+                    for (int r = 1; r < R; r *= 2) w[r] = __ldg(&tw[r * jm * STEP]);
+                }
 #pragma unroll
                 for (int r = 3; r < R; ++r) {
                     if ((r & (r - 1)) != 0) { // not a power of two: highest set bit times the rest

@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(FftPlan<M>::T *LPB, (FftPlan<M>::T * LPB <= 12
 #pragma unroll
             for (int e = 0; e < E; ++e) v[e] = active ? lp[tid + e * T] : make_double2(0.0, 0.0);
         }
-        fft_line<M, 2, 1>(v, tid, tw, xc);
+        fft_line<M, 2, 2>(v, tid, tw, xc);
         if constexpr (P::R2 > 1) xc.sync();
 #pragma unroll
         for (int e = 0; e < E; ++e) xc.put_lin(tid + e * T, v[e]);
@@ -136,7 +136,7 @@ __global__ void __launch_bounds__(FftPlan<M>::T *LPB, (FftPlan<M>::T * LPB <= 12
         }
         // every global read of the line precedes the first barrier inside fft_line (or, for a
         // single-pass transform, is done by the one thread that owns the line): in place is safe
-        fft_line<M, 2, 1>(v, tid, tw, xc);
+        fft_line<M, 2, 2>(v, tid, tw, xc);
         if (active) {
 #pragma unroll
             for (int e = 0; e < E; ++e) lp[tid + e * T] = make_double2(v[e].x * scale, -v[e].y * scale);

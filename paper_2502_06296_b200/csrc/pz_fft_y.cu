@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(FftPlan<L>::T *TC, (FftPlan<L>::T * TC <= 256)
             v[e] = INV ? cconj(t) : t;
         }
     }
-    fft_line<L, 1, (L >= 1024) ? 1 : 0>(v, tid, tw, xc); // long lines: factored twiddles (fewer L1 look-ups)
+    fft_line<L, 1, (L >= 1024) ? 2 : 0>(v, tid, tw, xc); // long lines: factored twiddles (fewer L1 look-ups)
     if (!INV && p0) {
         __syncthreads();
         if (c == 0)
