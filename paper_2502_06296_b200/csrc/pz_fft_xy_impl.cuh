@@ -152,8 +152,9 @@ __device__ __forceinline__ void x_item_fwd(double *__restrict__ plane_base, cons
         for (int r = 0; r < R2; ++r) v[r] = xc.get(t + r * R1);
         next();
         dif<R2, 1>(v);
+        // every result goes to global memory as soon as it is formed: nothing but v is held (an
+        // array of the 32 results beside v spilled 800 bytes per thread)
         const int src = (32 - t) & 31;
-        double2 o[R2];
 #pragma unroll
         for (int rp = 0; rp < R2; ++rp) {
             const double2 mine = v[slot_of<R2>(R2 - 1 - rp)];
@@ -161,11 +162,10 @@ __device__ __forceinline__ void x_item_fwd(double *__restrict__ plane_base, cons
             pa.x = __shfl_sync(0xffffffffu, mine.x, src);
             pa.y = __shfl_sync(0xffffffffu, mine.y, src);
             if (t == 0) pa = v[slot_of<R2>((R2 - rp) % R2)];
-            o[rp] = r2c_split<2, 0>(v[slot_of<R2>(rp)], pa, __ldg(&tw[t + 32 * rp]));
+            double2 o = r2c_split<2, 0>(v[slot_of<R2>(rp)], pa, __ldg(&tw[t + 32 * rp]));
+            if (rp == 0 && t == 0) o = make_double2(v[0].x + v[0].y, v[0].x - v[0].y);
+            st2h(&lp[t + 32 * rp], o, pol);
         }
-        if (t == 0) o[0] = make_double2(v[0].x + v[0].y, v[0].x - v[0].y);
-#pragma unroll
-        for (int rp = 0; rp < R2; ++rp) st2h(&lp[t + 32 * rp], o[rp], pol);
     }
 }
 
@@ -225,20 +225,27 @@ __device__ __forceinline__ void x_item_inv(double *__restrict__ plane_base, cons
         static_assert(T == 32, "one warp per line");
 #pragma unroll
         for (int r = 0; r < R1; ++r) v[r] = in[t + 32 * r];
+        // merged in place, indices r and R1-1-r together (partners of each other in the other lanes);
+        // lane 0 pairs r with (R1 - r) mod R1 instead, whose old value is carried along in `hi`
         const int src = (32 - t) & 31;
-        double2 z[R1];
+        double2 hi = v[0];   // old v[(R1 - r) % R1] for lane 0 at step r
 #pragma unroll
-        for (int r = 0; r < R1; ++r) {
-            const double2 mine = v[R1 - 1 - r];
-            double2 pa;
-            pa.x = __shfl_sync(0xffffffffu, mine.x, src);
-            pa.y = __shfl_sync(0xffffffffu, mine.y, src);
-            if (t == 0) pa = v[(R1 - r) % R1];
-            z[r] = c2r_merge_conj<2, 0>(v[r], pa, __ldg(&tw[t + 32 * r]));
+        for (int r = 0; r < R1 / 2; ++r) {
+            const int q = R1 - 1 - r;
+            const double2 a = v[r], b = v[q];
+            double2 pa, pb;   // partners of index r and of index q
+            pa.x = __shfl_sync(0xffffffffu, b.x, src);
+            pa.y = __shfl_sync(0xffffffffu, b.y, src);
+            pb.x = __shfl_sync(0xffffffffu, a.x, src);
+            pb.y = __shfl_sync(0xffffffffu, a.y, src);
+            if (t == 0) { pa = hi; pb = v[r + 1]; }   // (R1 - q) mod R1 = r + 1: not yet overwritten
+            double2 za = c2r_merge_conj<2, 0>(a, pa, __ldg(&tw[t + 32 * r]));
+            const double2 zb = c2r_merge_conj<2, 0>(b, pb, __ldg(&tw[t + 32 * q]));
+            if (r == 0 && t == 0) za = make_double2(a.x + a.y, -(a.x - a.y));
+            hi = b;           // = old v[R1 - (r + 1)]
+            v[r] = za;
+            v[q] = zb;
         }
-        if (t == 0) z[0] = make_double2(v[0].x + v[0].y, -(v[0].x - v[0].y));
-#pragma unroll
-        for (int r = 0; r < R1; ++r) v[r] = z[r];
         dif<R1, 1>(v);
         __syncthreads();
 #pragma unroll
@@ -560,11 +567,18 @@ int launch_xy(pz_plan *pl, double *p, cudaStream_t st)
     if (blocks > total) blocks = total;
     // D: the first phase may run this many planes ahead (what is in flight stays in L2); enough
     // that half the CTAs find first-phase work while the other half runs the second phase
+    // Planes of 16 MB: what is in flight between the phases must still fit L2 (126 MB) beside the
+    // streams: at most three planes ahead, one plane of prefetch (2048 x 1024 x 512: 6.3 + 6.0 ms
+    // against 6.4 + 8.0 ms with the defaults below)
+    const bool big_planes = (size_t)pl->nx * pl->ny * sizeof(double) >= ((size_t)16 << 20);
     int D = pl->opt.xy_lag;
-    if (D <= 0) D = 2 + (int)((blocks + a.n1 - 1) / a.n1);
+    if (D <= 0) {
+        D = 2 + (int)((blocks + a.n1 - 1) / a.n1);
+        if (big_planes && D > 3) D = 3;
+    }
     if (D > pl->nz) D = pl->nz;
     a.D = D;
-    a.pf = pl->opt.xy_prefetch > 0 ? pl->opt.xy_prefetch : 3;
+    a.pf = pl->opt.xy_prefetch > 0 ? pl->opt.xy_prefetch : (big_planes ? 1 : 3);
     // SMs of a role group run the same phase (the two SMs of a TPC share an instruction-cache level);
     // measured at 512^3: forward 0.598 ms with groups of 4 against 0.612 with 2, inverse 0.572 with 2 against 0.582
     a.group = pl->opt.xy_group > 0 ? pl->opt.xy_group : (INV ? 2 : 4);

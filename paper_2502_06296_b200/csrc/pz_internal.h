@@ -33,7 +33,7 @@ struct Options {
                               // 2 = the same solve inside a TMA load / solve / TMA store pipeline
     int zsolve_probe = 0;     // diagnostic (variant 2): 2 = no arithmetic (results are wrong)
     int zsolve_stages = 0;    // variant 2: shared-memory stages (0 = as many as fit, at most 3)
-    int fft_fused = -1;       // -1 = auto (currently the separate kernels); 0 = separate kernels; 1 = fused x/y kernel
+    int fft_fused = -1;       // -1 = auto (use_fused, pz_api.cu); 0 = separate kernels; 1 = fused x/y kernel
                               // (nx, ny in {256, 512, 1024, 2048})
     int xy_lag = 0;           // fused kernel: planes by which the first phase runs ahead (0 = auto)
     int xy_bps = 0;           // fused kernel: resident CTAs per SM (0 = as many as fit)

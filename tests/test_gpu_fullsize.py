@@ -167,21 +167,25 @@ def _c3_like(wl, nx, ny, nz):
 
 @pytest.mark.parametrize("shape", [(2048, 1024, 128), (64, 64, 512), (2048, 64, 512), (64, 1024, 512)])
 def test_c3_templates_element_by_element(env, shape):
-    """The kernels c3 runs (x transform of 2048 reals, y transform of 1024 points, z-solve with
-    16-row sub-domains on the beta = 2.0 grid), whole solves compared with the oracle element by
-    element (Eq. 12; verification style PAPER.md:256)."""
+    """The kernels c3 runs (x transform of 2048 reals, y transform of 1024 points -- in one fused
+    kernel by default at 2048 x 1024, and as the separate kernels --, z-solve with 16-row sub-domains
+    on the beta = 2.0 grid), whole solves compared with the oracle element by element (Eq. 12,
+    PAPER.md:86; verification style PAPER.md:256)."""
     torch, pz, wl, oracle = env
     w = _c3_like(wl, *shape)
     zc, zf = wl.grid(w)
     plan = pz.poisson_plan_create(w.nx, w.ny, w.nz, w.lx, w.ly, zc, zf)
     f = wl.poisson_rhs(w)
-    p = torch.from_numpy(f).cuda()
-    pz.poisson_solve(plan, p)
-    torch.cuda.synchronize()
-    got = p.cpu().numpy()
-    del p
     ref = oracle.poisson_solve(w.lx, w.ly, zc, zf, f, 1)
-    assert rel_err(got, ref) <= TOL
+    for fused in (None, 0):               # None: the plan's own choice (bench.py's configuration)
+        if fused is not None:
+            pz.pz_set_option(plan, "fft_fused", fused)
+        p = torch.from_numpy(f).cuda()
+        pz.poisson_solve(plan, p)
+        torch.cuda.synchronize()
+        got = p.cpu().numpy()
+        del p
+        assert rel_err(got, ref) <= TOL, fused
     pz.poisson_plan_destroy(plan)
 
 
