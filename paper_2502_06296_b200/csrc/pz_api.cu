@@ -149,18 +149,13 @@ bool use_fused(const pz_plan *pl)
     if (pl->opt.slab_planes > 0 || pl->opt.fft_fused == 0 || !fused_sizes(pl) || pl->bcx || pl->bcy) return false;
     if (pl->opt.fft_fused == 1) return true;
     // auto: the fused kernel hands a plane from the x to the y transform through L2 (16 instead of
-    // 32 DRAM bytes per point, ncu r02); that needs a few planes in flight to stay L2-resident: up to
-    // 4 MB per plane always (512^3: 0.60 + 0.57 ms against 0.71 + 0.72 ms for the separate kernels),
-    // and the 8 / 16 MB planes with ny = 1024, where the first phase runs no more than three planes
-    // ahead and prefetches one (launch_xy): 1024 x 1024 x 256 3.58 against 4.24 ms per solve,
-    // 2048 x 1024 x 512 16.2 against 18.2 ms (ncu: 17.6 / 21.8 GB of DRAM traffic per direction
-    // against 34.4).  2048 x 512 planes tie (8.0 ms either way) and keep the separate kernels; a 256^3
-    // field is L2-sized as a whole and the separate kernels already hit L2: 0.30 against 0.32 ms.
-    // Lines of nx = 2048 (1024-point items, one warp per line) with short columns lose to the separate
-    // kernels: 2048 x 256 x 1024 5.97 against 5.60 ms for the four transforms.
-    const size_t plane_bytes = (size_t)pl->nx * pl->ny * sizeof(double);
-    const bool sizes = (pl->nx == 2048) ? pl->ny == 1024 : (plane_bytes <= ((size_t)4 << 20) || pl->ny == 1024);
-    return sizes && pl->n * sizeof(double) >= ((size_t)512 << 20);
+    // 32 DRAM bytes per point, ncu r02), which needs the few planes in flight to stay L2-resident
+    // (planes of 16 MB: at most three planes ahead, one plane of prefetch, launch_xy).  Against the
+    // separate kernels, per solve: 512^3 1.63 / 1.90 ms, 1024 x 1024 x 256 3.51 / 4.24 ms,
+    // 2048 x 512 x 512 7.4 / 7.9 ms, 2048 x 256 x 1024 9.1 / 9.4 ms, 2048 x 1024 x 512 15.5 / 18.2 ms
+    // (ncu: 17.6 / 21.8 GB of DRAM traffic per direction against 34.4).  A field of L2 size is served
+    // from L2 by the separate kernels anyway (256^3: 0.30 against 0.32 ms).
+    return pl->n * sizeof(double) >= ((size_t)512 << 20);
 }
 
 int forward_xy(pz_plan *pl, double *p, cudaStream_t st)

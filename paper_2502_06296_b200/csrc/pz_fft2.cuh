@@ -77,12 +77,17 @@ struct Xchg2X {
 template <int L, int R1> __host__ __device__ constexpr int xline_elems() { return (L / R1) * (R1 + 1); }
 
 // y columns: TC neighbouring complex columns side by side, c fastest: 8 lanes = 128 contiguous bytes
-template <int TC>
+// With TC = 4 (columns of 1024 points) a quarter warp holds two butterflies j1 whose pass-1 outputs
+// lie 32 rows = 2 KB apart: the same banks.  PAD skips one row every 32 (as Xchg2X does), which puts
+// them 64 bytes apart modulo 128: conflict-free (ncu r02: 606 M shared-memory wavefronts per launch at
+// 2048 x 1024 x 512 where 470 M are needed).
+template <int TC, bool PAD = false>
 struct Xchg2Y {
     double2 *buf;
     int c;
-    __device__ __forceinline__ void put(int pos, double2 v) const { buf[pos * TC + c] = v; }
-    __device__ __forceinline__ double2 get(int pos) const { return buf[pos * TC + c]; }
+    __device__ __forceinline__ static int idx(int pos) { return PAD ? pos + (pos >> 5) : pos; }
+    __device__ __forceinline__ void put(int pos, double2 v) const { buf[idx(pos) * TC + c] = v; }
+    __device__ __forceinline__ double2 get(int pos) const { return buf[idx(pos) * TC + c]; }
 };
 
 // Residue classes mod 32 closed under negation for thread t of T (x lines): 32 / T classes per
@@ -113,6 +118,54 @@ __device__ __forceinline__ double2 c2r_merge_conj(double2 xk, double2 xmk, doubl
     const double2 xm = cconj(xmk);
     const double2 s = cadd(xk, xm);
     const double2 c = cmul_conj(mul_wc<R2X, ROT>(csub(xk, xm)), wj);
+    return make_double2(s.x - c.y, -(s.y + c.x));
+}
+
+// ---- lines of n = 2048 reals (M = 1024): w_n^k with k = t + 32 r' is w_n^t w_64^{r'}; the first
+// factor is one look-up per thread, the second a compile-time constant (32 look-ups per thread and
+// line cost as many L1 wavefronts as an exchange and their latency was the kernel's second stall).
+__host__ __device__ constexpr double cos64(int m) // cos(2 pi m / 64), m = 0..16
+{
+    constexpr double c[17] = {1.0,
+                              0.995184726672196886245, 0.980785280403230449126, 0.956940335732208864936, 0.923879532511286756128,
+                              0.881921264348355029713, 0.831469612302545237079, 0.773010453362736960811, 0.707106781186547524401,
+                              0.634393284163645498215, 0.555570233019602224743, 0.471396736825997648556, 0.382683432365089771728,
+                              0.290284677254462367636, 0.195090322016128267848, 0.0980171403295606019942, 0.0};
+    return c[m];
+}
+__host__ __device__ constexpr double c64(int m) { return m <= 16 ? cos64(m) : -cos64(32 - m); } // cos(2 pi m / 64), m <= 32
+__host__ __device__ constexpr double s64(int m) { return m <= 16 ? cos64(16 - m) : cos64(m - 16); } // sin
+// d * w_64^r (CONJ: d * conj(w_64^r)), r = 0..31
+template <int r, bool CONJ>
+__device__ __forceinline__ double2 rot64(double2 d)
+{
+    static_assert(r >= 0 && r < 32, "w_64^r with r < 32");
+    if constexpr (r == 0) {
+        return d;
+    } else if constexpr (r == 16) {
+        return CONJ ? make_double2(-d.y, d.x) : make_double2(d.y, -d.x);
+    } else {
+        constexpr double c = c64(r), sg = CONJ ? -s64(r) : s64(r);
+        // (d.x + i d.y)(c - i sg)
+        return make_double2(fma(d.x, c, d.y * sg), fma(d.y, c, -(d.x * sg)));
+    }
+}
+// r2c_split / c2r_merge_conj with the twiddle w_n^{t + 32 r} = wt w_64^r
+template <int r>
+__device__ __forceinline__ double2 r2c_split64(double2 zk, double2 zmk, double2 wt)
+{
+    const double2 zm = cconj(zmk);
+    const double2 ev = make_double2(0.5 * (zk.x + zm.x), 0.5 * (zk.y + zm.y));
+    const double2 d = csub(zk, zm);
+    const double2 od = make_double2(0.5 * d.y, -0.5 * d.x);
+    return cadd(ev, cmul(rot64<r, false>(od), wt));
+}
+template <int r>
+__device__ __forceinline__ double2 c2r_merge_conj64(double2 xk, double2 xmk, double2 wt)
+{
+    const double2 xm = cconj(xmk);
+    const double2 s = cadd(xk, xm);
+    const double2 c = cmul_conj(rot64<r, true>(csub(xk, xm)), wt);
     return make_double2(s.x - c.y, -(s.y + c.x));
 }
 

@@ -155,17 +155,18 @@ __device__ __forceinline__ void x_item_fwd(double *__restrict__ plane_base, cons
         // every result goes to global memory as soon as it is formed: nothing but v is held (an
         // array of the 32 results beside v spilled 800 bytes per thread)
         const int src = (32 - t) & 31;
-#pragma unroll
-        for (int rp = 0; rp < R2; ++rp) {
+        const double2 wt = __ldg(&tw[t]);   // w_n^t; w_n^{t + 32 r'} = wt w_64^{r'}
+        static_for<0, R2>([&](auto ic) {
+            constexpr int rp = decltype(ic)::value;
             const double2 mine = v[slot_of<R2>(R2 - 1 - rp)];
             double2 pa;
             pa.x = __shfl_sync(0xffffffffu, mine.x, src);
             pa.y = __shfl_sync(0xffffffffu, mine.y, src);
             if (t == 0) pa = v[slot_of<R2>((R2 - rp) % R2)];
-            double2 o = r2c_split<2, 0>(v[slot_of<R2>(rp)], pa, __ldg(&tw[t + 32 * rp]));
+            double2 o = r2c_split64<rp>(v[slot_of<R2>(rp)], pa, wt);
             if (rp == 0 && t == 0) o = make_double2(v[0].x + v[0].y, v[0].x - v[0].y);
             st2h(&lp[t + 32 * rp], o, pol);
-        }
+        });
     }
 }
 
@@ -229,9 +230,9 @@ __device__ __forceinline__ void x_item_inv(double *__restrict__ plane_base, cons
         // lane 0 pairs r with (R1 - r) mod R1 instead, whose old value is carried along in `hi`
         const int src = (32 - t) & 31;
         double2 hi = v[0];   // old v[(R1 - r) % R1] for lane 0 at step r
-#pragma unroll
-        for (int r = 0; r < R1 / 2; ++r) {
-            const int q = R1 - 1 - r;
+        const double2 wt = __ldg(&tw[t]);   // w_n^t; w_n^{t + 32 r} = wt w_64^r
+        static_for<0, R1 / 2>([&](auto ic) {
+            constexpr int r = decltype(ic)::value, q = R1 - 1 - r;
             const double2 a = v[r], b = v[q];
             double2 pa, pb;   // partners of index r and of index q
             pa.x = __shfl_sync(0xffffffffu, b.x, src);
@@ -239,13 +240,13 @@ __device__ __forceinline__ void x_item_inv(double *__restrict__ plane_base, cons
             pb.x = __shfl_sync(0xffffffffu, a.x, src);
             pb.y = __shfl_sync(0xffffffffu, a.y, src);
             if (t == 0) { pa = hi; pb = v[r + 1]; }   // (R1 - q) mod R1 = r + 1: not yet overwritten
-            double2 za = c2r_merge_conj<2, 0>(a, pa, __ldg(&tw[t + 32 * r]));
-            const double2 zb = c2r_merge_conj<2, 0>(b, pb, __ldg(&tw[t + 32 * q]));
+            double2 za = c2r_merge_conj64<r>(a, pa, wt);
+            const double2 zb = c2r_merge_conj64<q>(b, pb, wt);
             if (r == 0 && t == 0) za = make_double2(a.x + a.y, -(a.x - a.y));
             hi = b;           // = old v[R1 - (r + 1)]
             v[r] = za;
             v[q] = zb;
-        }
+        });
         dif<R1, 1>(v);
         __syncthreads();
 #pragma unroll
@@ -278,14 +279,14 @@ __device__ __forceinline__ void y_item(double *__restrict__ plane_base, const do
     constexpr int R1 = 32, R2 = L / 32, T = R2, NB = 32 / R2, TC = kThreads / T;
     const int c = threadIdx.x % TC, t = threadIdx.x / TC;
     double *base = plane_base + 2 * ((size_t)idx * TC + c);
-    Xchg2Y<TC> xc{smem, c};
+    Xchg2Y<TC, (TC < 8)> xc{smem, c};   // the exchange; the tile the TMA boxes deliver is dense
     constexpr int h = L / 2;
 
     double2 v[kE2];
 #pragma unroll
     for (int r = 0; r < R1; ++r) {
         const int row = t + r * T;
-        double2 x = xc.get(row);
+        double2 x = smem[row * TC + c];
         if (INV && P0 && c == 0) {
             // re-merge the packed spectra of columns 0 and 1 into W_row = A + i B
             if (row == 0 || row == h) {
@@ -391,7 +392,7 @@ template <int MX, int LY> struct XYGeo {
     static constexpr size_t SMEM_XF = (size_t)LPB * xline_elems<MX, 32>() * sizeof(double2);
     static constexpr size_t SMEM_XI = (size_t)LPB * xline_elems<MX, MX / 32>() * sizeof(double2);
     static constexpr size_t SMEM_X = SMEM_XF > SMEM_XI ? SMEM_XF : SMEM_XI;
-    static constexpr size_t SMEM_Y = (size_t)LY * TC * sizeof(double2);
+    static constexpr size_t SMEM_Y = (size_t)(TC < 8 ? LY + LY / 32 : LY) * TC * sizeof(double2);   // padded exchange (Xchg2Y)
     static constexpr size_t SMEM = (SMEM_X > SMEM_Y ? SMEM_X : SMEM_Y) + 128; // + alignment slack
     static constexpr unsigned X_BYTES = (unsigned)((size_t)LPB * MX * sizeof(double2));
     static constexpr unsigned Y_BYTES = (unsigned)((size_t)LY * TC * sizeof(double2));
