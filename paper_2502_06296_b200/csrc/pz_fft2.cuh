@@ -64,17 +64,39 @@ template <int R, int r>
 __device__ __forceinline__ double2 mul_wc(double2 d) { return cconj(mul_w<R, r>(cconj(d))); }
 
 // ---- exchange buffers
-// x lines: one line per T threads, 16-byte elements, indexed (pos / R1)(R1 + 1) + pos % R1: lanes of
-// pass 1 (consecutive j1 = pos / R1) write with stride R1 + 1, lanes of pass 2 (consecutive
-// j2 = pos % R1) read consecutive elements; both are conflict-free (8 lanes x 16 B per wavefront).
-template <int R1>
+// x lines: one line per T <= 32 threads, 16-byte elements.  Lanes of pass 1 (consecutive
+// j1 = pos / R1) write with a stride of R1 elements, lanes of pass 2 (consecutive j2 = pos % R1) read
+// consecutive elements.
+// PADDED (INPLACE = false): element pos at (pos / R1)(R1 + 1) + pos % R1; both accesses are
+//   conflict-free (8 lanes x 16 B per wavefront); the padded line reaches into the space of the next
+//   line's input, so the exchange is bracketed by CTA barriers.
+// IN PLACE (R1 >= 8): element pos at pos ^ ((pos / R1) & 7) -- the 16-byte chunk index is swizzled
+//   with the butterfly index: conflict-free as well, and a line stays inside its own M elements; the
+//   lines of a warp being its own, the exchange needs __syncwarp only (ncu r02: the CTA barriers are
+//   the largest stall of the fused kernel).  Used by the forward items (R1 = 32: 0.599 -> 0.572 ms at
+//   512^3); in the inverse items of 256-point lines (R1 = 8) the 32 run-time store addresses per
+//   thread spilled 400 bytes and lost more than the barriers cost.
+template <int R1, bool INPLACE = false>
 struct Xchg2X {
+    static_assert(!INPLACE || R1 >= 8, "the swizzle permutes the low three bits of the position");
     double2 *buf;
-    __device__ __forceinline__ static int idx(int pos) { return (pos / R1) * (R1 + 1) + (pos % R1); }
+    __device__ __forceinline__ static int idx(int pos)
+    {
+        if constexpr (INPLACE) return pos ^ ((pos / R1) & 7);
+        else return (pos / R1) * (R1 + 1) + (pos % R1);
+    }
     __device__ __forceinline__ void put(int pos, double2 v) const { buf[idx(pos)] = v; }
     __device__ __forceinline__ double2 get(int pos) const { return buf[idx(pos)]; }
+    // orders the accesses of the threads that may touch the same elements
+    __device__ __forceinline__ static void sync()
+    {
+        if constexpr (INPLACE) __syncwarp();
+        else __syncthreads();
+    }
 };
-template <int L, int R1> __host__ __device__ constexpr int xline_elems() { return (L / R1) * (R1 + 1); }
+template <int L, int R1, bool INPLACE = false> __host__ __device__ constexpr int xline_elems() { return INPLACE ? L : (L / R1) * (R1 + 1); }
+// forward x items of the fused kernel: in place from 256-point lines (128-point lines measured slower)
+template <int M> __host__ __device__ constexpr bool x_fwd_inplace() { return M >= 256; }
 
 // y columns: TC neighbouring complex columns side by side, c fastest: 8 lanes = 128 contiguous bytes
 // With TC = 4 (columns of 1024 points) a quarter warp holds two butterflies j1 whose pass-1 outputs

@@ -87,28 +87,29 @@ template <int TX, int TY> struct TwTab {
 // x item, forward: LPB = 128 / T lines of one plane, T = M / 32 threads per line (M = nx / 2).
 // pass 1: radix 32, butterfly j1 = t, twiddle w_M^{t r'} on its outputs;  pass 2: radix M / 32 on
 // the residue classes (+-t) of the thread, then the real-to-complex split in registers.
-// `in` holds the LPB lines back to back (M complex each); the exchange re-uses the buffer with a
-// padded pitch.  next() is called by every thread once the buffer is free again.
+// `in` holds the LPB lines back to back (M complex each); the exchange re-uses the buffer, in place
+// (Xchg2X).  next() is called by every thread once the buffer is free again.
 template <int M, class Next>
 __device__ __forceinline__ void x_item_fwd(double *__restrict__ plane_base, const double2 *__restrict__ tw,
                                            const double2 *xp, const double2 *xs, int idx, double2 *smem, uint64_t pol, Next next)
 {
     constexpr int R1 = 32, R2 = M / 32, T = R2, NB = 32 / R2, LPB = kThreads / T;
-    constexpr int LD = xline_elems<M, R1>();
+    constexpr bool IP = x_fwd_inplace<M>();
+    constexpr int LD = xline_elems<M, R1, IP>();
     const int t = threadIdx.x % T, ll = threadIdx.x / T;
     double2 *lp = reinterpret_cast<double2 *>(plane_base + ((size_t)idx * LPB + ll) * (2 * (size_t)M));
     const double2 *in = smem + (size_t)ll * M;
-    Xchg2X<R1> xc{smem + (size_t)ll * LD};
+    Xchg2X<R1, IP> xc{smem + (size_t)ll * LD};
 
     double2 v[kE2];
 #pragma unroll
     for (int r = 0; r < R1; ++r) v[r] = in[t + r * T];
     dif<R1, 1>(v);
     apply_twiddles32<true>(v, xp + t, T);
-    __syncthreads(); // every line has been read: the padded exchange layout may overwrite it
+    xc.sync(); // every line has been read: the exchange may overwrite it
 #pragma unroll
     for (int rp = 0; rp < R1; ++rp) xc.put(t * R1 + rp, v[slot_of<R1>(rp)]);
-    __syncthreads();
+    xc.sync();
 
     if constexpr (NB >= 2) {
         constexpr int NP = NB / 2;
@@ -389,7 +390,7 @@ template <int MX, int LY> struct XYGeo {
     static constexpr int TC = kThreads / TY;    // complex pairs per y item
     static constexpr int BOXR = LY < 256 ? LY : 256; // rows per TMA box of a y tile
     // x exchange: R1 = 32 forward, R1 = MX / 32 inverse
-    static constexpr size_t SMEM_XF = (size_t)LPB * xline_elems<MX, 32>() * sizeof(double2);
+    static constexpr size_t SMEM_XF = (size_t)LPB * xline_elems<MX, 32, x_fwd_inplace<MX>()>() * sizeof(double2);
     static constexpr size_t SMEM_XI = (size_t)LPB * xline_elems<MX, MX / 32>() * sizeof(double2);
     static constexpr size_t SMEM_X = SMEM_XF > SMEM_XI ? SMEM_XF : SMEM_XI;
     static constexpr size_t SMEM_Y = (size_t)(TC < 8 ? LY + LY / 32 : LY) * TC * sizeof(double2);   // padded exchange (Xchg2Y)
