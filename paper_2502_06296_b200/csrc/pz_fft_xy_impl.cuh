@@ -171,9 +171,12 @@ __device__ __forceinline__ void x_item_fwd(double *__restrict__ plane_base, cons
     }
 }
 
+// elements of a warp's region in the inverse x items: its 1024 points + the padding of their exchange
+template <int M> constexpr int kWarpPitchInv = (32 / (M / 32)) * xline_elems<M, M / 32>();
+
 // x item, inverse: merge in registers on the classes (+-t), pass 1 radix M / 32, pass 2 radix 32
 // with butterfly j2 = t and the twiddle w_M^{t r} on its inputs; output x[t + r' T], natural order.
-// `in` holds the LPB packed lines back to back.
+// The packed lines arrive per warp (see below).
 template <int M, class Next>
 __device__ __forceinline__ void x_item_inv(double *__restrict__ plane_base, const double2 *__restrict__ tw,
                                            const double2 *xp, const double2 *xs, int idx, double scale, double2 *smem,
@@ -183,8 +186,14 @@ __device__ __forceinline__ void x_item_inv(double *__restrict__ plane_base, cons
     constexpr int LD = xline_elems<M, R1>();
     const int t = threadIdx.x % T, ll = threadIdx.x / T;
     double2 *lp = reinterpret_cast<double2 *>(plane_base + ((size_t)idx * LPB + ll) * (2 * (size_t)M));
-    const double2 *in = smem + (size_t)ll * M;
-    Xchg2X<R1> xc{smem + (size_t)ll * LD};
+    // A warp's lines (1024 points in all) arrive back to back in the warp's own region of
+    // kWarpPitchInv<M> elements (one bulk copy per warp); the padded exchange of a line reaches into
+    // the next line's input and, for the last line, into the region's tail: only this warp's
+    // threads ever touch the region, so the exchange is ordered by __syncwarp alone.
+    constexpr int LPW = 32 / T;   // lines per warp
+    double2 *region = smem + (size_t)(ll / LPW) * kWarpPitchInv<M>;
+    const double2 *in = region + (size_t)(ll % LPW) * M;
+    Xchg2X<R1> xc{region + (size_t)(ll % LPW) * LD};
 
     double2 v[kE2];
     if constexpr (NB >= 2) {
@@ -218,7 +227,7 @@ __device__ __forceinline__ void x_item_inv(double *__restrict__ plane_base, cons
         }
 #pragma unroll
         for (int b = 0; b < NB; ++b) dif<R1, 1>(v + b * R1);
-        __syncthreads(); // every packed line has been read
+        __syncwarp(); // every packed line of the warp has been read
 #pragma unroll
         for (int b = 0; b < NB; ++b)
 #pragma unroll
@@ -249,11 +258,11 @@ __device__ __forceinline__ void x_item_inv(double *__restrict__ plane_base, cons
             v[q] = zb;
         });
         dif<R1, 1>(v);
-        __syncthreads();
+        __syncwarp();
 #pragma unroll
         for (int rp = 0; rp < R1; ++rp) xc.put(t * R1 + rp, v[slot_of<R1>(rp)]);
     }
-    __syncthreads();
+    __syncwarp();
 #pragma unroll
     for (int r = 0; r < R2; ++r) v[r] = xc.get(t + r * R1);
     next();
@@ -480,7 +489,14 @@ __global__ void __launch_bounds__(kThreads, 3) fft_xy_kernel(const __grid_consta
         if (is_x) {
             const double *src = a.p + (size_t)it.k * plane_sz + (size_t)it.idx * G::LPB * (2 * (size_t)MX);
             mbar_arrive_expect_tx(&s_bar, G::X_BYTES);
-            bulk_load_1d_hint(smem, src, G::X_BYTES, &s_bar, pol_stream);
+            if constexpr (INV) {
+                // one copy per warp: its 1024 points into its own region (x_item_inv)
+#pragma unroll
+                for (int w = 0; w < kThreads / 32; ++w)
+                    bulk_load_1d_hint(smem + (size_t)w * kWarpPitchInv<MX>, src + (size_t)w * 2048, 1024 * sizeof(double2), &s_bar, pol_stream);
+            } else {
+                bulk_load_1d_hint(smem, src, G::X_BYTES, &s_bar, pol_stream);
+            }
             if (it.phase == 1 && it.k + a.pf < a.nz) bulk_prefetch_l2(src + (size_t)a.pf * plane_sz, G::X_BYTES);
         } else {
             mbar_arrive_expect_tx(&s_bar, G::Y_BYTES);
