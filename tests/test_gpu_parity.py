@@ -735,10 +735,11 @@ def test_error_paths_of_the_widened_entry_points(torch, pz, wl):
     pz.poisson_plan_destroy(plan)
 
 
-def test_host_batch_pipeline(torch, pz, wl, oracle):
+@pytest.mark.parametrize("nx,ny,nz", [(64, 32, 48), (24, 20, 33), (128, 64, 300)])
+def test_host_batch_pipeline(torch, pz, wl, oracle, nx, ny, nz):
     """pz_solve_host_batch: Poisson + several Helmholtz fields on pinned host buffers, more fields
     than staging buffers, twice in a row on a side stream."""
-    w = wl.scaled(wl.CONFIGS["c1"], 64, 32, 48)
+    w = wl.scaled(wl.CONFIGS["c1"], nx, ny, nz)
     zc, zf = wl.grid(w)
     f = wl.poisson_rhs(w)
     rs = [np.random.default_rng(40 + c).standard_normal((w.nz, w.ny, w.nx)) for c in range(5)]
